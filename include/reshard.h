@@ -1,0 +1,202 @@
+/*
+ * reshard.h -- C ABI of the B200-native cross-mesh resharding hot path (arXiv 2211.05322).
+ *
+ * One shared library, paper_2211_05322_b200/libreshard.so, exports exactly the symbols declared
+ * here.  No torch types, no C++ types: plain pointers and sizes.  Every pointer argument says
+ * whether it is a HOST or a DEVICE pointer.  Citations are PAPER.md:<line> (section).
+ *
+ * The operation (S2.2 "Cross-mesh resharding"): a tensor D of shape l[0..N) is held
+ * by the devices of a source mesh Mesh_A under sharding spec X_A; materialise it on a disjoint
+ * destination mesh Mesh_B under spec X_B.  Both meshes are VIRTUAL here: every virtual device is
+ * one dense row-major shard buffer in the one GPU's HBM.
+ *
+ *   device mesh     PAPER.md:78-82  n-D array of devices, row-major ids: (2,2) = [[0,1],[2,3]]
+ *   sharding spec   PAPER.md:84     one entry per tensor dim: R, or S followed by the mesh axes the
+ *                                   dim is sharded over ("S0", "S1", "S01"); first listed axis is
+ *                                   the most significant digit of the shard index (R2)
+ *   data slice      PAPER.md:86     device r holds the box [p_i*l_i/k_i, (p_i+1)*l_i/k_i) of D,
+ *                                   dense row-major, no padding (R11)
+ *   unit task       PAPER.md:90, 482-492 (App. B.2): slices = product of the per-dim intervals cut
+ *                                   at every source and destination shard boundary; senders N_i =
+ *                                   source devices holding the slice, receivers M_i = destination
+ *                                   devices requiring it.  Slice id = row-major rank in
+ *                                   I_0 x ... x I_{N-1} (dim 0 slowest).
+ *   sender choice   PAPER.md:163 (naive: lowest-indexed device), Eq. 4 (load
+ *                                   balance: minimise the maximum per-sender bytes)
+ *   broadcast       PAPER.md:137    one sender, all receivers; here: slice read ONCE from the
+ *                                   chosen sender's shard and written to EVERY receiver shard
+ *
+ * Spec text accepted: entries 'R' or 'S<axes>' separated by optional commas/spaces/parentheses,
+ * '^', '{', '}', '_' ignored after 'S': "S0,R,S1", "(S01, R, R)", "RRR", "RS^{01}R".
+ *
+ * Threading: a plan is immutable after reshard_plan returns; any number of host threads may
+ * execute the same plan concurrently on different streams.  reshard_last_error is thread-local.
+ */
+#ifndef RESHARD_H_
+#define RESHARD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define RS_API __attribute__((visibility("default")))
+#else
+#define RS_API
+#endif
+
+#define RS_MAX_NDIM       8     /* tensor dims                                              */
+#define RS_MAX_MESH_NDIM  4     /* mesh dims (the paper uses the 2-D view)      */
+#define RS_MAX_DEVICES    128   /* virtual devices per mesh                                  */
+
+typedef struct rs_plan rs_plan; /* opaque; owns its host tables and ONE device allocation    */
+
+typedef enum rs_status {
+    RS_OK = 0,
+    RS_EINVAL = 1,        /* null pointer, non-positive extent, bad elem_bytes, bad index      */
+    RS_ESPEC = 2,         /* unparsable spec, wrong entry count, mesh axis out of range or used
+                             by two tensor dims (R3)                                 */
+    RS_EDIVIS = 3,        /* l_i not divisible by the sharding degree k_i (R5)        */
+    RS_EUNSUPPORTED = 4,  /* more than RS_MAX_DEVICES devices, > 2^31-1 rows per slice, ...     */
+    RS_ENOMEM = 5,
+    RS_ECUDA = 6          /* a CUDA runtime call failed; text via reshard_last_error()          */
+} rs_status;
+
+/* flags of reshard_plan (OR together) */
+enum {
+    RS_LB_GREEDY   = 0x0,   /* Eq. 4 load balance: tasks by descending bytes, each
+                               to the lightest candidate; groups of <= 16 tasks are finished by an
+                               exact branch-and-bound (R9).  Default.                  */
+    RS_LB_NAIVE    = 0x1,   /* always the lowest-indexed candidate                  */
+    RS_PATH_AUTO   = 0x00,  /* executor chosen per operation from alignment and run length        */
+    RS_PATH_LSU    = 0x10,  /* force the register path: 128-bit ld.global -> st.global x k        */
+    RS_PATH_BULK   = 0x20,  /* force the TMA path: cp.async.bulk global->smem ring->global x k    */
+    RS_HOST_ONLY   = 0x100  /* build host tables only: no CUDA call, execute/pack/unpack refuse   */
+};
+#define RS_PATH_MASK 0xF0
+
+/* operations a plan can run */
+enum { RS_OP_EXECUTE = 0, RS_OP_PACK = 1, RS_OP_UNPACK = 2 };
+/* sides */
+enum { RS_SRC = 0, RS_DST = 1 };
+
+typedef struct rs_plan_info {
+    int32_t ndim, elem_bytes;
+    int32_t n_src, n_dst;            /* devices in Mesh_A, Mesh_B                                  */
+    int32_t n_slices;                /* unit tasks (App. B.2)                                      */
+    int32_t n_messages;              /* non-empty (sender, receiver) pairs                         */
+    int64_t tensor_bytes;            /* size(D) * e                                                */
+    int64_t src_shard_bytes;         /* bytes of ONE source shard (all equal)                      */
+    int64_t dst_shard_bytes;         /* bytes of ONE destination shard                             */
+    int64_t unique_read_bytes;       /* = tensor_bytes: every element read once      */
+    int64_t write_bytes;             /* = tensor_bytes * r_B (r_B = destination replication)       */
+    int64_t max_sender_bytes;        /* objective of Eq. 4 under the chosen senders                */
+    int64_t arena_bytes;             /* message arena for pack/unpack = write_bytes (+alignment)   */
+    int32_t lb_mode;                 /* RS_LB_GREEDY or RS_LB_NAIVE                                */
+    int32_t device;                  /* CUDA device the tables live on, -1 if RS_HOST_ONLY         */
+} rs_plan_info;
+
+typedef struct rs_op_info {
+    int32_t path;                    /* RS_PATH_LSU or RS_PATH_BULK actually selected              */
+    int32_t vec_bytes;               /* widest access every offset/stride/run of the op allows     */
+    int32_t n_tasks;                 /* copy tasks (execute/pack: one per slice; unpack: per
+                                        (slice, receiver))                                         */
+    int32_t n_dsts;                  /* (task, destination) entries                                */
+    int32_t n_tiles;                 /* entries of the flat tile table                             */
+    int32_t tile_bytes;              /* target bytes read per tile                                 */
+    int32_t grid, block;             /* launch configuration                                       */
+    int32_t smem_bytes;              /* dynamic shared memory per CTA                              */
+    int64_t read_bytes, write_bytes; /* algorithmic bytes of one launch                            */
+    int64_t min_run_bytes;           /* shortest contiguous run any tile copies                    */
+} rs_op_info;
+
+/*
+ * reshard_plan -- steps a1..a5 of the path (host): tile boxes, unit tasks, sender choice, flat
+ * task/tile tables for execute, pack and unpack, message layout; uploads the tables to the
+ * current CUDA device (one cudaMalloc + one cudaMemcpy) unless RS_HOST_ONLY.
+ *   global_shape [HOST, ndim]   l_i >= 1, 1 <= ndim <= RS_MAX_NDIM
+ *   elem_bytes                  1, 2, 4, 8 or 16; the payload is opaque bytes (R22)
+ *   src/dst_mesh_shape [HOST]   m_a >= 1, 1 <= mesh_ndim <= RS_MAX_MESH_NDIM, product <= RS_MAX_DEVICES
+ *   src/dst_spec [HOST]         NUL-terminated spec text, see above
+ *   out_plan [HOST]             receives the plan; untouched on failure.  Caller frees it with
+ *                               reshard_plan_destroy.
+ */
+RS_API rs_status reshard_plan(const int64_t *global_shape, int32_t ndim, int32_t elem_bytes,
+                       const int32_t *src_mesh_shape, int32_t src_mesh_ndim, const char *src_spec,
+                       const int32_t *dst_mesh_shape, int32_t dst_mesh_ndim, const char *dst_spec,
+                       uint32_t flags, rs_plan **out_plan);
+
+RS_API void reshard_plan_destroy(rs_plan *plan);      /* NULL is allowed */
+
+/* ---- queries (all host-side, no CUDA) ------------------------------------------------------ */
+RS_API rs_status reshard_plan_info(const rs_plan *plan, rs_plan_info *out);
+RS_API rs_status reshard_op_info(const rs_plan *plan, int32_t op, rs_op_info *out);
+/* local shard shape l_i / k_i of one side; out [HOST, ndim] */
+RS_API rs_status reshard_plan_local_shape(const rs_plan *plan, int32_t side, int64_t *out);
+/* box [lo, hi) of D that device `dev` of `side` holds; lo, hi [HOST, ndim] */
+RS_API rs_status reshard_plan_device_box(const rs_plan *plan, int32_t side, int32_t dev, int64_t *lo, int64_t *hi);
+/* unit task i: box, chosen sender, candidate senders N_i, receivers M_i.
+ * senders [HOST, n_src] / receivers [HOST, n_dst] may be NULL. */
+RS_API rs_status reshard_plan_slice(const rs_plan *plan, int32_t i, int64_t *lo, int64_t *hi,
+                             int32_t *sender, int32_t *n_senders, int32_t *senders,
+                             int32_t *n_receivers, int32_t *receivers);
+/* bytes each source device sends under the chosen senders; out [HOST, n_src] */
+RS_API rs_status reshard_plan_sender_bytes(const rs_plan *plan, int64_t *out);
+/* message m (ordered by (sender, receiver)): the concatenation, in ascending slice id, of every
+ * slice with that sender needed by that receiver, each dense row-major (the wire model, north_star
+ * item 3).  offset = byte offset inside the arena.  slice_ids [HOST, n_slices] may be NULL. */
+RS_API rs_status reshard_plan_message(const rs_plan *plan, int32_t m, int32_t *sender, int32_t *receiver,
+                               int64_t *offset, int64_t *bytes, int32_t *n_slice_ids, int32_t *slice_ids);
+
+/* Raw copy of operation `op`'s flat tables (inspection and host-side tests; the layouts are the
+ * structs RsTask / RsDst / RsTile of paper_2211_05322_b200/csrc/tables.h: 192, 16 and 32 bytes).
+ * tasks [HOST, n_tasks*192], dsts [HOST, n_dsts*16], tiles [HOST, n_tiles*32]; each may be NULL. */
+RS_API rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *dsts, void *tiles);
+
+/* ---- the data path (steps a6..a8): asynchronous, allocate nothing, never synchronise -------- */
+/*
+ * reshard_execute (PAPER.md:137 on-chip: read once, write to every receiver): for every unit task
+ * copy the slice from the chosen sender's shard into each receiver's shard.
+ *   src_shards [HOST array of n_src DEVICE pointers]  shard r = dense row-major local box of device r
+ *   dst_shards [HOST array of n_dst DEVICE pointers]  written completely (every element exactly once)
+ *   cuda_stream                                       cudaStream_t (NULL = legacy default stream)
+ * Preconditions (undefined behaviour otherwise, not checked): replicas on the source side hold
+ * identical bytes; no destination shard overlaps any other shard (Mesh_A and Mesh_B are
+ * disjoint).  Pointers of source shards that no task reads may be NULL.
+ * One kernel launch.  Returns RS_ECUDA if the launch fails, RS_EINVAL for a host-only plan.
+ */
+RS_API rs_status reshard_execute(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
+                          void *cuda_stream);
+/* reshard_pack: sender shards -> message arena [DEVICE, arena_bytes].  A slice needed by k receivers
+ * is read once and written into k messages.  One kernel launch. */
+RS_API rs_status reshard_pack(const rs_plan *plan, const void *const *src_shards, void *msg_arena, void *cuda_stream);
+/* reshard_unpack: message arena -> receiver shards.  unpack(pack(x)) == execute(x) bit for bit. */
+RS_API rs_status reshard_unpack(const rs_plan *plan, const void *msg_arena, void *const *dst_shards, void *cuda_stream);
+
+/*
+ * reshard_execute_host -- the same operation with HOST shard buffers (the end-to-end call):
+ * copies the source shards the plan reads host->device into `workspace`, runs the execute kernel,
+ * copies every destination shard device->host; all on `cuda_stream`, returns without synchronising.
+ *   src_shards_host [HOST array of n_src HOST pointers]  (pinned memory makes the copies async)
+ *   dst_shards_host [HOST array of n_dst HOST pointers]
+ *   workspace [DEVICE]  at least reshard_host_workspace_bytes(plan) bytes, 256-byte aligned
+ *   h2d_bytes, d2h_bytes [HOST, may be NULL]  receive the bytes copied in each direction
+ */
+RS_API rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shards_host,
+                               void *const *dst_shards_host, void *workspace, void *cuda_stream,
+                               int64_t *h2d_bytes, int64_t *d2h_bytes);
+RS_API int64_t reshard_host_workspace_bytes(const rs_plan *plan);
+
+/* kernels launched by this library in the calling thread since it was loaded (bench bookkeeping) */
+RS_API int64_t reshard_launch_count(void);
+
+RS_API const char *reshard_strerror(rs_status s);
+RS_API const char *reshard_last_error(void);          /* thread-local text of the last failure, "" if none */
+RS_API const char *reshard_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RESHARD_H_ */

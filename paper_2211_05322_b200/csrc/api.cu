@@ -1,0 +1,343 @@
+// api.cu -- the C ABI of include/reshard.h: plan creation / upload / queries and the launch glue of
+// execute, pack, unpack and the host-buffer entry point.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/reshard.h"
+#include "config.h"
+#include "kernels.h"
+#include "plan.hpp"
+
+static_assert(sizeof(RsTask) == 192 && sizeof(RsDst) == 16 && sizeof(RsTile) == 32, "table layouts are part of reshard_op_tables");
+
+struct rs_plan {
+    rs::Plan p;
+};
+
+namespace {
+
+rs_status cuda_fail(cudaError_t e, const char *what) {
+    rs::set_error(std::string(what) + ": " + cudaGetErrorString(e));
+    return RS_ECUDA;
+}
+
+size_t round256(size_t x) { return (x + 255) / 256 * 256; }
+
+// one device allocation holding the three operations' task / destination / tile tables
+rs_status upload(rs::Plan *P) {
+    cudaError_t e = cudaGetDevice(&P->device);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->device);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    if (sms != P->sm_count) {                                 // grids are sized in multiples of the SM count
+        P->sm_count = sms;
+        rs_status st = rs::build_tables(P);
+        if (st != RS_OK) return st;
+    }
+    size_t total = 0;
+    for (rs::OpTables &o : P->op)
+        total += round256(o.tasks.size() * sizeof(RsTask)) + round256(o.dsts.size() * sizeof(RsDst)) +
+                 round256(o.tiles.size() * sizeof(RsTile));
+    std::vector<char> host(total, 0);
+    e = cudaMalloc(&P->dev_blob, std::max<size_t>(total, 256));
+    if (e != cudaSuccess) { P->dev_blob = nullptr; return e == cudaErrorMemoryAllocation ? RS_ENOMEM : cuda_fail(e, "cudaMalloc"); }
+    size_t off = 0;
+    char *base = static_cast<char *>(P->dev_blob);
+    for (rs::OpTables &o : P->op) {
+        o.dev.tasks = reinterpret_cast<const RsTask *>(base + off);
+        std::memcpy(host.data() + off, o.tasks.data(), o.tasks.size() * sizeof(RsTask));
+        off += round256(o.tasks.size() * sizeof(RsTask));
+        o.dev.dsts = reinterpret_cast<const RsDst *>(base + off);
+        std::memcpy(host.data() + off, o.dsts.data(), o.dsts.size() * sizeof(RsDst));
+        off += round256(o.dsts.size() * sizeof(RsDst));
+        o.dev.tiles = reinterpret_cast<const RsTile *>(base + off);
+        std::memcpy(host.data() + off, o.tiles.data(), o.tiles.size() * sizeof(RsTile));
+        off += round256(o.tiles.size() * sizeof(RsTile));
+        o.dev.n_tiles = (uint32_t)o.tiles.size();
+    }
+    e = cudaMemcpy(P->dev_blob, host.data(), total, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpy(tables)");
+    int smem = 0;
+    for (rs::OpTables &o : P->op) smem = std::max(smem, (int)RS_SMEM_MAX);
+    e = rs::prepare_bulk(smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(rs_copy_bulk)");
+    return RS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+rs_status reshard_plan(const int64_t *global_shape, int32_t ndim, int32_t elem_bytes,
+                       const int32_t *src_mesh_shape, int32_t src_mesh_ndim, const char *src_spec,
+                       const int32_t *dst_mesh_shape, int32_t dst_mesh_ndim, const char *dst_spec,
+                       uint32_t flags, rs_plan **out_plan) {
+    rs::set_error("");
+    if (!out_plan) { rs::set_error("out_plan is null"); return RS_EINVAL; }
+    if (elem_bytes != 1 && elem_bytes != 2 && elem_bytes != 4 && elem_bytes != 8 && elem_bytes != 16) {
+        rs::set_error("elem_bytes must be 1, 2, 4, 8 or 16");
+        return RS_EINVAL;
+    }
+    rs_plan *h = new (std::nothrow) rs_plan();
+    if (!h) return RS_ENOMEM;
+    rs::Plan *P = &h->p;
+    P->elem_bytes = elem_bytes;
+    P->flags = flags;
+    rs_status st;
+    try {
+        st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, &P->A);
+        if (st == RS_OK) st = rs::make_layout(global_shape, ndim, dst_mesh_shape, dst_mesh_ndim, dst_spec, &P->B);
+        if (st == RS_OK) st = rs::build_slices(P);
+        if (st == RS_OK) { rs::choose_senders(P); st = rs::build_messages(P); }
+        if (st == RS_OK) st = rs::build_tables(P);
+        if (st == RS_OK && !(flags & RS_HOST_ONLY)) st = upload(P);
+    } catch (const std::bad_alloc &) {
+        st = RS_ENOMEM;
+    }
+    if (st != RS_OK) { reshard_plan_destroy(h); return st; }
+    *out_plan = h;
+    return RS_OK;
+}
+
+void reshard_plan_destroy(rs_plan *plan) {
+    if (!plan) return;
+    if (plan->p.dev_blob) cudaFree(plan->p.dev_blob);
+    delete plan;
+}
+
+rs_status reshard_plan_info(const rs_plan *plan, rs_plan_info *out) {
+    if (!plan || !out) return RS_EINVAL;
+    const rs::Plan &P = plan->p;
+    std::memset(out, 0, sizeof(*out));
+    out->ndim = P.A.ndim;
+    out->elem_bytes = P.elem_bytes;
+    out->n_src = P.A.n_dev;
+    out->n_dst = P.B.n_dev;
+    out->n_slices = (int32_t)P.slices.size();
+    out->n_messages = (int32_t)P.messages.size();
+    int64_t tb = P.elem_bytes;
+    for (int d = 0; d < P.A.ndim; d++) tb *= P.A.shape[d];
+    out->tensor_bytes = tb;
+    out->src_shard_bytes = P.A.shard_elems() * P.elem_bytes;
+    out->dst_shard_bytes = P.B.shard_elems() * P.elem_bytes;
+    out->unique_read_bytes = tb;
+    out->write_bytes = tb * P.r_B;
+    out->max_sender_bytes = P.max_sender_bytes;
+    out->arena_bytes = P.arena_bytes;
+    out->lb_mode = (P.flags & RS_LB_NAIVE) ? RS_LB_NAIVE : RS_LB_GREEDY;
+    out->device = P.device;
+    return RS_OK;
+}
+
+rs_status reshard_op_info(const rs_plan *plan, int32_t op, rs_op_info *out) {
+    if (!plan || !out || op < 0 || op > 2) return RS_EINVAL;
+    *out = plan->p.op[op].info;
+    return RS_OK;
+}
+
+rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *dsts, void *tiles) {
+    if (!plan || op < 0 || op > 2) return RS_EINVAL;
+    const rs::OpTables &o = plan->p.op[op];
+    if (tasks) std::memcpy(tasks, o.tasks.data(), o.tasks.size() * sizeof(RsTask));
+    if (dsts) std::memcpy(dsts, o.dsts.data(), o.dsts.size() * sizeof(RsDst));
+    if (tiles) std::memcpy(tiles, o.tiles.data(), o.tiles.size() * sizeof(RsTile));
+    return RS_OK;
+}
+
+rs_status reshard_plan_local_shape(const rs_plan *plan, int32_t side, int64_t *out) {
+    if (!plan || !out || (side != RS_SRC && side != RS_DST)) return RS_EINVAL;
+    const rs::Layout &L = side == RS_SRC ? plan->p.A : plan->p.B;
+    for (int d = 0; d < L.ndim; d++) out[d] = L.local[d];
+    return RS_OK;
+}
+
+rs_status reshard_plan_device_box(const rs_plan *plan, int32_t side, int32_t dev, int64_t *lo, int64_t *hi) {
+    if (!plan || !lo || !hi || (side != RS_SRC && side != RS_DST)) return RS_EINVAL;
+    const rs::Layout &L = side == RS_SRC ? plan->p.A : plan->p.B;
+    if (dev < 0 || dev >= L.n_dev) return RS_EINVAL;
+    rs::device_box(L, dev, lo, hi);
+    return RS_OK;
+}
+
+rs_status reshard_plan_slice(const rs_plan *plan, int32_t i, int64_t *lo, int64_t *hi, int32_t *sender,
+                             int32_t *n_senders, int32_t *senders, int32_t *n_receivers, int32_t *receivers) {
+    if (!plan || i < 0 || (size_t)i >= plan->p.slices.size()) return RS_EINVAL;
+    const rs::Slice &S = plan->p.slices[(size_t)i];
+    for (int d = 0; d < plan->p.A.ndim; d++) {
+        if (lo) lo[d] = S.lo[d];
+        if (hi) hi[d] = S.hi[d];
+    }
+    if (sender) *sender = S.sender;
+    if (n_senders) *n_senders = (int32_t)S.senders.size();
+    if (senders) std::copy(S.senders.begin(), S.senders.end(), senders);
+    if (n_receivers) *n_receivers = (int32_t)S.receivers.size();
+    if (receivers) std::copy(S.receivers.begin(), S.receivers.end(), receivers);
+    return RS_OK;
+}
+
+rs_status reshard_plan_sender_bytes(const rs_plan *plan, int64_t *out) {
+    if (!plan || !out) return RS_EINVAL;
+    std::copy(plan->p.sender_bytes.begin(), plan->p.sender_bytes.end(), out);
+    return RS_OK;
+}
+
+rs_status reshard_plan_message(const rs_plan *plan, int32_t m, int32_t *sender, int32_t *receiver,
+                               int64_t *offset, int64_t *bytes, int32_t *n_slice_ids, int32_t *slice_ids) {
+    if (!plan || m < 0 || (size_t)m >= plan->p.messages.size()) return RS_EINVAL;
+    const rs::Message &M = plan->p.messages[(size_t)m];
+    if (sender) *sender = M.sender;
+    if (receiver) *receiver = M.receiver;
+    if (offset) *offset = M.offset;
+    if (bytes) *bytes = M.bytes;
+    if (n_slice_ids) *n_slice_ids = (int32_t)M.slice_ids.size();
+    if (slice_ids) std::copy(M.slice_ids.begin(), M.slice_ids.end(), slice_ids);
+    return RS_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// the data path
+
+namespace {
+
+int ptr_align(const void *p) {
+    uintptr_t x = reinterpret_cast<uintptr_t>(p);
+    int a = 16;
+    while (a > 1 && (x % (uintptr_t)a)) a /= 2;
+    return a;
+}
+
+// one launch of operation `opi` on the given buffers
+rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src, void *const *dst, int n_dst,
+                 const char *used_src, void *stream) {
+    rs::set_error("");
+    if (!plan || !src || !dst) { rs::set_error("null argument"); return RS_EINVAL; }
+    const rs::Plan &P = plan->p;
+    if (!P.dev_blob) { rs::set_error("plan was built with RS_HOST_ONLY"); return RS_EINVAL; }
+    const rs::OpTables &op = P.op[opi];
+    if (op.tiles.empty()) return RS_OK;
+    RsPtrTable pt;
+    int align = op.info.vec_bytes;
+    for (int i = 0; i < n_src; i++) {
+        pt.src[i] = static_cast<const char *>(src[i]);
+        if (used_src && !used_src[i]) continue;
+        if (!src[i]) { rs::set_error("a source shard pointer the plan reads is null"); return RS_EINVAL; }
+        align = std::min(align, ptr_align(src[i]));
+    }
+    for (int i = 0; i < n_dst; i++) {
+        if (!dst[i]) { rs::set_error("a destination pointer is null"); return RS_EINVAL; }
+        pt.dst[i] = static_cast<char *>(dst[i]);
+        align = std::min(align, ptr_align(dst[i]));
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    if (op.info.path == RS_PATH_BULK && align == 16) {
+        e = rs::launch_bulk(op.dev, pt, op.info.grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
+                            (uint32_t)op.info.tile_bytes, st);
+    } else {                                                  // also the fallback for under-aligned pointers
+        int grid = op.info.grid;
+        if (op.info.path == RS_PATH_BULK)
+            grid = (int)std::min<int64_t>(op.info.n_tiles, (int64_t)P.sm_count * RS_LSU_CTAS_PER_SM);
+        e = rs::launch_lsu(op.dev, pt, align, grid, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
+    return RS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+rs_status reshard_execute(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
+                          void *cuda_stream) {
+    if (!plan) return RS_EINVAL;
+    return run_op(plan, RS_OP_EXECUTE, src_shards, plan->p.A.n_dev, dst_shards, plan->p.B.n_dev,
+                  plan->p.used_src.data(), cuda_stream);
+}
+
+rs_status reshard_pack(const rs_plan *plan, const void *const *src_shards, void *msg_arena, void *cuda_stream) {
+    if (!plan) return RS_EINVAL;
+    void *dst[1] = {msg_arena};
+    return run_op(plan, RS_OP_PACK, src_shards, plan->p.A.n_dev, dst, 1, plan->p.used_src.data(), cuda_stream);
+}
+
+rs_status reshard_unpack(const rs_plan *plan, const void *msg_arena, void *const *dst_shards, void *cuda_stream) {
+    if (!plan) return RS_EINVAL;
+    const void *src[1] = {msg_arena};
+    return run_op(plan, RS_OP_UNPACK, src, 1, dst_shards, plan->p.B.n_dev, nullptr, cuda_stream);
+}
+
+int64_t reshard_host_workspace_bytes(const rs_plan *plan) {
+    if (!plan) return -1;
+    const rs::Plan &P = plan->p;
+    int64_t n_used = 0;
+    for (char u : P.used_src) n_used += u ? 1 : 0;
+    return n_used * (int64_t)round256((size_t)(P.A.shard_elems() * P.elem_bytes)) +
+           (int64_t)P.B.n_dev * (int64_t)round256((size_t)(P.B.shard_elems() * P.elem_bytes));
+}
+
+rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shards_host, void *const *dst_shards_host,
+                               void *workspace, void *cuda_stream, int64_t *h2d_bytes, int64_t *d2h_bytes) {
+    rs::set_error("");
+    if (!plan || !src_shards_host || !dst_shards_host || !workspace) { rs::set_error("null argument"); return RS_EINVAL; }
+    const rs::Plan &P = plan->p;
+    if (!P.dev_blob) { rs::set_error("plan was built with RS_HOST_ONLY"); return RS_EINVAL; }
+    if (ptr_align(workspace) < 16) { rs::set_error("workspace must be 256-byte aligned"); return RS_EINVAL; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t sb = (size_t)(P.A.shard_elems() * P.elem_bytes), db = (size_t)(P.B.shard_elems() * P.elem_bytes);
+    const void *src_dev[RS_MAX_DEVICES];
+    void *dst_dev[RS_MAX_DEVICES];
+    char *w = static_cast<char *>(workspace);
+    int64_t up = 0, down = 0;
+    // Replicas are identical by precondition, so only the shards the chosen senders read are uploaded:
+    // the bytes crossing the link are the lower bound size(D).
+    for (int r = 0; r < P.A.n_dev; r++) {
+        src_dev[r] = nullptr;
+        if (!P.used_src[(size_t)r]) continue;
+        if (!src_shards_host[r]) { rs::set_error("a source shard pointer the plan reads is null"); return RS_EINVAL; }
+        cudaError_t e = cudaMemcpyAsync(w, src_shards_host[r], sb, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(H2D)");
+        src_dev[r] = w;
+        w += round256(sb);
+        up += (int64_t)sb;
+    }
+    for (int q = 0; q < P.B.n_dev; q++) { dst_dev[q] = w; w += round256(db); }
+    rs_status rc = run_op(plan, RS_OP_EXECUTE, src_dev, P.A.n_dev, dst_dev, P.B.n_dev, P.used_src.data(), cuda_stream);
+    if (rc != RS_OK) return rc;
+    for (int q = 0; q < P.B.n_dev; q++) {
+        if (!dst_shards_host[q]) { rs::set_error("a destination pointer is null"); return RS_EINVAL; }
+        cudaError_t e = cudaMemcpyAsync(dst_shards_host[q], dst_dev[q], db, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(D2H)");
+        down += (int64_t)db;
+    }
+    if (h2d_bytes) *h2d_bytes = up;
+    if (d2h_bytes) *d2h_bytes = down;
+    return RS_OK;
+}
+
+int64_t reshard_launch_count(void) { return rs::launch_count(); }
+
+const char *reshard_strerror(rs_status s) {
+    switch (s) {
+        case RS_OK: return "ok";
+        case RS_EINVAL: return "invalid argument";
+        case RS_ESPEC: return "bad sharding spec";
+        case RS_EDIVIS: return "tensor dim not divisible by its sharding degree";
+        case RS_EUNSUPPORTED: return "unsupported size";
+        case RS_ENOMEM: return "out of memory";
+        case RS_ECUDA: return "CUDA error";
+    }
+    return "unknown status";
+}
+
+const char *reshard_last_error(void) { return rs::last_error().c_str(); }
+
+const char *reshard_version(void) { return "reshard-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,18 @@
+// config.h -- launch-shape defaults of the two executors.  Each can be overridden at plan time by
+// an environment variable of the same name (tuning sweeps on the GPU box without a rebuild).
+#pragma once
+
+// register path: 128-bit ld.global -> st.global x k
+#define RS_LSU_THREADS       256
+#define RS_LSU_CTAS_PER_SM   8          // persistent CTAs per SM (grid = 148 * this)
+#define RS_LSU_TILE_BYTES    32768
+#define RS_LSU_UNROLL        4          // independent 16-byte loads in flight per thread
+
+// TMA path: cp.async.bulk global -> shared ring -> global x k; every warp is its own pipeline
+#define RS_BULK_WARPS        2          // warps (independent pipelines) per CTA, one CTA per SM
+#define RS_BULK_STAGES       6          // ring slots per warp
+#define RS_BULK_LOOKAHEAD    3          // loads in flight per warp before the first store is issued
+#define RS_BULK_TILE_BYTES   16384      // bytes per ring slot
+#define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
+
+#define RS_SMEM_MAX          (227 * 1024)

@@ -1,0 +1,259 @@
+// kernels.cu -- the data path (steps a6, a7, a8): one persistent kernel launch per operation.
+//
+// What is computed (PAPER.md:88 task, PAPER.md:137 broadcast strategy, on chip): every copy task's
+// box is read ONCE from its source buffer and written to each of its k destination buffers.
+// reshard_execute / reshard_pack / reshard_unpack differ only in the task table they run.
+//
+// Two executors, both sm_100a, no tensor cores (pure data movement, HBM-bound):
+//   rs_copy_lsu   register path.  Every thread keeps RS_LSU_UNROLL independent vector loads
+//                 (ld.global.nc, 16/8/4/2/1 bytes wide) in flight and stores each value k times.
+//                 Handles any alignment and any run length.
+//   rs_copy_bulk  TMA path (SASS: UBLKCP).  Every warp owns a ring of shared-memory slots: lane r
+//                 issues cp.async.bulk global->shared for row r of the tile (mbarrier complete_tx),
+//                 and once the tile has landed, cp.async.bulk shared->global to each of the k
+//                 destinations (bulk_group).  No register staging, loads run LOOKAHEAD tiles ahead
+//                 of the stores.  Needs 16-byte alignment of every address and length.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "config.h"
+#include "kernels.h"
+#include "tables.h"
+
+namespace rs {
+
+// ------------------------------------------------------------------------------------------------
+// shared device helpers
+
+__device__ __forceinline__ RsTile load_tile(const RsTile *tiles, uint32_t t) {
+    const uint4 *p = reinterpret_cast<const uint4 *>(tiles + t);
+    uint4 x = __ldg(p), y = __ldg(p + 1);
+    RsTile r;
+    r.task = x.x; r.n_rows = x.y; r.col_bytes = x.z; r.flags = x.w;
+    r.a = (uint64_t)y.x | ((uint64_t)y.y << 32);
+    r.b = (uint64_t)y.z | ((uint64_t)y.w << 32);
+    return r;
+}
+
+// byte offsets (relative to the task's box origin on each side) of byte 0 of row `row` of a tile
+__device__ __forceinline__ void row_offsets(const RsTile &tile, const RsTask *__restrict__ T, uint32_t row,
+                                            int64_t s0, int64_t d0, int64_t *so, int64_t *doff) {
+    if (tile.flags & RS_TILE_FAST) {
+        *so = (int64_t)tile.a + (int64_t)row * s0;
+        *doff = (int64_t)tile.b + (int64_t)row * d0;
+    } else {                                                  // GENERIC: decode the linear row index
+        uint64_t lin = tile.a + row;
+        int64_t s = (int64_t)tile.b, d = (int64_t)tile.b;
+        const int nd = T->nd;
+        for (int i = 0; i < nd; i++) {
+            uint32_t e = T->ext[i];
+            uint64_t q = lin / e;
+            uint32_t c = (uint32_t)(lin - q * e);
+            lin = q;
+            s += (int64_t)c * T->sstride[i];
+            d += (int64_t)c * T->dstride[i];
+        }
+        *so = s; *doff = d;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// register path
+
+template <typename V> __device__ __forceinline__ V ld_stream(const char *p) {
+    return *reinterpret_cast<const V *>(p);
+}
+template <> __device__ __forceinline__ uint4 ld_stream<uint4>(const char *p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+template <typename V> __device__ __forceinline__ void st_stream(char *p, const V &v) {
+    *reinterpret_cast<V *>(p) = v;
+}
+template <> __device__ __forceinline__ void st_stream<uint4>(char *p, const uint4 &v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1, %2, %3, %4};"
+                 :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+template <typename V, int U>
+__global__ void __launch_bounds__(RS_LSU_THREADS)
+rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs) {
+    constexpr uint32_t VB = sizeof(V);
+    for (uint32_t t = blockIdx.x; t < op.n_tiles; t += gridDim.x) {
+        const RsTile tile = load_tile(op.tiles, t);
+        const RsTask *__restrict__ T = op.tasks + tile.task;
+        const int k = T->k;
+        const RsDst *__restrict__ dsts = op.dsts + T->dst_first;
+        const char *src = ptrs.src[T->src_buf] + T->src_off;
+        const int64_t s0 = T->sstride[0], d0 = T->dstride[0];
+        const uint32_t vpr = tile.col_bytes / VB;             // vectors per row
+        const uint32_t total = tile.n_rows * vpr;
+        for (uint32_t v0 = threadIdx.x; v0 < total; v0 += RS_LSU_THREADS * U) {
+            V data[U];
+            int64_t doff[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const uint32_t v = v0 + u * RS_LSU_THREADS;
+                if (v < total) {
+                    const uint32_t row = tile.n_rows == 1 ? 0u : v / vpr;
+                    const uint32_t col = v - row * vpr;
+                    int64_t so;
+                    row_offsets(tile, T, row, s0, d0, &so, &doff[u]);
+                    doff[u] += (int64_t)col * VB;
+                    data[u] = ld_stream<V>(src + so + (int64_t)col * VB);
+                }
+            }
+            for (int j = 0; j < k; j++) {                     // read once, write k times
+                const RsDst d = dsts[j];
+                char *dp = ptrs.dst[d.buf] + d.off;
+#pragma unroll
+                for (int u = 0; u < U; u++)
+                    if (v0 + u * RS_LSU_THREADS < total) st_stream<V>(dp + doff[u], data[u]);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// TMA path
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}"
+        :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void *gsrc, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *gdst, uint32_t smem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 :: "l"(gdst), "r"(smem_src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read(int pending) {  // immediate operand: dispatch on the value
+    switch (pending) {
+        case 0: asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); break;
+        case 1: asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); break;
+        case 2: asm volatile("cp.async.bulk.wait_group.read 2;" ::: "memory"); break;
+        case 3: asm volatile("cp.async.bulk.wait_group.read 3;" ::: "memory"); break;
+        case 4: asm volatile("cp.async.bulk.wait_group.read 4;" ::: "memory"); break;
+        case 5: asm volatile("cp.async.bulk.wait_group.read 5;" ::: "memory"); break;
+        default: asm volatile("cp.async.bulk.wait_group.read 6;" ::: "memory"); break;
+    }
+}
+
+__global__ void __launch_bounds__(256, 1)
+rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const int stages, const int lookahead,
+             const uint32_t stage_bytes) {
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    const uint32_t bars = smem_u32(smem) + warp * 64;                       // <= 8 mbarriers per warp
+    const uint32_t ring = smem_u32(smem) + 1024 + (uint32_t)warp * stages * stage_bytes;
+    if (lane == 0) {
+        for (int s = 0; s < stages; s++) mbar_init(bars + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
+    const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
+    const int pending_ok = stages - lookahead - 1;            // store groups that may still read smem
+
+    for (int it = 0; it < n_my + lookahead; ++it) {
+        if (it < n_my) {                                      // ---- load tile `it` into slot it % stages
+            const int s = it % stages;
+            if (it >= stages) {                               // slot reuse: its stores must have read it
+                bulk_wait_read(pending_ok);
+                __syncwarp();
+            }
+            const RsTile tile = load_tile(op.tiles, worker + (uint32_t)it * n_workers);
+            const RsTask *__restrict__ T = op.tasks + tile.task;
+            const char *src = ptrs.src[T->src_buf] + T->src_off;
+            const int64_t s0 = T->sstride[0], d0 = T->dstride[0];
+            const uint32_t bar = bars + 8 * s, slot = ring + (uint32_t)s * stage_bytes;
+            if (lane == 0) mbar_expect_tx(bar, tile.n_rows * tile.col_bytes);
+            __syncwarp();
+            for (uint32_t r = lane; r < tile.n_rows; r += 32) {
+                int64_t so, doff;
+                row_offsets(tile, T, r, s0, d0, &so, &doff);
+                bulk_g2s(slot + r * tile.col_bytes, src + so, tile.col_bytes, bar);
+            }
+        }
+        const int j = it - lookahead;
+        if (j >= 0) {                                         // ---- store tile j to its k destinations
+            const int s = j % stages;
+            const RsTile tile = load_tile(op.tiles, worker + (uint32_t)j * n_workers);
+            const RsTask *__restrict__ T = op.tasks + tile.task;
+            const int k = T->k;
+            const RsDst *__restrict__ dsts = op.dsts + T->dst_first;
+            const int64_t s0 = T->sstride[0], d0 = T->dstride[0];
+            const uint32_t slot = ring + (uint32_t)s * stage_bytes;
+            mbar_wait(bars + 8 * s, (uint32_t)(j / stages) & 1u);
+            for (uint32_t r = lane; r < tile.n_rows; r += 32) {
+                int64_t so, doff;
+                row_offsets(tile, T, r, s0, d0, &so, &doff);
+                for (int q = 0; q < k; q++) {                 // read once, write k times
+                    const RsDst d = dsts[q];
+                    bulk_s2g(ptrs.dst[d.buf] + d.off + doff, slot + r * tile.col_bytes, tile.col_bytes);
+                }
+            }
+            bulk_commit();
+        }
+    }
+    bulk_wait_read(0);                                        // shared memory must outlive the stores' reads
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-side launchers
+
+static thread_local int64_t g_launches = 0;
+int64_t launch_count() { return g_launches; }
+
+template <typename V>
+static cudaError_t launch_lsu_t(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st) {
+    rs_copy_lsu<V, RS_LSU_UNROLL><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int vec_bytes, int grid, cudaStream_t st) {
+    cudaError_t e;
+    switch (vec_bytes) {
+        case 16: e = launch_lsu_t<uint4>(op, ptrs, grid, st); break;
+        case 8:  e = launch_lsu_t<uint2>(op, ptrs, grid, st); break;
+        case 4:  e = launch_lsu_t<uint32_t>(op, ptrs, grid, st); break;
+        case 2:  e = launch_lsu_t<uint16_t>(op, ptrs, grid, st); break;
+        default: e = launch_lsu_t<uint8_t>(op, ptrs, grid, st); break;
+    }
+    if (e == cudaSuccess) ++g_launches;
+    return e;
+}
+
+cudaError_t prepare_bulk(int smem_bytes) {
+    return cudaFuncSetAttribute(rs_copy_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+}
+
+cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
+                        int lookahead, uint32_t stage_bytes, cudaStream_t st) {
+    rs_copy_bulk<<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) ++g_launches;
+    return e;
+}
+
+}  // namespace rs

@@ -1,0 +1,14 @@
+// kernels.h -- launchers of the two executors (kernels.cu).  Internal header.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "tables.h"
+
+namespace rs {
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int vec_bytes, int grid, cudaStream_t st);
+cudaError_t prepare_bulk(int smem_bytes);
+cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
+                        int lookahead, uint32_t stage_bytes, cudaStream_t st);
+int64_t launch_count();
+}  // namespace rs

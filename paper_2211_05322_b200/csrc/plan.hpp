@@ -1,0 +1,84 @@
+// plan.hpp -- host planner of a cross-mesh resharding task (steps a1..a5).  Internal header.
+//
+//   a1 spec -> tile boxes                      PAPER.md:78-86   (S2.2)
+//   a2 cutpoints -> intervals -> slices        PAPER.md:488-492 (App. B.2)
+//   a3 sender / receiver sets N_i, M_i
+//   a4 load-balanced sender choice             PAPER.md:163 (naive), 167-171 Eq. 4 (greedy/LPT)
+//   a5 flat task / tile tables, message layout north_star items (1), (3)
+#pragma once
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/reshard.h"
+#include "tables.h"
+
+namespace rs {
+
+struct Layout {                          // one side of the task: (shape, mesh, spec)
+    int ndim = 0;
+    int64_t shape[RS_MAX_NDIM];          // l_i
+    int mesh_ndim = 0;
+    int64_t mesh[RS_MAX_MESH_NDIM];      // m_a
+    int n_axes[RS_MAX_NDIM];             // 0 => R
+    int axes[RS_MAX_NDIM][RS_MAX_MESH_NDIM];
+    int64_t degree[RS_MAX_NDIM];         // k_i
+    int64_t local[RS_MAX_NDIM];          // l_i / k_i
+    int n_dev = 0;
+    std::vector<int64_t> shard_index;    // [n_dev][ndim]: p_i of every device
+    int64_t shard_elems() const { int64_t n = 1; for (int i = 0; i < ndim; i++) n *= local[i]; return n; }
+};
+
+struct Slice {                           // one unit task
+    int64_t lo[RS_MAX_NDIM], hi[RS_MAX_NDIM];
+    int64_t elems = 0;
+    std::vector<int> senders;            // N_i, ascending device id
+    std::vector<int> receivers;          // M_i, ascending device id
+    int sender = -1;                     // n_i*
+};
+
+struct Message {                         // wire model: everything sender s ships to receiver r
+    int sender, receiver;
+    int64_t offset = 0, bytes = 0;       // inside the arena
+    std::vector<int> slice_ids;          // ascending
+    std::vector<int64_t> slice_off;      // byte offset of each slice inside the arena
+};
+
+struct OpTables {                        // one operation (execute / pack / unpack)
+    std::vector<RsTask> tasks;
+    std::vector<RsDst> dsts;
+    std::vector<RsTile> tiles;
+    rs_op_info info{};
+    int stages = 0, lookahead = 0;       // TMA path: ring slots per warp, loads in flight
+    RsOpDev dev{};                       // device copies (null for a host-only plan)
+};
+
+struct Plan {
+    Layout A, B;
+    int elem_bytes = 0;
+    uint32_t flags = 0;
+    std::vector<Slice> slices;
+    std::vector<int64_t> sender_bytes;
+    int64_t max_sender_bytes = 0;
+    std::vector<Message> messages;
+    int64_t arena_bytes = 0;
+    int64_t r_B = 1;                     // destination replication factor
+    OpTables op[3];
+    std::vector<char> used_src;          // [n_src] 1 if some task reads that shard
+    int device = -1;
+    int sm_count = 148;
+    void *dev_blob = nullptr;            // the ONE device allocation
+};
+
+void set_error(const std::string &msg);
+const std::string &last_error();
+
+rs_status make_layout(const int64_t *shape, int ndim, const int32_t *mesh, int mesh_ndim, const char *spec,
+                      Layout *L);
+void device_box(const Layout &L, int dev, int64_t *lo, int64_t *hi);
+rs_status build_slices(Plan *P);                       // a2 + a3
+void choose_senders(Plan *P);                          // a4
+rs_status build_messages(Plan *P);                     // message layout
+rs_status build_tables(Plan *P);                       // a5 (host side), tables.cpp
+
+}  // namespace rs

@@ -1,0 +1,295 @@
+// tables.cpp -- step a5: unit tasks -> collapsed copy tasks -> flat tile tables for the three
+// operations (execute / pack / unpack), plus the per-operation launch configuration.
+// Paper analogue: "choose the better result as the schedule to launch broadcasts";
+// north_star item (1): "emits a flat task table".  No CUDA here.
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+
+#include "config.h"
+#include "plan.hpp"
+
+namespace rs {
+
+namespace {
+
+struct BoxDesc {                         // one box seen from both sides, per TENSOR dim, in bytes
+    int ndim;
+    int64_t ext[RS_MAX_NDIM];            // elements
+    int64_t sstride[RS_MAX_NDIM];
+    int64_t dstride[RS_MAX_NDIM];
+};
+
+// dense row-major byte strides of a local array
+void dense_strides(const int64_t *shape, int ndim, int64_t e, int64_t *stride) {
+    int64_t s = e;
+    for (int d = ndim - 1; d >= 0; d--) { stride[d] = s; s *= shape[d]; }
+}
+
+int64_t box_offset(const int64_t *lo, const int64_t *origin, const int64_t *stride, int ndim) {
+    int64_t off = 0;
+    for (int d = 0; d < ndim; d++) off += (lo[d] - origin[d]) * stride[d];
+    return off;
+}
+
+// Collapse a box: drop unit dims, merge dims that are contiguous on BOTH sides, turn the innermost
+// dim into the byte run if it is dense on both sides.  Returns false if a row dim overflows 32 bits.
+bool collapse(const BoxDesc &bx, int64_t e, RsTask *T) {
+    int64_t ext[RS_MAX_NDIM + 1], ss[RS_MAX_NDIM + 1], ds[RS_MAX_NDIM + 1];
+    int n = 0;
+    for (int d = 0; d < bx.ndim; d++) {                       // outermost first
+        if (bx.ext[d] == 1) continue;
+        if (n > 0 && ss[n - 1] == bx.ext[d] * bx.sstride[d] && ds[n - 1] == bx.ext[d] * bx.dstride[d]) {
+            ext[n - 1] *= bx.ext[d];                          // outer dim steps exactly over this one
+            ss[n - 1] = bx.sstride[d];
+            ds[n - 1] = bx.dstride[d];
+        } else {
+            ext[n] = bx.ext[d]; ss[n] = bx.sstride[d]; ds[n] = bx.dstride[d];
+            n++;
+        }
+    }
+    T->run_bytes = e;
+    if (n > 0 && ss[n - 1] == e && ds[n - 1] == e) { T->run_bytes = ext[n - 1] * e; n--; }
+    if (n > RS_ROW_DIMS) return false;
+    T->nd = n;
+    for (int i = 0; i <= RS_ROW_DIMS; i++) { T->ext[i] = 1; T->sstride[i] = 0; T->dstride[i] = 0; }
+    for (int i = 0; i < n; i++) {                             // ext[0] = innermost row dim
+        int src = n - 1 - i;
+        if (ext[src] > 0xFFFFFFFFll) return false;
+        T->ext[i] = (uint32_t)ext[src];
+        T->sstride[i] = ss[src];
+        T->dstride[i] = ds[src];
+    }
+    return true;
+}
+
+int64_t task_rows(const RsTask &T) {
+    int64_t r = 1;
+    for (int i = 0; i < T.nd; i++) r *= T.ext[i];
+    return r;
+}
+
+int64_t pow2_align(int64_t x) {                               // largest power of two <= 16 dividing x
+    if (x == 0) return 16;
+    int64_t a = 1;
+    while (a < 16 && x % (a * 2) == 0) a *= 2;
+    return a;
+}
+
+int env_int(const char *name, int dflt) {
+    const char *v = std::getenv(name);
+    if (!v || !*v) return dflt;
+    return std::atoi(v);
+}
+
+// Emit the tiles of one task.  tile_bytes is a multiple of 128.
+void emit_tiles(const RsTask &T, uint32_t task_id, int64_t tile_bytes, std::vector<RsTile> *out) {
+    const int64_t R = task_rows(T), B = T.run_bytes;
+    auto row_offsets = [&](int64_t row, int64_t *so, int64_t *doff) {
+        int64_t s = 0, d = 0;
+        for (int i = 0; i < T.nd; i++) {
+            int64_t c = row % T.ext[i];
+            row /= T.ext[i];
+            s += c * T.sstride[i];
+            d += c * T.dstride[i];
+        }
+        *so = s; *doff = d;
+    };
+    if (B > tile_bytes) {                                     // long runs: split every row into column chunks
+        int64_t n = (B + tile_bytes - 1) / tile_bytes;
+        int64_t chunk = ((B + n - 1) / n + 127) / 128 * 128;
+        for (int64_t r = 0; r < R; r++) {
+            int64_t so, doff;
+            row_offsets(r, &so, &doff);
+            for (int64_t c = 0; c < B; c += chunk) {
+                RsTile t{};
+                t.task = task_id; t.n_rows = 1; t.col_bytes = (uint32_t)std::min(chunk, B - c);
+                t.flags = RS_TILE_FAST;
+                t.a = (uint64_t)(so + c); t.b = (uint64_t)(doff + c);
+                out->push_back(t);
+            }
+        }
+        return;
+    }
+    const int64_t rpt = std::max<int64_t>(1, tile_bytes / B);  // rows per tile
+    const int64_t ext0 = T.nd > 0 ? T.ext[0] : 1;
+    if (T.nd <= 1 || ext0 >= rpt) {                           // FAST tiles inside one span of row dim 0
+        int64_t n = (ext0 + rpt - 1) / rpt, sz = (ext0 + n - 1) / n;
+        for (int64_t span = 0; span < R / ext0; span++) {
+            int64_t so, doff;
+            row_offsets(span * ext0, &so, &doff);
+            for (int64_t r0 = 0; r0 < ext0; r0 += sz) {
+                RsTile t{};
+                t.task = task_id; t.n_rows = (uint32_t)std::min(sz, ext0 - r0); t.col_bytes = (uint32_t)B;
+                t.flags = RS_TILE_FAST;
+                t.a = (uint64_t)(so + r0 * T.sstride[0]); t.b = (uint64_t)(doff + r0 * T.dstride[0]);
+                out->push_back(t);
+            }
+        }
+        return;
+    }
+    int64_t n = (R + rpt - 1) / rpt, sz = (R + n - 1) / n;     // GENERIC tiles: any run of linear rows
+    for (int64_t r0 = 0; r0 < R; r0 += sz) {
+        RsTile t{};
+        t.task = task_id; t.n_rows = (uint32_t)std::min(sz, R - r0); t.col_bytes = (uint32_t)B;
+        t.flags = 0;
+        t.a = (uint64_t)r0; t.b = 0;
+        out->push_back(t);
+    }
+}
+
+// Alignment class, path, tile size, grid of one operation; then its tile table.
+rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes) {
+    int64_t align = 16, min_run = INT64_MAX, max_rows = 0;
+    for (const RsTask &T : op->tasks) {
+        align = std::min(align, pow2_align(T.run_bytes));
+        align = std::min(align, pow2_align(T.src_off));
+        for (int i = 0; i < T.nd; i++) {
+            align = std::min(align, pow2_align(T.sstride[i]));
+            align = std::min(align, pow2_align(T.dstride[i]));
+        }
+        for (int j = 0; j < T.k; j++) align = std::min(align, pow2_align(op->dsts[(size_t)T.dst_first + j].off));
+        min_run = std::min(min_run, T.run_bytes);
+        max_rows = std::max(max_rows, task_rows(T));
+        if (task_rows(T) > 0x7FFFFFFFll) { set_error("more than 2^31-1 rows in one slice"); return RS_EUNSUPPORTED; }
+    }
+    rs_op_info &I = op->info;
+    I.vec_bytes = (int32_t)align;
+    I.n_tasks = (int32_t)op->tasks.size();
+    I.n_dsts = (int32_t)op->dsts.size();
+    I.read_bytes = read_bytes;
+    I.write_bytes = write_bytes;
+
+    const uint32_t forced = P->flags & RS_PATH_MASK;
+    const bool bulk_ok = align == 16 && min_run >= 16;
+    int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
+             : (bulk_ok && min_run >= RS_BULK_MIN_RUN) ? RS_PATH_BULK : RS_PATH_LSU;
+    if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_LSU;   // cp.async.bulk needs 16-byte everything
+    I.path = path;
+
+    int64_t tile_bytes;
+    int workers;                                               // independent tile consumers in one launch
+    if (path == RS_PATH_BULK) {
+        int warps = std::max(1, std::min(8, env_int("RS_BULK_WARPS", RS_BULK_WARPS)));
+        int stages = std::max(2, std::min(8, env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+        tile_bytes = env_int("RS_BULK_TILE_BYTES", RS_BULK_TILE_BYTES);
+        tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
+        while ((int64_t)warps * stages * tile_bytes + 1024 > RS_SMEM_MAX && tile_bytes > 1024) tile_bytes -= 1024;
+        I.block = warps * 32;
+        I.grid = P->sm_count;
+        workers = I.grid * warps;
+    } else {
+        tile_bytes = env_int("RS_LSU_TILE_BYTES", RS_LSU_TILE_BYTES);
+        tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
+        I.block = RS_LSU_THREADS;
+        I.grid = P->sm_count * std::max(1, env_int("RS_LSU_CTAS_PER_SM", RS_LSU_CTAS_PER_SM));
+        workers = I.grid;
+    }
+    // small problems: shrink tiles until every worker has a few (tail balance), floor 2 KiB
+    while (tile_bytes > 2048 && read_bytes / tile_bytes < (int64_t)workers * 4) tile_bytes = tile_bytes / 2 / 128 * 128;
+    tile_bytes = std::max<int64_t>(tile_bytes, 128);
+    I.tile_bytes = (int32_t)tile_bytes;
+
+    op->tiles.clear();
+    for (size_t t = 0; t < op->tasks.size(); t++) emit_tiles(op->tasks[t], (uint32_t)t, tile_bytes, &op->tiles);
+    if (op->tiles.size() > 0x7FFFFFFFull) { set_error("tile table too large"); return RS_EUNSUPPORTED; }
+    I.n_tiles = (int32_t)op->tiles.size();
+    int64_t mr = INT64_MAX;
+    for (const RsTile &t : op->tiles) mr = std::min<int64_t>(mr, t.col_bytes);
+    I.min_run_bytes = op->tiles.empty() ? 0 : mr;
+    if (path == RS_PATH_BULK) {
+        int warps = I.block / 32;
+        int stages = std::max(2, std::min(8, env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+        op->stages = stages;
+        op->lookahead = std::max(1, std::min(stages - 1, env_int("RS_BULK_LOOKAHEAD", RS_BULK_LOOKAHEAD)));
+        I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
+        I.smem_bytes = (int32_t)(warps * stages * tile_bytes + 1024);
+    } else {
+        I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, I.n_tiles));
+        I.smem_bytes = 0;
+    }
+    return RS_OK;
+}
+
+}  // namespace
+
+rs_status build_tables(Plan *P) {
+    const Layout &A = P->A, &B = P->B;
+    const int N = A.ndim;
+    const int64_t e = P->elem_bytes;
+    int64_t sA[RS_MAX_NDIM], sB[RS_MAX_NDIM];
+    dense_strides(A.local, N, e, sA);
+    dense_strides(B.local, N, e, sB);
+    const int64_t tensor_bytes = [&] { int64_t n = e; for (int d = 0; d < N; d++) n *= A.shape[d]; return n; }();
+
+    // which (message, position) holds slice i for receiver r
+    std::vector<std::vector<int64_t>> arena_off(P->slices.size());
+    for (size_t i = 0; i < P->slices.size(); i++) arena_off[i].assign(P->slices[i].receivers.size(), -1);
+    for (const Message &M : P->messages)
+        for (size_t j = 0; j < M.slice_ids.size(); j++) {
+            const Slice &S = P->slices[(size_t)M.slice_ids[j]];
+            size_t pos = (size_t)(std::find(S.receivers.begin(), S.receivers.end(), M.receiver) - S.receivers.begin());
+            arena_off[(size_t)M.slice_ids[j]][pos] = M.slice_off[j];
+        }
+
+    OpTables &X = P->op[RS_OP_EXECUTE], &PK = P->op[RS_OP_PACK], &UP = P->op[RS_OP_UNPACK];
+    for (OpTables *o : {&X, &PK, &UP}) { o->tasks.clear(); o->dsts.clear(); o->tiles.clear(); }
+
+    for (size_t i = 0; i < P->slices.size(); i++) {
+        const Slice &S = P->slices[i];
+        int64_t lo_s[RS_MAX_NDIM], hi_s[RS_MAX_NDIM], ext[RS_MAX_NDIM], dense[RS_MAX_NDIM];
+        device_box(A, S.sender, lo_s, hi_s);
+        for (int d = 0; d < N; d++) ext[d] = S.hi[d] - S.lo[d];
+        dense_strides(ext, N, e, dense);
+        const int64_t src_off = box_offset(S.lo, lo_s, sA, N);
+        BoxDesc bx;
+        bx.ndim = N;
+        for (int d = 0; d < N; d++) { bx.ext[d] = ext[d]; bx.sstride[d] = sA[d]; }
+
+        // execute: sender shard -> every receiver shard (read once, write k times)
+        {
+            RsTask T{};
+            for (int d = 0; d < N; d++) bx.dstride[d] = sB[d];
+            if (!collapse(bx, e, &T)) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+            T.src_buf = S.sender; T.src_off = src_off;
+            T.k = (int32_t)S.receivers.size(); T.dst_first = (int32_t)X.dsts.size();
+            for (int r : S.receivers) {
+                int64_t lo_r[RS_MAX_NDIM], hi_r[RS_MAX_NDIM];
+                device_box(B, r, lo_r, hi_r);
+                X.dsts.push_back(RsDst{box_offset(S.lo, lo_r, sB, N), r, 0});
+            }
+            X.tasks.push_back(T);
+        }
+        // pack: sender shard -> k dense copies in the arena
+        {
+            RsTask T{};
+            for (int d = 0; d < N; d++) bx.dstride[d] = dense[d];
+            if (!collapse(bx, e, &T)) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+            T.src_buf = S.sender; T.src_off = src_off;
+            T.k = (int32_t)S.receivers.size(); T.dst_first = (int32_t)PK.dsts.size();
+            for (size_t j = 0; j < S.receivers.size(); j++) PK.dsts.push_back(RsDst{arena_off[i][j], 0, 0});
+            PK.tasks.push_back(T);
+        }
+        // unpack: one dense copy in the arena -> one receiver shard
+        for (size_t j = 0; j < S.receivers.size(); j++) {
+            RsTask T{};
+            BoxDesc ux;
+            ux.ndim = N;
+            for (int d = 0; d < N; d++) { ux.ext[d] = ext[d]; ux.sstride[d] = dense[d]; ux.dstride[d] = sB[d]; }
+            if (!collapse(ux, e, &T)) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+            T.src_buf = 0; T.src_off = arena_off[i][j];
+            T.k = 1; T.dst_first = (int32_t)UP.dsts.size();
+            int64_t lo_r[RS_MAX_NDIM], hi_r[RS_MAX_NDIM];
+            device_box(B, S.receivers[j], lo_r, hi_r);
+            UP.dsts.push_back(RsDst{box_offset(S.lo, lo_r, sB, N), S.receivers[j], 0});
+            UP.tasks.push_back(T);
+        }
+    }
+    rs_status st;
+    if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
+    if ((st = finish_op(P, &PK, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
+    if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B)) != RS_OK) return st;
+    return RS_OK;
+}
+
+}  // namespace rs

@@ -1,0 +1,195 @@
+"""Thin ctypes binding of libreshard.so (include/reshard.h): argument marshalling only.
+
+Every step of the path runs inside the library: the planner in C++ on the host, the data path in
+the sm_100a kernels.  There is no Python or CPU fallback: if the library is missing, loading
+fails; if no CUDA device is present, reshard_plan without RS_HOST_ONLY fails with RS_ECUDA.
+
+Function names mirror the C ABI:  reshard_plan -> Plan(...), reshard_execute -> Plan.execute, ...
+Device buffers are passed as integer addresses (e.g. torch.Tensor.data_ptr()); streams as the
+integer cudaStream_t (torch.cuda.current_stream().cuda_stream).
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libreshard.so")
+
+RS_OK, RS_EINVAL, RS_ESPEC, RS_EDIVIS, RS_EUNSUPPORTED, RS_ENOMEM, RS_ECUDA = range(7)
+RS_LB_GREEDY, RS_LB_NAIVE = 0x0, 0x1
+RS_PATH_AUTO, RS_PATH_LSU, RS_PATH_BULK = 0x00, 0x10, 0x20
+RS_HOST_ONLY = 0x100
+RS_OP_EXECUTE, RS_OP_PACK, RS_OP_UNPACK = 0, 1, 2
+RS_SRC, RS_DST = 0, 1
+RS_MAX_NDIM, RS_MAX_MESH_NDIM, RS_MAX_DEVICES = 8, 4, 128
+
+# every symbol include/reshard.h declares (tests check the library exports exactly these)
+SYMBOLS = [
+    "reshard_plan", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
+    "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
+    "reshard_plan_message", "reshard_execute", "reshard_pack", "reshard_unpack", "reshard_execute_host",
+    "reshard_host_workspace_bytes", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
+    "reshard_version",
+]
+
+
+class PlanInfo(C.Structure):
+    _fields_ = [("ndim", C.c_int32), ("elem_bytes", C.c_int32), ("n_src", C.c_int32), ("n_dst", C.c_int32),
+                ("n_slices", C.c_int32), ("n_messages", C.c_int32),
+                ("tensor_bytes", C.c_int64), ("src_shard_bytes", C.c_int64), ("dst_shard_bytes", C.c_int64),
+                ("unique_read_bytes", C.c_int64), ("write_bytes", C.c_int64), ("max_sender_bytes", C.c_int64),
+                ("arena_bytes", C.c_int64), ("lb_mode", C.c_int32), ("device", C.c_int32)]
+
+
+class OpInfo(C.Structure):
+    _fields_ = [("path", C.c_int32), ("vec_bytes", C.c_int32), ("n_tasks", C.c_int32), ("n_dsts", C.c_int32),
+                ("n_tiles", C.c_int32), ("tile_bytes", C.c_int32), ("grid", C.c_int32), ("block", C.c_int32),
+                ("smem_bytes", C.c_int32), ("read_bytes", C.c_int64), ("write_bytes", C.c_int64),
+                ("min_run_bytes", C.c_int64)]
+
+
+class ReshardError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("reshard: %s (%s)" % (text, _lib().reshard_strerror(code).decode()))
+        self.code = code
+
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libreshard.so is not built: run `python -m paper_2211_05322_b200.build` "
+                              "(there is no fallback path)")
+        try:
+            L = C.CDLL(LIB_PATH)
+        except OSError:                      # libcudart not on the loader path: torch ships one
+            import torch  # noqa: F401
+            L = C.CDLL(LIB_PATH)
+        for name in SYMBOLS:
+            getattr(L, name).restype = C.c_int
+        L.reshard_plan_destroy.restype = None
+        L.reshard_host_workspace_bytes.restype = C.c_int64
+        L.reshard_launch_count.restype = C.c_int64
+        for name in ("reshard_strerror", "reshard_last_error", "reshard_version"):
+            getattr(L, name).restype = C.c_char_p
+        _LIB = L
+    return _LIB
+
+
+def _chk(rc):
+    if rc != RS_OK:
+        raise ReshardError(rc, _lib().reshard_last_error().decode() or "error %d" % rc)
+
+
+def _i64(xs):
+    return (C.c_int64 * len(xs))(*[int(x) for x in xs])
+
+
+def _i32(xs):
+    return (C.c_int32 * len(xs))(*[int(x) for x in xs])
+
+
+def _ptrs(addrs):
+    return (C.c_void_p * len(addrs))(*[C.c_void_p(int(a) if a else None) for a in addrs])
+
+
+def version():
+    return _lib().reshard_version().decode()
+
+
+def launch_count():
+    return int(_lib().reshard_launch_count())
+
+
+class Plan:
+    """reshard_plan(...) handle.  See include/reshard.h for the contract of every call."""
+
+    def __init__(self, global_shape, elem_bytes, src_mesh, src_spec, dst_mesh, dst_spec, flags=0):
+        self._h = C.c_void_p()
+        _chk(_lib().reshard_plan(_i64(global_shape), len(global_shape), int(elem_bytes),
+                                 _i32(src_mesh), len(src_mesh), src_spec.encode(),
+                                 _i32(dst_mesh), len(dst_mesh), dst_spec.encode(),
+                                 C.c_uint32(flags), C.byref(self._h)))
+        self.info = PlanInfo()
+        _chk(_lib().reshard_plan_info(self._h, C.byref(self.info)))
+        self.ndim = self.info.ndim
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib().reshard_plan_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # ---- queries
+    def op_info(self, op):
+        out = OpInfo()
+        _chk(_lib().reshard_op_info(self._h, op, C.byref(out)))
+        return out
+
+    def op_tables(self, op):
+        """raw bytes of (tasks, dsts, tiles); layouts in csrc/tables.h"""
+        oi = self.op_info(op)
+        t, d, l = (C.create_string_buffer(max(1, oi.n_tasks * 192)), C.create_string_buffer(max(1, oi.n_dsts * 16)),
+                   C.create_string_buffer(max(1, oi.n_tiles * 32)))
+        _chk(_lib().reshard_op_tables(self._h, op, t, d, l))
+        return t.raw[:oi.n_tasks * 192], d.raw[:oi.n_dsts * 16], l.raw[:oi.n_tiles * 32]
+
+    def local_shape(self, side):
+        out = (C.c_int64 * self.ndim)()
+        _chk(_lib().reshard_plan_local_shape(self._h, side, out))
+        return tuple(out)
+
+    def device_box(self, side, dev):
+        lo, hi = (C.c_int64 * self.ndim)(), (C.c_int64 * self.ndim)()
+        _chk(_lib().reshard_plan_device_box(self._h, side, dev, lo, hi))
+        return tuple(lo), tuple(hi)
+
+    def slice(self, i):
+        lo, hi = (C.c_int64 * self.ndim)(), (C.c_int64 * self.ndim)()
+        sender, ns, nr = C.c_int32(), C.c_int32(), C.c_int32()
+        senders, receivers = (C.c_int32 * self.info.n_src)(), (C.c_int32 * self.info.n_dst)()
+        _chk(_lib().reshard_plan_slice(self._h, i, lo, hi, C.byref(sender), C.byref(ns), senders, C.byref(nr),
+                                       receivers))
+        return dict(lo=tuple(lo), hi=tuple(hi), sender=sender.value, senders=list(senders[:ns.value]),
+                    receivers=list(receivers[:nr.value]))
+
+    def slices(self):
+        return [self.slice(i) for i in range(self.info.n_slices)]
+
+    def sender_bytes(self):
+        out = (C.c_int64 * self.info.n_src)()
+        _chk(_lib().reshard_plan_sender_bytes(self._h, out))
+        return list(out)
+
+    def message(self, m):
+        s, r, n = C.c_int32(), C.c_int32(), C.c_int32()
+        off, nb = C.c_int64(), C.c_int64()
+        ids = (C.c_int32 * self.info.n_slices)()
+        _chk(_lib().reshard_plan_message(self._h, m, C.byref(s), C.byref(r), C.byref(off), C.byref(nb), C.byref(n), ids))
+        return dict(sender=s.value, receiver=r.value, offset=off.value, bytes=nb.value, slice_ids=list(ids[:n.value]))
+
+    def messages(self):
+        return [self.message(m) for m in range(self.info.n_messages)]
+
+    def host_workspace_bytes(self):
+        return int(_lib().reshard_host_workspace_bytes(self._h))
+
+    # ---- data path (device addresses in, nothing out; asynchronous on `stream`)
+    def execute(self, src_ptrs, dst_ptrs, stream=0):
+        _chk(_lib().reshard_execute(self._h, _ptrs(src_ptrs), _ptrs(dst_ptrs), C.c_void_p(stream)))
+
+    def pack(self, src_ptrs, arena_ptr, stream=0):
+        _chk(_lib().reshard_pack(self._h, _ptrs(src_ptrs), C.c_void_p(arena_ptr), C.c_void_p(stream)))
+
+    def unpack(self, arena_ptr, dst_ptrs, stream=0):
+        _chk(_lib().reshard_unpack(self._h, C.c_void_p(arena_ptr), _ptrs(dst_ptrs), C.c_void_p(stream)))
+
+    def execute_host(self, src_host_ptrs, dst_host_ptrs, workspace_ptr, stream=0):
+        """returns (h2d_bytes, d2h_bytes)"""
+        up, down = C.c_int64(), C.c_int64()
+        _chk(_lib().reshard_execute_host(self._h, _ptrs(src_host_ptrs), _ptrs(dst_host_ptrs),
+                                         C.c_void_p(workspace_ptr), C.c_void_p(stream), C.byref(up), C.byref(down)))
+        return up.value, down.value

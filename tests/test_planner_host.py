@@ -1,0 +1,354 @@
+"""Host logic of libreshard.so on the CPU box (no compute calls, RS_HOST_ONLY plans):
+exported symbols, planner (a1..a4) against the plan oracle and the paper's facts, and the flat
+task/tile tables (a5) replayed by the TEST-ONLY interpreter tests/table_interp.py against the
+C data oracle."""
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+from hypothesis import given, settings, strategies as st
+
+import golden_io
+import table_interp as ti
+from oracle import data_oracle as do
+from oracle import plan_oracle as po
+from paper_2211_05322_b200 import inputs
+from paper_2211_05322_b200 import reshard as rs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HOST = rs.RS_HOST_ONLY
+
+LAYOUTS = [
+    ((8, 16), (1, 2), "S0,R", (1, 2), "R,S0"),
+    ((8, 16), (1, 2), "S1,R", (1, 2), "R,S1"),
+    ((4, 8, 16), (2, 4), "S0,R,S1", (2, 4), "S0,S1,R"),
+    ((4, 8, 4, 4), (1, 4), "S0,R,R,R", (2, 2), "R,S0,S1,R"),
+    ((4, 8, 4, 4), (1, 4), "S1,R,R,R", (2, 2), "R,S0,R,R"),
+    ((8, 16, 12), (2, 4), "S0,S1,R", (4, 2), "S1,R,S0"),
+    ((8, 8, 4), (2, 4), "R,S01,R", (2, 4), "S01,R,R"),
+    ((6, 6, 2), (2, 3), "RRR", (3, 2), "RRR"),
+    ((12, 6), (2, 3), "S0,S1", (3, 2), "S0,S1"),
+    ((12, 6), (2, 3), "S0,R", (3, 2), "S0,R"),
+    ((8, 8, 8), (2, 4), "R,R,S0", (2, 4), "S0,R,R"),
+    ((8, 8, 8), (2, 4), "S0,R,R", (2, 4), "R,R,R"),
+    ((8, 8, 8), (2, 4), "R,R,R", (2, 4), "S0,S1,R"),
+    ((8, 4), (2, 2), "S0,S1", (4,), "S0,R"),
+    ((4, 6, 5, 3), (2, 2), "S0,S1,R,R", (2, 2), "S1,R,R,R"),      # odd inner extents: narrow vectors
+    ((16, 7), (4,), "S0,R", (2,), "R,R"),
+]
+
+
+def _plan(shape, e, sm, ss, dm, ds, flags=0):
+    return rs.Plan(shape, e, sm, ss, dm, ds, flags | HOST)
+
+
+# ---------------------------------------------------------------- the boundary
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "reshard.h")).read()
+    declared = sorted(set(re.findall(r"RS_API[^;(]*?\b(reshard_\w+)\s*\(", hdr)))
+    assert declared == sorted(rs.SYMBOLS)
+    out = subprocess.run(["nm", "-D", "--defined-only", rs.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l)
+    assert exported == declared                       # nothing else leaks out of the library
+    for name in declared:
+        assert hasattr(rs._lib(), name)
+    assert "sm_100a" in rs.version()
+
+
+def test_only_sm_100a_code_in_library():
+    out = subprocess.run(["cuobjdump", "-lelf", rs.LIB_PATH], capture_output=True, text=True)
+    if out.returncode != 0:
+        pytest.skip("cuobjdump unavailable")
+    archs = set(re.findall(r"sm_\d+a?", out.stdout))
+    assert archs == {"sm_100a"}
+
+
+def test_error_codes():
+    def code(*a, **k):
+        with pytest.raises(rs.ReshardError) as ei:
+            _plan(*a, **k)
+        return ei.value.code
+    assert code((8, 8), 2, (2, 2), "S0,S0", (2, 2), "R,R") == rs.RS_ESPEC          # axis used twice (R3)
+    assert code((8, 8), 2, (2, 2), "S2,R", (2, 2), "R,R") == rs.RS_ESPEC           # axis out of range
+    assert code((8, 8), 2, (2, 2), "S0", (2, 2), "R,R") == rs.RS_ESPEC             # too few entries
+    assert code((8, 8), 2, (2, 2), "S0,R,R", (2, 2), "R,R") == rs.RS_ESPEC         # too many
+    assert code((8, 8), 2, (2, 2), "S,R", (2, 2), "R,R") == rs.RS_ESPEC            # S without axis
+    assert code((8, 8), 2, (2, 2), "X,R", (2, 2), "R,R") == rs.RS_ESPEC
+    assert code((6, 8), 2, (2, 4), "S1,R", (2, 2), "R,R") == rs.RS_EDIVIS          # 6 % 4 (R5)
+    assert code((1024, 1024, 512), 2, (2, 4), "S0RR", (3, 4), "S0RR") == rs.RS_EDIVIS   # Table 2 case 6
+    assert code((8, 8), 3, (2, 2), "R,R", (2, 2), "R,R") == rs.RS_EINVAL           # elem_bytes
+    assert code((8, 0), 2, (2, 2), "R,R", (2, 2), "R,R") == rs.RS_EINVAL
+    assert code((8, 8), 2, (0, 2), "R,R", (2, 2), "R,R") == rs.RS_EINVAL
+    assert code((8, 8), 2, (16, 16), "R,R", (2, 2), "R,R") == rs.RS_EUNSUPPORTED   # > RS_MAX_DEVICES
+    p = _plan((8, 8), 2, (2, 2), "R,R", (2, 2), "R,R")
+    with pytest.raises(rs.ReshardError) as ei:                                      # host-only plan refuses to run
+        p.execute([1] * 4, [1] * 4)
+    assert ei.value.code == rs.RS_EINVAL
+
+
+def test_spec_spellings():
+    a = _plan((8, 8, 8), 2, (2, 4), "S01,R,R", (2, 4), "R,S0,S1").slices()
+    for text in ("(S01, R, R)", "S^{01}RR", "s01 r r", "[S_01,R,R]"):
+        assert _plan((8, 8, 8), 2, (2, 4), text, (2, 4), "RS0S1").slices() == a
+
+
+# ---------------------------------------------------------------- a1..a3 against the paper and the plan oracle
+
+def test_fig2_worked_example():
+    """PAPER.md:62, 86, 90."""
+    g = golden_io.load("fig2_example.txt")
+    shape = tuple(g["matrix_shape"])
+    a0, b0 = g["mesh_a_devices"][0], g["mesh_b_devices"][0]
+    D = np.array(g["matrix_values"]).reshape(shape)
+    p1 = _plan(shape, 4, g["mesh_a"], g["spec1"], g["mesh_b"], g["spec2"])
+    s = p1.slices()
+    assert len(s) == g["task1_num_unit_tasks"][0]
+    box = tuple(slice(l, h) for l, h in zip(s[0]["lo"], s[0]["hi"]))
+    assert D[box].reshape(-1).tolist() == g["task1_first_slice_elements"]
+    assert [r + b0 for r in s[0]["receivers"]] == g["task1_first_receivers"]
+    for local in (0, 1):                                   # devices 4, 5 hold elements 0..7
+        lo, hi = p1.device_box(rs.RS_DST, local)
+        assert D[lo[0]:hi[0], lo[1]:hi[1]].reshape(-1).tolist() == g["spec2_device4_elements"]
+    p2 = _plan(shape, 4, g["mesh_b"], g["spec2"], g["mesh_a"], g["spec3"])
+    s = p2.slices()
+    assert len(s) == g["task2_num_unit_tasks"][0]
+    box = tuple(slice(l, h) for l, h in zip(s[0]["lo"], s[0]["hi"]))
+    assert D[box].reshape(-1).tolist() == g["task2_first_slice_elements"]
+    assert [r + a0 for r in s[0]["receivers"]] == g["task2_first_receivers"]
+    assert [x + b0 for x in s[0]["senders"]] == [4, 5]
+
+
+def test_table2_facts():
+    """PAPER.md:282 (case 4: 64 unit tasks), 320 (case 8: one broadcast; case 2 naive: first node)."""
+    g = golden_io.load("table2_facts.txt")
+    shape = tuple(g["tensor_shape"])
+
+    def plan(case, flags=0):
+        ss, ds, sm, dm = inputs.TABLE2[case]
+        return _plan(shape, 2, sm, ss, dm, ds, flags)
+    assert plan(4).info.n_slices == g["case4_num_unit_tasks"][0]
+    p8 = plan(8)
+    assert p8.info.n_slices == g["case8_num_unit_tasks"][0]
+    assert len(p8.slice(0)["senders"]) == 6 and len(p8.slice(0)["receivers"]) == 6
+    naive = plan(2, rs.RS_LB_NAIVE)
+    assert {s["sender"] // 4 for s in naive.slices()} == {g["case2_naive_sender_node"][0]}
+    assert naive.info.max_sender_bytes == naive.info.tensor_bytes            # everything from one device
+    greedy = plan(2)
+    assert greedy.info.max_sender_bytes == greedy.info.tensor_bytes // 2
+    for case in (1, 2, 3, 4, 5, 7, 8, 9):
+        p = plan(case)
+        assert sum(p.sender_bytes()) == p.info.tensor_bytes                  # lower bound
+
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", LAYOUTS)
+def test_slices_match_plan_oracle(shape, sm, ss, dm, ds):
+    p = _plan(shape, 2, sm, ss, dm, ds)
+    tasks = po.unit_tasks(shape, sm, ss, dm, ds)
+    got = p.slices()
+    assert len(got) == len(tasks) == p.info.n_slices
+    for g, t in zip(got, tasks):
+        assert g["lo"] == t["lo"] and g["hi"] == t["hi"]
+        assert g["senders"] == t["senders"] and g["receivers"] == t["receivers"]
+        assert g["sender"] in t["senders"]                                   # Eq. 2
+    for side, mesh, spec in ((rs.RS_SRC, sm, ss), (rs.RS_DST, dm, ds)):
+        assert p.local_shape(side) == do.local_shape(shape, mesh, spec)
+        for r in range(po.n_devices(mesh)):
+            assert p.device_box(side, r) == po.tile_box(shape, mesh, spec, r)
+    assert p.info.write_bytes == sum(t["size"] * len(t["receivers"]) for t in tasks) * 2
+    assert p.info.unique_read_bytes == int(np.prod(shape)) * 2
+
+
+# ---------------------------------------------------------------- a4: sender choice
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", LAYOUTS)
+def test_sender_choice_objective(shape, sm, ss, dm, ds):
+    tasks = po.unit_tasks(shape, sm, ss, dm, ds)
+    n_src = po.n_devices(sm)
+    greedy = _plan(shape, 2, sm, ss, dm, ds)
+    naive = _plan(shape, 2, sm, ss, dm, ds, rs.RS_LB_NAIVE)
+    assert [s["sender"] for s in naive.slices()] == po.naive_senders(tasks)
+    assert naive.info.max_sender_bytes == po.max_load(tasks, po.naive_senders(tasks), n_src, 2)
+    loads = po.sender_loads(tasks, [s["sender"] for s in greedy.slices()], n_src, 2)
+    assert loads == greedy.sender_bytes() and max(loads) == greedy.info.max_sender_bytes
+    assert greedy.info.max_sender_bytes <= po.max_load(tasks, po.greedy_senders(tasks, 2), n_src, 2)
+    assert greedy.info.max_sender_bytes <= naive.info.max_sender_bytes
+    try:
+        opt = po.bruteforce_optimum(tasks, n_src, 2)
+    except ValueError:
+        return
+    assert greedy.info.max_sender_bytes == opt            # BASELINE: equals the brute-force optimum
+
+
+def test_unequal_slices_need_the_exact_finish():
+    """2-way x 3-way cuts give slices of 3 sizes; LPT alone can miss the optimum (R9)."""
+    shape, sm, ss, dm, ds = (12, 12), (2, 3), "S0,R", (3, 2), "S0,S1"
+    for shape, sm, ss, dm, ds in [((12, 12), (2, 3), "S0,R", (3, 2), "S0,S1"), ((12, 6), (2, 3), "S0,R", (3, 2), "S0,R"),
+                                  ((24, 12), (4, 3), "R,R", (3, 4), "S0,S1")]:
+        tasks = po.unit_tasks(shape, sm, ss, dm, ds)
+        p = _plan(shape, 1, sm, ss, dm, ds)
+        try:
+            assert p.info.max_sender_bytes == po.bruteforce_optimum(tasks, po.n_devices(sm), 1)
+        except ValueError:
+            assert p.info.max_sender_bytes <= po.max_load(tasks, po.greedy_senders(tasks, 1), po.n_devices(sm), 1)
+
+
+# ---------------------------------------------------------------- a5: tables replayed against the data oracle
+
+def _bytes(a):
+    return np.ascontiguousarray(a).view(np.uint8).reshape(-1)
+
+
+def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None):
+    e = np.dtype(dtype).itemsize
+    old = {}
+    for k, v in (env or {}).items():
+        old[k] = os.environ.get(k)
+        os.environ[k] = str(v)
+    try:
+        p = _plan(shape, e, sm, ss, dm, ds, flags)
+    finally:
+        for k, v in old.items():
+            if v is None:
+                os.environ.pop(k)
+            else:
+                os.environ[k] = v
+    D = (np.arange(int(np.prod(shape)), dtype=np.int64) * 2654435761 % 251 + 1).astype(dtype).reshape(shape)
+    src = do.shards_from_global(D, sm, ss)
+    want = do.reshard(shape, sm, ss, dm, ds, src)
+    n_dst = len(want)
+    # execute
+    dst = [np.zeros(want[0].nbytes, np.uint8) for _ in range(n_dst)]
+    cnt = [np.zeros(want[0].nbytes, np.int32) for _ in range(n_dst)]
+    ti.replay(p, rs.RS_OP_EXECUTE, [_bytes(s) for s in src], dst, cnt)
+    for q in range(n_dst):
+        assert np.array_equal(dst[q], _bytes(want[q])), "execute tables differ from the oracle on device %d" % q
+        assert (cnt[q] == 1).all(), "execute tables do not write every byte exactly once"
+    # pack -> message contents as the plan oracle states them -> unpack
+    arena = [np.zeros(p.info.arena_bytes, np.uint8)]
+    acnt = [np.zeros(p.info.arena_bytes, np.int32)]
+    ti.replay(p, rs.RS_OP_PACK, [_bytes(s) for s in src], arena, acnt)
+    tasks = po.unit_tasks(shape, sm, ss, dm, ds)
+    senders = [s["sender"] for s in p.slices()]
+    msgs = p.messages()
+    ref = po.pack_messages(shape, sm, ss, tasks, senders, src)
+    assert [(m["sender"], m["receiver"]) for m in msgs] == [(s, r) for s, r, _ in ref]
+    covered = np.zeros(p.info.arena_bytes, bool)
+    for m, (s, r, payload) in zip(msgs, ref):
+        assert m["bytes"] == payload.nbytes and m["offset"] % 256 == 0
+        assert np.array_equal(arena[0][m["offset"]:m["offset"] + m["bytes"]], _bytes(payload))
+        covered[m["offset"]:m["offset"] + m["bytes"]] = True
+    assert sum(m["bytes"] for m in msgs) == p.info.write_bytes
+    assert np.array_equal(acnt[0] == 1, covered) and (acnt[0][~covered] == 0).all()
+    dst2 = [np.zeros(want[0].nbytes, np.uint8) for _ in range(n_dst)]
+    cnt2 = [np.zeros(want[0].nbytes, np.int32) for _ in range(n_dst)]
+    ti.replay(p, rs.RS_OP_UNPACK, arena, dst2, cnt2)
+    for q in range(n_dst):
+        assert np.array_equal(dst2[q], _bytes(want[q]))
+        assert (cnt2[q] == 1).all()
+    return p
+
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", LAYOUTS)
+@pytest.mark.parametrize("dtype", [np.uint8, np.int16, np.int64])
+def test_tables_replay_equals_oracle(shape, sm, ss, dm, ds, dtype):
+    _check_tables(shape, dtype, sm, ss, dm, ds)
+
+
+@pytest.mark.parametrize("tile", [128, 256, 1024])
+@pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK])
+def test_tables_with_tiny_tiles_cover_every_tile_kind(tile, path):
+    """small tile sizes force column-split rows, FAST row groups and GENERIC tiles at test sizes"""
+    env = {"RS_LSU_TILE_BYTES": tile, "RS_BULK_TILE_BYTES": tile}
+    kinds = set()
+    for shape, sm, ss, dm, ds in [((4, 6, 64), (2, 2), "S0,S1,R", (2, 2), "S1,S0,R"),      # long runs -> column split
+                                  ((8, 16, 16), (2, 4), "S0,R,S1", (2, 4), "S0,S1,R"),     # short runs, wide ext0
+                                  ((8, 6, 2, 16), (2, 2), "S0,R,R,S1", (2, 2), "R,S0,R,S1"),  # ext0 = 2 -> GENERIC
+                                  ((6, 4, 2, 3, 8), (2,), "R,R,R,R,S0", (2,), "S0,R,R,R,R")]:
+        p = _check_tables(shape, np.int32, sm, ss, dm, ds, flags=path, env=env)
+        _t, _d, tiles = ti.tables(p, rs.RS_OP_EXECUTE)
+        for t in tiles:
+            kinds.add("split" if t["n_rows"] == 1 and t["flags"] & 1 else "fast" if t["flags"] & 1 else "generic")
+        assert p.op_info(rs.RS_OP_EXECUTE).tile_bytes <= max(tile, 128)
+        assert all(int(t["n_rows"]) * int(t["col_bytes"]) <= max(tile, 128) for t in tiles)
+    assert kinds == {"split", "fast", "generic"}
+
+
+def test_alignment_class_and_path_choice():
+    p = _plan((16, 1024, 4096), 2, (2, 4), "S0,R,S1", (2, 4), "S0,S1,R")
+    oi = p.op_info(rs.RS_OP_EXECUTE)
+    assert oi.vec_bytes == 16 and oi.path == rs.RS_PATH_BULK and oi.min_run_bytes == 2048
+    assert oi.read_bytes == p.info.tensor_bytes and oi.write_bytes == p.info.tensor_bytes
+    p = _plan((4, 6, 5, 3), 2, (2, 2), "S0,S1,R,R", (2, 2), "S1,R,R,R")          # runs of 15 elements = 30 B
+    oi = p.op_info(rs.RS_OP_EXECUTE)
+    assert oi.vec_bytes == 2 and oi.path == rs.RS_PATH_LSU
+    p = _plan((4, 6, 5, 3), 2, (2, 2), "S0,S1,R,R", (2, 2), "S1,R,R,R", rs.RS_PATH_BULK)
+    assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_LSU                     # TMA needs 16-byte everything
+    p = _plan((8, 16), 4, (1, 2), "S1,R", (1, 2), "R,S1")                         # c1i: 32-byte runs
+    assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_LSU
+    assert _plan((8, 16), 4, (1, 2), "S1,R", (1, 2), "R,S1", rs.RS_PATH_BULK).op_info(0).path == rs.RS_PATH_BULK
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c3i", "c3ii", "c4", "t2_4", "sweep_P5_m8_1024MiB", "sweep_P2_m8_4096MiB"])
+def test_full_size_tables_cover_every_byte_once(name):
+    """at BASELINE sizes: interval arithmetic over the tile table instead of replaying bytes"""
+    w = inputs.get_workload(name)
+    p = _plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    for op in (rs.RS_OP_EXECUTE, rs.RS_OP_PACK, rs.RS_OP_UNPACK):
+        tasks, dsts, tiles = ti.tables(p, op)
+        oi = p.op_info(op)
+        T = tasks[tiles["task"]]
+        nbytes = tiles["n_rows"].astype(np.int64) * tiles["col_bytes"].astype(np.int64)
+        assert int(nbytes.sum()) == oi.read_bytes
+        assert int((nbytes * T["k"]).sum()) == oi.write_bytes
+        assert int(nbytes.max()) <= oi.tile_bytes
+        assert (tiles["col_bytes"] % 16 == 0).all() and oi.vec_bytes == 16
+        # the largest byte any FAST tile touches stays inside its buffers
+        fast = (tiles["flags"] & 1) == 1
+        assert fast.all()
+        last_s = T["src_off"] + tiles["a"].astype(np.int64) + (tiles["n_rows"].astype(np.int64) - 1) * T["sstride"][:, 0] + tiles["col_bytes"]
+        src_cap = p.info.src_shard_bytes if op != rs.RS_OP_UNPACK else p.info.arena_bytes
+        assert int(last_s.max()) <= src_cap
+        dst_cap = p.info.dst_shard_bytes if op != rs.RS_OP_PACK else p.info.arena_bytes
+        for j in range(int(T["k"].max())):
+            has = T["k"] > j
+            D = dsts[(T["dst_first"] + j)[has]]
+            last_d = D["off"] + tiles["b"].astype(np.int64)[has] + (tiles["n_rows"].astype(np.int64)[has] - 1) * T["dstride"][:, 0][has] + tiles["col_bytes"][has]
+            assert int(last_d.max()) <= dst_cap
+
+
+_SPECS2 = ["R", "S0", "S1", "S01", "S10"]
+
+
+@st.composite
+def _layouts(draw):
+    ndim = draw(st.integers(1, 4))
+
+    def side():
+        mesh = draw(st.sampled_from([(1, 2), (2, 2), (2, 4), (4, 2), (2, 3), (3, 2), (1, 4), (4,), (3,)]))
+        while True:
+            spec = [draw(st.sampled_from(_SPECS2)) for _ in range(ndim)]
+            axes = "".join(s[1:] for s in spec)
+            if len(set(axes)) == len(axes) and all(int(a) < len(mesh) for a in axes):
+                return mesh, ",".join(spec)
+    sm, ss = side()
+    dm, ds = side()
+    shape = tuple(draw(st.sampled_from([12, 24])) for _ in range(ndim))
+    if ndim >= 3:
+        shape = tuple(min(s, 12) for s in shape)
+    return shape, sm, ss, dm, ds, draw(st.sampled_from([np.uint8, np.int16, np.int32])), draw(st.sampled_from([128, 512, 16384]))
+
+
+@settings(max_examples=60, deadline=None)
+@given(_layouts())
+def test_random_layouts_tables_equal_oracle(layout):
+    shape, sm, ss, dm, ds, dtype, tile = layout
+    try:
+        do.local_shape(shape, sm, ss), do.local_shape(shape, dm, ds)
+    except do.OracleError:
+        with pytest.raises(rs.ReshardError):
+            _plan(shape, 1, sm, ss, dm, ds)
+        return
+    _check_tables(shape, dtype, sm, ss, dm, ds, env={"RS_LSU_TILE_BYTES": tile, "RS_BULK_TILE_BYTES": tile})
