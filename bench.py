@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- resharding GB/s (unique bytes read + bytes written) of the hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4] [--impl ours|reference]
+
+A STEP is one pass of the device rows of the hot path over one synthetic
+tensor: reshard_execute, reshard_pack, reshard_unpack, one kernel launch each, back to back on one
+stream.  The host rows a1..a5 (reshard_plan) run once before the timed region (SURVEY.md S8(d):
+"plan once outside the timed region"); their time is reported as plan_ms.
+value = algorithmic bytes of the three launches / step time, inputs resident in HBM.
+e2e   = the same metric for reshard_execute_host: HOST (pinned) shards in, HOST shards out, copies
+        inside the timed region.
+One JSON line on stdout (rank 0).  Multi-GPU: "replicas only": every rank runs the same
+task on its own GPU, no data-path collective; value = N x bytes / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "resharding GB/s (unique read+write bytes)"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json: "~8 TB/s"; the >=70 % bar refers to this
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE rs_copy_* launch of reshard_execute, from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists)
+NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", help="c4 (default, 1.5 GiB GPT activation), c2, c3, t2_<n>, sweep_<pair>_<m8|m4>_<MiB>MiB")
+    ap.add_argument("--path", default="auto", choices=["auto", "lsu", "bulk"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU work of the oracle sample")
+    return ap.parse_args()
+
+
+def peak_hbm():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------ oracle timing (CPU baseline / reference arm)
+
+def oracle_sample(w, seconds, steps=1, warmup=0):
+    """Time the oracle AS IT STANDS on a bounded sample of workload w: whole destination shards
+    (devices 0, 1, ...) until about `seconds` of wall time, all host cores.  Source shards hold a
+    cheap seeded byte pattern (the oracle's cost does not depend on values).  Returns dict."""
+    import numpy as np
+    from oracle import data_oracle as do
+    from paper_2211_05322_b200 import inputs
+    e = inputs.elem_bytes(w.dtype)
+    ct = np.dtype({1: np.uint8, 2: np.int16, 4: np.int32, 8: np.int64}[e])
+    cores = do.max_threads()
+    n_src, n_dst = do.num_devices(w.src_mesh), do.num_devices(w.dst_mesh)
+    lshape = do.local_shape(w.shape, w.src_mesh, w.src_spec)
+    # only the lowest-index replica of each source tile is dereferenced: alias replicas of a tile
+    bufs, src = {}, []
+    for r in range(n_src):
+        key = do.device_box(w.shape, w.src_mesh, w.src_spec, r)
+        if key not in bufs:
+            a = np.arange(int(np.prod(lshape)), dtype=np.int64)
+            bufs[key] = ((a * 2654435761 + w.seed + r) >> 7).astype(ct).reshape(lshape)
+        src.append(bufs[key])
+    out = np.empty(do.local_shape(w.shape, w.dst_mesh, w.dst_spec), dtype=ct)
+    shard_bytes = out.nbytes
+    r_B = n_dst * shard_bytes / (int(np.prod(w.shape)) * e)           # destination replication
+    per_shard_metric_bytes = shard_bytes * (1.0 + 1.0 / r_B)            # written + its share of the unique read
+    times, shards_done = [], 0
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        q = 0
+        while True:
+            do.reshard_device(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, src, q % n_dst, ct,
+                              n_threads=cores, out=out)
+            q += 1
+            if time.perf_counter() - t0 >= seconds or q >= n_dst:
+                break
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt / q)
+            shards_done = q
+    t = statistics.median(times)
+    return {"value": per_shard_metric_bytes / t / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
+            "sample": "%d of %d destination shards of %s (%.0f MiB each), all elements, %d threads, %.2f s per shard"
+                      % (shards_done, n_dst, w.name, shard_bytes / 2**20, cores, t),
+            "seconds_per_shard": t, "shards": shards_done}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on host cores, same metric/config; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    from paper_2211_05322_b200 import inputs
+    w = inputs.get_workload(args.workload)
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    budget = 150.0                                                     # whole run within a few minutes
+    per_step = max(1.0, min(args.cpu_seconds, budget / (steps + warmup)))
+    r = oracle_sample(w, per_step, steps=steps, warmup=warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": "GB/s", "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": r["seconds_per_shard"] * r["shards"] * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": _config(w, "cpu-oracle"), "gpu_launches": 0,
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def _config(w, path):
+    return {"workload": "%s: %s %s, src mesh %s spec (%s) -> dst mesh %s spec (%s)" % (
+                w.name, w.dtype, list(w.shape), "x".join(map(str, w.src_mesh)), w.src_spec,
+                "x".join(map(str, w.dst_mesh)), w.dst_spec),
+            "step": "reshard_execute + reshard_pack + reshard_unpack (plan outside the timed region)",
+            "executor": path, "l2": "inputs larger than L2 (no flush needed)", "parallelism": "replicas only"}
+
+
+# ------------------------------------------------------------------ clocks
+
+SMI_FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+
+class ClockSampler:
+    """nvidia-smi -lms 50 in the background while the timed region runs"""
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + SMI_FIELDS,
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def n_samples(self):
+        try:
+            with open(self.f.name) as f:
+                return sum(1 for _ in f)
+        except OSError:
+            return 0
+
+    def stop(self):
+        if self.p is not None:
+            self.p.terminate()
+            try:
+                self.p.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.p.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            with open(self.f.name) as f:
+                for line in f:
+                    c = [x.strip() for x in line.split(",")]
+                    if len(c) < 8:
+                        continue
+                    try:
+                        sm.append(float(c[0])); mx.append(float(c[1]))
+                    except ValueError:
+                        continue
+                    for name, v in zip(names, c[4:8]):
+                        if v.lower().startswith("active"):
+                            reasons.add(name)
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------ our arm
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2211_05322_b200 import harness, inputs
+    from paper_2211_05322_b200 import reshard as rs
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = inputs.get_workload(args.workload)
+    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK}[args.path]
+    t0 = time.perf_counter()
+    plan = harness.make_plan(w, flags)                     # rows a1..a5, once, outside the timed region
+    plan_ms = (time.perf_counter() - t0) * 1e3
+    info = plan.info
+    ops = [plan.op_info(o) for o in (rs.RS_OP_EXECUTE, rs.RS_OP_PACK, rs.RS_OP_UNPACK)]
+    op_bytes = [o.read_bytes + o.write_bytes for o in ops]
+    step_bytes = sum(op_bytes)
+
+    D, src = harness.device_inputs(w, plan, dev)
+    dst = harness.device_outputs(plan, D, dev)
+    arena = torch.empty(info.arena_bytes, dtype=torch.uint8, device=dev)
+    del D
+    sp, dp, ap = harness.ptrs(src), harness.ptrs(dst), arena.data_ptr()
+    stream = torch.cuda.current_stream()
+    sh = stream.cuda_stream
+    flush = None
+    if step_bytes < (1 << 30):                              # working set comparable to the 126 MB L2: flush it
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+
+    K, W = max(1, args.steps), max(3, args.warmup)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
+
+    def step(e4=None):
+        if flush is not None:
+            flush.fill_(1)
+        if e4: e4[0].record(stream)
+        plan.execute(sp, dp, sh)
+        if e4: e4[1].record(stream)
+        plan.pack(sp, ap, sh)
+        if e4: e4[2].record(stream)
+        plan.unpack(ap, dp, sh)
+        if e4: e4[3].record(stream)
+
+    for _ in range(W):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    n0 = rs.launch_count()
+    barrier()
+    for i in range(K):
+        step(ev[i])
+    barrier()
+    launches = rs.launch_count() - n0
+    if sampler is not None:
+        t_end = time.perf_counter() + 2.0                   # short regions: keep the same load until >= 3 samples
+        while sampler.n_samples() < 3 and time.perf_counter() < t_end:
+            for _ in range(20):
+                step()
+            torch.cuda.synchronize()
+        clocks = sampler.stop()
+    if flush is None:
+        total_ms = ev[0][0].elapsed_time(ev[-1][3])
+    else:
+        total_ms = sum(e[0].elapsed_time(e[3]) for e in ev)
+    k_ms = [statistics.mean(e[j].elapsed_time(e[j + 1]) for e in ev) for j in range(3)]
+    k_best = [min(e[j].elapsed_time(e[j + 1]) for e in ev) for j in range(3)]
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / K
+    value = world * step_bytes / (ms_per_step * 1e-3) / 1e9
+
+    # ---- end to end: host (pinned) shards in, host shards out, through reshard_execute_host
+    e2e = None
+    if not args.no_e2e:
+        src_h = [torch.empty(s.shape, dtype=s.dtype).pin_memory() for s in src]
+        for h, s in zip(src_h, src):
+            h.copy_(s)
+        dst_h = [torch.empty(d.shape, dtype=d.dtype).pin_memory() for d in dst]
+        ws = torch.empty(plan.host_workspace_bytes(), dtype=torch.uint8, device=dev)
+        shp, dhp = harness.ptrs(src_h), harness.ptrs(dst_h)
+        up = down = 0
+        for _ in range(2):
+            up, down = plan.execute_host(shp, dhp, ws.data_ptr(), sh)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_e2e = max(1, args.e2e_steps)
+        e0.record(stream)
+        for _ in range(n_e2e):
+            plan.execute_host(shp, dhp, ws.data_ptr(), sh)
+            stream.synchronize()                            # the caller reads the result on the host
+        e1.record(stream)
+        barrier()
+        t = torch.tensor([e0.elapsed_time(e1) / n_e2e], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+        e2e = {"value": world * op_bytes[0] / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": up,
+               "d2h_bytes_per_step": down, "ms_per_step": e2e_ms, "steps": n_e2e,
+               "call": "reshard_execute_host (pinned host shards -> H2D -> rs_copy kernel -> D2H)"}
+        del src_h, dst_h, ws
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = peak_hbm()
+    names = ["reshard_execute", "reshard_pack", "reshard_unpack"]
+    pname = {rs.RS_PATH_LSU: "rs_copy_lsu", rs.RS_PATH_BULK: "rs_copy_bulk"}
+    kernels = {n: {"kernel": pname[o.path], "ms": k_ms[j], "best_ms": k_best[j], "bytes": op_bytes[j],
+                   "GB/s": op_bytes[j] / (k_ms[j] * 1e-3) / 1e9, "grid": o.grid, "block": o.block,
+                   "smem": o.smem_bytes, "tiles": o.n_tiles, "tile_bytes": o.tile_bytes}
+               for j, (n, o) in enumerate(zip(names, ops))}
+    achieved = kernels["reshard_execute"]["GB/s"]
+    line = {"metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u8", "data": "synthetic", "config": _config(w, kernels["reshard_execute"]["kernel"]),
+            "clocks": clocks, "gpu_launches": launches, "plan_ms": plan_ms,
+            "pct_of_nominal_8TBs": 100.0 * achieved / NOMINAL_HBM_GBS,
+            "roofline": {"bound": "hbm", "kernel": "reshard_execute (%s)" % kernels["reshard_execute"]["kernel"],
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "peak_source": peak_src, "algorithmic_bytes": op_bytes[0],
+                         "traffic": NCU_TRAFFIC_BYTES.get(w.name)},
+            "kernels": kernels}
+    if flush is not None:
+        line["config"]["l2"] = "L2 flushed between steps (512 MiB fill); working set is L2-sized: effective GB/s"
+    if e2e is not None:
+        line["e2e"] = e2e
+    if world == 1 and not args.no_cpu_baseline:
+        r = oracle_sample(w, args.cpu_seconds)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

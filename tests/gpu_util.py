@@ -1,0 +1,71 @@
+"""helpers of the -m gpu parity tests: device buffers (torch is only memory + streams here),
+shards cut with the ORACLE's boxes, calls through the C ABI binding."""
+import numpy as np
+import torch
+
+from oracle import data_oracle as do
+from paper_2211_05322_b200 import inputs
+from paper_2211_05322_b200 import reshard as rs
+
+_TORCH_CT = {1: torch.uint8, 2: torch.int16, 4: torch.int32, 8: torch.int64}
+
+
+def dev():
+    return torch.device("cuda:0")
+
+
+def to_dev(a):
+    """numpy array (any itemsize, incl. 16-byte void) -> device uint8 tensor of its bytes"""
+    return torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1).copy()).to(dev())
+
+
+def ptrs(ts):
+    return [t.data_ptr() for t in ts]
+
+
+def stream():
+    return torch.cuda.current_stream().cuda_stream
+
+
+def oracle_slices(shape, mesh, spec):
+    """per device the torch/numpy basic-slicing index of its box, from the oracle's device_box"""
+    out = []
+    for r in range(do.num_devices(mesh)):
+        lo, hi = do.device_box(shape, mesh, spec, r)
+        out.append(tuple(slice(l, h) for l, h in zip(lo, hi)))
+    return out
+
+
+def device_shards_from_global(D, mesh, spec):
+    """D: device tensor of the global shape -> list of dense device shards (oracle boxes)"""
+    return [D[idx].contiguous() for idx in oracle_slices(tuple(D.shape), mesh, spec)]
+
+
+def run_small(shape, np_dtype, sm, ss, dm, ds, flags=0, seed=1, src_offset=0, dst_offset=0):
+    """execute on the GPU and return (plan, got dst shards as numpy, oracle dst shards as numpy)."""
+    e = np.dtype(np_dtype).itemsize
+    rng = np.random.default_rng(seed)
+    D = np.frombuffer(rng.bytes(int(np.prod(shape)) * e), dtype=np_dtype).reshape(shape)
+    src = do.shards_from_global(D, sm, ss)
+    want = do.reshard(shape, sm, ss, dm, ds, src)
+    p = rs.Plan(shape, e, sm, ss, dm, ds, flags)
+    src_d = [torch.zeros(s.nbytes + 64, dtype=torch.uint8, device=dev()) for s in src]
+    for t, s in zip(src_d, src):
+        t[src_offset:src_offset + s.nbytes] = to_dev(s)
+    dst_d = [torch.full((want[0].nbytes + 64,), 0xA5, dtype=torch.uint8, device=dev()) for _ in want]
+    p.execute([t.data_ptr() + src_offset for t in src_d], [t.data_ptr() + dst_offset for t in dst_d], stream())
+    torch.cuda.synchronize()
+    got = []
+    for t, w in zip(dst_d, want):
+        raw = t.cpu().numpy()
+        assert (raw[:dst_offset] == 0xA5).all() and (raw[dst_offset + w.nbytes:] == 0xA5).all(), "wrote outside the shard"
+        got.append(raw[dst_offset:dst_offset + w.nbytes].view(np_dtype).reshape(w.shape))
+    return p, got, want
+
+
+def workload_on_device(w):
+    """(D on device in its container dtype, src shards, expected dst shards) for a named workload;
+    expected = basic slicing of D with the oracle's destination boxes."""
+    D = inputs.global_tensor_torch(w, dev())
+    src = device_shards_from_global(D, w.src_mesh, w.src_spec)
+    return D, src

@@ -1,0 +1,267 @@
+"""-m gpu parity tests: the CUDA path, called through the C ABI, against the CPU oracle.
+Bar: bit-exact (pure copy, tolerance 0) -- BASELINE.json north_star."""
+import numpy as np
+import pytest
+import torch
+
+import gpu_util as gu
+from oracle import data_oracle as do
+from oracle import plan_oracle as po
+from paper_2211_05322_b200 import inputs
+from paper_2211_05322_b200 import reshard as rs
+
+pytestmark = pytest.mark.gpu
+
+PATHS = [rs.RS_PATH_AUTO, rs.RS_PATH_LSU, rs.RS_PATH_BULK]
+
+SMALL = [
+    ((8, 16), (1, 2), "S0,R", (1, 2), "R,S0"),                      # config 1 literal
+    ((8, 16), (1, 2), "S1,R", (1, 2), "R,S1"),                      # config 1 intent
+    ((4, 8, 16), (2, 4), "S0,R,S1", (2, 4), "S0,S1,R"),
+    ((4, 8, 4, 4), (1, 4), "S0,R,R,R", (2, 2), "R,S0,S1,R"),
+    ((4, 8, 4, 4), (1, 4), "S1,R,R,R", (2, 2), "R,S0,R,R"),
+    ((8, 16, 12), (2, 4), "S0,S1,R", (4, 2), "S1,R,S0"),
+    ((8, 8, 4), (2, 4), "R,S01,R", (2, 4), "S01,R,R"),
+    ((6, 6, 2), (2, 3), "RRR", (3, 2), "RRR"),
+    ((12, 6), (2, 3), "S0,S1", (3, 2), "S0,S1"),
+    ((8, 8, 8), (2, 4), "R,R,S0", (2, 4), "S0,R,R"),
+    ((8, 8, 8), (2, 4), "S0,R,R", (2, 4), "R,R,R"),
+    ((8, 8, 8), (2, 4), "R,R,R", (2, 4), "S0,S1,R"),
+    ((4, 6, 5, 3), (2, 2), "S0,S1,R,R", (2, 2), "S1,R,R,R"),        # odd extents: 2-byte vectors at most
+    ((16, 7), (4,), "S0,R", (2,), "R,R"),
+    ((1,), (1,), "R", (1,), "R"),                                    # degenerate: one element
+    ((8, 6, 2, 16), (2, 2), "S0,R,R,S1", (2, 2), "R,S0,R,S1"),       # GENERIC tiles
+    ((6, 4, 2, 3, 8), (2,), "R,R,R,R,S0", (2,), "S0,R,R,R,R"),
+    ((64, 96, 160), (2, 4), "S0,R,S1", (2, 4), "S0,S1,R"),           # several tiles + ragged tail (160*e/4)
+    ((48, 1000), (2, 2), "S0,S1", (2, 2), "S1,S0"),
+    ((3, 5, 7), (1,), "R,R,R", (1,), "R,R,R"),                       # 1 device -> 1 device: memcpy
+]
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("dtype", [np.uint8, np.int16, np.float32, np.int64, np.dtype("V16")])
+@pytest.mark.parametrize("case", SMALL, ids=[str(i) for i in range(len(SMALL))])
+def test_execute_bit_exact_small(case, dtype, path):
+    shape, sm, ss, dm, ds = case
+    _p, got, want = gu.run_small(shape, dtype, sm, ss, dm, ds, flags=path)
+    for q, (g, w) in enumerate(zip(got, want)):
+        assert g.tobytes() == w.tobytes(), "device %d differs" % q
+
+
+@pytest.mark.parametrize("off", [(2, 0), (0, 2), (4, 8), (1, 3), (16, 16)])
+@pytest.mark.parametrize("path", PATHS)
+def test_under_aligned_shard_pointers(off, path):
+    """plan allows 16-byte vectors; the caller's pointers do not: narrower accesses, same bytes"""
+    _p, got, want = gu.run_small((64, 96, 160), np.int16, (2, 4), "S0,R,S1", (2, 4), "S0,S1,R", flags=path,
+                                 src_offset=off[0], dst_offset=off[1])
+    for g, w in zip(got, want):
+        assert g.tobytes() == w.tobytes()
+
+
+@pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK])
+@pytest.mark.parametrize("tile", [128, 1024, 4096])
+def test_tile_sizes_and_ring_depths(tile, path, monkeypatch):
+    monkeypatch.setenv("RS_LSU_TILE_BYTES", str(tile))
+    monkeypatch.setenv("RS_BULK_TILE_BYTES", str(tile))
+    for stages, look, warps in [(2, 1, 1), (3, 2, 4), (8, 4, 2), (6, 5, 8)]:
+        monkeypatch.setenv("RS_BULK_STAGES", str(stages))
+        monkeypatch.setenv("RS_BULK_LOOKAHEAD", str(look))
+        monkeypatch.setenv("RS_BULK_WARPS", str(warps))
+        for case in (SMALL[2], SMALL[15], SMALL[17], SMALL[18]):
+            shape, sm, ss, dm, ds = case
+            _p, got, want = gu.run_small(shape, np.int32, sm, ss, dm, ds, flags=path)
+            for g, w in zip(got, want):
+                assert g.tobytes() == w.tobytes()
+        if path == rs.RS_PATH_LSU:
+            break
+
+
+@pytest.mark.parametrize("name", ["c1", "c1i", "c3", "c3i", "c3ii", "c2"])
+@pytest.mark.parametrize("path", PATHS)
+def test_baseline_configs_against_full_oracle(name, path):
+    """configs 1-3 of BASELINE.json (and the prose-intent variants, R21): every element vs the oracle"""
+    w = inputs.get_workload(name)
+    e = inputs.elem_bytes(w.dtype)
+    D = inputs.global_tensor(w)
+    src = do.shards_from_global(D, w.src_mesh, w.src_spec)
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, path)
+    src_d = [gu.to_dev(s) for s in src]
+    dst_d = [torch.full((p.info.dst_shard_bytes,), 0x5A, dtype=torch.uint8, device=gu.dev()) for _ in range(p.info.n_dst)]
+    p.execute(gu.ptrs(src_d), gu.ptrs(dst_d), gu.stream())
+    torch.cuda.synchronize()
+    n_thr = do.max_threads()
+    for q in range(p.info.n_dst):
+        want = do.reshard_device(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, src, q, D.dtype, n_threads=n_thr)
+        assert dst_d[q].cpu().numpy().tobytes() == want.tobytes(), "%s: device %d differs" % (name, q)
+
+
+def _check_full_size(w, path=rs.RS_PATH_AUTO, n_samples=4096):
+    """full-size check in the bench's launch configuration: (1) every element of every dst shard equals
+    basic slicing of D with the ORACLE's box (on device), (2) sampled elements equal what the oracle's
+    per-element source map says, (3) values are a function of the global index, so (1) needs no source."""
+    e = inputs.elem_bytes(w.dtype)
+    D, src = gu.workload_on_device(w)
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, path)
+    dst = [torch.empty(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+    for t in dst:
+        t.view(torch.uint8).fill_(0x5A)
+    p.execute(gu.ptrs(src), gu.ptrs(dst), gu.stream())
+    torch.cuda.synchronize()
+    idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
+    for q in range(p.info.n_dst):
+        assert torch.equal(dst[q].view(torch.uint8), D[idx[q]].contiguous().view(torch.uint8)), "%s dev %d" % (w.name, q)
+    rng = np.random.default_rng(7)
+    n_local = int(np.prod(p.local_shape(rs.RS_DST)))
+    flat_src = [s.reshape(-1) for s in src]
+    for q in range(p.info.n_dst):
+        js = rng.integers(0, n_local, size=n_samples // p.info.n_dst + 1)
+        js[0], js[-1] = 0, n_local - 1
+        srcs = [do.element_source(w.shape, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, q, int(j)) for j in js]
+        got = dst[q].reshape(-1)[torch.from_numpy(js).to(gu.dev())].cpu()
+        want = torch.stack([flat_src[d][l] for d, l, _g in srcs]).cpu()
+        assert torch.equal(got.view(torch.uint8), want.view(torch.uint8))
+        gl = D.reshape(-1)[torch.tensor([g for _d, _l, g in srcs], device=gu.dev())].cpu()
+        assert torch.equal(got.view(torch.uint8), gl.view(torch.uint8))
+    return p
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config4_full_size(path):
+    _check_full_size(inputs.get_workload("c4"), path)
+
+
+@pytest.mark.parametrize("pair", sorted(inputs.SWEEP_PAIRS))
+@pytest.mark.parametrize("meshes", ["m8", "m4"])
+def test_sweep_1gib_full_size(pair, meshes):
+    _check_full_size(inputs.sweep_workload(pair, meshes, 1 << 30))
+
+
+@pytest.mark.parametrize("pair,meshes", [("P1", "m8"), ("P5", "m8"), ("P2", "m4"), ("P6", "m8")])
+def test_sweep_4gib_maximum_size(pair, meshes):
+    """2^31 elements: byte offsets beyond 2^32"""
+    _check_full_size(inputs.sweep_workload(pair, meshes, 4 << 30), n_samples=1024)
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("mib", [1, 4, 16, 64, 256])
+@pytest.mark.parametrize("pair", ["P1", "P2", "P5"])
+def test_sweep_small_sizes(pair, mib):
+    _check_full_size(inputs.sweep_workload(pair, "m8", mib << 20), n_samples=512)
+
+
+@pytest.mark.parametrize("case", [1, 2, 3, 4, 5, 7, 8, 9])
+def test_table2_cases_full_size(case):
+    """the paper's microbenchmark layouts on (1024,1024,512) at 2 B/elt"""
+    _check_full_size(inputs.table2_workload(case), n_samples=512)
+
+
+def test_a_to_b_to_a_is_identity_on_every_replica():
+    for name in ("c3ii", "c2", "t2_3"):
+        w = inputs.get_workload(name)
+        e = inputs.elem_bytes(w.dtype)
+        _D, src = gu.workload_on_device(w)
+        fwd = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+        bwd = rs.Plan(w.shape, e, w.dst_mesh, w.dst_spec, w.src_mesh, w.src_spec)
+        mid = [torch.empty(fwd.info.dst_shard_bytes, dtype=torch.uint8, device=gu.dev()) for _ in range(fwd.info.n_dst)]
+        back = [torch.zeros_like(s) for s in src]
+        fwd.execute(gu.ptrs(src), gu.ptrs(mid), gu.stream())
+        bwd.execute(gu.ptrs(mid), gu.ptrs(back), gu.stream())
+        torch.cuda.synchronize()
+        for a, b in zip(src, back):
+            assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("lb", [rs.RS_LB_GREEDY, rs.RS_LB_NAIVE])
+@pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK])
+def test_executed_sender_is_the_planned_sender(lb, path):
+    """R12: replicas carry their device id; what lands tells which replica the kernel read"""
+    for shape, sm, ss, dm, ds in [((8, 8, 64), (2, 4), "R,R,S0", (2, 4), "S0,R,R"), ((8, 8, 64), (2, 4), "R,R,R", (2, 4), "S0,S1,R"),
+                                  ((16, 8, 64), (2, 3), "RRR", (3, 2), "RRR"), ((24, 64), (2, 3), "S0,R", (3, 2), "S0,R")]:
+        p = rs.Plan(shape, 4, sm, ss, dm, ds, lb | path)
+        src = [torch.full(p.local_shape(rs.RS_SRC), r, dtype=torch.int32, device=gu.dev()) for r in range(p.info.n_src)]
+        dst = [torch.full(p.local_shape(rs.RS_DST), -1, dtype=torch.int32, device=gu.dev()) for _ in range(p.info.n_dst)]
+        p.execute(gu.ptrs(src), gu.ptrs(dst), gu.stream())
+        torch.cuda.synchronize()
+        for s in p.slices():
+            for q in s["receivers"]:
+                lo, _hi = do.device_box(shape, dm, ds, q)
+                box = tuple(slice(a - l, b - l) for a, b, l in zip(s["lo"], s["hi"], lo))
+                assert (dst[q][box] == s["sender"]).all()
+        assert all((d >= 0).all() for d in dst)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("case", [SMALL[i] for i in (2, 4, 5, 8, 10, 12, 15, 17)])
+def test_pack_unpack_equals_execute_equals_oracle(case, path):
+    shape, sm, ss, dm, ds = case
+    D = np.frombuffer(np.random.default_rng(3).bytes(int(np.prod(shape)) * 2), dtype=np.int16).reshape(shape)
+    src = do.shards_from_global(D, sm, ss)
+    want = do.reshard(shape, sm, ss, dm, ds, src)
+    p = rs.Plan(shape, 2, sm, ss, dm, ds, path)
+    src_d = [gu.to_dev(s) for s in src]
+    arena = torch.full((p.info.arena_bytes,), 0x77, dtype=torch.uint8, device=gu.dev())
+    dst_d = [torch.full((p.info.dst_shard_bytes,), 0x5A, dtype=torch.uint8, device=gu.dev()) for _ in want]
+    p.pack(gu.ptrs(src_d), arena.data_ptr(), gu.stream())
+    p.unpack(arena.data_ptr(), gu.ptrs(dst_d), gu.stream())
+    torch.cuda.synchronize()
+    for q, wq in enumerate(want):
+        assert dst_d[q].cpu().numpy().tobytes() == wq.tobytes()
+    # message contents: concatenation of the sender's boxes in slice-id order (plan oracle, numpy slicing)
+    tasks = po.unit_tasks(shape, sm, ss, dm, ds)
+    ref = po.pack_messages(shape, sm, ss, tasks, [s["sender"] for s in p.slices()], src)
+    host = arena.cpu().numpy()
+    used = np.zeros(host.size, bool)
+    for m, (s, r, payload) in zip(p.messages(), ref):
+        assert (m["sender"], m["receiver"]) == (s, r)
+        assert host[m["offset"]:m["offset"] + m["bytes"]].tobytes() == payload.tobytes()
+        used[m["offset"]:m["offset"] + m["bytes"]] = True
+    assert (host[~used] == 0x77).all()                               # padding between messages untouched
+
+
+def test_pack_unpack_full_size_c4_and_multicast():
+    for name in ("c4", "sweep_P5_m8_1024MiB"):
+        w = inputs.get_workload(name)
+        e = inputs.elem_bytes(w.dtype)
+        D, src = gu.workload_on_device(w)
+        p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+        arena = torch.empty(p.info.arena_bytes, dtype=torch.uint8, device=gu.dev())
+        dst = [torch.empty(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+        p.pack(gu.ptrs(src), arena.data_ptr(), gu.stream())
+        p.unpack(arena.data_ptr(), gu.ptrs(dst), gu.stream())
+        torch.cuda.synchronize()
+        idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
+        for q in range(p.info.n_dst):
+            assert torch.equal(dst[q], D[idx[q]])
+        del arena, dst, src, D
+        torch.cuda.empty_cache()
+
+
+def test_execute_host_buffers_and_side_stream():
+    w = inputs.get_workload("c3ii")
+    e = inputs.elem_bytes(w.dtype)
+    D = inputs.global_tensor(w)
+    src = do.shards_from_global(D, w.src_mesh, w.src_spec)
+    want = do.reshard(w.shape, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, src, n_threads=do.max_threads())
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    src_h = [torch.from_numpy(s.copy()).pin_memory() for s in src]
+    dst_h = [torch.empty(p.local_shape(rs.RS_DST), dtype=torch.int16).pin_memory() for _ in want]
+    ws = torch.empty(p.host_workspace_bytes(), dtype=torch.uint8, device=gu.dev())
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        up, down = p.execute_host(gu.ptrs(src_h), gu.ptrs(dst_h), ws.data_ptr(), side.cuda_stream)
+    side.synchronize()
+    assert up == p.info.tensor_bytes and down == p.info.write_bytes
+    for g, wq in zip(dst_h, want):
+        assert g.numpy().tobytes() == wq.tobytes()
+
+
+def test_one_launch_per_call_and_loud_failure():
+    p = rs.Plan((8, 8, 64), 2, (2, 4), "S0,R,S1", (2, 4), "S0,S1,R")
+    src = [torch.zeros(p.info.src_shard_bytes, dtype=torch.uint8, device=gu.dev()) for _ in range(8)]
+    dst = [torch.zeros(p.info.dst_shard_bytes, dtype=torch.uint8, device=gu.dev()) for _ in range(8)]
+    n0 = rs.launch_count()
+    p.execute(gu.ptrs(src), gu.ptrs(dst), gu.stream())
+    assert rs.launch_count() == n0 + 1                                # single-launch kernel (north_star item 2)
+    with pytest.raises(rs.ReshardError):
+        p.execute(gu.ptrs(src), [0] * 8, gu.stream())                 # null destination: refused, not skipped
+    torch.cuda.synchronize()
