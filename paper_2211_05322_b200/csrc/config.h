@@ -15,4 +15,6 @@
 #define RS_BULK_TILE_BYTES   16384      // bytes per ring slot
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 
+#define RS_BULK_DESC_BYTES   4096       // per-warp descriptor ring: 64 tiles x 64 bytes
+
 #define RS_SMEM_MAX          (227 * 1024)

@@ -158,13 +158,42 @@ __device__ __forceinline__ void bulk_wait_read(int pending) {  // immediate oper
     }
 }
 
+// Per-warp descriptor ring: everything one tile needs, resolved 32 tiles at a time (lane i resolves
+// the warp's tile it+i: tile record -> task -> base pointers), so the per-tile critical path has
+// no dependent global load -- one shared-memory broadcast read instead.
+struct alignas(16) RsDesc {
+    const char *src;                     // FAST: address of the tile's first source byte; GENERIC: box origin
+    int64_t dst_rel;                     // FAST: tile.b; GENERIC: byte offset inside the run
+    int64_t s0, d0;                      // row strides (FAST)
+    uint64_t lin;                        // GENERIC: linear index of the first row
+    uint32_t n_rows, col_bytes, flags, k, dst_first, task;
+};
+static_assert(sizeof(RsDesc) == 64, "descriptor ring slot");
+#define RS_DESC_RING 64
+
+__device__ __forceinline__ void generic_row(const RsTask *__restrict__ T, uint64_t lin, int64_t *so, int64_t *doff) {
+    int64_t s = 0, d = 0;
+    const int nd = T->nd;
+    for (int i = 0; i < nd; i++) {
+        uint32_t e = T->ext[i];
+        uint64_t q = lin / e;
+        uint32_t c = (uint32_t)(lin - q * e);
+        lin = q;
+        s += (int64_t)c * T->sstride[i];
+        d += (int64_t)c * T->dstride[i];
+    }
+    *so = s; *doff = d;
+}
+
 __global__ void __launch_bounds__(256, 1)
 rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const int stages, const int lookahead,
              const uint32_t stage_bytes) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const uint32_t bars = smem_u32(smem) + warp * 64;                       // <= 8 mbarriers per warp
-    const uint32_t ring = smem_u32(smem) + 1024 + (uint32_t)warp * stages * stage_bytes;
+    RsDesc *descs = reinterpret_cast<RsDesc *>(smem + 1024) + warp * RS_DESC_RING;
+    const uint32_t ring = smem_u32(smem) + 1024 + (uint32_t)W * RS_DESC_RING * sizeof(RsDesc) +
+                          (uint32_t)warp * stages * stage_bytes;
     if (lane == 0) {
         for (int s = 0; s < stages; s++) mbar_init(bars + 8 * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -174,46 +203,78 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const in
     const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
     const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
     const int pending_ok = stages - lookahead - 1;            // store groups that may still read smem
+    int ld_slot = 0, st_slot = 0;                             // it % stages, j % stages without dividing
+    uint32_t st_parity = 0;
 
     for (int it = 0; it < n_my + lookahead; ++it) {
-        if (it < n_my) {                                      // ---- load tile `it` into slot it % stages
-            const int s = it % stages;
+        if (it < n_my) {                                      // ---- load tile `it` into slot ld_slot
+            if ((it & 31) == 0) {                             // resolve the next 32 tiles of this warp
+                const int mine = it + lane;
+                if (mine < n_my) {
+                    const RsTile tile = load_tile(op.tiles, worker + (uint32_t)mine * n_workers);
+                    const RsTask *__restrict__ T = op.tasks + tile.task;
+                    RsDesc d;
+                    const char *base = ptrs.src[T->src_buf] + T->src_off;
+                    const bool fast = tile.flags & RS_TILE_FAST;
+                    d.src = fast ? base + tile.a : base;
+                    d.dst_rel = (int64_t)tile.b;
+                    d.s0 = T->sstride[0]; d.d0 = T->dstride[0];
+                    d.lin = tile.a;
+                    d.n_rows = tile.n_rows; d.col_bytes = tile.col_bytes; d.flags = tile.flags;
+                    d.k = (uint32_t)T->k; d.dst_first = (uint32_t)T->dst_first; d.task = tile.task;
+                    descs[mine & (RS_DESC_RING - 1)] = d;
+                }
+                __syncwarp();
+            }
             if (it >= stages) {                               // slot reuse: its stores must have read it
                 bulk_wait_read(pending_ok);
                 __syncwarp();
             }
-            const RsTile tile = load_tile(op.tiles, worker + (uint32_t)it * n_workers);
-            const RsTask *__restrict__ T = op.tasks + tile.task;
-            const char *src = ptrs.src[T->src_buf] + T->src_off;
-            const int64_t s0 = T->sstride[0], d0 = T->dstride[0];
-            const uint32_t bar = bars + 8 * s, slot = ring + (uint32_t)s * stage_bytes;
-            if (lane == 0) mbar_expect_tx(bar, tile.n_rows * tile.col_bytes);
+            const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
+            const uint32_t n_rows = d->n_rows, col_bytes = d->col_bytes;
+            const uint32_t bar = bars + 8 * ld_slot, slot = ring + (uint32_t)ld_slot * stage_bytes;
+            if (lane == 0) mbar_expect_tx(bar, n_rows * col_bytes);
             __syncwarp();
-            for (uint32_t r = lane; r < tile.n_rows; r += 32) {
-                int64_t so, doff;
-                row_offsets(tile, T, r, s0, d0, &so, &doff);
-                bulk_g2s(slot + r * tile.col_bytes, src + so, tile.col_bytes, bar);
+            if (d->flags & RS_TILE_FAST) {
+                const char *src = d->src;
+                const int64_t s0 = d->s0;
+                for (uint32_t r = lane; r < n_rows; r += 32)
+                    bulk_g2s(slot + r * col_bytes, src + (int64_t)r * s0, col_bytes, bar);
+            } else {
+                const RsTask *__restrict__ T = op.tasks + d->task;
+                for (uint32_t r = lane; r < n_rows; r += 32) {
+                    int64_t so, doff;
+                    generic_row(T, d->lin + r, &so, &doff);
+                    bulk_g2s(slot + r * col_bytes, d->src + d->dst_rel + so, col_bytes, bar);
+                }
             }
+            if (++ld_slot == stages) ld_slot = 0;
         }
         const int j = it - lookahead;
         if (j >= 0) {                                         // ---- store tile j to its k destinations
-            const int s = j % stages;
-            const RsTile tile = load_tile(op.tiles, worker + (uint32_t)j * n_workers);
-            const RsTask *__restrict__ T = op.tasks + tile.task;
-            const int k = T->k;
-            const RsDst *__restrict__ dsts = op.dsts + T->dst_first;
-            const int64_t s0 = T->sstride[0], d0 = T->dstride[0];
-            const uint32_t slot = ring + (uint32_t)s * stage_bytes;
-            mbar_wait(bars + 8 * s, (uint32_t)(j / stages) & 1u);
-            for (uint32_t r = lane; r < tile.n_rows; r += 32) {
-                int64_t so, doff;
-                row_offsets(tile, T, r, s0, d0, &so, &doff);
-                for (int q = 0; q < k; q++) {                 // read once, write k times
-                    const RsDst d = dsts[q];
-                    bulk_s2g(ptrs.dst[d.buf] + d.off + doff, slot + r * tile.col_bytes, tile.col_bytes);
+            const RsDesc *d = descs + (j & (RS_DESC_RING - 1));
+            const uint32_t n_rows = d->n_rows, col_bytes = d->col_bytes, k = d->k;
+            const RsDst *__restrict__ dsts = op.dsts + d->dst_first;
+            const uint32_t slot = ring + (uint32_t)st_slot * stage_bytes;
+            const bool fast = d->flags & RS_TILE_FAST;
+            const RsTask *__restrict__ T = op.tasks + d->task;
+            mbar_wait(bars + 8 * st_slot, st_parity);
+            for (uint32_t r = lane; r < n_rows; r += 32) {
+                int64_t doff;
+                if (fast) {
+                    doff = d->dst_rel + (int64_t)r * d->d0;
+                } else {
+                    int64_t so;
+                    generic_row(T, d->lin + r, &so, &doff);
+                    doff += d->dst_rel;
+                }
+                for (uint32_t q = 0; q < k; q++) {            // read once, write k times
+                    const RsDst dd = dsts[q];
+                    bulk_s2g(ptrs.dst[dd.buf] + dd.off + doff, slot + r * col_bytes, col_bytes);
                 }
             }
             bulk_commit();
+            if (++st_slot == stages) { st_slot = 0; st_parity ^= 1u; }
         }
     }
     bulk_wait_read(0);                                        // shared memory must outlive the stores' reads

@@ -174,7 +174,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         int stages = std::max(2, std::min(8, env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
         tile_bytes = env_int("RS_BULK_TILE_BYTES", RS_BULK_TILE_BYTES);
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
-        while ((int64_t)warps * stages * tile_bytes + 1024 > RS_SMEM_MAX && tile_bytes > 1024) tile_bytes -= 1024;
+        while ((int64_t)warps * (stages * tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && tile_bytes > 1024) tile_bytes -= 1024;
         I.block = warps * 32;
         I.grid = P->sm_count;
         workers = I.grid * warps;
@@ -203,7 +203,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         op->stages = stages;
         op->lookahead = std::max(1, std::min(stages - 1, env_int("RS_BULK_LOOKAHEAD", RS_BULK_LOOKAHEAD)));
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
-        I.smem_bytes = (int32_t)(warps * stages * tile_bytes + 1024);
+        I.smem_bytes = (int32_t)(warps * (stages * tile_bytes + RS_BULK_DESC_BYTES) + 1024);
     } else {
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, I.n_tiles));
         I.smem_bytes = 0;
