@@ -10,9 +10,9 @@
 
 // TMA path: cp.async.bulk global -> shared ring -> global x k; every warp is its own pipeline
 #define RS_BULK_WARPS        2          // warps (independent pipelines) per CTA, one CTA per SM
-#define RS_BULK_STAGES       6          // ring slots per warp
-#define RS_BULK_LOOKAHEAD    3          // loads in flight per warp before the first store is issued
-#define RS_BULK_TILE_BYTES   16384      // bytes per ring slot
+#define RS_BULK_STAGES       4          // ring slots per warp
+#define RS_BULK_LOOKAHEAD    2          // loads in flight per warp before the first store is issued
+#define RS_BULK_TILE_BYTES   12288      // bytes per ring slot
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 
 #define RS_BULK_DESC_BYTES   4096       // per-warp descriptor ring: 64 tiles x 64 bytes
