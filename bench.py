@@ -30,8 +30,8 @@ METRIC = "resharding GB/s (unique read+write bytes)"
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json: "~8 TB/s"; the >=70 % bar refers to this
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE rs_copy_* launch of reshard_execute, from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists)
-NCU_TRAFFIC_BYTES = {}
+# `ncu --set full` capture summarised in profiles/ (null for workloads without a capture)
+NCU_TRAFFIC_BYTES = {"c4": 1614862000 + 1564753000}     # profiles/r01_ncu_full_c4.md
 
 
 def parse_args():
@@ -91,7 +91,7 @@ def oracle_sample(w, seconds, steps=1, warmup=0):
             do.reshard_device(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, src, q % n_dst, ct,
                               n_threads=cores, out=out)
             q += 1
-            if time.perf_counter() - t0 >= seconds or q >= n_dst:
+            if time.perf_counter() - t0 >= seconds:
                 break
         dt = time.perf_counter() - t0
         if it >= warmup:
@@ -99,8 +99,8 @@ def oracle_sample(w, seconds, steps=1, warmup=0):
             shards_done = q
     t = statistics.median(times)
     return {"value": per_shard_metric_bytes / t / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
-            "sample": "%d of %d destination shards of %s (%.0f MiB each), all elements, %d threads, %.2f s per shard"
-                      % (shards_done, n_dst, w.name, shard_bytes / 2**20, cores, t),
+            "sample": "%d destination shards of %s computed in full (devices 0..%d cyclically, %.0f MiB each), %d threads, %.2f s per shard"
+                      % (shards_done, w.name, n_dst - 1, shard_bytes / 2**20, cores, t),
             "seconds_per_shard": t, "shards": shards_done}
 
 
