@@ -193,8 +193,7 @@ class ClockSampler:
 
 def run_ours(args):
     import torch
-    import torch.distributed as dist
-    from paper_2211_05322_b200 import harness, inputs
+    from paper_2211_05322_b200 import harness, inputs, multi
     from paper_2211_05322_b200 import reshard as rs
 
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
@@ -204,12 +203,10 @@ def run_ours(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        multi.init("nccl", dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        multi.barrier(torch.cuda.synchronize)
 
     w = inputs.get_workload(args.workload)
     flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK}[args.path]
@@ -269,12 +266,9 @@ def run_ours(args):
         total_ms = sum(e[0].elapsed_time(e[3]) for e in ev)
     k_ms = [statistics.mean(e[j].elapsed_time(e[j + 1]) for e in ev) for j in range(3)]
     k_best = [min(e[j].elapsed_time(e[j + 1]) for e in ev) for j in range(3)]
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = multi.max_over_ranks(total_ms, dev)
     ms_per_step = total_ms / K
-    value = world * step_bytes / (ms_per_step * 1e-3) / 1e9
+    value = multi.job_gbs(step_bytes, ms_per_step, world)
 
     # ---- end to end: host (pinned) shards in, host shards out, through reshard_execute_host
     e2e = None
@@ -297,18 +291,14 @@ def run_ours(args):
             stream.synchronize()                            # the caller reads the result on the host
         e1.record(stream)
         barrier()
-        t = torch.tensor([e0.elapsed_time(e1) / n_e2e], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-        e2e = {"value": world * op_bytes[0] / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": up,
+        e2e_ms = multi.max_over_ranks(e0.elapsed_time(e1) / n_e2e, dev)
+        e2e = {"value": multi.job_gbs(op_bytes[0], e2e_ms, world), "unit": "GB/s", "h2d_bytes_per_step": up,
                "d2h_bytes_per_step": down, "ms_per_step": e2e_ms, "steps": n_e2e,
                "call": "reshard_execute_host (pinned host shards -> H2D -> rs_copy kernel -> D2H)"}
         del src_h, dst_h, ws
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        multi.shutdown()
         return 0
 
     peak, peak_src = peak_hbm()
@@ -337,8 +327,7 @@ def run_ours(args):
         r = oracle_sample(w, args.cpu_seconds)
         line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    multi.shutdown()
     return 0
 
 
