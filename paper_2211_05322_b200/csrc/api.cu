@@ -243,7 +243,7 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     } else {                                                  // also the fallback for under-aligned pointers
         int grid = op.info.grid;
         if (op.info.path == RS_PATH_BULK)
-            grid = (int)std::min<int64_t>(op.info.n_tiles, (int64_t)P.sm_count * RS_LSU_CTAS_PER_SM);
+            grid = (int)std::max<int64_t>(1, std::min<int64_t>((op.info.n_tiles + 7) / 8, (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT));
         e = rs::launch_lsu(op.dev, pt, align, grid, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");

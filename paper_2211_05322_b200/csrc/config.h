@@ -4,9 +4,10 @@
 
 // register path: 128-bit ld.global -> st.global x k
 #define RS_LSU_THREADS       256
-#define RS_LSU_CTAS_PER_SM   8          // persistent CTAs per SM (grid = 148 * this)
-#define RS_LSU_TILE_BYTES    32768
-#define RS_LSU_UNROLL        4          // independent 16-byte loads in flight per thread
+#define RS_LSU_CTAS_PER_SM   4          // persistent CTAs per SM (grid = 148 * this); every warp is a worker
+#define RS_LSU_CTAS_DEFAULT  2          // CTAs per SM actually launched (more bytes in flight is slower on B200)
+#define RS_LSU_TILE_BYTES    16384
+#define RS_LSU_UNROLL        8          // independent vector loads in flight per thread
 
 // TMA path: cp.async.bulk global -> shared ring -> global x k; every warp is its own pipeline
 #define RS_BULK_WARPS        2          // warps (independent pipelines) per CTA, one CTA per SM

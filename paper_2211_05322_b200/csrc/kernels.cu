@@ -35,26 +35,48 @@ __device__ __forceinline__ RsTile load_tile(const RsTile *tiles, uint32_t t) {
     return r;
 }
 
-// byte offsets (relative to the task's box origin on each side) of byte 0 of row `row` of a tile
-__device__ __forceinline__ void row_offsets(const RsTile &tile, const RsTask *__restrict__ T, uint32_t row,
-                                            int64_t s0, int64_t d0, int64_t *so, int64_t *doff) {
-    if (tile.flags & RS_TILE_FAST) {
-        *so = (int64_t)tile.a + (int64_t)row * s0;
-        *doff = (int64_t)tile.b + (int64_t)row * d0;
-    } else {                                                  // GENERIC: decode the linear row index
-        uint64_t lin = tile.a + row;
-        int64_t s = (int64_t)tile.b, d = (int64_t)tile.b;
-        const int nd = T->nd;
-        for (int i = 0; i < nd; i++) {
-            uint32_t e = T->ext[i];
-            uint64_t q = lin / e;
-            uint32_t c = (uint32_t)(lin - q * e);
-            lin = q;
-            s += (int64_t)c * T->sstride[i];
-            d += (int64_t)c * T->dstride[i];
-        }
-        *so = s; *doff = d;
+// Per-warp descriptor ring: everything one tile needs, resolved 32 tiles at a time (lane i resolves
+// the warp's tile it+i: tile record -> task -> base pointers), so the per-tile critical path has
+// no dependent global load -- one shared-memory broadcast read instead.
+struct alignas(16) RsDesc {
+    const char *src;                     // FAST: address of the tile's first source byte; GENERIC: box origin
+    int64_t dst_rel;                     // FAST: tile.b; GENERIC: byte offset inside the run
+    int64_t s0, d0;                      // row strides (FAST)
+    uint64_t lin;                        // GENERIC: linear index of the first row
+    uint32_t n_rows, col_bytes, flags, k, dst_first, task;
+};
+static_assert(sizeof(RsDesc) == 64, "descriptor ring slot");
+#define RS_DESC_RING 64
+static_assert(RS_DESC_RING * sizeof(RsDesc) == RS_BULK_DESC_BYTES, "config.h and the ring disagree");
+
+__device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsPtrTable &ptrs, uint32_t tile_index,
+                                             RsDesc *out) {
+    const RsTile tile = load_tile(op.tiles, tile_index);
+    const RsTask *__restrict__ T = op.tasks + tile.task;
+    RsDesc d;
+    const char *base = ptrs.src[T->src_buf] + T->src_off;
+    d.src = (tile.flags & RS_TILE_FAST) ? base + tile.a : base;
+    d.dst_rel = (int64_t)tile.b;
+    d.s0 = T->sstride[0]; d.d0 = T->dstride[0];
+    d.lin = tile.a;
+    d.n_rows = tile.n_rows; d.col_bytes = tile.col_bytes; d.flags = tile.flags;
+    d.k = (uint32_t)T->k; d.dst_first = (uint32_t)T->dst_first; d.task = tile.task;
+    *out = d;
+}
+
+// GENERIC tiles: byte offsets of linear row `lin` of a task's box, relative to the box origin on each side
+__device__ __forceinline__ void generic_row(const RsTask *__restrict__ T, uint64_t lin, int64_t *so, int64_t *doff) {
+    int64_t s = 0, d = 0;
+    const int nd = T->nd;
+    for (int i = 0; i < nd; i++) {
+        uint32_t e = T->ext[i];
+        uint64_t q = lin / e;
+        uint32_t c = (uint32_t)(lin - q * e);
+        lin = q;
+        s += (int64_t)c * T->sstride[i];
+        d += (int64_t)c * T->dstride[i];
     }
+    *so = s; *doff = d;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -77,41 +99,70 @@ template <> __device__ __forceinline__ void st_stream<uint4>(char *p, const uint
                  :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// Every WARP is an independent worker (no CTA-wide synchronisation anywhere).  Inside a tile the
+// warp walks the (row, column) grid of V-sized vectors 32 at a time; (row, col) advance incrementally,
+// so the only integer division is one per tile.  U loads are issued back to back, then U x k stores.
 template <typename V, int U>
-__global__ void __launch_bounds__(RS_LSU_THREADS)
+__global__ void __launch_bounds__(RS_LSU_THREADS, RS_LSU_CTAS_PER_SM)
 rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs) {
     constexpr uint32_t VB = sizeof(V);
-    for (uint32_t t = blockIdx.x; t < op.n_tiles; t += gridDim.x) {
-        const RsTile tile = load_tile(op.tiles, t);
-        const RsTask *__restrict__ T = op.tasks + tile.task;
-        const int k = T->k;
-        const RsDst *__restrict__ dsts = op.dsts + T->dst_first;
-        const char *src = ptrs.src[T->src_buf] + T->src_off;
-        const int64_t s0 = T->sstride[0], d0 = T->dstride[0];
-        const uint32_t vpr = tile.col_bytes / VB;             // vectors per row
-        const uint32_t total = tile.n_rows * vpr;
-        for (uint32_t v0 = threadIdx.x; v0 < total; v0 += RS_LSU_THREADS * U) {
-            V data[U];
-            int64_t doff[U];
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                const uint32_t v = v0 + u * RS_LSU_THREADS;
-                if (v < total) {
-                    const uint32_t row = tile.n_rows == 1 ? 0u : v / vpr;
-                    const uint32_t col = v - row * vpr;
-                    int64_t so;
-                    row_offsets(tile, T, row, s0, d0, &so, &doff[u]);
-                    doff[u] += (int64_t)col * VB;
-                    data[u] = ld_stream<V>(src + so + (int64_t)col * VB);
+    __shared__ RsDesc ring[RS_LSU_THREADS / 32][32];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = RS_LSU_THREADS / 32;
+    RsDesc *descs = ring[warp];
+    const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
+    const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
+
+    for (int it = 0; it < n_my; ++it) {
+        if ((it & 31) == 0) {                                 // resolve the next 32 tiles of this warp
+            __syncwarp();
+            if (it + lane < n_my) resolve_desc(op, ptrs, worker + (uint32_t)(it + lane) * n_workers, descs + lane);
+            __syncwarp();
+        }
+        const RsDesc *d = descs + (it & 31);
+        const uint32_t n_rows = d->n_rows, k = d->k;
+        const uint32_t vpr = d->col_bytes / VB;               // vectors per row
+        const uint32_t total = n_rows * vpr;
+        const RsDst *__restrict__ dsts = op.dsts + d->dst_first;
+        const bool fast = d->flags & RS_TILE_FAST;
+        const char *src = d->src;
+        const int64_t s0 = d->s0, d0 = d->d0, dst_rel = d->dst_rel;
+        const RsTask *__restrict__ T = op.tasks + d->task;
+        if (!fast) {                                          // GENERIC tiles (rare): one vector at a time
+            for (uint32_t v = lane; v < total; v += 32) {
+                const uint32_t r = v / vpr, c = v - r * vpr;
+                int64_t so, doff;
+                generic_row(T, d->lin + r, &so, &doff);
+                const V x = ld_stream<V>(src + dst_rel + so + (int64_t)c * VB);
+                for (uint32_t j = 0; j < k; j++) {
+                    const RsDst dd = dsts[j];
+                    st_stream<V>(ptrs.dst[dd.buf] + dd.off + dst_rel + doff + (int64_t)c * VB, x);
                 }
             }
-            for (int j = 0; j < k; j++) {                     // read once, write k times
-                const RsDst d = dsts[j];
-                char *dp = ptrs.dst[d.buf] + d.off;
+            continue;
+        }
+        const uint32_t q32 = 32u / vpr, r32 = 32u - q32 * vpr;   // how (row, col) move when v += 32
+        uint32_t row = (uint32_t)lane / vpr, col = (uint32_t)lane - row * vpr;
+        for (uint32_t v0 = lane; v0 < total; v0 += 32 * U) {
+            V data[U];
+            uint32_t r = row, c = col;
 #pragma unroll
-                for (int u = 0; u < U; u++)
-                    if (v0 + u * RS_LSU_THREADS < total) st_stream<V>(dp + doff[u], data[u]);
+            for (int u = 0; u < U; u++) {                     // U independent loads in flight
+                if (v0 + 32 * u < total) data[u] = ld_stream<V>(src + (int64_t)r * s0 + (int64_t)c * VB);
+                r += q32; c += r32;
+                if (c >= vpr) { c -= vpr; r++; }
             }
+            for (uint32_t j = 0; j < k; j++) {                // read once, write k times
+                const RsDst dd = dsts[j];
+                char *dp = ptrs.dst[dd.buf] + dd.off + dst_rel;
+                uint32_t r2 = row, c2 = col;                  // offsets are recomputed, not kept in registers
+#pragma unroll
+                for (int u = 0; u < U; u++) {
+                    if (v0 + 32 * u < total) st_stream<V>(dp + (int64_t)r2 * d0 + (int64_t)c2 * VB, data[u]);
+                    r2 += q32; c2 += r32;
+                    if (c2 >= vpr) { c2 -= vpr; r2++; }
+                }
+            }
+            row = r; col = c;
         }
     }
 }
@@ -158,33 +209,6 @@ __device__ __forceinline__ void bulk_wait_read(int pending) {  // immediate oper
     }
 }
 
-// Per-warp descriptor ring: everything one tile needs, resolved 32 tiles at a time (lane i resolves
-// the warp's tile it+i: tile record -> task -> base pointers), so the per-tile critical path has
-// no dependent global load -- one shared-memory broadcast read instead.
-struct alignas(16) RsDesc {
-    const char *src;                     // FAST: address of the tile's first source byte; GENERIC: box origin
-    int64_t dst_rel;                     // FAST: tile.b; GENERIC: byte offset inside the run
-    int64_t s0, d0;                      // row strides (FAST)
-    uint64_t lin;                        // GENERIC: linear index of the first row
-    uint32_t n_rows, col_bytes, flags, k, dst_first, task;
-};
-static_assert(sizeof(RsDesc) == 64, "descriptor ring slot");
-#define RS_DESC_RING 64
-
-__device__ __forceinline__ void generic_row(const RsTask *__restrict__ T, uint64_t lin, int64_t *so, int64_t *doff) {
-    int64_t s = 0, d = 0;
-    const int nd = T->nd;
-    for (int i = 0; i < nd; i++) {
-        uint32_t e = T->ext[i];
-        uint64_t q = lin / e;
-        uint32_t c = (uint32_t)(lin - q * e);
-        lin = q;
-        s += (int64_t)c * T->sstride[i];
-        d += (int64_t)c * T->dstride[i];
-    }
-    *so = s; *doff = d;
-}
-
 __global__ void __launch_bounds__(256, 1)
 rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const int stages, const int lookahead,
              const uint32_t stage_bytes) {
@@ -210,20 +234,8 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const in
         if (it < n_my) {                                      // ---- load tile `it` into slot ld_slot
             if ((it & 31) == 0) {                             // resolve the next 32 tiles of this warp
                 const int mine = it + lane;
-                if (mine < n_my) {
-                    const RsTile tile = load_tile(op.tiles, worker + (uint32_t)mine * n_workers);
-                    const RsTask *__restrict__ T = op.tasks + tile.task;
-                    RsDesc d;
-                    const char *base = ptrs.src[T->src_buf] + T->src_off;
-                    const bool fast = tile.flags & RS_TILE_FAST;
-                    d.src = fast ? base + tile.a : base;
-                    d.dst_rel = (int64_t)tile.b;
-                    d.s0 = T->sstride[0]; d.d0 = T->dstride[0];
-                    d.lin = tile.a;
-                    d.n_rows = tile.n_rows; d.col_bytes = tile.col_bytes; d.flags = tile.flags;
-                    d.k = (uint32_t)T->k; d.dst_first = (uint32_t)T->dst_first; d.task = tile.task;
-                    descs[mine & (RS_DESC_RING - 1)] = d;
-                }
+                if (mine < n_my)
+                    resolve_desc(op, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
                 __syncwarp();
             }
             if (it >= stages) {                               // slot reuse: its stores must have read it
@@ -288,7 +300,8 @@ int64_t launch_count() { return g_launches; }
 
 template <typename V>
 static cudaError_t launch_lsu_t(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st) {
-    rs_copy_lsu<V, RS_LSU_UNROLL><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
+    constexpr int U = sizeof(V) == 16 ? RS_LSU_UNROLL / 2 : RS_LSU_UNROLL;   // 64 B in flight per thread
+    rs_copy_lsu<V, U><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
     return cudaGetLastError();
 }
 

@@ -182,8 +182,8 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         tile_bytes = env_int("RS_LSU_TILE_BYTES", RS_LSU_TILE_BYTES);
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
         I.block = RS_LSU_THREADS;
-        I.grid = P->sm_count * std::max(1, env_int("RS_LSU_CTAS_PER_SM", RS_LSU_CTAS_PER_SM));
-        workers = I.grid;
+        I.grid = P->sm_count * std::max(1, std::min(RS_LSU_CTAS_PER_SM, env_int("RS_LSU_CTAS_PER_SM", RS_LSU_CTAS_DEFAULT)));
+        workers = I.grid * (RS_LSU_THREADS / 32);
     }
     // small problems: shrink tiles until every worker has a few (tail balance), floor 2 KiB
     while (tile_bytes > 2048 && read_bytes / tile_bytes < (int64_t)workers * 4) tile_bytes = tile_bytes / 2 / 128 * 128;
@@ -205,7 +205,8 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
         I.smem_bytes = (int32_t)(warps * (stages * tile_bytes + RS_BULK_DESC_BYTES) + 1024);
     } else {
-        I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, I.n_tiles));
+        const int warps = RS_LSU_THREADS / 32;
+        I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
         I.smem_bytes = 0;
     }
     return RS_OK;
