@@ -281,7 +281,9 @@ def run_ours(args):
         shp, dhp = harness.ptrs(src_h), harness.ptrs(dst_h)
         up = down = 0
         for _ in range(2):
+            c0 = rs.launch_count()
             up, down = plan.execute_host(shp, dhp, ws.data_ptr(), sh)
+            n_slabs = rs.launch_count() - c0                 # one kernel launch per slab
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         n_e2e = max(1, args.e2e_steps)
@@ -294,7 +296,7 @@ def run_ours(args):
         e2e_ms = multi.max_over_ranks(e0.elapsed_time(e1) / n_e2e, dev)
         e2e = {"value": multi.job_gbs(op_bytes[0], e2e_ms, world), "unit": "GB/s", "h2d_bytes_per_step": up,
                "d2h_bytes_per_step": down, "ms_per_step": e2e_ms, "steps": n_e2e,
-               "call": "reshard_execute_host (pinned host shards -> H2D -> rs_copy kernel -> D2H)"}
+               "call": "reshard_execute_host (pinned host shards; H2D, kernel and D2H pipelined over %d slabs of dim 0)" % n_slabs}
         del src_h, dst_h, ws
 
     if rank != 0:

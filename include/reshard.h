@@ -78,7 +78,8 @@ enum {
 #define RS_PATH_MASK 0xF0
 
 /* operations a plan can run */
-enum { RS_OP_EXECUTE = 0, RS_OP_PACK = 1, RS_OP_UNPACK = 2 };
+enum { RS_OP_EXECUTE = 0, RS_OP_PACK = 1, RS_OP_UNPACK = 2,
+       RS_OP_EXECUTE_SLABS = 3 /* execute cut into dim-0 slabs: the table reshard_execute_host runs (queries only) */ };
 /* sides */
 enum { RS_SRC = 0, RS_DST = 1 };
 
@@ -176,9 +177,13 @@ RS_API rs_status reshard_pack(const rs_plan *plan, const void *const *src_shards
 RS_API rs_status reshard_unpack(const rs_plan *plan, const void *msg_arena, void *const *dst_shards, void *cuda_stream);
 
 /*
- * reshard_execute_host -- the same operation with HOST shard buffers (the end-to-end call):
- * copies the source shards the plan reads host->device into `workspace`, runs the execute kernel,
- * copies every destination shard device->host; all on `cuda_stream`, returns without synchronising.
+ * reshard_execute_host -- the same operation with HOST shard buffers (the end-to-end call).
+ * Pipelined over slabs of tensor dim 0 (the chunk pipelining of PAPER.md:137 applied to the host
+ * link): slab c of the source shards the plan reads is copied host->device into `workspace` on a
+ * plan-owned upload stream, resharded by one kernel launch on `cuda_stream`, and its destination
+ * byte ranges are copied device->host on a plan-owned download stream while slab c+1 uploads.
+ * All work is ordered after prior work on `cuda_stream`, and `cuda_stream` waits for the last
+ * download; returns without synchronising.  Not reentrant per plan (the plan owns the side streams).
  *   src_shards_host [HOST array of n_src HOST pointers]  (pinned memory makes the copies async)
  *   dst_shards_host [HOST array of n_dst HOST pointers]
  *   workspace [DEVICE]  at least reshard_host_workspace_bytes(plan) bytes, 256-byte aligned

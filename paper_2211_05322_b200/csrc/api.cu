@@ -66,6 +66,19 @@ rs_status upload(rs::Plan *P) {
     for (rs::OpTables &o : P->op) smem = std::max(smem, (int)RS_SMEM_MAX);
     e = rs::prepare_bulk(smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(rs_copy_bulk)");
+    // reshard_execute_host pipeline: plan-owned upload / download streams and per-slab events
+    for (int i = 0; i < 2; i++) {
+        cudaStream_t st;
+        e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
+        P->streams[i] = st;
+    }
+    for (size_t i = 0; i < 2 * P->slabs.size() + 2; i++) {
+        cudaEvent_t ev;
+        e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
+        P->events.push_back(ev);
+    }
     return RS_OK;
 }
 
@@ -106,6 +119,8 @@ rs_status reshard_plan(const int64_t *global_shape, int32_t ndim, int32_t elem_b
 
 void reshard_plan_destroy(rs_plan *plan) {
     if (!plan) return;
+    for (void *ev : plan->p.events) cudaEventDestroy(static_cast<cudaEvent_t>(ev));
+    for (void *st : plan->p.streams) if (st) cudaStreamDestroy(static_cast<cudaStream_t>(st));
     if (plan->p.dev_blob) cudaFree(plan->p.dev_blob);
     delete plan;
 }
@@ -135,13 +150,13 @@ rs_status reshard_plan_info(const rs_plan *plan, rs_plan_info *out) {
 }
 
 rs_status reshard_op_info(const rs_plan *plan, int32_t op, rs_op_info *out) {
-    if (!plan || !out || op < 0 || op > 2) return RS_EINVAL;
+    if (!plan || !out || op < 0 || op >= rs::RS_N_OPS) return RS_EINVAL;
     *out = plan->p.op[op].info;
     return RS_OK;
 }
 
 rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *dsts, void *tiles) {
-    if (!plan || op < 0 || op > 2) return RS_EINVAL;
+    if (!plan || op < 0 || op >= rs::RS_N_OPS) return RS_EINVAL;
     const rs::OpTables &o = plan->p.op[op];
     if (tasks) std::memcpy(tasks, o.tasks.data(), o.tasks.size() * sizeof(RsTask));
     if (dsts) std::memcpy(dsts, o.dsts.data(), o.dsts.size() * sizeof(RsDst));
@@ -215,7 +230,7 @@ int ptr_align(const void *p) {
 
 // one launch of operation `opi` on the given buffers
 rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src, void *const *dst, int n_dst,
-                 const char *used_src, void *stream) {
+                 const char *used_src, void *stream, uint32_t tile_begin = 0, uint32_t tile_end = 0) {
     rs::set_error("");
     if (!plan || !src || !dst) { rs::set_error("null argument"); return RS_EINVAL; }
     const rs::Plan &P = plan->p;
@@ -237,14 +252,18 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaError_t e;
+    RsOpDev dev = op.dev;
+    if (tile_end > tile_begin) { dev.tiles += tile_begin; dev.n_tiles = tile_end - tile_begin; }   // one slab
+    const int64_t n_tiles = dev.n_tiles;
     if (op.info.path == RS_PATH_BULK && align == 16) {
-        e = rs::launch_bulk(op.dev, pt, op.info.grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
+        const int warps = op.info.block / 32;
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
+        e = rs::launch_bulk(dev, pt, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                             (uint32_t)op.info.tile_bytes, st);
     } else {                                                  // also the fallback for under-aligned pointers
-        int grid = op.info.grid;
-        if (op.info.path == RS_PATH_BULK)
-            grid = (int)std::max<int64_t>(1, std::min<int64_t>((op.info.n_tiles + 7) / 8, (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT));
-        e = rs::launch_lsu(op.dev, pt, align, grid, st);
+        const int64_t cap = op.info.path == RS_PATH_BULK ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));
+        e = rs::launch_lsu(dev, pt, align, grid, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
     return RS_OK;
@@ -290,32 +309,65 @@ rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shard
     if (!P.dev_blob) { rs::set_error("plan was built with RS_HOST_ONLY"); return RS_EINVAL; }
     if (ptr_align(workspace) < 16) { rs::set_error("workspace must be 256-byte aligned"); return RS_EINVAL; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaStream_t up_st = static_cast<cudaStream_t>(P.streams[0]), down_st = static_cast<cudaStream_t>(P.streams[1]);
     const size_t sb = (size_t)(P.A.shard_elems() * P.elem_bytes), db = (size_t)(P.B.shard_elems() * P.elem_bytes);
     const void *src_dev[RS_MAX_DEVICES];
     void *dst_dev[RS_MAX_DEVICES];
     char *w = static_cast<char *>(workspace);
-    int64_t up = 0, down = 0;
-    // Replicas are identical by precondition, so only the shards the chosen senders read are uploaded:
-    // the bytes crossing the link are the lower bound size(D).
+    // Replicas are identical by precondition, so only shards the chosen senders read get device space and
+    // uploads: the bytes crossing the link are the lower bound size(D).
     for (int r = 0; r < P.A.n_dev; r++) {
         src_dev[r] = nullptr;
         if (!P.used_src[(size_t)r]) continue;
         if (!src_shards_host[r]) { rs::set_error("a source shard pointer the plan reads is null"); return RS_EINVAL; }
-        cudaError_t e = cudaMemcpyAsync(w, src_shards_host[r], sb, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(H2D)");
         src_dev[r] = w;
         w += round256(sb);
-        up += (int64_t)sb;
     }
-    for (int q = 0; q < P.B.n_dev; q++) { dst_dev[q] = w; w += round256(db); }
-    rs_status rc = run_op(plan, RS_OP_EXECUTE, src_dev, P.A.n_dev, dst_dev, P.B.n_dev, P.used_src.data(), cuda_stream);
-    if (rc != RS_OK) return rc;
     for (int q = 0; q < P.B.n_dev; q++) {
         if (!dst_shards_host[q]) { rs::set_error("a destination pointer is null"); return RS_EINVAL; }
-        cudaError_t e = cudaMemcpyAsync(dst_shards_host[q], dst_dev[q], db, cudaMemcpyDeviceToHost, st);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(D2H)");
-        down += (int64_t)db;
+        dst_dev[q] = w;
+        w += round256(db);
     }
+    // Pipeline over slabs of tensor dim 0 (PAPER.md:137's chunk pipelining, applied to the host link):
+    //   upload stream:   H2D slab 0 | H2D slab 1 | ...
+    //   caller's stream:            | kernel 0   | kernel 1 | ...
+    //   download stream:                         | D2H 0    | D2H 1 | ...
+    auto ev = [&](size_t i) { return static_cast<cudaEvent_t>(P.events[i]); };
+    const size_t n = P.slabs.size();
+    cudaError_t e = cudaEventRecord(ev(2 * n), st);            // everything is ordered after the caller's prior work
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(up_st, ev(2 * n), 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(down_st, ev(2 * n), 0);
+    if (e != cudaSuccess) return cuda_fail(e, "stream fork");
+    int64_t up = 0, down = 0;
+    for (size_t c = 0; c < n; c++) {
+        const rs::HostSlab &S = P.slabs[c];
+        for (const rs::HostCopy &h : S.up) {
+            e = cudaMemcpyAsync(const_cast<char *>(static_cast<const char *>(src_dev[h.dev])) + h.off,
+                                static_cast<const char *>(src_shards_host[h.dev]) + h.off, (size_t)h.bytes,
+                                cudaMemcpyHostToDevice, up_st);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(H2D)");
+            up += h.bytes;
+        }
+        if ((e = cudaEventRecord(ev(2 * c), up_st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+        if ((e = cudaStreamWaitEvent(st, ev(2 * c), 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
+        if (S.tile_end > S.tile_begin) {
+            rs_status rc = run_op(plan, rs::RS_OP_SLABS, src_dev, P.A.n_dev, dst_dev, P.B.n_dev, P.used_src.data(),
+                                  cuda_stream, S.tile_begin, S.tile_end);
+            if (rc != RS_OK) return rc;
+        }
+        if ((e = cudaEventRecord(ev(2 * c + 1), st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+        if ((e = cudaStreamWaitEvent(down_st, ev(2 * c + 1), 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
+        for (const rs::HostCopy &h : S.down) {
+            e = cudaMemcpyAsync(static_cast<char *>(dst_shards_host[h.dev]) + h.off,
+                                static_cast<char *>(dst_dev[h.dev]) + h.off, (size_t)h.bytes, cudaMemcpyDeviceToHost,
+                                down_st);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(D2H)");
+            down += h.bytes;
+        }
+    }
+    e = cudaEventRecord(ev(2 * n + 1), down_st);               // join: the caller's stream sees the downloads
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev(2 * n + 1), 0);
+    if (e != cudaSuccess) return cuda_fail(e, "stream join");
     if (h2d_bytes) *h2d_bytes = up;
     if (d2h_bytes) *d2h_bytes = down;
     return RS_OK;

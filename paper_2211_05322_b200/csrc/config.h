@@ -18,4 +18,8 @@
 
 #define RS_BULK_DESC_BYTES   4096       // per-warp descriptor ring: 64 tiles x 64 bytes
 
+// reshard_execute_host: pipeline over slabs of tensor dim 0
+#define RS_HOST_SLABS_MAX        16
+#define RS_HOST_SLAB_MIN_BYTES  (8 << 20)
+
 #define RS_SMEM_MAX          (227 * 1024)

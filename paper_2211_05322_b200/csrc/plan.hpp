@@ -53,6 +53,18 @@ struct OpTables {                        // one operation (execute / pack / unpa
     RsOpDev dev{};                       // device copies (null for a host-only plan)
 };
 
+struct HostCopy {                        // one contiguous host<->device copy of a shard byte range
+    int dev;                             // device id on its side
+    int64_t off, bytes;                  // inside the shard
+};
+
+struct HostSlab {                        // one stage of the reshard_execute_host pipeline: a slab of tensor dim 0
+    uint32_t tile_begin = 0, tile_end = 0;       // range in op[RS_OP_SLABS].tiles
+    std::vector<HostCopy> up, down;      // source ranges to upload before, destination ranges to download after
+};
+
+enum { RS_OP_SLABS = 3, RS_N_OPS = 4 };  // internal 4th table: execute, cut into dim-0 slabs
+
 struct Plan {
     Layout A, B;
     int elem_bytes = 0;
@@ -63,7 +75,10 @@ struct Plan {
     std::vector<Message> messages;
     int64_t arena_bytes = 0;
     int64_t r_B = 1;                     // destination replication factor
-    OpTables op[3];
+    OpTables op[RS_N_OPS];
+    std::vector<HostSlab> slabs;         // reshard_execute_host pipeline (PAPER.md:137's chunked pipelining, over PCIe)
+    void *streams[2] = {nullptr, nullptr};   // plan-owned upload / download streams (cudaStream_t)
+    std::vector<void *> events;          // plan-owned cudaEvent_t: 2 per slab + 2
     std::vector<char> used_src;          // [n_src] 1 if some task reads that shard
     int device = -1;
     int sm_count = 148;

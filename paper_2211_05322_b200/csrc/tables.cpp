@@ -139,7 +139,8 @@ void emit_tiles(const RsTask &T, uint32_t task_id, int64_t tile_bytes, std::vect
 }
 
 // Alignment class, path, tile size, grid of one operation; then its tile table.
-rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes) {
+rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes,
+                    std::vector<uint32_t> *task_tile_begin = nullptr) {
     int64_t align = 16, min_run = INT64_MAX, max_rows = 0;
     for (const RsTask &T : op->tasks) {
         align = std::min(align, pow2_align(T.run_bytes));
@@ -191,7 +192,11 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     I.tile_bytes = (int32_t)tile_bytes;
 
     op->tiles.clear();
-    for (size_t t = 0; t < op->tasks.size(); t++) emit_tiles(op->tasks[t], (uint32_t)t, tile_bytes, &op->tiles);
+    for (size_t t = 0; t < op->tasks.size(); t++) {
+        if (task_tile_begin) task_tile_begin->push_back((uint32_t)op->tiles.size());
+        emit_tiles(op->tasks[t], (uint32_t)t, tile_bytes, &op->tiles);
+    }
+    if (task_tile_begin) task_tile_begin->push_back((uint32_t)op->tiles.size());
     if (op->tiles.size() > 0x7FFFFFFFull) { set_error("tile table too large"); return RS_EUNSUPPORTED; }
     I.n_tiles = (int32_t)op->tiles.size();
     int64_t mr = INT64_MAX;
@@ -208,6 +213,77 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         const int warps = RS_LSU_THREADS / 32;
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
         I.smem_bytes = 0;
+    }
+    return RS_OK;
+}
+
+// reshard_execute_host pipeline: cut tensor dim 0 into slabs.  Dim 0 is the outermost dim of every
+// local layout, so a slab is ONE contiguous byte range in each source shard and each destination
+// shard it touches: slab c can be uploaded, resharded and downloaded while slab c+1 is uploading.
+// This is the paper's chunked pipelining (K chunks) applied to the host link.
+rs_status build_slabs(Plan *P, const int64_t *sA, const int64_t *sB, int64_t tensor_bytes) {
+    const Layout &A = P->A, &B = P->B;
+    const int N = A.ndim;
+    const int64_t e = P->elem_bytes, l0 = A.shape[0];
+    OpTables &H = P->op[RS_OP_SLABS];
+    H.tasks.clear(); H.dsts.clear(); H.tiles.clear();
+    P->slabs.clear();
+    int64_t C = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(l0, RS_HOST_SLABS_MAX),
+                                                       tensor_bytes / RS_HOST_SLAB_MIN_BYTES));
+    std::vector<int64_t> bound((size_t)C + 1);
+    for (int64_t c = 0; c <= C; c++) bound[(size_t)c] = c * l0 / C;
+    std::vector<uint32_t> task_slab;
+    for (int64_t c = 0; c < C; c++) {
+        const int64_t b0 = bound[(size_t)c], b1 = bound[(size_t)c + 1];
+        HostSlab S;
+        std::vector<char> up_used((size_t)A.n_dev, 0);
+        for (size_t i = 0; i < P->slices.size(); i++) {
+            const Slice &sl = P->slices[i];
+            int64_t lo[RS_MAX_NDIM], hi[RS_MAX_NDIM];
+            for (int d = 0; d < N; d++) { lo[d] = sl.lo[d]; hi[d] = sl.hi[d]; }
+            lo[0] = std::max(lo[0], b0); hi[0] = std::min(hi[0], b1);
+            if (lo[0] >= hi[0]) continue;
+            int64_t lo_s[RS_MAX_NDIM], hi_s[RS_MAX_NDIM];
+            device_box(A, sl.sender, lo_s, hi_s);
+            BoxDesc bx;
+            bx.ndim = N;
+            for (int d = 0; d < N; d++) { bx.ext[d] = hi[d] - lo[d]; bx.sstride[d] = sA[d]; bx.dstride[d] = sB[d]; }
+            RsTask T{};
+            if (!collapse(bx, e, &T)) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+            T.src_buf = sl.sender; T.src_off = box_offset(lo, lo_s, sA, N);
+            T.k = (int32_t)sl.receivers.size(); T.dst_first = (int32_t)H.dsts.size();
+            for (int r : sl.receivers) {
+                int64_t lo_r[RS_MAX_NDIM], hi_r[RS_MAX_NDIM];
+                device_box(B, r, lo_r, hi_r);
+                H.dsts.push_back(RsDst{box_offset(lo, lo_r, sB, N), r, 0});
+            }
+            H.tasks.push_back(T);
+            task_slab.push_back((uint32_t)c);
+            up_used[(size_t)sl.sender] = 1;
+        }
+        for (int r = 0; r < A.n_dev; r++) {                   // byte range of the slab inside every shard read
+            if (!up_used[(size_t)r]) continue;
+            int64_t lo_s[RS_MAX_NDIM], hi_s[RS_MAX_NDIM];
+            device_box(A, r, lo_s, hi_s);
+            int64_t a = std::max(b0, lo_s[0]), b = std::min(b1, hi_s[0]);
+            if (a < b) S.up.push_back(HostCopy{r, (a - lo_s[0]) * sA[0], (b - a) * sA[0]});
+        }
+        for (int q = 0; q < B.n_dev; q++) {
+            int64_t lo_r[RS_MAX_NDIM], hi_r[RS_MAX_NDIM];
+            device_box(B, q, lo_r, hi_r);
+            int64_t a = std::max(b0, lo_r[0]), b = std::min(b1, hi_r[0]);
+            if (a < b) S.down.push_back(HostCopy{q, (a - lo_r[0]) * sB[0], (b - a) * sB[0]});
+        }
+        P->slabs.push_back(std::move(S));
+    }
+    std::vector<uint32_t> ttb;
+    rs_status st = finish_op(P, &H, tensor_bytes, tensor_bytes * P->r_B, &ttb);
+    if (st != RS_OK) return st;
+    for (HostSlab &S : P->slabs) { S.tile_begin = 0xFFFFFFFFu; S.tile_end = 0; }
+    for (size_t t = 0; t < task_slab.size(); t++) {
+        HostSlab &S = P->slabs[task_slab[t]];
+        S.tile_begin = std::min(S.tile_begin, ttb[t]);
+        S.tile_end = std::max(S.tile_end, ttb[t + 1]);
     }
     return RS_OK;
 }
@@ -287,6 +363,7 @@ rs_status build_tables(Plan *P) {
         }
     }
     rs_status st;
+    if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
     if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
     if ((st = finish_op(P, &PK, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
     if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B)) != RS_OK) return st;

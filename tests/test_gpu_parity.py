@@ -265,3 +265,30 @@ def test_one_launch_per_call_and_loud_failure():
     with pytest.raises(rs.ReshardError):
         p.execute(gu.ptrs(src), [0] * 8, gu.stream())                 # null destination: refused, not skipped
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("case", [
+    ((6, 1024, 2048), (2, 2), "S0,R,S1", (3,), "S0,R,R"),            # 3 slabs, l_0 = 6, 2-way x 3-way cuts on dim 0
+    ((64, 512, 1024), (2, 4), "R,R,S0", (2, 4), "S0,R,R"),           # replicas: only the chosen senders are uploaded
+    ((48, 256, 1024), (2, 4), "S0,R,R", (2, 4), "R,R,R"),            # full broadcast: every slab lands on 8 devices
+    ((5, 1024, 2048), (2,), "R,S0,R", (4,), "R,R,S0"),               # l_0 = 5 not divisible by the slab count
+    ((40, 300, 1000), (2, 2), "S0,S1,R", (2, 2), "S1,S0,R"),         # 8-byte-aligned runs only: LSU path per slab
+])
+def test_execute_host_pipeline_cases(case):
+    shape, sm, ss, dm, ds = case
+    D = np.frombuffer(np.random.default_rng(11).bytes(int(np.prod(shape)) * 2), dtype=np.int16).reshape(shape)
+    src = do.shards_from_global(D, sm, ss)
+    want = do.reshard(shape, sm, ss, dm, ds, src, n_threads=do.max_threads())
+    p = rs.Plan(shape, 2, sm, ss, dm, ds)
+    used = {s["sender"] for s in p.slices()}
+    src_h = [torch.from_numpy(s.copy()).pin_memory() if r in used else None for r, s in enumerate(src)]
+    dst_h = [torch.full(p.local_shape(rs.RS_DST), 0x5A5A, dtype=torch.int16).pin_memory() for _ in want]
+    ws = torch.empty(p.host_workspace_bytes(), dtype=torch.uint8, device=gu.dev())
+    for _ in range(2):                                               # twice: the plan-owned streams/events are reused
+        up, down = p.execute_host([t.data_ptr() if t is not None else 0 for t in src_h], gu.ptrs(dst_h),
+                                  ws.data_ptr(), gu.stream())
+        torch.cuda.current_stream().synchronize()                    # the caller's stream alone must be enough
+        assert up == p.info.tensor_bytes and down == p.info.write_bytes
+        for q, (g, wq) in enumerate(zip(dst_h, want)):
+            assert g.numpy().tobytes() == wq.tobytes(), "device %d" % q
+            g.fill_(0x5A5A)

@@ -226,6 +226,12 @@ def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None):
     for q in range(n_dst):
         assert np.array_equal(dst[q], _bytes(want[q])), "execute tables differ from the oracle on device %d" % q
         assert (cnt[q] == 1).all(), "execute tables do not write every byte exactly once"
+    # the slab-cut execute table that reshard_execute_host pipelines over: same result, same exactly-once
+    dst3 = [np.zeros(want[0].nbytes, np.uint8) for _ in range(n_dst)]
+    cnt3 = [np.zeros(want[0].nbytes, np.int32) for _ in range(n_dst)]
+    ti.replay(p, rs.RS_OP_EXECUTE_SLABS, [_bytes(s) for s in src], dst3, cnt3)
+    for q in range(n_dst):
+        assert np.array_equal(dst3[q], _bytes(want[q])) and (cnt3[q] == 1).all()
     # pack -> message contents as the plan oracle states them -> unpack
     arena = [np.zeros(p.info.arena_bytes, np.uint8)]
     acnt = [np.zeros(p.info.arena_bytes, np.int32)]
@@ -352,3 +358,15 @@ def test_random_layouts_tables_equal_oracle(layout):
             _plan(shape, 1, sm, ss, dm, ds)
         return
     _check_tables(shape, dtype, sm, ss, dm, ds, env={"RS_LSU_TILE_BYTES": tile, "RS_BULK_TILE_BYTES": tile})
+
+
+def test_slab_table_cuts_dim0_when_large():
+    """>= 8 MiB per slab, at most 16 slabs, never more than l_0"""
+    p = _plan((32, 2048, 12288), 2, (2, 4), "S0,S1,R", (4, 2), "S1,R,S0")
+    assert p.op_info(rs.RS_OP_EXECUTE_SLABS).n_tasks == 16 * 32 // 2      # 16 slabs x the 16 slices each slab meets
+    p = _plan((6, 1024, 2048), 2, (2, 2), "S0,R,S1", (3,), "S0,R,R")       # 24 MiB -> 3 slabs over l_0 = 6
+    tasks, _d, tiles = ti.tables(p, rs.RS_OP_EXECUTE_SLABS)
+    assert p.op_info(rs.RS_OP_EXECUTE_SLABS).read_bytes == p.info.tensor_bytes
+    assert int((tiles["n_rows"].astype(np.int64) * tiles["col_bytes"]).sum()) == p.info.tensor_bytes
+    p = _plan((8, 16), 4, (1, 2), "S1,R", (1, 2), "R,S1")                  # tiny: one slab == the execute table
+    assert p.op_info(rs.RS_OP_EXECUTE_SLABS).n_tasks == p.op_info(rs.RS_OP_EXECUTE).n_tasks
