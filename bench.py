@@ -46,6 +46,10 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU work of the oracle sample")
+    ap.add_argument("--sweep", default=None, help="time execute/pack/unpack on a list of workloads instead of the step: "
+                    "'configs' (c2,c3,c3i,c3ii,c4), 'pairs' (6 pairs x 2 mesh pairs x 1 MiB..4 GiB), 'table2', 'all', "
+                    "or comma-separated workload names; one JSON line per workload")
+    ap.add_argument("--sweep-md", default=None, help="also write the sweep as a markdown table to this file")
     return ap.parse_args()
 
 
@@ -333,8 +337,93 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------ sweep
+
+def sweep_names(what):
+    from paper_2211_05322_b200 import inputs
+    cfg = ["c2", "c3", "c3i", "c3ii", "c4"]
+    pairs = ["sweep_%s_%s_%dMiB" % (p, m, b >> 20) for p in inputs.SWEEP_PAIRS for m in inputs.SWEEP_MESHES
+             for b in inputs.SWEEP_BYTES]
+    t2 = ["t2_%d" % c for c in (1, 2, 3, 4, 5, 7, 8, 9)]
+    return {"configs": cfg, "pairs": pairs, "table2": t2, "all": cfg + pairs + t2}.get(what) or what.split(",")
+
+
+def run_sweep(args):
+    """Per workload: plan, then each of execute / pack / unpack timed alone with CUDA events on the
+    launching stream (3 warm-up + --steps launches, L2 flushed before every launch when the
+    operation moves < 1 GiB).  Buffer contents are irrelevant to a copy: shards are seeded bytes."""
+    import torch
+    from paper_2211_05322_b200 import harness, inputs
+    from paper_2211_05322_b200 import reshard as rs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream()
+    sh = stream.cuda_stream
+    peak, _ = peak_hbm()
+    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK}[args.path]
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    K = max(3, min(args.steps, 30))
+    rows = []
+    for name in sweep_names(args.sweep):
+        w = inputs.get_workload(name)
+        plan = harness.make_plan(w, flags)
+        info = plan.info
+        g = torch.Generator(device=dev); g.manual_seed(w.seed % (1 << 31))
+        def buf(n):
+            t = torch.empty(n, dtype=torch.uint8, device=dev)
+            t[: min(n, 1 << 26)].random_(0, 256, generator=g)
+            return t
+        src = [buf(info.src_shard_bytes) for _ in range(info.n_src)]
+        dst = [torch.empty(info.dst_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_dst)]
+        arena = buf(info.arena_bytes)
+        sp, dp, ap = harness.ptrs(src), harness.ptrs(dst), arena.data_ptr()
+        calls = [("execute", rs.RS_OP_EXECUTE, lambda: plan.execute(sp, dp, sh)),
+                 ("pack", rs.RS_OP_PACK, lambda: plan.pack(sp, ap, sh)),
+                 ("unpack", rs.RS_OP_UNPACK, lambda: plan.unpack(ap, dp, sh))]
+        row = {"workload": name, "shape": list(w.shape), "src": "%s %s" % ("x".join(map(str, w.src_mesh)), w.src_spec),
+               "dst": "%s %s" % ("x".join(map(str, w.dst_mesh)), w.dst_spec), "n_slices": info.n_slices,
+               "tensor_bytes": info.tensor_bytes}
+        for opname, op, call in calls:
+            o = plan.op_info(op)
+            nbytes = o.read_bytes + o.write_bytes
+            do_flush = nbytes < (1 << 30)
+            for _ in range(3):
+                call()
+            ts = []
+            for _ in range(K):
+                if do_flush:
+                    flush.fill_(1)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); call(); e1.record(stream)
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            med = statistics.median(ts)
+            row[opname] = {"kernel": "rs_copy_bulk" if o.path == rs.RS_PATH_BULK else "rs_copy_lsu", "bytes": nbytes,
+                           "ms": med, "best_ms": min(ts), "GB/s": nbytes / med / 1e6, "frac_of_copy_peak": nbytes / med / 1e6 / peak,
+                           "tiles": o.n_tiles, "tile_bytes": o.tile_bytes, "grid": o.grid, "l2_flushed": do_flush}
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+        plan.close()
+        del src, dst, arena
+        torch.cuda.empty_cache()
+    if args.sweep_md:
+        with open(args.sweep_md, "w") as f:
+            f.write("| workload | tensor | src -> dst | slices | bytes moved (execute) | execute GB/s (frac of %.0f) | pack GB/s | unpack GB/s | kernel |\n" % peak)
+            f.write("|---|---|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %s | %s | %s -> %s | %d | %.1f MiB | %.0f (%.3f) | %.0f | %.0f | %s |\n" % (
+                    r["workload"], r["shape"], r["src"], r["dst"], r["n_slices"], r["execute"]["bytes"] / 2**20,
+                    r["execute"]["GB/s"], r["execute"]["frac_of_copy_peak"], r["pack"]["GB/s"], r["unpack"]["GB/s"],
+                    r["execute"]["kernel"]))
+    return 0
+
+
 def main():
     args = parse_args()
+    if args.sweep:
+        return run_sweep(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)
