@@ -14,6 +14,9 @@
 #define RS_BULK_STAGES       4          // ring slots per warp
 #define RS_BULK_LOOKAHEAD    2          // loads in flight per warp before the first store is issued
 #define RS_BULK_TILE_BYTES   12288      // bytes per ring slot
+#define RS_BULK_SHORT_RUN    1024       // runs up to this long: many copies per tile, use the SHORT shape
+#define RS_BULK_WARPS_SHORT  4
+#define RS_BULK_TILE_BYTES_SHORT 8192
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 
 #define RS_BULK_DESC_BYTES   4096       // per-warp descriptor ring: 64 tiles x 64 bytes
