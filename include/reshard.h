@@ -77,6 +77,40 @@ enum {
 };
 #define RS_PATH_MASK 0xF0
 
+/* load balance + ORDER of the unit tasks at host level (S3.2) */
+enum {
+    RS_SCHED_NONE = 0,          /* Eq. 4 per device, tables in slice-id order (reshard_plan's behaviour)   */
+    RS_SCHED_NAIVE = 1,         /* lowest-indexed sender, slice-id order                      */
+    RS_SCHED_LOAD_BALANCE = 2,  /* Eq. 4 greedy over hosts, order = the greedy's order   */
+    RS_SCHED_DFS = 3,           /* DFS over (next task, sender host), pruned, node budget */
+    RS_SCHED_GREEDY = 4,        /* rounds of non-overlapping tasks covering the most hosts,
+                                   found by `trials` random orderings (R24)                       */
+    RS_SCHED_ENSEMBLE = 5       /* DFS and greedy, the better one (ties: DFS)                 */
+};
+
+typedef struct rs_plan_opts {
+    uint32_t flags;                  /* as reshard_plan; RS_LB_* is ignored when schedule != RS_SCHED_NONE  */
+    int32_t schedule;                /* RS_SCHED_*                                                          */
+    int32_t src_devices_per_host;    /* host = device id / this (R8); 0 or 1: every device a host */
+    int32_t dst_devices_per_host;
+    int32_t trials;                  /* random orderings per round of RS_SCHED_GREEDY; 0 = 32               */
+    int32_t reserved;
+    int64_t node_budget;             /* DFS nodes before giving up with the best found; 0 = 200000          */
+    uint64_t seed;                   /* of the counter-based generator the greedy search draws from         */
+} rs_plan_opts;
+
+typedef struct rs_schedule_info {
+    int32_t algorithm;               /* RS_SCHED_* the plan was built with                                  */
+    int32_t winner;                  /* ensemble: RS_SCHED_DFS or RS_SCHED_GREEDY; else = algorithm         */
+    int32_t n_tasks, n_rounds;       /* unit tasks; rounds of the greedy search (0 if it did not run)       */
+    int32_t n_src_hosts, n_dst_hosts;
+    int32_t dfs_finished, reserved;  /* 1 if the search ended before the node budget (its result is optimal)*/
+    int64_t dfs_nodes;
+    int64_t makespan;                /* Eq. 1 with T_i = slice bytes (R7)                         */
+    int64_t busiest_host_bytes;      /* max over hosts of the bytes it sends or receives: no schedule of
+                                        these senders can finish earlier                     */
+} rs_schedule_info;
+
 /* operations a plan can run */
 enum { RS_OP_EXECUTE = 0, RS_OP_PACK = 1, RS_OP_UNPACK = 2,
        RS_OP_EXECUTE_SLABS = 3 /* execute cut into dim-0 slabs: the table reshard_execute_host runs (queries only) */ };
@@ -128,6 +162,20 @@ RS_API rs_status reshard_plan(const int64_t *global_shape, int32_t ndim, int32_t
                        const int32_t *src_mesh_shape, int32_t src_mesh_ndim, const char *src_spec,
                        const int32_t *dst_mesh_shape, int32_t dst_mesh_ndim, const char *dst_spec,
                        uint32_t flags, rs_plan **out_plan);
+
+/* reshard_plan with options: opts->schedule != RS_SCHED_NONE runs S3.2 at host level; the chosen
+ * host's least-loaded candidate device (lowest id on ties; RS_SCHED_NAIVE: its lowest-indexed device)
+ * becomes the sender, and the task tables list the unit tasks in order of their start time S_i.
+ * The data result is the same whatever the schedule (R10).  opts [HOST] may be NULL. */
+RS_API rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int32_t elem_bytes,
+                          const int32_t *src_mesh_shape, int32_t src_mesh_ndim, const char *src_spec,
+                          const int32_t *dst_mesh_shape, int32_t dst_mesh_ndim, const char *dst_spec,
+                          const rs_plan_opts *opts, rs_plan **out_plan);
+/* the schedule of a plan built with schedule != RS_SCHED_NONE (else RS_EINVAL): per unit task its
+ * sender HOST, its start time S_i (bytes), and the global order.
+ * sender_host, start, order [HOST, n_slices] may each be NULL. */
+RS_API rs_status reshard_plan_schedule(const rs_plan *plan, rs_schedule_info *info, int32_t *sender_host,
+                                int64_t *start, int32_t *order);
 
 RS_API void reshard_plan_destroy(rs_plan *plan);      /* NULL is allowed */
 

@@ -90,7 +90,22 @@ rs_status reshard_plan(const int64_t *global_shape, int32_t ndim, int32_t elem_b
                        const int32_t *src_mesh_shape, int32_t src_mesh_ndim, const char *src_spec,
                        const int32_t *dst_mesh_shape, int32_t dst_mesh_ndim, const char *dst_spec,
                        uint32_t flags, rs_plan **out_plan) {
+    rs_plan_opts o;
+    std::memset(&o, 0, sizeof(o));
+    o.flags = flags;
+    return reshard_plan_ex(global_shape, ndim, elem_bytes, src_mesh_shape, src_mesh_ndim, src_spec, dst_mesh_shape,
+                           dst_mesh_ndim, dst_spec, &o, out_plan);
+}
+
+rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int32_t elem_bytes,
+                          const int32_t *src_mesh_shape, int32_t src_mesh_ndim, const char *src_spec,
+                          const int32_t *dst_mesh_shape, int32_t dst_mesh_ndim, const char *dst_spec,
+                          const rs_plan_opts *opts, rs_plan **out_plan) {
     rs::set_error("");
+    rs_plan_opts defaults;
+    std::memset(&defaults, 0, sizeof(defaults));
+    if (!opts) opts = &defaults;
+    const uint32_t flags = opts->flags;
     if (!out_plan) { rs::set_error("out_plan is null"); return RS_EINVAL; }
     if (elem_bytes != 1 && elem_bytes != 2 && elem_bytes != 4 && elem_bytes != 8 && elem_bytes != 16) {
         rs::set_error("elem_bytes must be 1, 2, 4, 8 or 16");
@@ -101,12 +116,24 @@ rs_status reshard_plan(const int64_t *global_shape, int32_t ndim, int32_t elem_b
     rs::Plan *P = &h->p;
     P->elem_bytes = elem_bytes;
     P->flags = flags;
+    P->sched.algorithm = opts->schedule;
+    P->sched.src_dph = std::max(1, opts->src_devices_per_host);
+    P->sched.dst_dph = std::max(1, opts->dst_devices_per_host);
+    P->sched.trials = opts->trials;
+    P->sched.node_budget = opts->node_budget;
+    P->sched.seed = opts->seed;
     rs_status st;
     try {
         st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, &P->A);
         if (st == RS_OK) st = rs::make_layout(global_shape, ndim, dst_mesh_shape, dst_mesh_ndim, dst_spec, &P->B);
         if (st == RS_OK) st = rs::build_slices(P);
-        if (st == RS_OK) { rs::choose_senders(P); st = rs::build_messages(P); }
+        if (st == RS_OK) {
+            P->exec_order.resize(P->slices.size());
+            for (size_t i = 0; i < P->slices.size(); i++) P->exec_order[i] = (int)i;
+            if (opts->schedule == RS_SCHED_NONE) rs::choose_senders(P);
+            else st = rs::schedule_plan(P);
+        }
+        if (st == RS_OK) st = rs::build_messages(P);
         if (st == RS_OK) st = rs::build_tables(P);
         if (st == RS_OK && !(flags & RS_HOST_ONLY)) st = upload(P);
     } catch (const std::bad_alloc &) {
@@ -192,6 +219,27 @@ rs_status reshard_plan_slice(const rs_plan *plan, int32_t i, int64_t *lo, int64_
     if (senders) std::copy(S.senders.begin(), S.senders.end(), senders);
     if (n_receivers) *n_receivers = (int32_t)S.receivers.size();
     if (receivers) std::copy(S.receivers.begin(), S.receivers.end(), receivers);
+    return RS_OK;
+}
+
+rs_status reshard_plan_schedule(const rs_plan *plan, rs_schedule_info *info, int32_t *sender_host, int64_t *start,
+                                int32_t *order) {
+    if (!plan) return RS_EINVAL;
+    const rs::Plan &P = plan->p;
+    const rs::Schedule &S = P.sched;
+    if (S.algorithm == RS_SCHED_NONE) { rs::set_error("plan was built without a schedule"); return RS_EINVAL; }
+    if (info) {
+        std::memset(info, 0, sizeof(*info));
+        info->algorithm = S.algorithm; info->winner = S.winner;
+        info->n_tasks = (int32_t)P.slices.size(); info->n_rounds = S.n_rounds;
+        info->n_src_hosts = (P.A.n_dev + S.src_dph - 1) / S.src_dph;
+        info->n_dst_hosts = (P.B.n_dev + S.dst_dph - 1) / S.dst_dph;
+        info->dfs_finished = S.dfs_finished; info->dfs_nodes = S.dfs_nodes;
+        info->makespan = S.makespan; info->busiest_host_bytes = S.busiest_host_bytes;
+    }
+    if (sender_host) std::copy(S.sender_host.begin(), S.sender_host.end(), sender_host);
+    if (start) std::copy(S.start.begin(), S.start.end(), start);
+    if (order) std::copy(S.order.begin(), S.order.end(), order);
     return RS_OK;
 }
 

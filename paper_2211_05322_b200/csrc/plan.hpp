@@ -63,6 +63,20 @@ struct HostSlab {                        // one stage of the reshard_execute_hos
     std::vector<HostCopy> up, down;      // source ranges to upload before, destination ranges to download after
 };
 
+struct Schedule {                        // S3.2 at host level (schedule.cpp); algorithm 0 = not scheduled
+    int algorithm = 0;
+    int src_dph = 1, dst_dph = 1;        // devices per host (R8)
+    int trials = 0;
+    int64_t node_budget = 0;
+    uint64_t seed = 0;
+    int64_t makespan = 0;                // Eq. 1, in bytes (T_i = slice bytes, R7)
+    int64_t busiest_host_bytes = 0;      // Eq. 4-style bound under the chosen senders
+    int n_rounds = 0, winner = 0, dfs_finished = 1;
+    int64_t dfs_nodes = 0;
+    std::vector<int> sender_host, order; // per slice; global order
+    std::vector<int64_t> start;          // S_i
+};
+
 enum { RS_OP_SLABS = 3, RS_N_OPS = 4 };  // internal 4th table: execute, cut into dim-0 slabs
 
 struct Plan {
@@ -70,6 +84,8 @@ struct Plan {
     int elem_bytes = 0;
     uint32_t flags = 0;
     std::vector<Slice> slices;
+    Schedule sched;
+    std::vector<int> exec_order;         // slice ids in the order the tables list them (identity unless scheduled)
     std::vector<int64_t> sender_bytes;
     int64_t max_sender_bytes = 0;
     std::vector<Message> messages;
@@ -93,6 +109,7 @@ rs_status make_layout(const int64_t *shape, int ndim, const int32_t *mesh, int m
 void device_box(const Layout &L, int dev, int64_t *lo, int64_t *hi);
 rs_status build_slices(Plan *P);                       // a2 + a3
 void choose_senders(Plan *P);                          // a4
+rs_status schedule_plan(Plan *P);                      // S3.2: senders + order at host level, schedule.cpp
 rs_status build_messages(Plan *P);                     // message layout
 rs_status build_tables(Plan *P);                       // a5 (host side), tables.cpp
 

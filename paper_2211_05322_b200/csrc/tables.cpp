@@ -240,8 +240,8 @@ rs_status build_slabs(Plan *P, const int64_t *sA, const int64_t *sB, int64_t ten
         const int64_t b0 = bound[(size_t)c], b1 = bound[(size_t)c + 1];
         HostSlab S;
         std::vector<char> up_used((size_t)A.n_dev, 0);
-        for (size_t i = 0; i < P->slices.size(); i++) {
-            const Slice &sl = P->slices[i];
+        for (int i : P->exec_order) {
+            const Slice &sl = P->slices[(size_t)i];
             int64_t lo[RS_MAX_NDIM], hi[RS_MAX_NDIM];
             for (int d = 0; d < N; d++) { lo[d] = sl.lo[d]; hi[d] = sl.hi[d]; }
             lo[0] = std::max(lo[0], b0); hi[0] = std::min(hi[0], b1);
@@ -315,8 +315,8 @@ rs_status build_tables(Plan *P) {
     OpTables &X = P->op[RS_OP_EXECUTE], &PK = P->op[RS_OP_PACK], &UP = P->op[RS_OP_UNPACK];
     for (OpTables *o : {&X, &PK, &UP}) { o->tasks.clear(); o->dsts.clear(); o->tiles.clear(); }
 
-    for (size_t i = 0; i < P->slices.size(); i++) {
-        const Slice &S = P->slices[i];
+    for (int i : P->exec_order) {                              // slice-id order, or the schedule's (S3.2)
+        const Slice &S = P->slices[(size_t)i];
         int64_t lo_s[RS_MAX_NDIM], hi_s[RS_MAX_NDIM], ext[RS_MAX_NDIM], dense[RS_MAX_NDIM];
         device_box(A, S.sender, lo_s, hi_s);
         for (int d = 0; d < N; d++) ext[d] = S.hi[d] - S.lo[d];
@@ -347,7 +347,7 @@ rs_status build_tables(Plan *P) {
             if (!collapse(bx, e, &T)) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
             T.src_buf = S.sender; T.src_off = src_off;
             T.k = (int32_t)S.receivers.size(); T.dst_first = (int32_t)PK.dsts.size();
-            for (size_t j = 0; j < S.receivers.size(); j++) PK.dsts.push_back(RsDst{arena_off[i][j], 0, 0});
+            for (size_t j = 0; j < S.receivers.size(); j++) PK.dsts.push_back(RsDst{arena_off[(size_t)i][j], 0, 0});
             PK.tasks.push_back(T);
         }
         // unpack: one dense copy in the arena -> one receiver shard
@@ -357,7 +357,7 @@ rs_status build_tables(Plan *P) {
             ux.ndim = N;
             for (int d = 0; d < N; d++) { ux.ext[d] = ext[d]; ux.sstride[d] = dense[d]; ux.dstride[d] = sB[d]; }
             if (!collapse(ux, e, &T)) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
-            T.src_buf = 0; T.src_off = arena_off[i][j];
+            T.src_buf = 0; T.src_off = arena_off[(size_t)i][j];
             T.k = 1; T.dst_first = (int32_t)UP.dsts.size();
             int64_t lo_r[RS_MAX_NDIM], hi_r[RS_MAX_NDIM];
             device_box(B, S.receivers[j], lo_r, hi_r);

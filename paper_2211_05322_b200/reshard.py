@@ -20,11 +20,12 @@ RS_PATH_AUTO, RS_PATH_LSU, RS_PATH_BULK = 0x00, 0x10, 0x20
 RS_HOST_ONLY = 0x100
 RS_OP_EXECUTE, RS_OP_PACK, RS_OP_UNPACK, RS_OP_EXECUTE_SLABS = 0, 1, 2, 3
 RS_SRC, RS_DST = 0, 1
+RS_SCHED_NONE, RS_SCHED_NAIVE, RS_SCHED_LOAD_BALANCE, RS_SCHED_DFS, RS_SCHED_GREEDY, RS_SCHED_ENSEMBLE = range(6)
 RS_MAX_NDIM, RS_MAX_MESH_NDIM, RS_MAX_DEVICES = 8, 4, 128
 
 # every symbol include/reshard.h declares (tests check the library exports exactly these)
 SYMBOLS = [
-    "reshard_plan", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
+    "reshard_plan", "reshard_plan_ex", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
     "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
     "reshard_plan_message", "reshard_execute", "reshard_pack", "reshard_unpack", "reshard_execute_host",
     "reshard_host_workspace_bytes", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
@@ -45,6 +46,19 @@ class OpInfo(C.Structure):
                 ("n_tiles", C.c_int32), ("tile_bytes", C.c_int32), ("grid", C.c_int32), ("block", C.c_int32),
                 ("smem_bytes", C.c_int32), ("read_bytes", C.c_int64), ("write_bytes", C.c_int64),
                 ("min_run_bytes", C.c_int64)]
+
+
+class PlanOpts(C.Structure):
+    _fields_ = [("flags", C.c_uint32), ("schedule", C.c_int32), ("src_devices_per_host", C.c_int32),
+                ("dst_devices_per_host", C.c_int32), ("trials", C.c_int32), ("reserved", C.c_int32),
+                ("node_budget", C.c_int64), ("seed", C.c_uint64)]
+
+
+class ScheduleInfo(C.Structure):
+    _fields_ = [("algorithm", C.c_int32), ("winner", C.c_int32), ("n_tasks", C.c_int32), ("n_rounds", C.c_int32),
+                ("n_src_hosts", C.c_int32), ("n_dst_hosts", C.c_int32), ("dfs_finished", C.c_int32),
+                ("reserved", C.c_int32), ("dfs_nodes", C.c_int64), ("makespan", C.c_int64),
+                ("busiest_host_bytes", C.c_int64)]
 
 
 class ReshardError(RuntimeError):
@@ -106,12 +120,20 @@ def launch_count():
 class Plan:
     """reshard_plan(...) handle.  See include/reshard.h for the contract of every call."""
 
-    def __init__(self, global_shape, elem_bytes, src_mesh, src_spec, dst_mesh, dst_spec, flags=0):
+    def __init__(self, global_shape, elem_bytes, src_mesh, src_spec, dst_mesh, dst_spec, flags=0, opts=None):
+        """opts: dict of rs_plan_opts fields (schedule, src_devices_per_host, ...) -> reshard_plan_ex"""
         self._h = C.c_void_p()
-        _chk(_lib().reshard_plan(_i64(global_shape), len(global_shape), int(elem_bytes),
-                                 _i32(src_mesh), len(src_mesh), src_spec.encode(),
-                                 _i32(dst_mesh), len(dst_mesh), dst_spec.encode(),
-                                 C.c_uint32(flags), C.byref(self._h)))
+        if opts is None:
+            _chk(_lib().reshard_plan(_i64(global_shape), len(global_shape), int(elem_bytes),
+                                     _i32(src_mesh), len(src_mesh), src_spec.encode(),
+                                     _i32(dst_mesh), len(dst_mesh), dst_spec.encode(),
+                                     C.c_uint32(flags), C.byref(self._h)))
+        else:
+            o = PlanOpts(flags=flags, **opts)
+            _chk(_lib().reshard_plan_ex(_i64(global_shape), len(global_shape), int(elem_bytes),
+                                        _i32(src_mesh), len(src_mesh), src_spec.encode(),
+                                        _i32(dst_mesh), len(dst_mesh), dst_spec.encode(),
+                                        C.byref(o), C.byref(self._h)))
         self.info = PlanInfo()
         _chk(_lib().reshard_plan_info(self._h, C.byref(self.info)))
         self.ndim = self.info.ndim
@@ -158,6 +180,13 @@ class Plan:
 
     def slices(self):
         return [self.slice(i) for i in range(self.info.n_slices)]
+
+    def schedule(self):
+        """reshard_plan_schedule -> dict(info=ScheduleInfo, sender_host, start, order)"""
+        n = self.info.n_slices
+        info, sh, st, od = ScheduleInfo(), (C.c_int32 * n)(), (C.c_int64 * n)(), (C.c_int32 * n)()
+        _chk(_lib().reshard_plan_schedule(self._h, C.byref(info), sh, st, od))
+        return dict(info=info, sender_host=list(sh), start=list(st), order=list(od))
 
     def sender_bytes(self):
         out = (C.c_int64 * self.info.n_src)()

@@ -41,14 +41,14 @@ def device_shards_from_global(D, mesh, spec):
     return [D[idx].contiguous() for idx in oracle_slices(tuple(D.shape), mesh, spec)]
 
 
-def run_small(shape, np_dtype, sm, ss, dm, ds, flags=0, seed=1, src_offset=0, dst_offset=0):
+def run_small(shape, np_dtype, sm, ss, dm, ds, flags=0, seed=1, src_offset=0, dst_offset=0, opts=None):
     """execute on the GPU and return (plan, got dst shards as numpy, oracle dst shards as numpy)."""
     e = np.dtype(np_dtype).itemsize
     rng = np.random.default_rng(seed)
     D = np.frombuffer(rng.bytes(int(np.prod(shape)) * e), dtype=np_dtype).reshape(shape)
     src = do.shards_from_global(D, sm, ss)
     want = do.reshard(shape, sm, ss, dm, ds, src)
-    p = rs.Plan(shape, e, sm, ss, dm, ds, flags)
+    p = rs.Plan(shape, e, sm, ss, dm, ds, flags, opts)
     src_d = [torch.zeros(s.nbytes + 64, dtype=torch.uint8, device=dev()) for s in src]
     for t, s in zip(src_d, src):
         t[src_offset:src_offset + s.nbytes] = to_dev(s)

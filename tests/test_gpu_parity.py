@@ -48,6 +48,19 @@ def test_execute_bit_exact_small(case, dtype, path):
         assert g.tobytes() == w.tobytes(), "device %d differs" % q
 
 
+@pytest.mark.parametrize("alg", [rs.RS_SCHED_NAIVE, rs.RS_SCHED_LOAD_BALANCE, rs.RS_SCHED_DFS, rs.RS_SCHED_GREEDY, rs.RS_SCHED_ENSEMBLE])
+@pytest.mark.parametrize("case", [SMALL[i] for i in (3, 4, 6, 7, 9, 10, 11, 17)])
+def test_scheduled_plans_move_the_same_bytes(case, alg):
+    """S3.2 changes senders and table order, never the result (R10)"""
+    shape, sm, ss, dm, ds = case
+    for dph in (1, 2):
+        p, got, want = gu.run_small(shape, np.int16, sm, ss, dm, ds, opts=dict(
+            schedule=alg, src_devices_per_host=dph, dst_devices_per_host=dph, seed=3, node_budget=5000))
+        assert p.schedule()["info"].makespan >= p.schedule()["info"].busiest_host_bytes
+        for g, w in zip(got, want):
+            assert g.tobytes() == w.tobytes()
+
+
 @pytest.mark.parametrize("off", [(2, 0), (0, 2), (4, 8), (1, 3), (16, 16)])
 @pytest.mark.parametrize("path", PATHS)
 def test_under_aligned_shard_pointers(off, path):

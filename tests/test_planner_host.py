@@ -40,8 +40,8 @@ LAYOUTS = [
 ]
 
 
-def _plan(shape, e, sm, ss, dm, ds, flags=0):
-    return rs.Plan(shape, e, sm, ss, dm, ds, flags | HOST)
+def _plan(shape, e, sm, ss, dm, ds, flags=0, opts=None):
+    return rs.Plan(shape, e, sm, ss, dm, ds, flags | HOST, opts)
 
 
 # ---------------------------------------------------------------- the boundary
@@ -201,14 +201,14 @@ def _bytes(a):
     return np.ascontiguousarray(a).view(np.uint8).reshape(-1)
 
 
-def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None):
+def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None, opts=None):
     e = np.dtype(dtype).itemsize
     old = {}
     for k, v in (env or {}).items():
         old[k] = os.environ.get(k)
         os.environ[k] = str(v)
     try:
-        p = _plan(shape, e, sm, ss, dm, ds, flags)
+        p = _plan(shape, e, sm, ss, dm, ds, flags, opts)
     finally:
         for k, v in old.items():
             if v is None:
