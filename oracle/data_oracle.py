@@ -67,19 +67,22 @@ def device_box(shape, mesh, spec, r):
     return tuple(lo), tuple(hi)
 
 
-def shard_from_global(D, mesh, spec, r):
-    """shard of device r: the oracle's own statement of the layout."""
+def shard_from_global(D, mesh, spec, r, pad=0):
+    """shard of device r: the oracle's own statement of the layout; padded local
+    shape (R5), padding elements = `pad`."""
     D = np.ascontiguousarray(D)
     shape = D.shape
-    out = np.empty(local_shape(shape, mesh, spec), dtype=D.dtype)
+    out = np.zeros(local_shape(shape, mesh, spec), dtype=D.dtype)
+    if pad:
+        out.view(np.uint8)[...] = pad
     _chk(lib().oracle_shard_from_global(_i64(shape), len(shape), D.dtype.itemsize, _i32(mesh), len(mesh),
                                         spec.encode(), C.c_int64(r), C.c_void_p(D.ctypes.data),
                                         C.c_void_p(out.ctypes.data)))
     return out
 
 
-def shards_from_global(D, mesh, spec):
-    return [shard_from_global(D, mesh, spec, r) for r in range(num_devices(mesh))]
+def shards_from_global(D, mesh, spec, pad=0):
+    return [shard_from_global(D, mesh, spec, r, pad) for r in range(num_devices(mesh))]
 
 
 def element_source(shape, src_mesh, src_spec, dst_mesh, dst_spec, q, j):
@@ -99,7 +102,7 @@ def reshard_device(shape, elem_bytes, src_mesh, src_spec, dst_mesh, dst_spec, sr
                    n_threads=1, out=None):
     """destination shard of device q computed by the oracle from host source shards."""
     if out is None:
-        out = np.empty(local_shape(shape, dst_mesh, dst_spec), dtype=dtype)
+        out = np.zeros(local_shape(shape, dst_mesh, dst_spec), dtype=dtype)
     assert out.flags.c_contiguous and out.dtype.itemsize == elem_bytes
     for s in src_shards:
         assert s.flags.c_contiguous
@@ -111,11 +114,15 @@ def reshard_device(shape, elem_bytes, src_mesh, src_spec, dst_mesh, dst_spec, sr
     return out
 
 
-def reshard(shape, src_mesh, src_spec, dst_mesh, dst_spec, src_shards, n_threads=1):
-    """the whole task: list of destination shards, one per dst device."""
+def reshard(shape, src_mesh, src_spec, dst_mesh, dst_spec, src_shards, n_threads=1, fill=0):
+    """the whole task: list of destination shards, one per dst device.  Padding bytes of
+    the destination shards (R5) keep the byte value `fill`: the oracle never writes them."""
     dtype = src_shards[0].dtype
     lshape = local_shape(shape, dst_mesh, dst_spec)
-    outs = [np.empty(lshape, dtype=dtype) for _ in range(num_devices(dst_mesh))]
+    outs = [np.zeros(lshape, dtype=dtype) for _ in range(num_devices(dst_mesh))]
+    if fill:
+        for o in outs:
+            o.view(np.uint8)[...] = fill
     for s in src_shards:
         assert s.flags.c_contiguous and s.dtype == dtype
     _chk(lib().reshard_oracle(_i64(shape), len(shape), dtype.itemsize,

@@ -14,7 +14,8 @@ What it follows (PAPER.md:<line>, section):
   optimum of Eq. 4  PAPER.md:169     brute force over all sender assignments (tiny inputs)
 
 Readings (DESIGN.md): R1 row-major device ids; R2 S^{01}: first listed axis most significant;
-R3 a mesh axis shards at most one tensor dim; R5 even partitions only; R6 one unit task per
+R3 a mesh axis shards at most one tensor dim; R5 uneven partitions: every shard has the padded
+extent c = ceil(l/k), shard p holds [min(pc, l), min((p+1)c, l)); R6 one unit task per
 B.2 slice; R7 T_i = slice bytes (independent of #receivers); R8 balance per (virtual) device;
 R9 ties: tasks by (bytes desc, slice id asc), senders by (load, device id).
 Slice id = row-major rank in I_0 x ... x I_{n-1} (dim 0 slowest): a convention of this build,
@@ -74,16 +75,20 @@ def device_coords(mesh, r):
     return tuple(int(x) for x in np.unravel_index(r, tuple(mesh)))
 
 
-def degrees(shape, mesh, axes_per_dim):
+def degrees(shape, mesh, axes_per_dim, even_only=False):
     ks = []
     for l, axes in zip(shape, axes_per_dim):
         k = 1
         for a in axes:
             k *= mesh[a]
-        if l % k:
-            raise DivisError("dim of length %d not divisible by degree %d" % (l, k))  # R5
+        if even_only and l % k:
+            raise DivisError("dim of length %d not divisible by degree %d" % (l, k))
         ks.append(k)
     return ks
+
+
+def ceil_div(a, b):
+    return -(-a // b)
 
 
 def tile_box(shape, mesh, spec, r):
@@ -96,20 +101,22 @@ def tile_box(shape, mesh, spec, r):
         p = 0
         for a in axes:               # R2: first listed axis most significant
             p = p * mesh[a] + c[a]
-        lo.append(p * (l // k))
-        hi.append((p + 1) * (l // k))
+        ext = ceil_div(l, k)                                # R5: padded extent, clipped box
+        lo.append(min(p * ext, l))
+        hi.append(min((p + 1) * ext, l))
     return tuple(lo), tuple(hi)
 
 
 def cutpoints(shape, src_mesh, src_spec, dst_mesh, dst_spec):
-    """Cut(d) = {0, l_d} U {j l_d/k_A} U {j l_d/k_B}."""
+    """Cut(d) = {0, l_d} U {j l_d/k_A} U {j l_d/k_B}; with uneven partitions the
+    shard boundaries are j*ceil(l_d/k), clipped to l_d (R5)."""
     ka = degrees(shape, src_mesh, parse_spec(src_spec, len(shape), len(src_mesh)))
     kb = degrees(shape, dst_mesh, parse_spec(dst_spec, len(shape), len(dst_mesh)))
     cuts = []
     for l, a, b in zip(shape, ka, kb):
         s = {0, l}
-        s.update(j * (l // a) for j in range(1, a))
-        s.update(j * (l // b) for j in range(1, b))
+        s.update(min(j * ceil_div(l, a), l) for j in range(1, a))
+        s.update(min(j * ceil_div(l, b), l) for j in range(1, b))
         cuts.append(sorted(s))
     return cuts
 

@@ -17,7 +17,7 @@
  *
  *   for every destination device q, for every local multi-index j of q's shard:
  *       g_i        = lo_i(q) + j_i                      (global index of that element)
- *       p_i        = g_i / (l_i / k^A_i)                (which source shard holds it on dim i)
+ *       p_i        = g_i / c^A_i, c_i = ceil(l_i / k_i)  (which source shard holds it on dim i)
  *       source dev = the device whose mesh coordinates on the axes X_A uses give p, and whose
  *                    coordinates on the axes X_A does not use are 0 (lowest-index replica)
  *       dst_q[j]   = src_dev[g - lo(src_dev)]           (copy elem_bytes bytes)
@@ -32,8 +32,12 @@
  *       FIRST listed axis most significant (S^{01} on (2,4): p = c0*4 + c1, degree 8).
  *   R3  one mesh axis may shard at most one tensor dim -> OR_ESPEC otherwise.
  *   R4  a mesh axis of size 1 is legal; it shards into 1 piece (behaves as R).
- *   R5  l_i must be divisible by k_i -> OR_EDIVIS otherwise (even partitions only).
- *   R11 a shard is the device's box of D stored dense row-major, no padding.
+ *   R5  uneven partitions ("handles tiling, padding", "pad it in case 6"):
+ *       every shard has the padded extent c_i = ceil(l_i / k_i); shard p holds
+ *       [min(p c_i, l_i), min((p+1) c_i, l_i)) -- the last one short, later ones possibly empty.
+ *       Divisible dims (all of the paper's other cases) are the special case c_i = l_i / k_i.
+ *   R11 a shard buffer is dense row-major of the PADDED local shape (c_0, ..., c_{N-1}), the same on
+ *       every device; the device's box sits at its origin; padding is never read and never written.
  *   R12 replicas are assumed identical; the oracle reads the lowest-index replica.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): the Fig. 2 worked example,
@@ -65,7 +69,7 @@ typedef struct {
     int64_t mesh[OR_MAX_MESH_NDIM];  /* m_a */
     or_dimspec spec[OR_MAX_NDIM];
     int64_t degree[OR_MAX_NDIM];     /* k_i */
-    int64_t local[OR_MAX_NDIM];      /* l_i / k_i */
+    int64_t local[OR_MAX_NDIM];      /* c_i = ceil(l_i / k_i): padded local extent (R5) */
     int64_t n_devices;
 } or_layout;
 
@@ -135,9 +139,8 @@ static int or_make_layout(const int64_t *shape, int ndim, const int32_t *mesh, i
     for (i = 0; i < ndim; i++) {
         int64_t k = 1;
         for (a = 0; a < L->spec[i].n_axes; a++) k *= L->mesh[L->spec[i].axes[a]];
-        if (L->shape[i] % k != 0) return OR_EDIVIS;       /* R5 */
         L->degree[i] = k;
-        L->local[i] = L->shape[i] / k;
+        L->local[i] = (L->shape[i] + k - 1) / k;          /* R5: ceil */
     }
     return OR_OK;
 }
@@ -193,7 +196,7 @@ int64_t oracle_num_devices(const int32_t *mesh, int mesh_ndim)
     return n;
 }
 
-/* local shard shape l_i / k_i. */
+/* (padded) local shard shape c_i = ceil(l_i / k_i) (R5). */
 int oracle_local_shape(const int64_t *shape, int ndim, const int32_t *mesh, int mesh_ndim,
                        const char *spec, int64_t *local_out)
 {
@@ -218,12 +221,15 @@ int oracle_device_box(const int64_t *shape, int ndim, const int32_t *mesh, int m
         int64_t p = or_shard_index(&L, c, i);
         lo[i] = p * L.local[i];
         hi[i] = lo[i] + L.local[i];
+        if (lo[i] > L.shape[i]) lo[i] = L.shape[i];        /* R5: clipped to the tensor */
+        if (hi[i] > L.shape[i]) hi[i] = L.shape[i];
     }
     return OR_OK;
 }
 
-/* Layout definition: shard_r[j] = D[lo(r) + j], dense row-major (R11).
- * D is the whole tensor, dense row-major, on the host. */
+/* Layout definition: shard_r[j] = D[lo(r) + j] for every j with lo(r) + j inside D, dense row-major
+ * of the padded local shape (R5, R11); padding elements of shard_out are left as
+ * the caller filled them.  D is the whole tensor, dense row-major, on the host. */
 int oracle_shard_from_global(const int64_t *shape, int ndim, int elem_bytes,
                              const int32_t *mesh, int mesh_ndim, const char *spec,
                              int64_t r, const void *D, void *shard_out)
@@ -241,16 +247,21 @@ int oracle_shard_from_global(const int64_t *shape, int ndim, int elem_bytes,
     }
     for (j = 0; j < n_local; j++) {
         int64_t rem = j, g = 0, ji[OR_MAX_NDIM];
+        int pad = 0;
         for (i = ndim - 1; i >= 0; i--) { ji[i] = rem % L.local[i]; rem /= L.local[i]; }
-        for (i = 0; i < ndim; i++) g = g * L.shape[i] + (lo[i] + ji[i]);
+        for (i = 0; i < ndim; i++) {
+            if (lo[i] + ji[i] >= L.shape[i]) pad = 1;
+            g = g * L.shape[i] + (lo[i] + ji[i]);
+        }
+        if (pad) continue;
         memcpy((char *)shard_out + j * elem_bytes, (const char *)D + g * elem_bytes, (size_t)elem_bytes);
     }
     return OR_OK;
 }
 
-/* where one destination element comes from: (q, local linear index j) -> (source device,
- * source local linear index, global linear index).  Used for sampled checks at sizes where
- * running the whole oracle would take too long. */
+/* where one destination element comes from: (q, local linear index j in the padded shard) ->
+ * (source device, source local linear index, global linear index); source device -1 if (q, j) is
+ * padding.  Used for sampled checks at sizes where running the whole oracle would take too long. */
 static void or_element_source(const or_layout *A, const or_layout *B, const int64_t *lo_q,
                               int64_t j, int64_t *src_dev, int64_t *src_lin, int64_t *g_lin)
 {
@@ -259,6 +270,7 @@ static void or_element_source(const or_layout *A, const or_layout *B, const int6
     for (i = B->ndim - 1; i >= 0; i--) { ji[i] = rem % B->local[i]; rem /= B->local[i]; }
     for (i = 0; i < B->ndim; i++) {
         int64_t gi = lo_q[i] + ji[i];
+        if (gi >= B->shape[i]) { *src_dev = -1; *src_lin = -1; if (g_lin) *g_lin = -1; return; }   /* padding */
         p[i] = gi / A->local[i];
         s = s * A->local[i] + (gi - p[i] * A->local[i]);
         g = g * A->shape[i] + gi;
@@ -306,6 +318,7 @@ static void or_fill_device(const or_layout *A, const or_layout *B, int elem_byte
         for (t = 0; t < inner; t++) {
             int64_t j = j0 * inner + t, dev, s;
             or_element_source(A, B, lo, j, &dev, &s, NULL);
+            if (dev < 0) continue;                         /* padding of the destination shard: untouched */
             memcpy((char *)dst_shard_q + j * elem_bytes,
                    (const char *)src_shards[dev] + s * elem_bytes, (size_t)elem_bytes);
         }

@@ -92,7 +92,11 @@ def _numpy_expected(D, mesh, spec, q):
     itself pinned in test_plan_oracle_pins.py)."""
     from oracle import plan_oracle as po
     lo, hi = po.tile_box(D.shape, mesh, spec, q)
-    return D[tuple(slice(l, h) for l, h in zip(lo, hi))]
+    box = D[tuple(slice(l, h) for l, h in zip(lo, hi))]
+    lo0, hi0 = po.tile_box(D.shape, mesh, spec, 0)        # device 0's box has the padded extents (R5)
+    out = np.zeros([h - l for l, h in zip(lo0, hi0)], dtype=D.dtype)
+    out[tuple(slice(0, n) for n in box.shape)] = box
+    return out
 
 
 # ---------------------------------------------------------------- whole-task checks
@@ -201,9 +205,7 @@ def test_error_codes():
     with pytest.raises(do.OracleError) as e:
         do.local_shape((4, 4), (2, 2), "S0")             # wrong length
     assert e.value.code == do.OR_ESPEC
-    with pytest.raises(do.OracleError) as e:
-        do.local_shape((5, 4), (2, 2), "S0,R")           # uneven (R5)
-    assert e.value.code == do.OR_EDIVIS
+    assert do.local_shape((5, 4), (2, 2), "S0,R") == (3, 4)   # uneven: padded extent ceil(5/2) (R5)
     assert do.local_shape((4, 8, 6), (2, 4), "RS^{01}R") == (4, 1, 6)
     assert do.local_shape((4, 8, 6), (2, 4), "(S0, S1, R)") == (2, 2, 6)
 
@@ -225,7 +227,7 @@ def _layouts(draw):
                 return mesh, ",".join(spec)
     sm, ss = side()
     dm, ds = side()
-    shape = tuple(draw(st.sampled_from([12, 24])) for _ in range(ndim))     # divisible by 1,2,3,4,6,8,12
+    shape = tuple(draw(st.sampled_from([12, 24, 7, 10, 1])) for _ in range(ndim))   # even and uneven (R5) splits
     if ndim >= 3:
         shape = tuple(min(s, 12) for s in shape)
     return shape, sm, ss, dm, ds
@@ -235,10 +237,6 @@ def _layouts(draw):
 @given(_layouts())
 def test_random_layouts_equal_numpy_slicing(layout):
     shape, sm, ss, dm, ds = layout
-    try:
-        do.local_shape(shape, sm, ss), do.local_shape(shape, dm, ds)
-    except do.OracleError:
-        return    # 24 % 8 etc. always divide; 12 % 8 does not -> skip
     D = np.arange(np.prod(shape), dtype=np.int32).reshape(shape)
     src = do.shards_from_global(D, sm, ss)
     for r, s in enumerate(src):
@@ -246,3 +244,81 @@ def test_random_layouts_equal_numpy_slicing(layout):
     dst = do.reshard(shape, sm, ss, dm, ds, src)
     for q, got in enumerate(dst):
         assert np.array_equal(got, _numpy_expected(D, dm, ds, q))
+
+
+# ---------------------------------------------------------------- uneven partitions (R5)
+
+UNEVEN = [
+    ((10,), (3,), "S0", (4,), "S0"),
+    ((5, 4), (2, 2), "S0,R", (2, 2), "R,S1"),
+    ((7, 9), (2, 4), "S1,S0", (4, 2), "S0,S1"),
+    ((7, 5, 3), (2, 3), "S1,R,S0", (3, 2), "R,S0,S1"),
+    ((2, 6), (4,), "S0,R", (2,), "S0,R"),                 # more shards than rows: devices 2, 3 hold nothing
+    ((9, 10, 4), (2, 4), "S0,R,R", (3, 4), "S0,R,R"),     # Table 2 case 6 in small
+    ((11, 6), (2, 4), "S01,R", (2, 3), "R,S10"),
+]
+
+
+def _torch_chunks(D, mesh, spec, r):
+    """LIBRARY ROUTINE statement of the ceil-div convention: torch.chunk(x, k, dim) returns chunks of
+    ceil(l/k) rows, the last one shorter, and FEWER than k chunks when l is small (those shards are
+    empty).  Device r takes chunk p_i on every sharded dim."""
+    import torch
+    from oracle import plan_oracle as po
+    axes = po.parse_spec(spec, D.ndim, len(mesh))
+    c = po.device_coords(mesh, r)
+    x = torch.from_numpy(np.ascontiguousarray(D))
+    for dim, ax in enumerate(axes):
+        k, p = 1, 0
+        for a in ax:
+            k *= mesh[a]
+            p = p * mesh[a] + c[a]
+        chunks = torch.chunk(x, k, dim)
+        x = chunks[p] if p < len(chunks) else x.narrow(dim, 0, 0)
+    return x.numpy()
+
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", UNEVEN)
+def test_uneven_shards_are_torch_chunks(shape, sm, ss, dm, ds):
+    D = np.arange(1, np.prod(shape) + 1, dtype=np.int32).reshape(shape)
+    for mesh, spec in ((sm, ss), (dm, ds)):
+        local = do.local_shape(shape, mesh, spec)
+        assert local == tuple(_torch_chunks(D, mesh, spec, 0).shape)          # padded extent = first chunk
+        for r in range(do.num_devices(mesh)):
+            want = _torch_chunks(D, mesh, spec, r)
+            lo, hi = do.device_box(shape, mesh, spec, r)
+            assert tuple(h - l for l, h in zip(lo, hi)) == want.shape
+            got = do.shard_from_global(D, mesh, spec, r, pad=0xEE)
+            valid = tuple(slice(0, n) for n in want.shape)
+            assert np.array_equal(got[valid], want)
+            mask = np.ones(local, bool); mask[valid] = False
+            assert (got.view(np.uint8).reshape(local + (4,))[mask] == 0xEE).all()   # padding left alone
+
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", UNEVEN)
+def test_uneven_reshard_values_cover_and_identity(shape, sm, ss, dm, ds):
+    D = np.arange(1, np.prod(shape) + 1, dtype=np.int64).reshape(shape)       # value = global index + 1, never 0
+    src = do.shards_from_global(D, sm, ss, pad=0x77)
+    dst = do.reshard(shape, sm, ss, dm, ds, src, fill=0)
+    holders = np.zeros(shape, np.int32)
+    for q, got in enumerate(dst):
+        want = _torch_chunks(D, dm, ds, q)
+        valid = tuple(slice(0, n) for n in want.shape)
+        assert np.array_equal(got[valid], want)
+        mask = np.ones(got.shape, bool); mask[valid] = False
+        assert (got[mask] == 0).all()                                         # padding never written
+        lo, hi = do.device_box(shape, dm, ds, q)
+        holders[tuple(slice(l, h) for l, h in zip(lo, hi))] += 1
+    assert (holders == holders.flat[0]).all() and holders.flat[0] >= 1       # every element on r_B devices
+    back = do.reshard(shape, dm, ds, sm, ss, dst, fill=0x77)                  # A -> B -> A
+    for a, b in zip(src, back):
+        assert a.tobytes() == b.tobytes()
+
+
+def test_uneven_element_source_flags_padding():
+    shape, sm, ss, dm, ds = (5, 4), (2, 2), "S0,R", (2, 2), "R,S1"
+    assert do.local_shape(shape, sm, ss) == (3, 4) and do.device_box(shape, sm, ss, 2) == ((3, 0), (5, 4))
+    # destination device 0 holds D[:, 0:2]; its element (4, 1) comes from source device 2 (rows 3..4), local (1, 1)
+    assert do.element_source(shape, sm, ss, dm, ds, 0, 4 * 2 + 1) == (2, 1 * 4 + 1, 4 * 4 + 1)
+    # source side padded: shard of device 2 has 3 rows, the last one padding; as a DESTINATION it is flagged
+    assert do.element_source(shape, dm, ds, sm, ss, 2, 2 * 4 + 0) == (-1, -1, -1)

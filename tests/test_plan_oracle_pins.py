@@ -98,10 +98,35 @@ def test_table2_decomposition_counts(case):
     assert sum(t["size"] for t in tasks) == np.prod(shape)            # lower bound
 
 
-def test_table2_case6_uneven_is_rejected():
+def test_table2_case6_uneven_partition():
+    """(2,4) -> (3,4), dim 0 = 1024 over 3 shards, "pad it in case 6" (R5)."""
+    g = golden_io.load("table2_facts.txt")
     ss, ds, sm, dm = inputs.TABLE2[6]
-    with pytest.raises(po.DivisError):
-        po.unit_tasks((1024, 1024, 512), sm, ss, dm, ds)              # 1024 % 3 != 0 (R5)
+    shape = tuple(g["tensor_shape"])
+    c = g["case6_padded_extent"][0]
+    assert po.ceil_div(shape[0], 3) == c and 3 * c == g["case6_padded_dim0"][0]
+    boxes = sorted({(po.tile_box(shape, dm, ds, r)[0][0], po.tile_box(shape, dm, ds, r)[1][0]) for r in range(12)})
+    assert [x for b in boxes for x in b] == g["case6_dst_dim0_boxes"]
+    assert po.cutpoints(shape, sm, ss, dm, ds)[0] == g["case6_dim0_cutpoints"]
+    tasks = po.unit_tasks(shape, sm, ss, dm, ds)
+    assert len(tasks) == g["case6_num_unit_tasks"][0]
+    assert sum(t["size"] for t in tasks) == np.prod(shape)            # PAPER.md:90, padding is never sent
+    assert [len(t["senders"]) for t in tasks] == [4] * 4 and [len(t["receivers"]) for t in tasks] == [4] * 4
+    with pytest.raises(po.DivisError):                                # the strict "evenly sharded" reading (PAPER.md:64)
+        po.degrees(shape, dm, po.parse_spec(ds, 3, 2), even_only=True)
+
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", [((10,), (3,), "S0", (4,), "S0"), ((7, 9), (2, 4), "S1,S0", (4, 2), "S0,S1"),
+                                               ((2, 6), (4,), "S0,R", (2,), "S0,R"), ((11, 6), (2, 4), "S01,R", (2, 3), "R,S10")])
+def test_uneven_unit_tasks_cover_exactly_once(shape, sm, ss, dm, ds):
+    tasks = po.unit_tasks(shape, sm, ss, dm, ds)
+    assert sum(t["size"] for t in tasks) == np.prod(shape) and all(t["size"] > 0 for t in tasks)
+    assert all(t["senders"] and t["receivers"] for t in tasks)
+    for cnt in po.paint_cover(shape, dm, ds, tasks):
+        assert (cnt == 1).all()
+    # the brute-force optimum of Eq. 4 is reachable although slice sizes differ
+    n_src = po.n_devices(sm)
+    assert po.max_load(tasks, po.greedy_senders(tasks), n_src) >= po.bruteforce_optimum(tasks, n_src)
 
 
 def test_cutpoints_follow_b2():
