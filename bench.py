@@ -344,7 +344,7 @@ def sweep_names(what):
     cfg = ["c2", "c3", "c3i", "c3ii", "c4"]
     pairs = ["sweep_%s_%s_%dMiB" % (p, m, b >> 20) for p in inputs.SWEEP_PAIRS for m in inputs.SWEEP_MESHES
              for b in inputs.SWEEP_BYTES]
-    t2 = ["t2_%d" % c for c in (1, 2, 3, 4, 5, 7, 8, 9)]
+    t2 = ["t2_%d" % c for c in (1, 2, 3, 4, 5, 6, 7, 8, 9)]
     return {"configs": cfg, "pairs": pairs, "table2": t2, "all": cfg + pairs + t2}.get(what) or what.split(",")
 
 

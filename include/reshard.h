@@ -14,8 +14,15 @@
  *   sharding spec   PAPER.md:84     one entry per tensor dim: R, or S followed by the mesh axes the
  *                                   dim is sharded over ("S0", "S1", "S01"); first listed axis is
  *                                   the most significant digit of the shard index (R2)
- *   data slice      PAPER.md:86     device r holds the box [p_i*l_i/k_i, (p_i+1)*l_i/k_i) of D,
- *                                   dense row-major, no padding (R11)
+ *   data slice      PAPER.md:86     device r holds the box [p_i*c_i, (p_i+1)*c_i) of D, c_i = l_i/k_i,
+ *                                   dense row-major (R11)
+ *   uneven split    PAPER.md:259, 263 ("tiling, padding", "pad it in case 6"; R5): when k_i
+ *                                   does not divide l_i, c_i = ceil(l_i/k_i) and the box is clipped to
+ *                                   D: the last shard is short, later ones may be empty.  EVERY shard
+ *                                   buffer is dense row-major of the padded local shape (c_0..c_{N-1}),
+ *                                   the box at its origin; padding is never read, and its content after
+ *                                   a call is unspecified (execute/pack/unpack leave it untouched,
+ *                                   reshard_execute_host may overwrite it)
  *   unit task       PAPER.md:90, 482-492 (App. B.2): slices = product of the per-dim intervals cut
  *                                   at every source and destination shard boundary; senders N_i =
  *                                   source devices holding the slice, receivers M_i = destination
@@ -58,7 +65,7 @@ typedef enum rs_status {
     RS_EINVAL = 1,        /* null pointer, non-positive extent, bad elem_bytes, bad index      */
     RS_ESPEC = 2,         /* unparsable spec, wrong entry count, mesh axis out of range or used
                              by two tensor dims (R3)                                 */
-    RS_EDIVIS = 3,        /* l_i not divisible by the sharding degree k_i (R5)        */
+    RS_EDIVIS = 3,        /* l_i not divisible by the sharding degree k_i, with RS_EVEN_ONLY    */
     RS_EUNSUPPORTED = 4,  /* more than RS_MAX_DEVICES devices, > 2^31-1 rows per slice, ...     */
     RS_ENOMEM = 5,
     RS_ECUDA = 6          /* a CUDA runtime call failed; text via reshard_last_error()          */
@@ -73,7 +80,9 @@ enum {
     RS_PATH_AUTO   = 0x00,  /* executor chosen per operation from alignment and run length        */
     RS_PATH_LSU    = 0x10,  /* force the register path: 128-bit ld.global -> st.global x k        */
     RS_PATH_BULK   = 0x20,  /* force the TMA path: cp.async.bulk global->smem ring->global x k    */
-    RS_HOST_ONLY   = 0x100  /* build host tables only: no CUDA call, execute/pack/unpack refuse   */
+    RS_HOST_ONLY   = 0x100, /* build host tables only: no CUDA call, execute/pack/unpack refuse   */
+    RS_EVEN_ONLY   = 0x200  /* reject l_i not divisible by k_i with RS_EDIVIS ("evenly sharded",
+                               PAPER.md:64) instead of padding the last shard (R5)      */
 };
 #define RS_PATH_MASK 0xF0
 
@@ -123,7 +132,7 @@ typedef struct rs_plan_info {
     int32_t n_slices;                /* unit tasks (App. B.2)                                      */
     int32_t n_messages;              /* non-empty (sender, receiver) pairs                         */
     int64_t tensor_bytes;            /* size(D) * e                                                */
-    int64_t src_shard_bytes;         /* bytes of ONE source shard (all equal)                      */
+    int64_t src_shard_bytes;         /* bytes of ONE source shard buffer (all equal; padded, R5)   */
     int64_t dst_shard_bytes;         /* bytes of ONE destination shard                             */
     int64_t unique_read_bytes;       /* = tensor_bytes: every element read once      */
     int64_t write_bytes;             /* = tensor_bytes * r_B (r_B = destination replication)       */
@@ -182,9 +191,9 @@ RS_API void reshard_plan_destroy(rs_plan *plan);      /* NULL is allowed */
 /* ---- queries (all host-side, no CUDA) ------------------------------------------------------ */
 RS_API rs_status reshard_plan_info(const rs_plan *plan, rs_plan_info *out);
 RS_API rs_status reshard_op_info(const rs_plan *plan, int32_t op, rs_op_info *out);
-/* local shard shape l_i / k_i of one side; out [HOST, ndim] */
+/* (padded) local shard shape c_i = ceil(l_i / k_i) of one side; out [HOST, ndim] */
 RS_API rs_status reshard_plan_local_shape(const rs_plan *plan, int32_t side, int64_t *out);
-/* box [lo, hi) of D that device `dev` of `side` holds; lo, hi [HOST, ndim] */
+/* box [lo, hi) of D that device `dev` of `side` holds (clipped to D, may be empty); lo, hi [HOST, ndim] */
 RS_API rs_status reshard_plan_device_box(const rs_plan *plan, int32_t side, int32_t dev, int64_t *lo, int64_t *hi);
 /* unit task i: box, chosen sender, candidate senders N_i, receivers M_i.
  * senders [HOST, n_src] / receivers [HOST, n_dst] may be NULL. */

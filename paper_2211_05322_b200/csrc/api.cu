@@ -124,8 +124,8 @@ rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int32_t ele
     P->sched.seed = opts->seed;
     rs_status st;
     try {
-        st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, &P->A);
-        if (st == RS_OK) st = rs::make_layout(global_shape, ndim, dst_mesh_shape, dst_mesh_ndim, dst_spec, &P->B);
+        st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, (flags & RS_EVEN_ONLY) != 0, &P->A);
+        if (st == RS_OK) st = rs::make_layout(global_shape, ndim, dst_mesh_shape, dst_mesh_ndim, dst_spec, (flags & RS_EVEN_ONLY) != 0, &P->B);
         if (st == RS_OK) st = rs::build_slices(P);
         if (st == RS_OK) {
             P->exec_order.resize(P->slices.size());

@@ -52,7 +52,7 @@ static rs_status parse_spec(const char *text, int ndim, int mesh_ndim, Layout *L
 }
 
 rs_status make_layout(const int64_t *shape, int ndim, const int32_t *mesh, int mesh_ndim, const char *spec,
-                      Layout *L) {
+                      bool even_only, Layout *L) {
     if (!shape || !mesh || !spec) { set_error("null argument"); return RS_EINVAL; }
     if (ndim < 1 || ndim > RS_MAX_NDIM) { set_error("ndim out of range"); return RS_EINVAL; }
     if (mesh_ndim < 1 || mesh_ndim > RS_MAX_MESH_NDIM) { set_error("mesh_ndim out of range"); return RS_EINVAL; }
@@ -75,9 +75,9 @@ rs_status make_layout(const int64_t *shape, int ndim, const int32_t *mesh, int m
     for (int i = 0; i < ndim; i++) {
         int64_t k = 1;
         for (int j = 0; j < L->n_axes[i]; j++) k *= L->mesh[L->axes[i][j]];
-        if (L->shape[i] % k) { set_error("tensor dim not divisible by its sharding degree (R5)"); return RS_EDIVIS; }
+        if (even_only && L->shape[i] % k) { set_error("tensor dim not divisible by its sharding degree (RS_EVEN_ONLY)"); return RS_EDIVIS; }
         L->degree[i] = k;
-        L->local[i] = L->shape[i] / k;
+        L->local[i] = (L->shape[i] + k - 1) / k;              // R5: padded extent c_i = ceil(l_i / k_i)
     }
     // shard index p_i of every device: row-major coordinates, first listed axis most
     // significant (R2).
@@ -98,8 +98,8 @@ rs_status make_layout(const int64_t *shape, int ndim, const int32_t *mesh, int m
 void device_box(const Layout &L, int dev, int64_t *lo, int64_t *hi) {
     for (int i = 0; i < L.ndim; i++) {
         int64_t p = L.shard_index[(size_t)dev * L.ndim + i];
-        lo[i] = p * L.local[i];
-        hi[i] = lo[i] + L.local[i];
+        lo[i] = std::min(p * L.local[i], L.shape[i]);         // R5: clipped; empty when p c_i >= l_i
+        hi[i] = std::min((p + 1) * L.local[i], L.shape[i]);
     }
 }
 
@@ -113,8 +113,8 @@ rs_status build_slices(Plan *P) {
     int64_t n_slices = 1;
     for (int d = 0; d < N; d++) {
         std::vector<int64_t> &c = cut[d];
-        for (int64_t j = 0; j <= A.degree[d]; j++) c.push_back(j * A.local[d]);
-        for (int64_t j = 0; j <= B.degree[d]; j++) c.push_back(j * B.local[d]);
+        for (int64_t j = 0; j <= A.degree[d]; j++) c.push_back(std::min(j * A.local[d], A.shape[d]));
+        for (int64_t j = 0; j <= B.degree[d]; j++) c.push_back(std::min(j * B.local[d], A.shape[d]));
         std::sort(c.begin(), c.end());
         c.erase(std::unique(c.begin(), c.end()), c.end());
         n_slices *= (int64_t)c.size() - 1;                    // #slices = prod (#Cut(d) - 1)

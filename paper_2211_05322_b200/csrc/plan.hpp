@@ -23,7 +23,7 @@ struct Layout {                          // one side of the task: (shape, mesh, 
     int n_axes[RS_MAX_NDIM];             // 0 => R
     int axes[RS_MAX_NDIM][RS_MAX_MESH_NDIM];
     int64_t degree[RS_MAX_NDIM];         // k_i
-    int64_t local[RS_MAX_NDIM];          // l_i / k_i
+    int64_t local[RS_MAX_NDIM];          // c_i = ceil(l_i / k_i): padded local extent (R5)
     int n_dev = 0;
     std::vector<int64_t> shard_index;    // [n_dev][ndim]: p_i of every device
     int64_t shard_elems() const { int64_t n = 1; for (int i = 0; i < ndim; i++) n *= local[i]; return n; }
@@ -105,7 +105,7 @@ void set_error(const std::string &msg);
 const std::string &last_error();
 
 rs_status make_layout(const int64_t *shape, int ndim, const int32_t *mesh, int mesh_ndim, const char *spec,
-                      Layout *L);
+                      bool even_only, Layout *L);
 void device_box(const Layout &L, int dev, int64_t *lo, int64_t *hi);
 rs_status build_slices(Plan *P);                       // a2 + a3
 void choose_senders(Plan *P);                          // a4

@@ -274,8 +274,10 @@ rs_status build_slabs(Plan *P, const int64_t *sA, const int64_t *sB, int64_t ten
         for (int q = 0; q < B.n_dev; q++) {
             int64_t lo_r[RS_MAX_NDIM], hi_r[RS_MAX_NDIM];
             device_box(B, q, lo_r, hi_r);
+            bool empty = false;                               // R5: a device past the end of some dim holds nothing
+            for (int d = 1; d < N; d++) empty = empty || lo_r[d] >= hi_r[d];
             int64_t a = std::max(b0, lo_r[0]), b = std::min(b1, hi_r[0]);
-            if (a < b) S.down.push_back(HostCopy{q, (a - lo_r[0]) * sB[0], (b - a) * sB[0]});
+            if (a < b && !empty) S.down.push_back(HostCopy{q, (a - lo_r[0]) * sB[0], (b - a) * sB[0]});
         }
         P->slabs.push_back(std::move(S));
     }

@@ -12,12 +12,20 @@ def make_plan(w, flags=0):
 
 
 def device_inputs(w, plan, device):
-    """(D, src shards) on `device`; shard r = D[box_r].contiguous() in the container dtype."""
+    """(D, src shards) on `device`; shard r = D[box_r] at the origin of a dense buffer of the padded
+    local shape (zero padding when the partition is uneven), in the container dtype."""
     D = inputs.global_tensor_torch(w, device)
+    local = plan.local_shape(rs.RS_SRC)
     src = []
     for r in range(plan.info.n_src):
         lo, hi = plan.device_box(rs.RS_SRC, r)
-        src.append(D[tuple(slice(a, b) for a, b in zip(lo, hi))].contiguous())
+        box = D[tuple(slice(a, b) for a, b in zip(lo, hi))]
+        if tuple(box.shape) == tuple(local):
+            src.append(box.contiguous())
+        else:
+            t = torch.zeros(local, dtype=D.dtype, device=device)
+            t[tuple(slice(0, n) for n in box.shape)] = box
+            src.append(t)
     return D, src
 
 

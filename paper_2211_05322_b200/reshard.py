@@ -18,6 +18,7 @@ RS_OK, RS_EINVAL, RS_ESPEC, RS_EDIVIS, RS_EUNSUPPORTED, RS_ENOMEM, RS_ECUDA = ra
 RS_LB_GREEDY, RS_LB_NAIVE = 0x0, 0x1
 RS_PATH_AUTO, RS_PATH_LSU, RS_PATH_BULK = 0x00, 0x10, 0x20
 RS_HOST_ONLY = 0x100
+RS_EVEN_ONLY = 0x200
 RS_OP_EXECUTE, RS_OP_PACK, RS_OP_UNPACK, RS_OP_EXECUTE_SLABS = 0, 1, 2, 3
 RS_SRC, RS_DST = 0, 1
 RS_SCHED_NONE, RS_SCHED_NAIVE, RS_SCHED_LOAD_BALANCE, RS_SCHED_DFS, RS_SCHED_GREEDY, RS_SCHED_ENSEMBLE = range(6)

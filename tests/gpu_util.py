@@ -36,9 +36,22 @@ def oracle_slices(shape, mesh, spec):
     return out
 
 
-def device_shards_from_global(D, mesh, spec):
-    """D: device tensor of the global shape -> list of dense device shards (oracle boxes)"""
-    return [D[idx].contiguous() for idx in oracle_slices(tuple(D.shape), mesh, spec)]
+def padded(D, idx, local, fill=0):
+    """the shard buffer of one device: dense, padded local shape (R5), D[idx] at its origin, every
+    padding byte = fill"""
+    box = D[idx]
+    if tuple(box.shape) == tuple(local):
+        return box.contiguous()
+    out = torch.empty(tuple(local), dtype=D.dtype, device=D.device)
+    out.view(torch.uint8).fill_(fill)
+    out[tuple(slice(0, n) for n in box.shape)] = box
+    return out
+
+
+def device_shards_from_global(D, mesh, spec, fill=0):
+    """D: device tensor of the global shape -> list of dense (padded) device shards (oracle boxes)"""
+    local = do.local_shape(tuple(D.shape), mesh, spec)
+    return [padded(D, idx, local, fill) for idx in oracle_slices(tuple(D.shape), mesh, spec)]
 
 
 def run_small(shape, np_dtype, sm, ss, dm, ds, flags=0, seed=1, src_offset=0, dst_offset=0, opts=None):
@@ -47,7 +60,7 @@ def run_small(shape, np_dtype, sm, ss, dm, ds, flags=0, seed=1, src_offset=0, ds
     rng = np.random.default_rng(seed)
     D = np.frombuffer(rng.bytes(int(np.prod(shape)) * e), dtype=np_dtype).reshape(shape)
     src = do.shards_from_global(D, sm, ss)
-    want = do.reshard(shape, sm, ss, dm, ds, src)
+    want = do.reshard(shape, sm, ss, dm, ds, src, fill=0xA5)      # padding (R5) must come back untouched
     p = rs.Plan(shape, e, sm, ss, dm, ds, flags, opts)
     src_d = [torch.zeros(s.nbytes + 64, dtype=torch.uint8, device=dev()) for s in src]
     for t, s in zip(src_d, src):

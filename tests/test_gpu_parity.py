@@ -35,6 +35,13 @@ SMALL = [
     ((64, 96, 160), (2, 4), "S0,R,S1", (2, 4), "S0,S1,R"),           # several tiles + ragged tail (160*e/4)
     ((48, 1000), (2, 2), "S0,S1", (2, 2), "S1,S0"),
     ((3, 5, 7), (1,), "R,R,R", (1,), "R,R,R"),                       # 1 device -> 1 device: memcpy
+    # uneven partitions (R5): padded buffers, short and empty shards
+    ((10,), (3,), "S0", (4,), "S0"),
+    ((7, 9), (2, 4), "S1,S0", (4, 2), "S0,S1"),
+    ((7, 5, 3), (2, 3), "S1,R,S0", (3, 2), "R,S0,S1"),
+    ((2, 6), (4,), "S0,R", (2,), "S0,R"),
+    ((90, 100, 40), (2, 4), "S0,R,R", (3, 4), "S0,R,R"),             # Table 2 case 6 in small
+    ((50, 70, 96), (2, 4), "S0,S1,R", (3, 2), "S1,R,S0"),            # uneven on three dims, several tiles
 ]
 
 
@@ -121,8 +128,10 @@ def _check_full_size(w, path=rs.RS_PATH_AUTO, n_samples=4096):
     p.execute(gu.ptrs(src), gu.ptrs(dst), gu.stream())
     torch.cuda.synchronize()
     idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
-    for q in range(p.info.n_dst):
-        assert torch.equal(dst[q].view(torch.uint8), D[idx[q]].contiguous().view(torch.uint8)), "%s dev %d" % (w.name, q)
+    local = do.local_shape(w.shape, w.dst_mesh, w.dst_spec)
+    assert tuple(local) == tuple(p.local_shape(rs.RS_DST))
+    for q in range(p.info.n_dst):                             # padding (R5) must still hold the 0x5A fill
+        assert torch.equal(dst[q].view(torch.uint8), gu.padded(D, idx[q], local, 0x5A).view(torch.uint8)), "%s dev %d" % (w.name, q)
     rng = np.random.default_rng(7)
     n_local = int(np.prod(p.local_shape(rs.RS_DST)))
     flat_src = [s.reshape(-1) for s in src]
@@ -130,6 +139,10 @@ def _check_full_size(w, path=rs.RS_PATH_AUTO, n_samples=4096):
         js = rng.integers(0, n_local, size=n_samples // p.info.n_dst + 1)
         js[0], js[-1] = 0, n_local - 1
         srcs = [do.element_source(w.shape, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, q, int(j)) for j in js]
+        keep = [i for i, s in enumerate(srcs) if s[0] >= 0]   # (q, j) in the padding has no source
+        if not keep:
+            continue
+        js, srcs = js[keep], [srcs[i] for i in keep]
         got = dst[q].reshape(-1)[torch.from_numpy(js).to(gu.dev())].cpu()
         want = torch.stack([flat_src[d][l] for d, l, _g in srcs]).cpu()
         assert torch.equal(got.view(torch.uint8), want.view(torch.uint8))
@@ -162,7 +175,7 @@ def test_sweep_small_sizes(pair, mib):
     _check_full_size(inputs.sweep_workload(pair, "m8", mib << 20), n_samples=512)
 
 
-@pytest.mark.parametrize("case", [1, 2, 3, 4, 5, 7, 8, 9])
+@pytest.mark.parametrize("case", [1, 2, 3, 4, 5, 6, 7, 8, 9])
 def test_table2_cases_full_size(case):
     """the paper's microbenchmark layouts on (1024,1024,512) at 2 B/elt"""
     _check_full_size(inputs.table2_workload(case), n_samples=512)

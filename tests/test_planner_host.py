@@ -37,6 +37,14 @@ LAYOUTS = [
     ((8, 4), (2, 2), "S0,S1", (4,), "S0,R"),
     ((4, 6, 5, 3), (2, 2), "S0,S1,R,R", (2, 2), "S1,R,R,R"),      # odd inner extents: narrow vectors
     ((16, 7), (4,), "S0,R", (2,), "R,R"),
+    # uneven partitions (R5): padded shard buffers, short / empty last shards, unequal slices
+    ((10,), (3,), "S0", (4,), "S0"),
+    ((5, 4), (2, 2), "S0,R", (2, 2), "R,S1"),
+    ((7, 9), (2, 4), "S1,S0", (4, 2), "S0,S1"),
+    ((7, 5, 3), (2, 3), "S1,R,S0", (3, 2), "R,S0,S1"),
+    ((2, 6), (4,), "S0,R", (2,), "S0,R"),
+    ((9, 10, 4), (2, 4), "S0,R,R", (3, 4), "S0,R,R"),               # Table 2 case 6 in small
+    ((11, 6), (2, 4), "S01,R", (2, 3), "R,S10"),
 ]
 
 
@@ -77,8 +85,9 @@ def test_error_codes():
     assert code((8, 8), 2, (2, 2), "S0,R,R", (2, 2), "R,R") == rs.RS_ESPEC         # too many
     assert code((8, 8), 2, (2, 2), "S,R", (2, 2), "R,R") == rs.RS_ESPEC            # S without axis
     assert code((8, 8), 2, (2, 2), "X,R", (2, 2), "R,R") == rs.RS_ESPEC
-    assert code((6, 8), 2, (2, 4), "S1,R", (2, 2), "R,R") == rs.RS_EDIVIS          # 6 % 4 (R5)
-    assert code((1024, 1024, 512), 2, (2, 4), "S0RR", (3, 4), "S0RR") == rs.RS_EDIVIS   # Table 2 case 6
+    assert code((6, 8), 2, (2, 4), "S1,R", (2, 2), "R,R", rs.RS_EVEN_ONLY) == rs.RS_EDIVIS     # 6 % 4, strict mode (R5)
+    assert code((1024, 1024, 512), 2, (2, 4), "S0RR", (3, 4), "S0RR", rs.RS_EVEN_ONLY) == rs.RS_EDIVIS   # Table 2 case 6
+    assert _plan((6, 8), 2, (2, 4), "S1,R", (2, 2), "R,R").local_shape(rs.RS_SRC) == (2, 8)    # default: padded last shard
     assert code((8, 8), 3, (2, 2), "R,R", (2, 2), "R,R") == rs.RS_EINVAL           # elem_bytes
     assert code((8, 0), 2, (2, 2), "R,R", (2, 2), "R,R") == rs.RS_EINVAL
     assert code((8, 8), 2, (0, 2), "R,R", (2, 2), "R,R") == rs.RS_EINVAL
@@ -201,8 +210,21 @@ def _bytes(a):
     return np.ascontiguousarray(a).view(np.uint8).reshape(-1)
 
 
+def _valid_bytes(shape, mesh, spec, e):
+    """per device: 1 for every byte of the padded shard buffer that holds an element of D (oracle boxes)"""
+    out = []
+    local = do.local_shape(shape, mesh, spec)
+    for r in range(do.num_devices(mesh)):
+        lo, hi = do.device_box(shape, mesh, spec, r)
+        m = np.zeros(local + (e,), np.int32)
+        m[tuple(slice(0, h - l) for l, h in zip(lo, hi))] = 1
+        out.append(m.reshape(-1))
+    return out
+
+
 def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None, opts=None):
     e = np.dtype(dtype).itemsize
+    once = _valid_bytes(shape, dm, ds, e)
     old = {}
     for k, v in (env or {}).items():
         old[k] = os.environ.get(k)
@@ -225,13 +247,13 @@ def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None, opts=None):
     ti.replay(p, rs.RS_OP_EXECUTE, [_bytes(s) for s in src], dst, cnt)
     for q in range(n_dst):
         assert np.array_equal(dst[q], _bytes(want[q])), "execute tables differ from the oracle on device %d" % q
-        assert (cnt[q] == 1).all(), "execute tables do not write every byte exactly once"
+        assert np.array_equal(cnt[q], once[q]), "execute tables do not write every byte exactly once (padding: never)"
     # the slab-cut execute table that reshard_execute_host pipelines over: same result, same exactly-once
     dst3 = [np.zeros(want[0].nbytes, np.uint8) for _ in range(n_dst)]
     cnt3 = [np.zeros(want[0].nbytes, np.int32) for _ in range(n_dst)]
     ti.replay(p, rs.RS_OP_EXECUTE_SLABS, [_bytes(s) for s in src], dst3, cnt3)
     for q in range(n_dst):
-        assert np.array_equal(dst3[q], _bytes(want[q])) and (cnt3[q] == 1).all()
+        assert np.array_equal(dst3[q], _bytes(want[q])) and np.array_equal(cnt3[q], once[q])
     # pack -> message contents as the plan oracle states them -> unpack
     arena = [np.zeros(p.info.arena_bytes, np.uint8)]
     acnt = [np.zeros(p.info.arena_bytes, np.int32)]
@@ -253,7 +275,7 @@ def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None, opts=None):
     ti.replay(p, rs.RS_OP_UNPACK, arena, dst2, cnt2)
     for q in range(n_dst):
         assert np.array_equal(dst2[q], _bytes(want[q]))
-        assert (cnt2[q] == 1).all()
+        assert np.array_equal(cnt2[q], once[q])
     return p
 
 
@@ -341,7 +363,7 @@ def _layouts(draw):
                 return mesh, ",".join(spec)
     sm, ss = side()
     dm, ds = side()
-    shape = tuple(draw(st.sampled_from([12, 24])) for _ in range(ndim))
+    shape = tuple(draw(st.sampled_from([12, 24, 7, 10, 1])) for _ in range(ndim))     # even and uneven (R5) splits
     if ndim >= 3:
         shape = tuple(min(s, 12) for s in shape)
     return shape, sm, ss, dm, ds, draw(st.sampled_from([np.uint8, np.int16, np.int32])), draw(st.sampled_from([128, 512, 16384]))
@@ -351,12 +373,12 @@ def _layouts(draw):
 @given(_layouts())
 def test_random_layouts_tables_equal_oracle(layout):
     shape, sm, ss, dm, ds, dtype, tile = layout
-    try:
-        do.local_shape(shape, sm, ss), do.local_shape(shape, dm, ds)
-    except do.OracleError:
-        with pytest.raises(rs.ReshardError):
-            _plan(shape, 1, sm, ss, dm, ds)
-        return
+    even = all(l % k == 0 for mesh, spec in ((sm, ss), (dm, ds))
+               for l, k in zip(shape, po.degrees(shape, mesh, po.parse_spec(spec, len(shape), len(mesh)))))
+    if not even:
+        with pytest.raises(rs.ReshardError) as ei:
+            _plan(shape, 1, sm, ss, dm, ds, rs.RS_EVEN_ONLY)
+        assert ei.value.code == rs.RS_EDIVIS
     _check_tables(shape, dtype, sm, ss, dm, ds, env={"RS_LSU_TILE_BYTES": tile, "RS_BULK_TILE_BYTES": tile})
 
 
