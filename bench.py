@@ -41,7 +41,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", help="c4 (default, 1.5 GiB GPT activation), c2, c3, t2_<n>, sweep_<pair>_<m8|m4>_<MiB>MiB")
-    ap.add_argument("--path", default="auto", choices=["auto", "lsu", "bulk"])
+    ap.add_argument("--path", default="auto", choices=["auto", "lsu", "bulk", "shift"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -213,7 +213,7 @@ def run_ours(args):
         multi.barrier(torch.cuda.synchronize)
 
     w = inputs.get_workload(args.workload)
-    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK}[args.path]
+    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK, "shift": rs.RS_PATH_BULK_SHIFT}[args.path]
     t0 = time.perf_counter()
     plan = harness.make_plan(w, flags)                     # rows a1..a5, once, outside the timed region
     plan_ms = (time.perf_counter() - t0) * 1e3
@@ -309,7 +309,7 @@ def run_ours(args):
 
     peak, peak_src = peak_hbm()
     names = ["reshard_execute", "reshard_pack", "reshard_unpack"]
-    pname = {rs.RS_PATH_LSU: "rs_copy_lsu", rs.RS_PATH_BULK: "rs_copy_bulk"}
+    pname = {rs.RS_PATH_LSU: "rs_copy_lsu", rs.RS_PATH_BULK: "rs_copy_bulk", rs.RS_PATH_BULK_SHIFT: "rs_copy_bulk_shift"}
     kernels = {n: {"kernel": pname[o.path], "ms": k_ms[j], "best_ms": k_best[j], "bytes": op_bytes[j],
                    "GB/s": op_bytes[j] / (k_ms[j] * 1e-3) / 1e9, "grid": o.grid, "block": o.block,
                    "smem": o.smem_bytes, "tiles": o.n_tiles, "tile_bytes": o.tile_bytes}
@@ -362,7 +362,7 @@ def run_sweep(args):
     stream = torch.cuda.current_stream()
     sh = stream.cuda_stream
     peak, _ = peak_hbm()
-    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK}[args.path]
+    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK, "shift": rs.RS_PATH_BULK_SHIFT}[args.path]
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     K = max(3, min(args.steps, 30))
     rows = []
@@ -400,7 +400,7 @@ def run_sweep(args):
                 e1.synchronize()
                 ts.append(e0.elapsed_time(e1))
             med = statistics.median(ts)
-            row[opname] = {"kernel": "rs_copy_bulk" if o.path == rs.RS_PATH_BULK else "rs_copy_lsu", "bytes": nbytes,
+            row[opname] = {"kernel": {rs.RS_PATH_BULK: "rs_copy_bulk", rs.RS_PATH_BULK_SHIFT: "rs_copy_bulk_shift"}.get(o.path, "rs_copy_lsu"), "bytes": nbytes,
                            "ms": med, "best_ms": min(ts), "GB/s": nbytes / med / 1e6, "frac_of_copy_peak": nbytes / med / 1e6 / peak,
                            "tiles": o.n_tiles, "tile_bytes": o.tile_bytes, "grid": o.grid, "l2_flushed": do_flush}
         plan.close()

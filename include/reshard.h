@@ -80,6 +80,8 @@ enum {
     RS_PATH_AUTO   = 0x00,  /* executor chosen per operation from alignment and run length        */
     RS_PATH_LSU    = 0x10,  /* force the register path: 128-bit ld.global -> st.global x k        */
     RS_PATH_BULK   = 0x20,  /* force the TMA path: cp.async.bulk global->smem ring->global x k    */
+    RS_PATH_BULK_SHIFT = 0x30, /* force TMA loads + byte-shifted 128-bit register stores (any alignment;
+                               what AUTO picks for runs >= 512 B that are not 16-byte aligned)     */
     RS_HOST_ONLY   = 0x100, /* build host tables only: no CUDA call, execute/pack/unpack refuse   */
     RS_EVEN_ONLY   = 0x200  /* reject l_i not divisible by k_i with RS_EDIVIS ("evenly sharded",
                                PAPER.md:64) instead of padding the last shard (R5)      */
@@ -143,7 +145,7 @@ typedef struct rs_plan_info {
 } rs_plan_info;
 
 typedef struct rs_op_info {
-    int32_t path;                    /* RS_PATH_LSU or RS_PATH_BULK actually selected              */
+    int32_t path;                    /* RS_PATH_LSU, RS_PATH_BULK or RS_PATH_BULK_SHIFT selected   */
     int32_t vec_bytes;               /* widest access every offset/stride/run of the op allows     */
     int32_t n_tasks;                 /* copy tasks (execute/pack: one per slice; unpack: per
                                         (slice, receiver))                                         */

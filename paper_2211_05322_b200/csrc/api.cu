@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -66,6 +67,8 @@ rs_status upload(rs::Plan *P) {
     for (rs::OpTables &o : P->op) smem = std::max(smem, (int)RS_SMEM_MAX);
     e = rs::prepare_bulk(smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(rs_copy_bulk)");
+    e = rs::prepare_bulk_shift(smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(rs_copy_bulk_shift)");
     // reshard_execute_host pipeline: plan-owned upload / download streams and per-slab events
     for (int i = 0; i < 2; i++) {
         cudaStream_t st;
@@ -303,15 +306,22 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     RsOpDev dev = op.dev;
     if (tile_end > tile_begin) { dev.tiles += tile_begin; dev.n_tiles = tile_end - tile_begin; }   // one slab
     const int64_t n_tiles = dev.n_tiles;
+    const bool bulk_family = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_BULK_SHIFT;
+    const int warps = op.info.block / 32;
     if (op.info.path == RS_PATH_BULK && align == 16) {
-        const int warps = op.info.block / 32;
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         e = rs::launch_bulk(dev, pt, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                             (uint32_t)op.info.tile_bytes, st);
-    } else {                                                  // also the fallback for under-aligned pointers
-        const int64_t cap = op.info.path == RS_PATH_BULK ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
+    } else if (op.info.path == RS_PATH_BULK_SHIFT) {          // layout not 16-byte aligned: TMA loads, shifted stores
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
+        e = rs::launch_bulk_shift(dev, pt, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
+                                  op.shift_stage, st);
+    } else {                                                  // register paths (also: aligned plan, unaligned pointers)
+        const int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));
-        e = rs::launch_lsu(dev, pt, align, grid, st);
+        static const bool no_shift = std::getenv("RS_NO_SHIFT") != nullptr;   // A/B switch for measurements
+        if (align < 16 && !no_shift) e = rs::launch_shift(dev, pt, grid, st);  // any alignment, 16-byte accesses
+        else e = rs::launch_lsu(dev, pt, align, grid, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
     return RS_OK;

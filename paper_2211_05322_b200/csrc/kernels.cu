@@ -168,6 +168,122 @@ rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// shifted register path: any byte alignment on either side at 16-byte access width.
+//
+// A row of n bytes goes from s to d with s, d arbitrary.  The row is cut into SLOTS = the 16-byte
+// ALIGNED windows of the destination it touches.  The value of a slot is assembled from the two
+// aligned 16-byte source words that hold its bytes (byte-granular funnel shift).  A slot that lies
+// fully inside the row is written with one 16-byte store; the at most two partial slots of a row
+// (head, tail) are written with independent byte stores of the same assembled value.  A source word
+// is loaded only if it contains at least one byte of the row, so a load never leaves the page of a
+// byte the caller owns.  (row, slot) pairs are walked 32 at a time like the vectors of rs_copy_lsu.
+// With k destinations the shift differs per destination, so the source is re-read per destination
+// (L1/L2 hits).
+
+__device__ __forceinline__ uint4 ld_word16(const char *p) {       // ld.global.nc, allocating in L1: the
+    return __ldg(reinterpret_cast<const uint4 *>(p));              // neighbour slot re-reads this word
+}
+
+// bytes [delta, delta + 16) of the 32-byte window lo:hi (delta in 0..15)
+__device__ __forceinline__ uint4 shift_window(const uint4 lo, const uint4 hi, uint32_t delta) {
+    const bool w2 = delta & 8u, w1 = delta & 4u;
+    const uint32_t b = (delta & 3u) * 8u;
+    const uint32_t x0 = w2 ? lo.z : lo.x, x1 = w2 ? lo.w : lo.y, x2 = w2 ? hi.x : lo.z, x3 = w2 ? hi.y : lo.w,
+                   x4 = w2 ? hi.z : hi.x, x5 = w2 ? hi.w : hi.y;
+    const uint32_t y0 = w1 ? x1 : x0, y1 = w1 ? x2 : x1, y2 = w1 ? x3 : x2, y3 = w1 ? x4 : x3, y4 = w1 ? x5 : x4;
+    return make_uint4(__funnelshift_r(y0, y1, b), __funnelshift_r(y1, y2, b), __funnelshift_r(y2, y3, b),
+                      __funnelshift_r(y3, y4, b));
+}
+
+template <int U>
+__global__ void __launch_bounds__(RS_LSU_THREADS, RS_LSU_CTAS_DEFAULT)
+rs_copy_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs) {
+    __shared__ RsDesc ring[RS_LSU_THREADS / 32][32];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = RS_LSU_THREADS / 32;
+    RsDesc *descs = ring[warp];
+    const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
+    const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
+
+    for (int it = 0; it < n_my; ++it) {
+        if ((it & 31) == 0) {
+            __syncwarp();
+            if (it + lane < n_my) resolve_desc(op, ptrs, worker + (uint32_t)(it + lane) * n_workers, descs + lane);
+            __syncwarp();
+        }
+        const RsDesc *d = descs + (it & 31);
+        const uint32_t n_rows = d->n_rows, k = d->k, n = d->col_bytes;
+        const RsDst *__restrict__ dsts = op.dsts + d->dst_first;
+        const char *src = d->src;
+        const int64_t s0 = d->s0, d0 = d->d0, dst_rel = d->dst_rel;
+        if (!(d->flags & RS_TILE_FAST)) {                      // GENERIC tiles (rare): byte by byte
+            const RsTask *__restrict__ T = op.tasks + d->task;
+            const uint32_t total = n_rows * n;
+            for (uint32_t v = lane; v < total; v += 32) {
+                const uint32_t r = v / n, c = v - r * n;
+                int64_t so, doff;
+                generic_row(T, d->lin + r, &so, &doff);
+                const char x = src[dst_rel + so + c];
+                for (uint32_t j = 0; j < k; j++) {
+                    const RsDst dd = dsts[j];
+                    ptrs.dst[dd.buf][dd.off + dst_rel + doff + c] = x;
+                }
+            }
+            continue;
+        }
+        const uint32_t SL = (n + 30u) >> 4;                     // slots per row: ceil((15 + n) / 16) at most
+        const uint32_t total = n_rows * SL;
+        const uint32_t q32 = 32u / SL, r32 = 32u - q32 * SL;   // how (row, slot) move when the index grows by 32
+        for (uint32_t j = 0; j < k; j++) {
+            const RsDst dd = dsts[j];
+            char *dp = ptrs.dst[dd.buf] + dd.off + dst_rel;
+            uint32_t row = (uint32_t)lane / SL, slot = (uint32_t)lane - row * SL;
+            for (uint32_t v0 = lane; v0 < total; v0 += 32 * U) {
+                uint4 val[U];
+                uint32_t r = row, c = slot;
+#pragma unroll
+                for (int u = 0; u < U; u++) {                   // U independent slots in flight
+                    if (v0 + 32 * u < total) {
+                        const char *sr = src + (int64_t)r * s0;
+                        const int32_t X = (int32_t)(c * 16u) - (int32_t)((uintptr_t)(dp + (int64_t)r * d0) & 15u);
+                        const char *S = sr + X;                 // source of the slot's first byte (head slot: before the row)
+                        const uint32_t delta = (uint32_t)((uintptr_t)S & 15u);
+                        const char *A = S - delta;
+                        // a word is loaded only if it holds a byte of the row (always true for a full slot)
+                        const bool need_lo = A + 16 > sr && A < sr + n;
+                        const bool need_hi = delta && A + 32 > sr && A + 16 < sr + n;
+                        const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+                        const uint4 lo = need_lo ? ld_word16(A) : zero;
+                        const uint4 hi = need_hi ? ld_word16(A + 16) : zero;
+                        val[u] = shift_window(lo, hi, delta);
+                    }
+                    r += q32; c += r32;
+                    if (c >= SL) { c -= SL; r++; }
+                }
+                uint32_t r2 = row, c2 = slot;
+#pragma unroll
+                for (int u = 0; u < U; u++) {
+                    if (v0 + 32 * u < total) {
+                        char *dr = dp + (int64_t)r2 * d0;
+                        const int32_t X = (int32_t)(c2 * 16u) - (int32_t)((uintptr_t)dr & 15u);
+                        if (X >= 0 && X + 16 <= (int32_t)n) {
+                            *reinterpret_cast<uint4 *>(dr + X) = val[u];
+                        } else {                                // head / tail (or a slot past the end): independent byte stores
+                            const uint32_t w[4] = {val[u].x, val[u].y, val[u].z, val[u].w};
+#pragma unroll
+                            for (int i = 0; i < 16; i++)
+                                if (X + i >= 0 && X + i < (int32_t)n) dr[X + i] = (char)(w[i >> 2] >> (8 * (i & 3)));
+                        }
+                    }
+                    r2 += q32; c2 += r32;
+                    if (c2 >= SL) { c2 -= SL; r2++; }
+                }
+                row = r; slot = c;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // TMA path
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -293,6 +409,156 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const in
 }
 
 // ------------------------------------------------------------------------------------------------
+// TMA loads + shifted register stores: the deep asynchronous load pipeline of rs_copy_bulk for rows
+// whose addresses or lengths are NOT multiples of 16 bytes.
+//
+// Loads: lane r asks the copy engine for the 16-byte ALIGNED superset of row r (from floor16(src) to
+// ceil16(src + n): at most 15 bytes before and after the row, always inside aligned words that hold
+// bytes of the row).  Row r lands at  slot + r * pitch + 16  with its first byte at (src & 15).
+// Stores: once the tile has landed the warp walks the 16-byte aligned windows of every DESTINATION
+// row, assembles each from two aligned shared-memory words (shift_window) and stores it with one
+// st.global.v4 (head / tail windows: byte stores).  Shared-memory latency is short, so a few warps
+// keep up; DRAM latency is hidden by the loads running LOOKAHEAD tiles ahead.
+
+__device__ __forceinline__ uint32_t shift_pitch(uint32_t n) { return (n + 77u) & ~15u; }   // 16 slack + 15 + n + 46
+
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 r;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+    return r;
+}
+
+// One 16-byte aligned window of a destination row, in two steps so that several windows' shared-memory
+// loads can be in flight: n bytes of the row sit in shared memory from byte address `sm`.
+struct ShiftSlot { uint4 lo, hi; int32_t X; uint32_t delta; };
+
+__device__ __forceinline__ void slot_load(ShiftSlot &t, const char *dr, uint32_t sm, uint32_t n, uint32_t c) {
+    t.X = (int32_t)(c * 16u) - (int32_t)((uintptr_t)dr & 15u);              // row byte the window starts at (>= -15)
+    if (t.X >= (int32_t)n) return;                                          // window past the end of the row
+    const uint32_t q = sm + (uint32_t)t.X;                                  // 16 bytes of slack precede the row
+    t.delta = q & 15u;
+    t.lo = lds128(q - t.delta);
+    t.hi = lds128(q - t.delta + 16u);
+}
+
+__device__ __forceinline__ void slot_store(const ShiftSlot &t, char *dr, uint32_t n) {
+    if (t.X >= (int32_t)n) return;
+    const uint4 v = shift_window(t.lo, t.hi, t.delta);
+    if (t.X >= 0 && t.X + 16 <= (int32_t)n) {
+        *reinterpret_cast<uint4 *>(dr + t.X) = v;
+    } else {                                                                // head / tail: independent byte stores
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 16; i++)
+            if (t.X + i >= 0 && t.X + i < (int32_t)n) dr[t.X + i] = (char)(w[i >> 2] >> (8 * (i & 3)));
+    }
+}
+
+__global__ void __launch_bounds__(256, 1)
+rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const int stages, const int lookahead,
+                   const uint32_t stage_bytes) {
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    const uint32_t bars = smem_u32(smem) + warp * 64;
+    RsDesc *descs = reinterpret_cast<RsDesc *>(smem + 1024) + warp * RS_DESC_RING;
+    const uint32_t ring = smem_u32(smem) + 1024 + (uint32_t)W * RS_DESC_RING * sizeof(RsDesc) +
+                          (uint32_t)warp * stages * stage_bytes;
+    if (lane == 0) {
+        for (int s = 0; s < stages; s++) mbar_init(bars + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
+    const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
+    int ld_slot = 0, st_slot = 0;
+    uint32_t st_parity = 0;
+
+    for (int it = 0; it < n_my + lookahead; ++it) {
+        if (it < n_my) {                                      // ---- load tile `it` (its slot was drained in program order)
+            if ((it & 31) == 0) {
+                const int mine = it + lane;
+                if (mine < n_my)
+                    resolve_desc(op, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
+                __syncwarp();
+            }
+            const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
+            const uint32_t n_rows = d->n_rows, n = d->col_bytes, pitch = shift_pitch(n);
+            const uint32_t bar = bars + 8 * ld_slot, slot = ring + (uint32_t)ld_slot * stage_bytes;
+            const bool fast = d->flags & RS_TILE_FAST;
+            const RsTask *__restrict__ T = op.tasks + d->task;
+            uint32_t my_bytes = 0;
+            for (uint32_t r = lane; r < n_rows; r += 32) {     // bytes this lane will ask for
+                int64_t so = (int64_t)r * d->s0, doff;
+                if (!fast) { generic_row(T, d->lin + r, &so, &doff); so += d->dst_rel; }
+                const uint32_t a = (uint32_t)((uintptr_t)(d->src + so) & 15u);
+                my_bytes += (a + n + 15u) & ~15u;
+            }
+            const uint32_t tile_bytes = __reduce_add_sync(0xffffffffu, my_bytes);
+            if (lane == 0) mbar_expect_tx(bar, tile_bytes);
+            __syncwarp();
+            for (uint32_t r = lane; r < n_rows; r += 32) {
+                int64_t so = (int64_t)r * d->s0, doff;
+                if (!fast) { generic_row(T, d->lin + r, &so, &doff); so += d->dst_rel; }
+                const char *g = d->src + so;
+                const uint32_t a = (uint32_t)((uintptr_t)g & 15u);
+                bulk_g2s(slot + r * pitch + 16u, g - a, (a + n + 15u) & ~15u, bar);
+            }
+            if (++ld_slot == stages) ld_slot = 0;
+        }
+        const int j = it - lookahead;
+        if (j >= 0) {                                         // ---- store tile j to its k destinations
+            const RsDesc *d = descs + (j & (RS_DESC_RING - 1));
+            const uint32_t n_rows = d->n_rows, n = d->col_bytes, k = d->k, pitch = shift_pitch(n);
+            const RsDst *__restrict__ dsts = op.dsts + d->dst_first;
+            const uint32_t slot = ring + (uint32_t)st_slot * stage_bytes;
+            const bool fast = d->flags & RS_TILE_FAST;
+            const RsTask *__restrict__ T = op.tasks + d->task;
+            const uint32_t SL = (n + 30u) >> 4;               // destination windows per row, at most
+            mbar_wait(bars + 8 * st_slot, st_parity);
+            for (uint32_t q = 0; q < k; q++) {                // read once (from HBM), write k times
+                const RsDst dd = dsts[q];
+                char *dp = ptrs.dst[dd.buf] + dd.off + d->dst_rel;
+                if (fast) {                                   // flat walk over (row, window), 2 windows in flight per lane
+                    const uint32_t total = n_rows * SL, q32 = 32u / SL, r32 = 32u - q32 * SL;
+                    uint32_t r = (uint32_t)lane / SL, c = (uint32_t)lane - r * SL;
+                    for (uint32_t v = lane; v < total; v += 64) {
+                        ShiftSlot t0, t1;
+                        char *dr0 = dp + (int64_t)r * d->d0, *dr1 = dr0;
+                        slot_load(t0, dr0, slot + r * pitch + 16u + (uint32_t)((uintptr_t)(d->src + (int64_t)r * d->s0) & 15u), n, c);
+                        r += q32; c += r32;
+                        if (c >= SL) { c -= SL; r++; }
+                        const bool two = v + 32 < total;
+                        if (two) {
+                            dr1 = dp + (int64_t)r * d->d0;
+                            slot_load(t1, dr1, slot + r * pitch + 16u + (uint32_t)((uintptr_t)(d->src + (int64_t)r * d->s0) & 15u), n, c);
+                        }
+                        r += q32; c += r32;
+                        if (c >= SL) { c -= SL; r++; }
+                        slot_store(t0, dr0, n);
+                        if (two) slot_store(t1, dr1, n);
+                    }
+                } else {                                      // GENERIC tiles: row by row, lanes over windows
+                    for (uint32_t r = 0; r < n_rows; r++) {
+                        int64_t so, doff;
+                        generic_row(T, d->lin + r, &so, &doff);
+                        const uint32_t a = (uint32_t)((uintptr_t)(d->src + d->dst_rel + so) & 15u);
+                        for (uint32_t c = lane; c < SL; c += 32) {
+                            ShiftSlot t0;
+                            slot_load(t0, dp + doff, slot + r * pitch + 16u + a, n, c);
+                            slot_store(t0, dp + doff, n);
+                        }
+                    }
+                }
+            }
+            __syncwarp();                                     // every lane has read the slot ...
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // ... before the copy engine may overwrite it
+            if (++st_slot == stages) { st_slot = 0; st_parity ^= 1u; }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // host-side launchers
 
 static thread_local int64_t g_launches = 0;
@@ -318,8 +584,27 @@ cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int vec_bytes,
     return e;
 }
 
+cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st) {
+    rs_copy_shift<4><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) ++g_launches;
+    return e;
+}
+
 cudaError_t prepare_bulk(int smem_bytes) {
     return cudaFuncSetAttribute(rs_copy_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+}
+
+cudaError_t prepare_bulk_shift(int smem_bytes) {
+    return cudaFuncSetAttribute(rs_copy_bulk_shift, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+}
+
+cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
+                              int lookahead, uint32_t stage_bytes, cudaStream_t st) {
+    rs_copy_bulk_shift<<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) ++g_launches;
+    return e;
 }
 
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,

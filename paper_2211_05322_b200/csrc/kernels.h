@@ -7,8 +7,12 @@
 
 namespace rs {
 cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int vec_bytes, int grid, cudaStream_t st);
+cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st);
 cudaError_t prepare_bulk(int smem_bytes);
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
                         int lookahead, uint32_t stage_bytes, cudaStream_t st);
+cudaError_t prepare_bulk_shift(int smem_bytes);
+cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
+                              int lookahead, uint32_t stage_bytes, cudaStream_t st);
 int64_t launch_count();
 }  // namespace rs

@@ -50,6 +50,7 @@ struct OpTables {                        // one operation (execute / pack / unpa
     std::vector<RsTile> tiles;
     rs_op_info info{};
     int stages = 0, lookahead = 0;       // TMA path: ring slots per warp, loads in flight
+    uint32_t shift_stage = 0;            // rs_copy_bulk_shift: bytes per ring slot (rows padded), 0 if the path is not used
     RsOpDev dev{};                       // device copies (null for a host-only plan)
 };
 

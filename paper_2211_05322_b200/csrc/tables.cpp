@@ -164,19 +164,24 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     const uint32_t forced = P->flags & RS_PATH_MASK;
     const bool bulk_ok = align == 16 && min_run >= 16;
     int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
-             : (bulk_ok && min_run >= RS_BULK_MIN_RUN) ? RS_PATH_BULK : RS_PATH_LSU;
-    if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_LSU;   // cp.async.bulk needs 16-byte everything
+             : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
+             : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU : bulk_ok ? RS_PATH_BULK : RS_PATH_BULK_SHIFT;
+    if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_BULK_SHIFT;   // cp.async.bulk stores need 16-byte everything
     I.path = path;
+    const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT;
 
     int64_t tile_bytes;
     int workers;                                               // independent tile consumers in one launch
-    if (path == RS_PATH_BULK) {
+    if (bulk_family) {
         // short runs = many bulk copies per tile: one warp issues them too slowly, so use more,
         // smaller pipelines (t2 case 9, 512-byte runs: 3.6 TB/s with 2 warps, 5.7 with 4)
-        const bool short_runs = min_run <= RS_BULK_SHORT_RUN;
-        int warps = std::max(1, std::min(8, env_int("RS_BULK_WARPS", short_runs ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
-        int stages = std::max(2, std::min(8, env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
-        tile_bytes = env_int("RS_BULK_TILE_BYTES", short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
+        // the shifted variant assembles every 16 bytes in registers: many warps, small tiles
+        const bool short_runs = min_run <= RS_BULK_SHORT_RUN, shift = path == RS_PATH_BULK_SHIFT;
+        int warps = std::max(1, std::min(8, shift ? env_int("RS_SHIFT_WARPS", RS_SHIFT_WARPS)
+                                                  : env_int("RS_BULK_WARPS", short_runs ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
+        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+        tile_bytes = shift ? env_int("RS_SHIFT_TILE_BYTES", RS_SHIFT_TILE_BYTES)
+                           : env_int("RS_BULK_TILE_BYTES", short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
         while ((int64_t)warps * (stages * tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && tile_bytes > 1024) tile_bytes -= 1024;
         I.block = warps * 32;
@@ -205,13 +210,27 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     int64_t mr = INT64_MAX;
     for (const RsTile &t : op->tiles) mr = std::min<int64_t>(mr, t.col_bytes);
     I.min_run_bytes = op->tiles.empty() ? 0 : mr;
-    if (path == RS_PATH_BULK) {
+    op->shift_stage = 0;
+    if (bulk_family) {
+        const bool shift = path == RS_PATH_BULK_SHIFT;
         int warps = I.block / 32;
-        int stages = std::max(2, std::min(8, env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+        int64_t stage = tile_bytes;
+        if (shift) {                                           // a row of n bytes occupies (n + 77) & ~15 bytes of a ring slot
+            stage = 0;
+            for (const RsTile &t : op->tiles) stage = std::max<int64_t>(stage, (int64_t)t.n_rows * (((int64_t)t.col_bytes + 77) & ~15ll));
+            while (stages > 2 && (int64_t)warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) stages--;
+            while (warps > 1 && (int64_t)warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) warps--;
+            I.block = warps * 32;
+        }
         op->stages = stages;
-        op->lookahead = std::max(1, std::min(stages - 1, env_int("RS_BULK_LOOKAHEAD", RS_BULK_LOOKAHEAD)));
+        op->lookahead = std::max(1, std::min(stages - 1, shift ? env_int("RS_SHIFT_LOOKAHEAD", stages - 1) : env_int("RS_BULK_LOOKAHEAD", RS_BULK_LOOKAHEAD)));
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
-        I.smem_bytes = (int32_t)(warps * (stages * tile_bytes + RS_BULK_DESC_BYTES) + 1024);
+        I.smem_bytes = (int32_t)(warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024);
+        if (shift) {
+            op->shift_stage = (uint32_t)stage;
+            if (I.smem_bytes > RS_SMEM_MAX) { I.path = RS_PATH_LSU; I.smem_bytes = 0; op->shift_stage = 0; }   // rows too sparse for the ring
+        }
     } else {
         const int warps = RS_LSU_THREADS / 32;
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));

@@ -118,6 +118,10 @@ CONFIGS = {
     "c3i":  _w("c3i", (8, 320, 64, 64), "fp16", (1, 4), "S1,R,R,R", (2, 2), "R,S0,S1,R", "bits", 3),
     "c3ii": _w("c3ii", (8, 320, 64, 64), "fp16", (1, 4), "S1,R,R,R", (2, 2), "R,S0,R,R", "bits", 3),
     "c4":   _w("c4", (32, 2048, 12288), "bf16", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 4),
+    # config 4's layout pair on extents that divide nothing: uneven partitions on all three dims and runs of
+    # 6145 B at 2-byte alignment (the "tiling, padding" case of PAPER.md:259 at GPT-activation size)
+    "u4":   _w("u4", (30, 2047, 12290), "bf16", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 6),
+    "u4b":  _w("u4b", (30, 2047, 24579), "u8", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 7),
 }
 
 # config 5: six layout pairs (BASELINE.json configs[4]) on two mesh pairs.

@@ -12,7 +12,7 @@ from paper_2211_05322_b200 import reshard as rs
 
 pytestmark = pytest.mark.gpu
 
-PATHS = [rs.RS_PATH_AUTO, rs.RS_PATH_LSU, rs.RS_PATH_BULK]
+PATHS = [rs.RS_PATH_AUTO, rs.RS_PATH_LSU, rs.RS_PATH_BULK, rs.RS_PATH_BULK_SHIFT]
 
 SMALL = [
     ((8, 16), (1, 2), "S0,R", (1, 2), "R,S0"),                      # config 1 literal
@@ -78,7 +78,7 @@ def test_under_aligned_shard_pointers(off, path):
         assert g.tobytes() == w.tobytes()
 
 
-@pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK])
+@pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK, rs.RS_PATH_BULK_SHIFT])
 @pytest.mark.parametrize("tile", [128, 1024, 4096])
 def test_tile_sizes_and_ring_depths(tile, path, monkeypatch):
     monkeypatch.setenv("RS_LSU_TILE_BYTES", str(tile))
@@ -154,6 +154,14 @@ def _check_full_size(w, path=rs.RS_PATH_AUTO, n_samples=4096):
 @pytest.mark.parametrize("path", PATHS)
 def test_config4_full_size(path):
     _check_full_size(inputs.get_workload("c4"), path)
+
+
+@pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])
+@pytest.mark.parametrize("name", ["u4", "u4b"])
+def test_unaligned_uneven_full_size(name, path):
+    """1.4 GiB with nothing aligned: TMA loads + shifted stores (AUTO) and the register shift path (LSU)"""
+    p = _check_full_size(inputs.get_workload(name), path)
+    assert p.op_info(rs.RS_OP_EXECUTE).path == (rs.RS_PATH_BULK_SHIFT if path == rs.RS_PATH_AUTO else rs.RS_PATH_LSU)
 
 
 @pytest.mark.parametrize("pair", sorted(inputs.SWEEP_PAIRS))

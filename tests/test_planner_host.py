@@ -313,7 +313,12 @@ def test_alignment_class_and_path_choice():
     oi = p.op_info(rs.RS_OP_EXECUTE)
     assert oi.vec_bytes == 2 and oi.path == rs.RS_PATH_LSU
     p = _plan((4, 6, 5, 3), 2, (2, 2), "S0,S1,R,R", (2, 2), "S1,R,R,R", rs.RS_PATH_BULK)
-    assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_LSU                     # TMA needs 16-byte everything
+    assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_BULK_SHIFT              # TMA stores need 16-byte everything
+    p = _plan((32, 2048, 12290), 2, (2, 4), "S0,S1,R", (4, 2), "S1,R,S0")           # long runs of 6145 B: 2-byte class
+    oi = p.op_info(rs.RS_OP_EXECUTE)
+    assert oi.vec_bytes == 2 and oi.path == rs.RS_PATH_BULK_SHIFT and oi.smem_bytes <= 227 * 1024
+    p = _plan((16, 1024, 4096), 2, (2, 4), "S0,R,S1", (2, 4), "S0,S1,R", rs.RS_PATH_BULK_SHIFT)
+    assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_BULK_SHIFT              # forceable on aligned layouts too
     p = _plan((8, 16), 4, (1, 2), "S1,R", (1, 2), "R,S1")                         # c1i: 32-byte runs
     assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_LSU
     assert _plan((8, 16), 4, (1, 2), "S1,R", (1, 2), "R,S1", rs.RS_PATH_BULK).op_info(0).path == rs.RS_PATH_BULK
