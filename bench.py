@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--sweep", default=None, help="time execute/pack/unpack on a list of workloads instead of the step: "
                     "'configs' (c2,c3,c3i,c3ii,c4), 'pairs' (6 pairs x 2 mesh pairs x 1 MiB..4 GiB), 'table2', 'all', "
                     "or comma-separated workload names; one JSON line per workload")
+    ap.add_argument("--strategies", action="store_true", help="with --sweep: also time RS_STRATEGY_SENDRECV and "
+                    "RS_STRATEGY_ALLGATHER (PAPER.md S3.1) against the broadcast executor")
     ap.add_argument("--sweep-md", default=None, help="also write the sweep as a markdown table to this file")
     return ap.parse_args()
 
@@ -368,7 +370,7 @@ def run_sweep(args):
     rows = []
     for name in sweep_names(args.sweep):
         w = inputs.get_workload(name)
-        plan = harness.make_plan(w, flags)
+        plan = harness.make_plan(w, flags | (rs.RS_WITH_STRATEGIES if args.strategies else 0))
         info = plan.info
         g = torch.Generator(device=dev); g.manual_seed(w.seed % (1 << 31))
         def buf(n):
@@ -382,6 +384,10 @@ def run_sweep(args):
         calls = [("execute", rs.RS_OP_EXECUTE, lambda: plan.execute(sp, dp, sh)),
                  ("pack", rs.RS_OP_PACK, lambda: plan.pack(sp, ap, sh)),
                  ("unpack", rs.RS_OP_UNPACK, lambda: plan.unpack(ap, dp, sh))]
+        if args.strategies:      # same result by the paper's other strategies; GB/s counts the USEFUL bytes (1 + r_B) like execute
+            calls = [calls[0],
+                     ("sendrecv", rs.RS_OP_EXECUTE, lambda: plan.execute_strategy(rs.RS_STRATEGY_SENDRECV, sp, dp, sh)),
+                     ("allgather", rs.RS_OP_EXECUTE, lambda: plan.execute_strategy(rs.RS_STRATEGY_ALLGATHER, sp, dp, sh))]
         row = {"workload": name, "shape": list(w.shape), "src": "%s %s" % ("x".join(map(str, w.src_mesh)), w.src_spec),
                "dst": "%s %s" % ("x".join(map(str, w.dst_mesh)), w.dst_spec), "n_slices": info.n_slices,
                "tensor_bytes": info.tensor_bytes}
@@ -424,6 +430,17 @@ def run_sweep(args):
         torch.cuda.empty_cache()
         rows.append(row)
         print(json.dumps(row), flush=True)
+    if args.sweep_md and args.strategies:
+        with open(args.sweep_md, "w") as f:
+            f.write("| workload | src -> dst | receivers per slice | broadcast ms (GB/s useful) | send/recv ms (x broadcast) | all-gather ms (x broadcast) | bytes moved: broadcast / others |\n")
+            f.write("|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                k = (r["execute"]["bytes"] - r["tensor_bytes"]) // r["tensor_bytes"]
+                b = r["execute"]["ms"]
+                f.write("| %s | %s -> %s | %d | %.3f (%.0f) | %.3f (%.2f) | %.3f (%.2f) | %d / %d x size(D) |\n" % (
+                    r["workload"], r["src"], r["dst"], k, b, r["execute"]["GB/s"], r["sendrecv"]["ms"], r["sendrecv"]["ms"] / b,
+                    r["allgather"]["ms"], r["allgather"]["ms"] / b, 1 + k, 2 * k))
+        return 0
     if args.sweep_md:
         with open(args.sweep_md, "w") as f:
             f.write("| workload | tensor | src -> dst | slices | read + write (execute) | execute GB/s (frac of %.0f) | pack GB/s | unpack GB/s | torch copy_ same volume GB/s | kernel |\n" % peak)

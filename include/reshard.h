@@ -83,6 +83,8 @@ enum {
     RS_PATH_BULK_SHIFT = 0x30, /* force TMA loads + byte-shifted 128-bit register stores (any alignment;
                                what AUTO picks for runs >= 512 B that are not 16-byte aligned)     */
     RS_HOST_ONLY   = 0x100, /* build host tables only: no CUDA call, execute/pack/unpack refuse   */
+    RS_WITH_STRATEGIES = 0x400, /* also build the tables of RS_STRATEGY_SENDRECV / RS_STRATEGY_ALLGATHER
+                               (reshard_execute_strategy): the comparison of PAPER.md S3.1, S5.1         */
     RS_EVEN_ONLY   = 0x200  /* reject l_i not divisible by k_i with RS_EDIVIS ("evenly sharded",
                                PAPER.md:64) instead of padding the last shard (R5)      */
 };
@@ -124,7 +126,20 @@ typedef struct rs_schedule_info {
 
 /* operations a plan can run */
 enum { RS_OP_EXECUTE = 0, RS_OP_PACK = 1, RS_OP_UNPACK = 2,
-       RS_OP_EXECUTE_SLABS = 3 /* execute cut into dim-0 slabs: the table reshard_execute_host runs (queries only) */ };
+       RS_OP_EXECUTE_SLABS = 3, /* execute cut into dim-0 slabs: the table reshard_execute_host runs (queries only) */
+       RS_OP_SENDRECV = 4,      /* RS_STRATEGY_SENDRECV: one copy task per (unit task, receiver)                    */
+       RS_OP_AG_SCATTER = 5,    /* RS_STRATEGY_ALLGATHER phase 1: part j of every slice -> receiver j               */
+       RS_OP_AG_GATHER = 6      /* RS_STRATEGY_ALLGATHER phase 2: receivers copy the other parts from their peers   */ };
+
+/* communication strategies for a unit task (S3.1), on chip */
+enum {
+    RS_STRATEGY_BROADCAST = 0,  /* slice read once, written to every receiver (= reshard_execute)    */
+    RS_STRATEGY_SENDRECV = 1,   /* the sender sends the slice to each receiver one by one: the slice
+                                   is re-read per receiver (k reads + k writes)                                    */
+    RS_STRATEGY_ALLGATHER = 2   /* the slice is split over its k receivers, one part sent to each,
+                                   then the receivers all-gather: two dependent launches, 1 + (k-1) reads and
+                                   1 + (k-1) writes per slice byte                                                 */
+};
 /* sides */
 enum { RS_SRC = 0, RS_DST = 1 };
 
@@ -229,6 +244,12 @@ RS_API rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks,
  */
 RS_API rs_status reshard_execute(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
                           void *cuda_stream);
+/* reshard_execute_strategy: the same result as reshard_execute, reached with another of the paper's
+ * strategies for a unit task.  The plan must have been built with RS_WITH_STRATEGIES
+ * (else RS_EINVAL).  RS_STRATEGY_BROADCAST is reshard_execute; RS_STRATEGY_SENDRECV is one launch;
+ * RS_STRATEGY_ALLGATHER is two launches on `cuda_stream`, the second reading destination shards. */
+RS_API rs_status reshard_execute_strategy(const rs_plan *plan, int32_t strategy, const void *const *src_shards,
+                                   void *const *dst_shards, void *cuda_stream);
 /* reshard_pack: sender shards -> message arena [DEVICE, arena_bytes].  A slice needed by k receivers
  * is read once and written into k messages.  One kernel launch. */
 RS_API rs_status reshard_pack(const rs_plan *plan, const void *const *src_shards, void *msg_arena, void *cuda_stream);

@@ -386,7 +386,58 @@ rs_status build_tables(Plan *P) {
             UP.tasks.push_back(T);
         }
     }
+    // Alternative strategies for a unit task, as extra tables on request.  On chip
+    // they differ from the broadcast table in BYTES: send/recv re-reads the slice once per receiver
+    // (k reads + k writes instead of 1 + k); the all-gather strategy sends part j of the slice to
+    // receiver j (1 read + 1 write in total), then every receiver copies the other k - 1 parts from
+    // its peers' shards (k - 1 reads + k - 1 writes): again 2k, in two dependent launches.
+    OpTables &SR = P->op[RS_OP_SENDRECV], &AS = P->op[RS_OP_AG_SCATTER], &AG = P->op[RS_OP_AG_GATHER];
+    for (OpTables *o : {&SR, &AS, &AG}) { o->tasks.clear(); o->dsts.clear(); o->tiles.clear(); o->info = rs_op_info{}; }
+    if (P->flags & RS_WITH_STRATEGIES) {
+        auto add = [&](OpTables &O, const int64_t *lo, const int64_t *hi, int src_buf, const int64_t *src_origin,
+                       const int64_t *sstr, int dst_buf, const int64_t *dst_origin) -> bool {
+            BoxDesc bx;
+            bx.ndim = N;
+            for (int d = 0; d < N; d++) { bx.ext[d] = hi[d] - lo[d]; bx.sstride[d] = sstr[d]; bx.dstride[d] = sB[d]; }
+            RsTask T{};
+            if (!collapse(bx, e, &T)) return false;
+            T.src_buf = src_buf; T.src_off = box_offset(lo, src_origin, sstr, N);
+            T.k = 1; T.dst_first = (int32_t)O.dsts.size();
+            O.dsts.push_back(RsDst{box_offset(lo, dst_origin, sB, N), dst_buf, 0});
+            O.tasks.push_back(T);
+            return true;
+        };
+        for (int i : P->exec_order) {
+            const Slice &S = P->slices[(size_t)i];
+            const int k = (int)S.receivers.size();
+            int64_t lo_s[RS_MAX_NDIM], hi_s[RS_MAX_NDIM];
+            device_box(A, S.sender, lo_s, hi_s);
+            std::vector<std::vector<int64_t>> org((size_t)k, std::vector<int64_t>(RS_MAX_NDIM));
+            for (int j = 0; j < k; j++) { int64_t hi_r[RS_MAX_NDIM]; device_box(B, S.receivers[(size_t)j], org[(size_t)j].data(), hi_r); }
+            for (int j = 0; j < k; j++)                           // send/recv: the whole slice, once per receiver
+                if (!add(SR, S.lo, S.hi, S.sender, lo_s, sA, S.receivers[(size_t)j], org[(size_t)j].data())) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+            int cd = 0;                                        // all-gather: cut the outermost dim that has >= k rows (else the longest)
+            for (int d = 0; d < N; d++) if (S.hi[d] - S.lo[d] > S.hi[cd] - S.lo[cd]) cd = d;
+            for (int d = N - 1; d >= 0; d--) if (S.hi[d] - S.lo[d] >= k) cd = d;
+            const int64_t ext = S.hi[cd] - S.lo[cd], step = (ext + k - 1) / k;
+            for (int j = 0; j < k; j++) {
+                int64_t lo[RS_MAX_NDIM], hi[RS_MAX_NDIM];
+                for (int d = 0; d < N; d++) { lo[d] = S.lo[d]; hi[d] = S.hi[d]; }
+                lo[cd] = std::min(S.lo[cd] + j * step, S.hi[cd]);
+                hi[cd] = std::min(S.lo[cd] + (j + 1) * step, S.hi[cd]);
+                if (lo[cd] >= hi[cd]) continue;
+                if (!add(AS, lo, hi, S.sender, lo_s, sA, S.receivers[(size_t)j], org[(size_t)j].data())) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+                for (int q = 0; q < k; q++)                   // gather: part j from receiver j's shard into receiver q's
+                    if (q != j && !add(AG, lo, hi, S.receivers[(size_t)j], org[(size_t)j].data(), sB, S.receivers[(size_t)q], org[(size_t)q].data())) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+            }
+        }
+    }
     rs_status st;
+    if (P->flags & RS_WITH_STRATEGIES) {
+        if ((st = finish_op(P, &SR, tensor_bytes * P->r_B, tensor_bytes * P->r_B)) != RS_OK) return st;
+        if ((st = finish_op(P, &AS, tensor_bytes, tensor_bytes)) != RS_OK) return st;
+        if ((st = finish_op(P, &AG, tensor_bytes * (P->r_B - 1), tensor_bytes * (P->r_B - 1))) != RS_OK) return st;
+    }
     if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
     if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
     if ((st = finish_op(P, &PK, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;

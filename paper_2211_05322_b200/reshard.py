@@ -19,6 +19,9 @@ RS_LB_GREEDY, RS_LB_NAIVE = 0x0, 0x1
 RS_PATH_AUTO, RS_PATH_LSU, RS_PATH_BULK, RS_PATH_BULK_SHIFT = 0x00, 0x10, 0x20, 0x30
 RS_HOST_ONLY = 0x100
 RS_EVEN_ONLY = 0x200
+RS_WITH_STRATEGIES = 0x400
+RS_OP_SENDRECV, RS_OP_AG_SCATTER, RS_OP_AG_GATHER = 4, 5, 6
+RS_STRATEGY_BROADCAST, RS_STRATEGY_SENDRECV, RS_STRATEGY_ALLGATHER = 0, 1, 2
 RS_OP_EXECUTE, RS_OP_PACK, RS_OP_UNPACK, RS_OP_EXECUTE_SLABS = 0, 1, 2, 3
 RS_SRC, RS_DST = 0, 1
 RS_SCHED_NONE, RS_SCHED_NAIVE, RS_SCHED_LOAD_BALANCE, RS_SCHED_DFS, RS_SCHED_GREEDY, RS_SCHED_ENSEMBLE = range(6)
@@ -28,7 +31,7 @@ RS_MAX_NDIM, RS_MAX_MESH_NDIM, RS_MAX_DEVICES = 8, 4, 128
 SYMBOLS = [
     "reshard_plan", "reshard_plan_ex", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
     "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
-    "reshard_plan_message", "reshard_execute", "reshard_pack", "reshard_unpack", "reshard_execute_host",
+    "reshard_plan_message", "reshard_execute", "reshard_execute_strategy", "reshard_pack", "reshard_unpack", "reshard_execute_host",
     "reshard_host_workspace_bytes", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
     "reshard_version",
 ]
@@ -210,6 +213,9 @@ class Plan:
     # ---- data path (device addresses in, nothing out; asynchronous on `stream`)
     def execute(self, src_ptrs, dst_ptrs, stream=0):
         _chk(_lib().reshard_execute(self._h, _ptrs(src_ptrs), _ptrs(dst_ptrs), C.c_void_p(stream)))
+
+    def execute_strategy(self, strategy, src_ptrs, dst_ptrs, stream=0):
+        _chk(_lib().reshard_execute_strategy(self._h, int(strategy), _ptrs(src_ptrs), _ptrs(dst_ptrs), C.c_void_p(stream)))
 
     def pack(self, src_ptrs, arena_ptr, stream=0):
         _chk(_lib().reshard_pack(self._h, _ptrs(src_ptrs), C.c_void_p(arena_ptr), C.c_void_p(stream)))

@@ -326,3 +326,42 @@ def test_execute_host_pipeline_cases(case):
         for q, (g, wq) in enumerate(zip(dst_h, want)):
             assert g.numpy().tobytes() == wq.tobytes(), "device %d" % q
             g.fill_(0x5A5A)
+
+
+@pytest.mark.parametrize("strategy", [rs.RS_STRATEGY_BROADCAST, rs.RS_STRATEGY_SENDRECV, rs.RS_STRATEGY_ALLGATHER])
+@pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])
+@pytest.mark.parametrize("case", [SMALL[i] for i in (0, 3, 4, 7, 9, 10, 13, 17, 20, 23, 24)])
+def test_strategies_reach_the_oracle_result(case, path, strategy):
+    """send/recv, all-gather and broadcast are routes to the SAME destination layout"""
+    shape, sm, ss, dm, ds = case
+    rng = np.random.default_rng(11)
+    D = rng.integers(-2 ** 15, 2 ** 15, size=shape).astype(np.int16)
+    src = do.shards_from_global(D, sm, ss)
+    want = do.reshard(shape, sm, ss, dm, ds, src, fill=0xA5)
+    p = rs.Plan(shape, 2, sm, ss, dm, ds, path | rs.RS_WITH_STRATEGIES)
+    src_d = [gu.to_dev(s) for s in src]
+    dst_d = [torch.full((w.nbytes,), 0xA5, dtype=torch.uint8, device=gu.dev()) for w in want]
+    n0 = rs.launch_count()
+    p.execute_strategy(strategy, gu.ptrs(src_d), gu.ptrs(dst_d), gu.stream())
+    torch.cuda.synchronize()
+    r_B = p.info.write_bytes // p.info.tensor_bytes
+    assert rs.launch_count() - n0 == (1 if strategy != rs.RS_STRATEGY_ALLGATHER or r_B == 1 else 2)
+    for q, w in enumerate(want):
+        assert dst_d[q].cpu().numpy().tobytes() == w.tobytes(), "device %d differs" % q
+
+
+def test_strategies_full_size_multicast_and_refusal():
+    w = inputs.sweep_workload("P5", "m8", 256 << 20)               # 1 read + 8 writes at 256 MiB
+    e = inputs.elem_bytes(w.dtype)
+    D, src = gu.workload_on_device(w)
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, rs.RS_WITH_STRATEGIES)
+    idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
+    for strategy in (rs.RS_STRATEGY_SENDRECV, rs.RS_STRATEGY_ALLGATHER):
+        dst = [torch.zeros(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+        p.execute_strategy(strategy, gu.ptrs(src), gu.ptrs(dst), gu.stream())
+        torch.cuda.synchronize()
+        for q in range(p.info.n_dst):
+            assert torch.equal(dst[q], D[idx[q]])
+    plain = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    with pytest.raises(rs.ReshardError):
+        plain.execute_strategy(rs.RS_STRATEGY_SENDRECV, gu.ptrs(src), gu.ptrs(dst), gu.stream())

@@ -397,3 +397,38 @@ def test_slab_table_cuts_dim0_when_large():
     assert int((tiles["n_rows"].astype(np.int64) * tiles["col_bytes"]).sum()) == p.info.tensor_bytes
     p = _plan((8, 16), 4, (1, 2), "S1,R", (1, 2), "R,S1")                  # tiny: one slab == the execute table
     assert p.op_info(rs.RS_OP_EXECUTE_SLABS).n_tasks == p.op_info(rs.RS_OP_EXECUTE).n_tasks
+
+
+# ---------------------------------------------------------------- alternative strategies
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", LAYOUTS)
+def test_strategy_tables_replay_equals_oracle(shape, sm, ss, dm, ds):
+    """send/recv and scatter + all-gather reach the oracle's result; their byte counts are 2k per slice byte"""
+    dtype, e = np.int16, 2
+    p = _plan(shape, e, sm, ss, dm, ds, rs.RS_WITH_STRATEGIES)
+    D = (np.arange(int(np.prod(shape)), dtype=np.int64) * 2654435761 % 251 + 1).astype(dtype).reshape(shape)
+    src = do.shards_from_global(D, sm, ss)
+    want = do.reshard(shape, sm, ss, dm, ds, src)
+    once = _valid_bytes(shape, dm, ds, e)
+    n_dst, r_B = len(want), p.info.write_bytes // p.info.tensor_bytes
+    # send/recv: one launch, every destination byte written once, the source read r_B times
+    dst = [np.zeros(want[0].nbytes, np.uint8) for _ in range(n_dst)]
+    cnt = [np.zeros(want[0].nbytes, np.int32) for _ in range(n_dst)]
+    ti.replay(p, rs.RS_OP_SENDRECV, [_bytes(s) for s in src], dst, cnt)
+    for q in range(n_dst):
+        assert np.array_equal(dst[q], _bytes(want[q])) and np.array_equal(cnt[q], once[q])
+    oi = p.op_info(rs.RS_OP_SENDRECV)
+    assert oi.read_bytes == oi.write_bytes == p.info.tensor_bytes * r_B and oi.n_tasks == sum(len(s["receivers"]) for s in p.slices())
+    # all-gather: phase 1 writes every part once somewhere, phase 2 (reading destination shards) completes every shard
+    dst = [np.zeros(want[0].nbytes, np.uint8) for _ in range(n_dst)]
+    cnt = [np.zeros(want[0].nbytes, np.int32) for _ in range(n_dst)]
+    ti.replay(p, rs.RS_OP_AG_SCATTER, [_bytes(s) for s in src], dst, cnt)
+    assert sum(int(c.sum()) for c in cnt) == p.info.tensor_bytes            # one copy of D in total after the scatter
+    ti.replay(p, rs.RS_OP_AG_GATHER, dst, dst, cnt)
+    for q in range(n_dst):
+        assert np.array_equal(dst[q], _bytes(want[q])) and np.array_equal(cnt[q], once[q])
+    a, g = p.op_info(rs.RS_OP_AG_SCATTER), p.op_info(rs.RS_OP_AG_GATHER)
+    assert a.read_bytes == a.write_bytes == p.info.tensor_bytes
+    assert g.read_bytes == g.write_bytes == p.info.tensor_bytes * (r_B - 1)
+    # without the flag the tables are not built
+    assert _plan(shape, e, sm, ss, dm, ds).op_info(rs.RS_OP_SENDRECV).n_tasks == 0
