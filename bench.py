@@ -31,7 +31,13 @@ NOMINAL_HBM_GBS = 8000.0          # BASELINE.json: "~8 TB/s"; the >=70 % bar ref
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE rs_copy_* launch of reshard_execute, from the
 # `ncu --set full` capture summarised in profiles/ (null for workloads without a capture)
-NCU_TRAFFIC_BYTES = {"c4": 1614862000 + 1564753000}     # profiles/r01_ncu_full_c4.md
+NCU_TRAFFIC_BYTES = {            # profiles/r01_ncu_sweep.md (read + write, one reshard_execute launch)
+    "c4": 1614926000 + 1565091000, "c2": 134617344 + 85814784, "u4": 1542852000 + 1462126000,
+    "t2_9": 1077981000 + 4236750000,
+    "sweep_P1_m8_1024MiB": 1076611000 + 1024967000, "sweep_P2_m8_1024MiB": 1076635000 + 4238627000,
+    "sweep_P3_m8_1024MiB": 1076605000 + 1026876000, "sweep_P4_m8_1024MiB": 1076615000 + 1024249000,
+    "sweep_P5_m8_1024MiB": 1076862000 + 8532008000, "sweep_P6_m8_1024MiB": 1076596000 + 1026636000,
+}
 
 
 def parse_args():
