@@ -365,3 +365,66 @@ def test_strategies_full_size_multicast_and_refusal():
     plain = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
     with pytest.raises(rs.ReshardError):
         plain.execute_strategy(rs.RS_STRATEGY_SENDRECV, gu.ptrs(src), gu.ptrs(dst), gu.stream())
+
+
+def test_cuda_graph_capture_and_replay():
+    """execute / pack / unpack only enqueue kernels: a whole step can be captured once and replayed
+    (small, launch-bound reshards are the case for it)"""
+    w = inputs.get_workload("c3ii")
+    e = inputs.elem_bytes(w.dtype)
+    D, src = gu.workload_on_device(w)
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    dst = [torch.zeros(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+    dst2 = [torch.zeros_like(t) for t in dst]
+    arena = torch.zeros(p.info.arena_bytes, dtype=torch.uint8, device=gu.dev())
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.graph(g, stream=side):
+        s = torch.cuda.current_stream().cuda_stream
+        p.execute(gu.ptrs(src), gu.ptrs(dst), s)
+        p.pack(gu.ptrs(src), arena.data_ptr(), s)
+        p.unpack(arena.data_ptr(), gu.ptrs(dst2), s)
+    torch.cuda.synchronize()
+    assert all(int(t.abs().sum()) == 0 for t in dst)                   # capture does not execute
+    idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
+    for _ in range(3):
+        for t in dst + dst2:
+            t.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        for q in range(p.info.n_dst):
+            assert torch.equal(dst[q], D[idx[q]]) and torch.equal(dst2[q], D[idx[q]])
+
+
+def test_one_plan_many_host_threads_and_streams():
+    """include/reshard.h 'Threading': a plan is immutable; threads may execute it concurrently on their own streams"""
+    import threading
+    w = inputs.get_workload("c2")
+    e = inputs.elem_bytes(w.dtype)
+    D, src = gu.workload_on_device(w)
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
+    outs, errs = {}, []
+
+    def work(tid):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            dst = [torch.zeros(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+            st.wait_stream(torch.cuda.default_stream())
+            for _ in range(5):
+                p.execute(gu.ptrs(src), gu.ptrs(dst), st.cuda_stream)
+            st.synchronize()
+            outs[tid] = dst
+        except Exception as ex:                                        # noqa: BLE001
+            errs.append(ex)
+
+    torch.cuda.synchronize()
+    ts = [threading.Thread(target=work, args=(i,)) for i in range(4)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    assert not errs and len(outs) == 4
+    for dst in outs.values():
+        for q in range(p.info.n_dst):
+            assert torch.equal(dst[q], D[idx[q]])
