@@ -428,3 +428,17 @@ def test_one_plan_many_host_threads_and_streams():
     for dst in outs.values():
         for q in range(p.info.n_dst):
             assert torch.equal(dst[q], D[idx[q]])
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("case", [
+    ((2, 3, 2, 2, 4, 2, 2, 6), (2, 2, 2, 2), "S0,R,S1,R,S2,R,R,S3", (2, 2, 2, 2), "R,S3,R,S2,R,S1,S0,R"),
+    ((128, 4), (128,), "S0,R", (2, 4, 4, 4), "R,S0123"),
+    ((256, 64), (1,), "R,R", (128,), "R,R"),
+])
+def test_maximum_ranks_and_device_counts(case, path):
+    """RS_MAX_NDIM = 8 tensor dims, RS_MAX_MESH_NDIM = 4 mesh dims, RS_MAX_DEVICES = 128 devices per mesh"""
+    shape, sm, ss, dm, ds = case
+    _p, got, want = gu.run_small(shape, np.int16, sm, ss, dm, ds, flags=path)
+    for g, w in zip(got, want):
+        assert g.tobytes() == w.tobytes()

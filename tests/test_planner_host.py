@@ -432,3 +432,18 @@ def test_strategy_tables_replay_equals_oracle(shape, sm, ss, dm, ds):
     assert g.read_bytes == g.write_bytes == p.info.tensor_bytes * (r_B - 1)
     # without the flag the tables are not built
     assert _plan(shape, e, sm, ss, dm, ds).op_info(rs.RS_OP_SENDRECV).n_tasks == 0
+
+
+MAXIMA = [
+    ((2, 3, 2, 2, 4, 2, 2, 6), (2, 2, 2, 2), "S0,R,S1,R,S2,R,R,S3", (2, 2, 2, 2), "R,S3,R,S2,R,S1,S0,R"),   # RS_MAX_NDIM, RS_MAX_MESH_NDIM
+    ((128, 4), (128,), "S0,R", (2, 4, 4, 4), "R,S0123"),                                                    # RS_MAX_DEVICES on both sides
+    ((256, 2), (1,), "R,R", (128,), "R,R"),                                                                  # one slice, 128 receivers
+]
+
+
+@pytest.mark.parametrize("shape,sm,ss,dm,ds", MAXIMA)
+def test_maximum_ranks_and_device_counts(shape, sm, ss, dm, ds):
+    _check_tables(shape, np.int16, sm, ss, dm, ds)
+    with pytest.raises(rs.ReshardError) as ei:
+        _plan(shape + (2,) * (9 - len(shape)), 2, sm, ss + ",R" * (9 - len(shape)), dm, ds + ",R" * (9 - len(shape)))
+    assert ei.value.code == rs.RS_EINVAL                      # more than RS_MAX_NDIM dims
