@@ -274,6 +274,47 @@ RS_API rs_status reshard_execute_host(const rs_plan *plan, const void *const *sr
                                int64_t *h2d_bytes, int64_t *d2h_bytes);
 RS_API int64_t reshard_host_workspace_bytes(const rs_plan *plan);
 
+/* ---- S4: pipeline schedules around the resharding tasks (host only, no CUDA) ------------------- */
+#define RS_PIPE_MAX_STAGES 64
+enum { RS_PIPE_1F1B = 0,        /* stage i warms up with #stages - i + 1 forwards              */
+       RS_PIPE_EAGER_1F1B = 1   /* stage i warms up with 2 (#stages - i) + 1 forwards          */ };
+enum { RS_PIPE_F = 0, RS_PIPE_B = 1, RS_PIPE_BA = 2 /* activation gradients */, RS_PIPE_BW = 3 /* weight gradients */ };
+
+typedef struct rs_pipeline_opts {
+    int32_t schedule;                /* RS_PIPE_1F1B or RS_PIPE_EAGER_1F1B                                   */
+    int32_t n_stages;                /* 1..RS_PIPE_MAX_STAGES; stages are numbered 1..S in the paper, 0..S-1 in arrays */
+    int32_t n_micro_batches;         /* >= 1; warm-up counts are capped at it (R28)                */
+    int32_t overlap;                 /* 1: transfers run beside the sender's compute;
+                                        0: the sender stage is busy until its transfer has finished           */
+    int32_t bw_delay;                /* with bwd_act: ops by which the weight-gradient half is postponed (R32) */
+    int32_t reserved;
+    const int64_t *fwd, *bwd;        /* [HOST, n_stages] compute time of one forward / one whole backward, ticks */
+    const int64_t *bwd_act;          /* [HOST, n_stages] or NULL: time of the activation-gradient half; not NULL
+                                        splits every backward (backward weight delaying)    */
+    int64_t comm_fwd, comm_bwd;      /* ticks one micro-batch's tensor needs across a stage boundary, e.g. the
+                                        measured time of reshard_execute for that boundary's plan             */
+} rs_pipeline_opts;
+
+typedef struct rs_pipeline_result {
+    int64_t makespan;                /* end of the last op of the iteration                                  */
+    int32_t ops_per_stage;           /* 2 M, or 3 M with a split backward                                    */
+    int32_t reserved;
+    int32_t warmup[RS_PIPE_MAX_STAGES];            /* forwards before the first backward                     */
+    int32_t peak_activations[RS_PIPE_MAX_STAGES];  /* most micro-batches alive at once        */
+    int64_t busy[RS_PIPE_MAX_STAGES];              /* compute time of the stage                               */
+} rs_pipeline_result;
+
+/* Timeline of one iteration (R28-R32): every stage runs its op list strictly in order, an op starts
+ * when the stage is free and its input has arrived; every boundary has one link per direction.  The four output
+ * arrays [HOST, n_stages * ops_per_stage] (stage-major, in list order; query ops_per_stage with them NULL first)
+ * receive op kind (RS_PIPE_*), micro-batch, start and end; each may be NULL. */
+RS_API rs_status reshard_pipeline_simulate(const rs_pipeline_opts *opts, rs_pipeline_result *result, int32_t *op_kind,
+                                    int32_t *op_micro_batch, int64_t *op_start, int64_t *op_end);
+/* PAPER.md:217 "delay the least to cover all communications": the smallest bw_delay for which the compute a
+ * stage (1-based) runs between an activation-gradient op and its weight-gradient op covers comm_bwd. */
+RS_API int32_t reshard_pipeline_least_delay(int32_t schedule, int32_t n_stages, int32_t stage, int32_t n_micro_batches,
+                                     int64_t fwd, int64_t bwd, int64_t bwd_act, int64_t comm_bwd);
+
 /* kernels launched by this library in the calling thread since it was loaded (bench bookkeeping) */
 RS_API int64_t reshard_launch_count(void);
 

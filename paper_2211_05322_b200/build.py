@@ -10,7 +10,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["plan.cpp", "schedule.cpp", "tables.cpp", "kernels.cu", "api.cu"]
+SOURCES = ["plan.cpp", "schedule.cpp", "pipeline.cpp", "tables.cpp", "kernels.cu", "api.cu"]
 HEADERS = ["plan.hpp", "tables.h", "kernels.h", "config.h", os.path.join("..", "..", "include", "reshard.h")]
 OUT = os.path.join(HERE, "libreshard.so")
 

@@ -445,6 +445,23 @@ rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shard
     return RS_OK;
 }
 
+rs_status reshard_pipeline_simulate(const rs_pipeline_opts *opts, rs_pipeline_result *result, int32_t *op_kind,
+                                    int32_t *op_micro_batch, int64_t *op_start, int64_t *op_end) {
+    rs::set_error("");
+    if (!opts) { rs::set_error("null argument"); return RS_EINVAL; }
+    try {
+        return rs::pipeline_simulate(*opts, result, op_kind, op_micro_batch, op_start, op_end);
+    } catch (const std::bad_alloc &) {
+        return RS_ENOMEM;
+    }
+}
+
+int32_t reshard_pipeline_least_delay(int32_t schedule, int32_t n_stages, int32_t stage, int32_t n_micro_batches,
+                                     int64_t fwd, int64_t bwd, int64_t bwd_act, int64_t comm_bwd) {
+    if (n_stages < 1 || stage < 1 || stage > n_stages || n_micro_batches < 1) return -1;
+    return rs::pipeline_least_delay(schedule, n_stages, stage, n_micro_batches, fwd, bwd, bwd_act, comm_bwd);
+}
+
 int64_t reshard_launch_count(void) { return rs::launch_count(); }
 
 const char *reshard_strerror(rs_status s) {

@@ -113,5 +113,8 @@ void choose_senders(Plan *P);                          // a4
 rs_status schedule_plan(Plan *P);                      // S3.2: senders + order at host level, schedule.cpp
 rs_status build_messages(Plan *P);                     // message layout
 rs_status build_tables(Plan *P);                       // a5 (host side), tables.cpp
+rs_status pipeline_simulate(const rs_pipeline_opts &o, rs_pipeline_result *res, int32_t *op_kind, int32_t *op_micro,
+                            int64_t *op_start, int64_t *op_end);                    // S4, pipeline.cpp
+int pipeline_least_delay(int schedule, int S, int stage, int M, int64_t f, int64_t b, int64_t b_act, int64_t c_bwd);
 
 }  // namespace rs

@@ -32,7 +32,7 @@ SYMBOLS = [
     "reshard_plan", "reshard_plan_ex", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
     "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
     "reshard_plan_message", "reshard_execute", "reshard_execute_strategy", "reshard_pack", "reshard_unpack", "reshard_execute_host",
-    "reshard_host_workspace_bytes", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
+    "reshard_host_workspace_bytes", "reshard_pipeline_simulate", "reshard_pipeline_least_delay", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
     "reshard_version",
 ]
 
@@ -63,6 +63,23 @@ class ScheduleInfo(C.Structure):
                 ("n_src_hosts", C.c_int32), ("n_dst_hosts", C.c_int32), ("dfs_finished", C.c_int32),
                 ("reserved", C.c_int32), ("dfs_nodes", C.c_int64), ("makespan", C.c_int64),
                 ("busiest_host_bytes", C.c_int64)]
+
+
+RS_PIPE_MAX_STAGES = 64
+RS_PIPE_1F1B, RS_PIPE_EAGER_1F1B = 0, 1
+RS_PIPE_F, RS_PIPE_B, RS_PIPE_BA, RS_PIPE_BW = 0, 1, 2, 3
+
+
+class PipelineOpts(C.Structure):
+    _fields_ = [("schedule", C.c_int32), ("n_stages", C.c_int32), ("n_micro_batches", C.c_int32), ("overlap", C.c_int32),
+                ("bw_delay", C.c_int32), ("reserved", C.c_int32), ("fwd", C.POINTER(C.c_int64)), ("bwd", C.POINTER(C.c_int64)),
+                ("bwd_act", C.POINTER(C.c_int64)), ("comm_fwd", C.c_int64), ("comm_bwd", C.c_int64)]
+
+
+class PipelineResult(C.Structure):
+    _fields_ = [("makespan", C.c_int64), ("ops_per_stage", C.c_int32), ("reserved", C.c_int32),
+                ("warmup", C.c_int32 * RS_PIPE_MAX_STAGES), ("peak_activations", C.c_int32 * RS_PIPE_MAX_STAGES),
+                ("busy", C.c_int64 * RS_PIPE_MAX_STAGES)]
 
 
 class ReshardError(RuntimeError):
@@ -229,3 +246,29 @@ class Plan:
         _chk(_lib().reshard_execute_host(self._h, _ptrs(src_host_ptrs), _ptrs(dst_host_ptrs),
                                          C.c_void_p(workspace_ptr), C.c_void_p(stream), C.byref(up), C.byref(down)))
         return up.value, down.value
+
+
+def pipeline_simulate(schedule, n_stages, n_micro_batches, fwd, bwd, comm_fwd, comm_bwd, overlap=True, bwd_act=None,
+                      bw_delay=0):
+    """reshard_pipeline_simulate -> dict(makespan, warmup, peak, busy, ops=[per stage list of (kind, micro, start, end)]).
+    fwd / bwd / bwd_act: one int (every stage) or a list per stage."""
+    def per_stage(x):
+        return _i64(x if isinstance(x, (list, tuple)) else [x] * n_stages)
+    f, b = per_stage(fwd), per_stage(bwd)
+    ba = per_stage(bwd_act) if bwd_act is not None else None
+    o = PipelineOpts(schedule=schedule, n_stages=n_stages, n_micro_batches=n_micro_batches, overlap=int(bool(overlap)),
+                     bw_delay=bw_delay, fwd=f, bwd=b, bwd_act=ba, comm_fwd=comm_fwd, comm_bwd=comm_bwd)
+    res = PipelineResult()
+    _chk(_lib().reshard_pipeline_simulate(C.byref(o), C.byref(res), None, None, None, None))
+    n = n_stages * res.ops_per_stage
+    kind, micro, start, end = (C.c_int32 * n)(), (C.c_int32 * n)(), (C.c_int64 * n)(), (C.c_int64 * n)()
+    _chk(_lib().reshard_pipeline_simulate(C.byref(o), C.byref(res), kind, micro, start, end))
+    k = res.ops_per_stage
+    ops = [[(kind[i * k + j], micro[i * k + j], start[i * k + j], end[i * k + j]) for j in range(k)] for i in range(n_stages)]
+    return dict(makespan=res.makespan, warmup=list(res.warmup[:n_stages]), peak=list(res.peak_activations[:n_stages]),
+                busy=list(res.busy[:n_stages]), ops=ops)
+
+
+def pipeline_least_delay(schedule, n_stages, stage, n_micro_batches, fwd, bwd, bwd_act, comm_bwd):
+    return int(_lib().reshard_pipeline_least_delay(schedule, n_stages, stage, n_micro_batches, C.c_int64(fwd), C.c_int64(bwd),
+                                                   C.c_int64(bwd_act), C.c_int64(comm_bwd)))
