@@ -17,6 +17,11 @@
 #define RS_BULK_SHORT_RUN    1024       // runs up to this long: many copies per tile, use the SHORT shape
 #define RS_BULK_WARPS_SHORT  4
 #define RS_BULK_TILE_BYTES_SHORT 8192
+#define RS_BULK_CTAS_DEN       148    // CTA counts below are out of 148 SMs
+#define RS_BULK_CTAS_MCAST_NUM 96     // write-heavy (multicast) operations
+#define RS_BULK_CTAS_LONG_NUM  132    // 1 : 1 operations whose runs are at least RS_BULK_LONG_RUN
+#define RS_BULK_LONG_RUN       4096
+#define RS_BULK_CTAS_MIN_BYTES (256ll << 20)   // operations moving less than this keep one CTA on every SM
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 
 // TMA loads + shifted register stores (unaligned layouts): the stores are ALU work, so more warps, smaller tiles

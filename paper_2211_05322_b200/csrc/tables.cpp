@@ -185,7 +185,20 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
         while ((int64_t)warps * (stages * tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && tile_bytes > 1024) tile_bytes -= 1024;
         I.block = warps * 32;
-        I.grid = P->sm_count;
+        // At most one CTA per SM -- and FEWER where measurement says the memory system prefers it (B200, 148 SMs):
+        //  * write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes): 148 writers hold 5.65 TB/s
+        //    whatever the ring depth or tile size, 96 writers reach 6.1-6.2 TB/s (an SM sustains ~64 GB/s of this
+        //    mix; beyond ~104 SMs the writers contend);
+        //  * 1 : 1 operations with long runs (<= 3 bulk copies per tile): 132 CTAs are 1.5-3.7 % faster than 148;
+        //  * short runs and the shifted variant are issue-bound per SM and want every SM.
+        // Expressed as fractions of the SM count so the rule survives a different part.
+        // Small operations are latency-bound, not contention-bound: they keep every SM.
+        const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
+        int dflt = P->sm_count;
+        if (!big) dflt = P->sm_count;
+        else if (!shift && !short_runs && write_heavy) dflt = P->sm_count * RS_BULK_CTAS_MCAST_NUM / RS_BULK_CTAS_DEN;
+        else if (!shift && !write_heavy && min_run >= RS_BULK_LONG_RUN) dflt = P->sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
+        I.grid = std::max(1, std::min(P->sm_count, env_int(write_heavy ? "RS_BULK_CTAS_MCAST" : "RS_BULK_CTAS", std::max(1, dflt))));
         workers = I.grid * warps;
     } else {
         tile_bytes = env_int("RS_LSU_TILE_BYTES", RS_LSU_TILE_BYTES);
