@@ -57,6 +57,8 @@ def parse_args():
                     "or comma-separated workload names; one JSON line per workload")
     ap.add_argument("--strategies", action="store_true", help="with --sweep: also time RS_STRATEGY_SENDRECV and "
                     "RS_STRATEGY_ALLGATHER (PAPER.md S3.1) against the broadcast executor")
+    ap.add_argument("--overlap", action="store_true", help="resharding beside compute (PAPER.md S4, on chip): reshard_execute "
+                    "on a high-priority stream limited to max_ctas CTAs while torch.matmul (cuBLAS) runs on another stream")
     ap.add_argument("--sweep-md", default=None, help="also write the sweep as a markdown table to this file")
     return ap.parse_args()
 
@@ -460,8 +462,93 @@ def run_sweep(args):
     return 0
 
 
+def run_overlap(args):
+    """Per CTA cap: time N matmuls alone, M reshard_execute launches alone, then both started together on two
+    streams (wall time on the device between a common start event and the later of the two end events).
+    overlap gain = (t_gemm + t_reshard) / t_both: 1.0 = serialised, 2.0 = perfectly hidden."""
+    import torch
+    from paper_2211_05322_b200 import harness, inputs
+    from paper_2211_05322_b200 import reshard as rs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    w = inputs.get_workload(args.workload)
+    n = 8192
+    a = torch.randn(n, n, device=dev, dtype=torch.bfloat16)
+    b = torch.randn(n, n, device=dev, dtype=torch.bfloat16)
+    c = torch.empty(n, n, device=dev, dtype=torch.bfloat16)
+    s_gemm = torch.cuda.Stream()
+    s_copy = torch.cuda.Stream(priority=-1)                    # the copy's few CTAs get SMs as soon as they free up
+    n_gemm, n_copy = 12, 16
+
+    def timed(fn_g, fn_c):
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True)
+        eg, ec = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(torch.cuda.current_stream())
+        s_gemm.wait_event(e0); s_copy.wait_event(e0)
+        if fn_c:
+            with torch.cuda.stream(s_copy):
+                fn_c()
+                ec.record(s_copy)
+        if fn_g:
+            with torch.cuda.stream(s_gemm):
+                fn_g()
+                eg.record(s_gemm)
+        torch.cuda.synchronize()
+        return (e0.elapsed_time(eg) if fn_g else 0.0), (e0.elapsed_time(ec) if fn_c else 0.0)
+
+    def gemms():
+        for _ in range(n_gemm):
+            torch.matmul(a, b, out=c)
+
+    rows = []
+    for cap in (0, 96, 64, 48, 32, 16):
+        plan = rs.Plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0,
+                       dict(max_ctas=cap))
+        info = plan.info
+        src = [torch.empty(info.src_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_src)]
+        dst = [torch.empty(info.dst_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_dst)]
+        sp, dp = harness.ptrs(src), harness.ptrs(dst)
+        o = plan.op_info(rs.RS_OP_EXECUTE)
+
+        def copies():
+            for _ in range(n_copy):
+                plan.execute(sp, dp, s_copy.cuda_stream)
+
+        for _ in range(2):
+            timed(gemms, copies)
+        tg = statistics.median(timed(gemms, None)[0] for _ in range(5))
+        tc = statistics.median(timed(None, copies)[1] for _ in range(5))
+        both = [timed(gemms, copies) for _ in range(5)]
+        tb = statistics.median(max(x) for x in both)
+        nbytes = (o.read_bytes + o.write_bytes) * n_copy
+        row = {"max_ctas": cap, "grid": o.grid, "gemm_alone_ms": tg, "reshard_alone_ms": tc, "both_ms": tb,
+               "gemm_TFLOPs_alone": 2 * n ** 3 * n_gemm / tg / 1e9, "reshard_GBs_alone": nbytes / tc / 1e6,
+               "gemm_TFLOPs_concurrent": 2 * n ** 3 * n_gemm / statistics.median(x[0] for x in both) / 1e9,
+               "reshard_GBs_concurrent": nbytes / statistics.median(x[1] for x in both) / 1e6,
+               "overlap_gain": (tg + tc) / tb, "workload": w.name}
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+        plan.close()
+        del src, dst
+    if args.sweep_md:
+        with open(args.sweep_md, "w") as f:
+            f.write("| max_ctas (grid) | reshard alone GB/s | GEMM alone TFLOP/s | concurrent: reshard GB/s | concurrent: GEMM TFLOP/s | both ms vs sum of alone ms | gain |\n")
+            f.write("|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %s (%d) | %.0f | %.0f | %.0f | %.0f | %.2f vs %.2f | %.2f |\n" % (
+                    r["max_ctas"] or "library default", r["grid"], r["reshard_GBs_alone"], r["gemm_TFLOPs_alone"],
+                    r["reshard_GBs_concurrent"], r["gemm_TFLOPs_concurrent"], r["both_ms"],
+                    r["gemm_alone_ms"] + r["reshard_alone_ms"], r["overlap_gain"]))
+    return 0
+
+
 def main():
     args = parse_args()
+    if args.overlap:
+        return run_overlap(args)
     if args.sweep:
         return run_sweep(args)
     if args.impl == "reference":

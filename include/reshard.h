@@ -107,7 +107,9 @@ typedef struct rs_plan_opts {
     int32_t src_devices_per_host;    /* host = device id / this (R8); 0 or 1: every device a host */
     int32_t dst_devices_per_host;
     int32_t trials;                  /* random orderings per round of RS_SCHED_GREEDY; 0 = 32               */
-    int32_t reserved;
+    int32_t max_ctas;                /* 0 = launch shape chosen by the library; > 0: never more than this many
+                                        CTAs (one per SM) per launch, leaving the other SMs to kernels of other
+                                        streams -- overlapping a resharding with compute (PAPER.md S4) on chip  */
     int64_t node_budget;             /* DFS nodes before giving up with the best found; 0 = 200000          */
     uint64_t seed;                   /* of the counter-based generator the greedy search draws from         */
 } rs_plan_opts;

@@ -125,6 +125,7 @@ rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int32_t ele
     P->sched.trials = opts->trials;
     P->sched.node_budget = opts->node_budget;
     P->sched.seed = opts->seed;
+    P->max_ctas = std::max(0, opts->max_ctas);
     rs_status st;
     try {
         st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, (flags & RS_EVEN_ONLY) != 0, &P->A);
@@ -317,7 +318,8 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         e = rs::launch_bulk_shift(dev, pt, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                                   op.shift_stage, st);
     } else {                                                  // register paths (also: aligned plan, unaligned pointers)
-        const int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
+        int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
+        if (P.max_ctas > 0) cap = std::min<int64_t>(cap, P.max_ctas);
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));
         static const bool no_shift = std::getenv("RS_NO_SHIFT") != nullptr;   // A/B switch for measurements
         if (align < 16 && !no_shift) e = rs::launch_shift(dev, pt, grid, st);  // any alignment, 16-byte accesses

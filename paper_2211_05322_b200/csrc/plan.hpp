@@ -99,6 +99,7 @@ struct Plan {
     std::vector<char> used_src;          // [n_src] 1 if some task reads that shard
     int device = -1;
     int sm_count = 148;
+    int max_ctas = 0;                    // rs_plan_opts.max_ctas: cap on CTAs per launch (0: none)
     void *dev_blob = nullptr;            // the ONE device allocation
 };
 

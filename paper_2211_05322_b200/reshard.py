@@ -54,7 +54,7 @@ class OpInfo(C.Structure):
 
 class PlanOpts(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("schedule", C.c_int32), ("src_devices_per_host", C.c_int32),
-                ("dst_devices_per_host", C.c_int32), ("trials", C.c_int32), ("reserved", C.c_int32),
+                ("dst_devices_per_host", C.c_int32), ("trials", C.c_int32), ("max_ctas", C.c_int32),
                 ("node_budget", C.c_int64), ("seed", C.c_uint64)]
 
 

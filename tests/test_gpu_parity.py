@@ -442,3 +442,18 @@ def test_maximum_ranks_and_device_counts(case, path):
     _p, got, want = gu.run_small(shape, np.int16, sm, ss, dm, ds, flags=path)
     for g, w in zip(got, want):
         assert g.tobytes() == w.tobytes()
+
+
+@pytest.mark.parametrize("cap", [1, 7, 64])
+def test_max_ctas_caps_the_grid_not_the_result(cap):
+    """rs_plan_opts.max_ctas: fewer CTAs (SMs left to other streams), same bytes"""
+    for case in (SMALL[2], SMALL[10], SMALL[17], SMALL[25]):
+        shape, sm, ss, dm, ds = case
+        for path in (rs.RS_PATH_AUTO, rs.RS_PATH_LSU, rs.RS_PATH_BULK_SHIFT):
+            p, got, want = gu.run_small(shape, np.int16, sm, ss, dm, ds, flags=path, opts=dict(max_ctas=cap))
+            assert p.op_info(rs.RS_OP_EXECUTE).grid <= cap
+            for g, w in zip(got, want):
+                assert g.tobytes() == w.tobytes()
+    w = inputs.get_workload("c4")
+    p = rs.Plan(w.shape, 2, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, dict(max_ctas=cap))
+    assert p.op_info(rs.RS_OP_EXECUTE).grid == cap
