@@ -3,7 +3,6 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -321,9 +320,8 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
         if (P.max_ctas > 0) cap = std::min<int64_t>(cap, P.max_ctas);
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));
-        static const bool no_shift = std::getenv("RS_NO_SHIFT") != nullptr;   // A/B switch for measurements
-        if (align < 16 && !no_shift) e = rs::launch_shift(dev, pt, grid, st);  // any alignment, 16-byte accesses
-        else e = rs::launch_lsu(dev, pt, align, grid, st);
+        if (align < 16) e = rs::launch_shift(dev, pt, grid, st);   // any alignment, still 16-byte accesses
+        else e = rs::launch_lsu(dev, pt, grid, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
     return RS_OK;

@@ -5,9 +5,10 @@
 // reshard_execute / reshard_pack / reshard_unpack differ only in the task table they run.
 //
 // Two executors, both sm_100a, no tensor cores (pure data movement, HBM-bound):
-//   rs_copy_lsu   register path.  Every thread keeps RS_LSU_UNROLL independent vector loads
-//                 (ld.global.nc, 16/8/4/2/1 bytes wide) in flight and stores each value k times.
-//                 Handles any alignment and any run length.
+//   rs_copy_lsu   register path for 16-byte aligned layouts with short runs.  Every thread keeps 4
+//                 independent 128-bit loads (ld.global.nc) in flight and stores each value k times.
+//   rs_copy_shift / rs_copy_bulk_shift   the same two designs for layouts (or pointers) that are NOT
+//                 16-byte aligned: 128-bit accesses on both sides, bytes realigned by a funnel shift.
 //   rs_copy_bulk  TMA path (SASS: UBLKCP).  Every warp owns a ring of shared-memory slots: lane r
 //                 issues cp.async.bulk global->shared for row r of the tile (mbarrier complete_tx),
 //                 and once the tile has landed, cp.async.bulk shared->global to each of the k
@@ -564,22 +565,9 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, co
 static thread_local int64_t g_launches = 0;
 int64_t launch_count() { return g_launches; }
 
-template <typename V>
-static cudaError_t launch_lsu_t(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st) {
-    constexpr int U = sizeof(V) == 16 ? RS_LSU_UNROLL / 2 : RS_LSU_UNROLL;   // 64 B in flight per thread
-    rs_copy_lsu<V, U><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int vec_bytes, int grid, cudaStream_t st) {
-    cudaError_t e;
-    switch (vec_bytes) {
-        case 16: e = launch_lsu_t<uint4>(op, ptrs, grid, st); break;
-        case 8:  e = launch_lsu_t<uint2>(op, ptrs, grid, st); break;
-        case 4:  e = launch_lsu_t<uint32_t>(op, ptrs, grid, st); break;
-        case 2:  e = launch_lsu_t<uint16_t>(op, ptrs, grid, st); break;
-        default: e = launch_lsu_t<uint8_t>(op, ptrs, grid, st); break;
-    }
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st) {
+    rs_copy_lsu<uint4, RS_LSU_UNROLL / 2><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);   // 64 B in flight per thread
+    cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) ++g_launches;
     return e;
 }

@@ -6,7 +6,7 @@
 #include "tables.h"
 
 namespace rs {
-cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int vec_bytes, int grid, cudaStream_t st);
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st);      // 16-byte aligned only
 cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st);
 cudaError_t prepare_bulk(int smem_bytes);
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
