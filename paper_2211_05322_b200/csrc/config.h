@@ -19,6 +19,7 @@
 #define RS_BULK_TILE_BYTES_SHORT 8192
 #define RS_BULK_CTAS_DEN       148    // CTA counts below are out of 148 SMs
 #define RS_BULK_CTAS_MCAST_NUM 96     // write-heavy (multicast) operations
+#define RS_BULK_CTAS_MCAST_SHORT_NUM 136   // write-heavy operations with short runs (4 warps per CTA)
 #define RS_BULK_CTAS_LONG_NUM  132    // 1 : 1 operations whose runs are at least RS_BULK_LONG_RUN
 #define RS_BULK_LONG_RUN       4096
 #define RS_BULK_CTAS_MIN_BYTES (256ll << 20)   // operations moving less than this keep one CTA on every SM

@@ -193,13 +193,15 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         //    whatever the ring depth or tile size, 96 writers reach 6.1-6.2 TB/s (an SM sustains ~64 GB/s of this
         //    mix; beyond ~104 SMs the writers contend);
         //  * 1 : 1 operations with long runs (<= 3 bulk copies per tile): 132 CTAs are 1.5-3.7 % faster than 148;
-        //  * short runs and the shifted variant are issue-bound per SM and want every SM.
+        //  * short runs are issue-bound per SM: write-heavy ones do best from 136 CTAs (Table 2 case 9: 5.7 -> 6.2 TB/s),
+        //    1 : 1 ones and the shifted variant from every SM.
         // Expressed as fractions of the SM count so the rule survives a different part.
         // Small operations are latency-bound, not contention-bound: they keep every SM.
         const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
         int dflt = P->sm_count;
         if (!big) dflt = P->sm_count;
         else if (!shift && !short_runs && write_heavy) dflt = P->sm_count * RS_BULK_CTAS_MCAST_NUM / RS_BULK_CTAS_DEN;
+        else if (!shift && short_runs && write_heavy) dflt = P->sm_count * RS_BULK_CTAS_MCAST_SHORT_NUM / RS_BULK_CTAS_DEN;
         else if (!shift && !write_heavy && min_run >= RS_BULK_LONG_RUN) dflt = P->sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
         I.grid = std::max(1, std::min(P->sm_count, env_int(write_heavy ? "RS_BULK_CTAS_MCAST" : "RS_BULK_CTAS", std::max(1, dflt))));
         if (P->max_ctas > 0) I.grid = std::min(I.grid, P->max_ctas);
