@@ -429,6 +429,47 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return r;
 }
 
+// One destination row: n bytes sit in shared memory from byte address `sm`; write them to `dr`.
+// The row is cut at the destination's 16-byte boundaries: head bytes, `full` aligned windows, tail
+// bytes.  The byte shift between source and destination is the same for every window of the row, so
+// it is resolved ONCE per row (switch on its word part, funnel shift by its byte part): a window
+// costs two ld.shared.v4, four SHF.R and one st.global.v4.
+__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
+    uint32_t r;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(r) : "r"(addr));
+    return r;
+}
+
+template <int W>
+__device__ __forceinline__ void row_windows(char *dst16, uint32_t base, uint32_t full, uint32_t b, uint32_t lane) {
+#pragma unroll 2
+    for (uint32_t c = lane; c < full; c += 32) {
+        const uint4 lo = lds128(base + 16u * c), hi = lds128(base + 16u * c + 16u);
+        const uint32_t w[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+        *reinterpret_cast<uint4 *>(dst16 + 16u * c) =
+            make_uint4(__funnelshift_r(w[W], w[W + 1], b), __funnelshift_r(w[W + 1], w[W + 2], b),
+                       __funnelshift_r(w[W + 2], w[W + 3], b), __funnelshift_r(w[W + 3], w[W + 4], b));
+    }
+}
+
+__device__ __forceinline__ void store_row(char *dr, uint32_t sm, uint32_t n, uint32_t lane) {
+    uint32_t head = (16u - (uint32_t)((uintptr_t)dr & 15u)) & 15u;
+    if (head > n) head = n;
+    const uint32_t full = (n - head) >> 4, tail = n - head - (full << 4);
+    const uint32_t q0 = sm + head, delta = q0 & 15u, b = (delta & 3u) * 8u, base = q0 - delta;
+    switch (delta >> 2) {                                     // warp-uniform
+        case 0: row_windows<0>(dr + head, base, full, b, lane); break;
+        case 1: row_windows<1>(dr + head, base, full, b, lane); break;
+        case 2: row_windows<2>(dr + head, base, full, b, lane); break;
+        default: row_windows<3>(dr + head, base, full, b, lane); break;
+    }
+    if (lane < head) dr[lane] = (char)lds_u8(sm + lane);
+    else if (lane >= 16u && lane - 16u < tail) {
+        const uint32_t off = head + (full << 4) + lane - 16u;
+        dr[off] = (char)lds_u8(sm + off);
+    }
+}
+
 // One 16-byte aligned window of a destination row, in two steps so that several windows' shared-memory
 // loads can be in flight: n bytes of the row sit in shared memory from byte address `sm`.
 struct ShiftSlot { uint4 lo, hi; int32_t X; uint32_t delta; };
@@ -520,7 +561,7 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, co
             for (uint32_t q = 0; q < k; q++) {                // read once (from HBM), write k times
                 const RsDst dd = dsts[q];
                 char *dp = ptrs.dst[dd.buf] + dd.off + d->dst_rel;
-                if (fast) {                                   // flat walk over (row, window), 2 windows in flight per lane
+                if (fast && SL < 64u) {                       // short rows: flat walk over (row, window), 2 in flight per lane
                     const uint32_t total = n_rows * SL, q32 = 32u / SL, r32 = 32u - q32 * SL;
                     uint32_t r = (uint32_t)lane / SL, c = (uint32_t)lane - r * SL;
                     for (uint32_t v = lane; v < total; v += 64) {
@@ -539,16 +580,12 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, co
                         slot_store(t0, dr0, n);
                         if (two) slot_store(t1, dr1, n);
                     }
-                } else {                                      // GENERIC tiles: row by row, lanes over windows
+                } else {                                      // long rows: row by row, the shift is uniform inside a row
                     for (uint32_t r = 0; r < n_rows; r++) {
-                        int64_t so, doff;
-                        generic_row(T, d->lin + r, &so, &doff);
-                        const uint32_t a = (uint32_t)((uintptr_t)(d->src + d->dst_rel + so) & 15u);
-                        for (uint32_t c = lane; c < SL; c += 32) {
-                            ShiftSlot t0;
-                            slot_load(t0, dp + doff, slot + r * pitch + 16u + a, n, c);
-                            slot_store(t0, dp + doff, n);
-                        }
+                        int64_t so = (int64_t)r * d->s0, doff = (int64_t)r * d->d0;
+                        if (!fast) { generic_row(T, d->lin + r, &so, &doff); so += d->dst_rel; }
+                        const uint32_t a = (uint32_t)((uintptr_t)(d->src + so) & 15u);
+                        store_row(dp + doff, slot + r * pitch + 16u + a, n, (uint32_t)lane);
                     }
                 }
             }
