@@ -457,3 +457,27 @@ def test_max_ctas_caps_the_grid_not_the_result(cap):
     w = inputs.get_workload("c4")
     p = rs.Plan(w.shape, 2, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, dict(max_ctas=cap))
     assert p.op_info(rs.RS_OP_EXECUTE).grid == cap
+
+
+@pytest.mark.parametrize("case", [
+    ((70, 300, 1001), (2, 2), "S0,S1,R", (3, 2), "S1,S0,R"),          # uneven on dims 0 and 1, odd runs: shifted kernels per slab
+    ((45, 260, 1024), (2, 4), "S0,R,R", (3, 4), "S0,R,R"),            # Table 2 case 6 in small: short last shard on dim 0
+    ((9, 64, 4096), (4,), "S0,R,R", (2, 3), "S1,S0,R"),               # 9 rows over 4 and over 3 devices
+])
+def test_execute_host_uneven_layouts(case):
+    """host buffers are padded too (R5, R11); only the valid boxes are specified after reshard_execute_host"""
+    shape, sm, ss, dm, ds = case
+    D = np.frombuffer(np.random.default_rng(5).bytes(int(np.prod(shape)) * 2), dtype=np.int16).reshape(shape)
+    src = do.shards_from_global(D, sm, ss, pad=0x11)
+    want = do.reshard(shape, sm, ss, dm, ds, src, n_threads=do.max_threads())
+    for opts in (None, dict(schedule=rs.RS_SCHED_ENSEMBLE, src_devices_per_host=2, dst_devices_per_host=2)):
+        p = rs.Plan(shape, 2, sm, ss, dm, ds, 0, opts)
+        src_h = [torch.from_numpy(s.copy()).pin_memory() for s in src]
+        dst_h = [torch.zeros(p.local_shape(rs.RS_DST), dtype=torch.int16).pin_memory() for _ in want]
+        ws = torch.empty(p.host_workspace_bytes(), dtype=torch.uint8, device=gu.dev())
+        p.execute_host(gu.ptrs(src_h), gu.ptrs(dst_h), ws.data_ptr(), gu.stream())
+        torch.cuda.current_stream().synchronize()
+        for q, (g, wq) in enumerate(zip(dst_h, want)):
+            lo, hi = do.device_box(shape, dm, ds, q)
+            valid = tuple(slice(0, h - l) for l, h in zip(lo, hi))
+            assert np.array_equal(g.numpy()[valid], wq[valid]), "device %d" % q
