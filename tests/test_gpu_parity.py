@@ -481,3 +481,40 @@ def test_execute_host_uneven_layouts(case):
             lo, hi = do.device_box(shape, dm, ds, q)
             valid = tuple(slice(0, h - l) for l, h in zip(lo, hi))
             assert np.array_equal(g.numpy()[valid], wq[valid]), "device %d" % q
+
+
+def _random_layout(rng):
+    ndim = int(rng.integers(1, 5))
+    meshes = [(1, 2), (2, 2), (2, 4), (4, 2), (2, 3), (3, 2), (1, 4), (4,), (3,), (2, 2, 2)]
+
+    def side():
+        mesh = meshes[int(rng.integers(len(meshes)))]
+        axes = list(rng.permutation(len(mesh)))
+        spec = []
+        for _ in range(ndim):
+            take = int(rng.integers(0, 3)) if axes else 0
+            mine = [axes.pop() for _ in range(min(take, len(axes)))]
+            spec.append("S" + "".join(str(a) for a in mine) if mine else "R")
+        return mesh, ",".join(spec)
+    sm, ss = side()
+    dm, ds = side()
+    inner = int(rng.choice([1, 3, 8, 17, 64, 100, 257, 1000]))
+    shape = tuple(int(rng.choice([1, 2, 5, 7, 12, 16, 33])) for _ in range(ndim - 1)) + (inner,)
+    return shape, sm, ss, dm, ds
+
+
+@pytest.mark.parametrize("seed", range(20))
+def test_random_layouts_alignments_and_paths(seed):
+    """fuzz: 12 seeded layouts per seed (even and uneven, 1..4 dims, runs of 1..1000 elements), every element size,
+    shard pointers at random byte offsets, every executor, with and without a schedule -- bit-exact, guard bands intact"""
+    rng = np.random.default_rng(2211_05322 + seed)
+    dtypes = [np.uint8, np.int16, np.float32, np.int64, np.dtype("V16")]
+    for _ in range(12):
+        shape, sm, ss, dm, ds = _random_layout(rng)
+        dtype = dtypes[int(rng.integers(len(dtypes)))]
+        path = PATHS[int(rng.integers(len(PATHS)))]
+        so, dofs = (int(rng.integers(0, 16)), int(rng.integers(0, 16))) if rng.integers(2) else (0, 0)
+        opts = dict(schedule=int(rng.integers(1, 6)), src_devices_per_host=int(rng.integers(1, 3)), node_budget=2000) if rng.integers(3) == 0 else None
+        _p, got, want = gu.run_small(shape, dtype, sm, ss, dm, ds, flags=path, seed=seed, src_offset=so, dst_offset=dofs, opts=opts)
+        for q, (g, w) in enumerate(zip(got, want)):
+            assert g.tobytes() == w.tobytes(), (shape, sm, ss, dm, ds, dtype, path, so, dofs, opts, q)
