@@ -4,7 +4,8 @@
 // box is read ONCE from its source buffer and written to each of its k destination buffers.
 // reshard_execute / reshard_pack / reshard_unpack differ only in the task table they run.
 //
-// Two executors, both sm_100a, no tensor cores (pure data movement, HBM-bound):
+// Four kernels (a TMA and a register design, each with a variant for unaligned layouts), all sm_100a,
+// no tensor cores (pure data movement, HBM-bound):
 //   rs_copy_lsu   register path for 16-byte aligned layouts with short runs.  Every thread keeps 4
 //                 independent 128-bit loads (ld.global.nc) in flight and stores each value k times.
 //   rs_copy_shift / rs_copy_bulk_shift   the same two designs for layouts (or pointers) that are NOT
