@@ -23,6 +23,8 @@
 #define RS_BULK_CTAS_LONG_NUM  132    // 1 : 1 operations whose runs are at least RS_BULK_LONG_RUN
 #define RS_BULK_LONG_RUN       4096
 #define RS_BULK_CTAS_MIN_BYTES (256ll << 20)   // operations moving less than this keep one CTA on every SM
+#define RS_SMALL_OP_BYTES    (64ll << 20)   // AUTO: aligned operations moving no more than this take the register path
+                                            // (no shared-memory carve-out, no mbarriers: 16 % faster up to 8 MiB, 4 % up to 64 MiB)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 
 // TMA loads + shifted register stores (unaligned layouts): the stores are ALU work, so more warps, smaller tiles

@@ -165,7 +165,9 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     const bool bulk_ok = align == 16 && min_run >= 16;
     int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
              : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
-             : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU : bulk_ok ? RS_PATH_BULK : RS_PATH_BULK_SHIFT;
+             : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU
+             : bulk_ok ? (read_bytes + write_bytes <= RS_SMALL_OP_BYTES ? RS_PATH_LSU : RS_PATH_BULK)   // small: launch-bound, the
+             : RS_PATH_BULK_SHIFT;                                                                      // register kernel starts faster
     if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_BULK_SHIFT;   // cp.async.bulk stores need 16-byte everything
     I.path = path;
     const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT;
