@@ -73,7 +73,7 @@ def peak_hbm():
 
 # ------------------------------------------------------------------ oracle timing (CPU baseline / reference arm)
 
-def oracle_sample(w, seconds, steps=1, warmup=0):
+def oracle_sample(w, seconds, steps=1, warmup=0, one_core=False):
     """Time the oracle AS IT STANDS on a bounded sample of workload w: whole destination shards
     (devices 0, 1, ...) until about `seconds` of wall time, all host cores.  Source shards hold a
     cheap seeded byte pattern (the oracle's cost does not depend on values).  Returns dict."""
@@ -112,7 +112,12 @@ def oracle_sample(w, seconds, steps=1, warmup=0):
             times.append(dt / q)
             shards_done = q
     t = statistics.median(times)
-    return {"value": per_shard_metric_bytes / t / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
+    t1 = None
+    if one_core:                                                       # also at 1 thread (one shard)
+        t0 = time.perf_counter()
+        do.reshard_device(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, src, 0, ct, n_threads=1, out=out)
+        t1 = time.perf_counter() - t0
+    return {"value_1core": None if t1 is None else per_shard_metric_bytes / t1 / 1e9, "value": per_shard_metric_bytes / t / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
             "sample": "%d destination shards of %s computed in full (devices 0..%d cyclically, %.0f MiB each), %d threads, %.2f s per shard"
                       % (shards_done, w.name, n_dst - 1, shard_bytes / 2**20, cores, t),
             "seconds_per_shard": t, "shards": shards_done}
@@ -340,8 +345,8 @@ def run_ours(args):
     if e2e is not None:
         line["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:
-        r = oracle_sample(w, args.cpu_seconds)
-        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        r = oracle_sample(w, args.cpu_seconds, one_core=True)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "value_1core")}
     print(json.dumps(line))
     multi.shutdown()
     return 0
