@@ -383,7 +383,11 @@ def run_sweep(args):
     rows = []
     for name in sweep_names(args.sweep):
         w = inputs.get_workload(name)
-        plan = harness.make_plan(w, flags | (rs.RS_WITH_STRATEGIES if args.strategies else 0))
+        if args.strategies:                                 # a mesh row is a host: local all-gather per row
+            plan = rs.Plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec,
+                           flags | rs.RS_WITH_STRATEGIES, dict(dst_devices_per_host=w.dst_mesh[-1]))
+        else:
+            plan = harness.make_plan(w, flags)
         info = plan.info
         g = torch.Generator(device=dev); g.manual_seed(w.seed % (1 << 31))
         def buf(n):
@@ -400,7 +404,8 @@ def run_sweep(args):
         if args.strategies:      # same result by the paper's other strategies; GB/s counts the USEFUL bytes (1 + r_B) like execute
             calls = [calls[0],
                      ("sendrecv", rs.RS_OP_EXECUTE, lambda: plan.execute_strategy(rs.RS_STRATEGY_SENDRECV, sp, dp, sh)),
-                     ("allgather", rs.RS_OP_EXECUTE, lambda: plan.execute_strategy(rs.RS_STRATEGY_ALLGATHER, sp, dp, sh))]
+                     ("allgather", rs.RS_OP_EXECUTE, lambda: plan.execute_strategy(rs.RS_STRATEGY_ALLGATHER, sp, dp, sh)),
+                     ("allgather_local", rs.RS_OP_EXECUTE, lambda: plan.execute_strategy(rs.RS_STRATEGY_ALLGATHER_LOCAL, sp, dp, sh))]
         row = {"workload": name, "shape": list(w.shape), "src": "%s %s" % ("x".join(map(str, w.src_mesh)), w.src_spec),
                "dst": "%s %s" % ("x".join(map(str, w.dst_mesh)), w.dst_spec), "n_slices": info.n_slices,
                "tensor_bytes": info.tensor_bytes}
@@ -445,14 +450,15 @@ def run_sweep(args):
         print(json.dumps(row), flush=True)
     if args.sweep_md and args.strategies:
         with open(args.sweep_md, "w") as f:
-            f.write("| workload | src -> dst | receivers per slice | broadcast ms (GB/s useful) | send/recv ms (x broadcast) | all-gather ms (x broadcast) | bytes moved: broadcast / others |\n")
-            f.write("|---|---|---|---|---|---|---|\n")
+            f.write("| workload | src -> dst | receivers per slice | broadcast ms (GB/s useful) | send/recv ms (x broadcast) | global all-gather ms (x broadcast) | local all-gather ms (x broadcast) | bytes moved: broadcast / others |\n")
+            f.write("|---|---|---|---|---|---|---|---|\n")
             for r in rows:
                 k = (r["execute"]["bytes"] - r["tensor_bytes"]) // r["tensor_bytes"]
                 b = r["execute"]["ms"]
-                f.write("| %s | %s -> %s | %d | %.3f (%.0f) | %.3f (%.2f) | %.3f (%.2f) | %d / %d x size(D) |\n" % (
+                f.write("| %s | %s -> %s | %d | %.3f (%.0f) | %.3f (%.2f) | %.3f (%.2f) | %.3f (%.2f) | %d / %d x size(D) |\n" % (
                     r["workload"], r["src"], r["dst"], k, b, r["execute"]["GB/s"], r["sendrecv"]["ms"], r["sendrecv"]["ms"] / b,
-                    r["allgather"]["ms"], r["allgather"]["ms"] / b, 1 + k, 2 * k))
+                    r["allgather"]["ms"], r["allgather"]["ms"] / b, r["allgather_local"]["ms"], r["allgather_local"]["ms"] / b,
+                    1 + k, 2 * k))
         return 0
     if args.sweep_md:
         with open(args.sweep_md, "w") as f:

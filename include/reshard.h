@@ -131,16 +131,20 @@ enum { RS_OP_EXECUTE = 0, RS_OP_PACK = 1, RS_OP_UNPACK = 2,
        RS_OP_EXECUTE_SLABS = 3, /* execute cut into dim-0 slabs: the table reshard_execute_host runs (queries only) */
        RS_OP_SENDRECV = 4,      /* RS_STRATEGY_SENDRECV: one copy task per (unit task, receiver)                    */
        RS_OP_AG_SCATTER = 5,    /* RS_STRATEGY_ALLGATHER phase 1: part j of every slice -> receiver j               */
-       RS_OP_AG_GATHER = 6      /* RS_STRATEGY_ALLGATHER phase 2: receivers copy the other parts from their peers   */ };
+       RS_OP_AG_GATHER = 6,     /* RS_STRATEGY_ALLGATHER phase 2: receivers copy the other parts from their peers   */
+       RS_OP_AGL_SCATTER = 7,   /* RS_STRATEGY_ALLGATHER_LOCAL phase 1: per receiver host, part j -> its j-th receiver */
+       RS_OP_AGL_GATHER = 8     /* RS_STRATEGY_ALLGATHER_LOCAL phase 2: all-gather inside every receiver host        */ };
 
 /* communication strategies for a unit task (S3.1), on chip */
 enum {
     RS_STRATEGY_BROADCAST = 0,  /* slice read once, written to every receiver (= reshard_execute)    */
     RS_STRATEGY_SENDRECV = 1,   /* the sender sends the slice to each receiver one by one: the slice
                                    is re-read per receiver (k reads + k writes)                                    */
-    RS_STRATEGY_ALLGATHER = 2   /* the slice is split over its k receivers, one part sent to each,
-                                   then the receivers all-gather: two dependent launches, 1 + (k-1) reads and
-                                   1 + (k-1) writes per slice byte                                                 */
+    RS_STRATEGY_ALLGATHER = 2,  /* PAPER.md:133 (global all-gather): the slice is split over its k receivers, one part
+                                   sent to each, then the receivers all-gather: two dependent launches, 1 + (k-1)
+                                   reads and 1 + (k-1) writes per slice byte                                       */
+    RS_STRATEGY_ALLGATHER_LOCAL = 3 /* PAPER.md:131 (local all-gather): the same inside every receiver HOST
+                                   (rs_plan_opts.dst_devices_per_host): the slice leaves the sender once per host  */
 };
 /* sides */
 enum { RS_SRC = 0, RS_DST = 1 };

@@ -346,10 +346,12 @@ rs_status reshard_execute_strategy(const rs_plan *plan, int32_t strategy, const 
     if (!(P.flags & RS_WITH_STRATEGIES)) { rs::set_error("plan was built without RS_WITH_STRATEGIES"); return RS_EINVAL; }
     if (strategy == RS_STRATEGY_SENDRECV)
         return run_op(plan, RS_OP_SENDRECV, src_shards, P.A.n_dev, dst_shards, P.B.n_dev, P.used_src.data(), cuda_stream);
-    if (strategy != RS_STRATEGY_ALLGATHER) { rs::set_error("unknown strategy"); return RS_EINVAL; }
-    rs_status st = run_op(plan, RS_OP_AG_SCATTER, src_shards, P.A.n_dev, dst_shards, P.B.n_dev, P.used_src.data(), cuda_stream);
+    if (strategy != RS_STRATEGY_ALLGATHER && strategy != RS_STRATEGY_ALLGATHER_LOCAL) { rs::set_error("unknown strategy"); return RS_EINVAL; }
+    const int scatter = strategy == RS_STRATEGY_ALLGATHER ? RS_OP_AG_SCATTER : RS_OP_AGL_SCATTER;
+    const int gather = strategy == RS_STRATEGY_ALLGATHER ? RS_OP_AG_GATHER : RS_OP_AGL_GATHER;
+    rs_status st = run_op(plan, scatter, src_shards, P.A.n_dev, dst_shards, P.B.n_dev, P.used_src.data(), cuda_stream);
     if (st != RS_OK) return st;                               // phase 2 reads what phase 1 wrote: same stream, in order
-    return run_op(plan, RS_OP_AG_GATHER, dst_shards, P.B.n_dev, dst_shards, P.B.n_dev, nullptr, cuda_stream);
+    return run_op(plan, gather, dst_shards, P.B.n_dev, dst_shards, P.B.n_dev, nullptr, cuda_stream);
 }
 
 rs_status reshard_pack(const rs_plan *plan, const void *const *src_shards, void *msg_arena, void *cuda_stream) {

@@ -78,7 +78,7 @@ struct Schedule {                        // S3.2 at host level (schedule.cpp); a
     std::vector<int64_t> start;          // S_i
 };
 
-enum { RS_OP_SLABS = 3, RS_N_OPS = 7 };  // internal 4th table: execute, cut into dim-0 slabs; 4..6: alternative strategies
+enum { RS_OP_SLABS = 3, RS_N_OPS = 9 };  // internal 4th table: execute, cut into dim-0 slabs; 4..6: alternative strategies
 
 struct Plan {
     Layout A, B;

@@ -414,7 +414,8 @@ rs_status build_tables(Plan *P) {
     // receiver j (1 read + 1 write in total), then every receiver copies the other k - 1 parts from
     // its peers' shards (k - 1 reads + k - 1 writes): again 2k, in two dependent launches.
     OpTables &SR = P->op[RS_OP_SENDRECV], &AS = P->op[RS_OP_AG_SCATTER], &AG = P->op[RS_OP_AG_GATHER];
-    for (OpTables *o : {&SR, &AS, &AG}) { o->tasks.clear(); o->dsts.clear(); o->tiles.clear(); o->info = rs_op_info{}; }
+    OpTables &LS = P->op[RS_OP_AGL_SCATTER], &LG = P->op[RS_OP_AGL_GATHER];
+    for (OpTables *o : {&SR, &AS, &AG, &LS, &LG}) { o->tasks.clear(); o->dsts.clear(); o->tiles.clear(); o->info = rs_op_info{}; }
     if (P->flags & RS_WITH_STRATEGIES) {
         auto add = [&](OpTables &O, const int64_t *lo, const int64_t *hi, int src_buf, const int64_t *src_origin,
                        const int64_t *sstr, int dst_buf, const int64_t *dst_origin) -> bool {
@@ -438,20 +439,38 @@ rs_status build_tables(Plan *P) {
             for (int j = 0; j < k; j++) { int64_t hi_r[RS_MAX_NDIM]; device_box(B, S.receivers[(size_t)j], org[(size_t)j].data(), hi_r); }
             for (int j = 0; j < k; j++)                           // send/recv: the whole slice, once per receiver
                 if (!add(SR, S.lo, S.hi, S.sender, lo_s, sA, S.receivers[(size_t)j], org[(size_t)j].data())) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
-            int cd = 0;                                        // all-gather: cut the outermost dim that has >= k rows (else the longest)
-            for (int d = 0; d < N; d++) if (S.hi[d] - S.lo[d] > S.hi[cd] - S.lo[cd]) cd = d;
-            for (int d = N - 1; d >= 0; d--) if (S.hi[d] - S.lo[d] >= k) cd = d;
-            const int64_t ext = S.hi[cd] - S.lo[cd], step = (ext + k - 1) / k;
-            for (int j = 0; j < k; j++) {
-                int64_t lo[RS_MAX_NDIM], hi[RS_MAX_NDIM];
-                for (int d = 0; d < N; d++) { lo[d] = S.lo[d]; hi[d] = S.hi[d]; }
-                lo[cd] = std::min(S.lo[cd] + j * step, S.hi[cd]);
-                hi[cd] = std::min(S.lo[cd] + (j + 1) * step, S.hi[cd]);
-                if (lo[cd] >= hi[cd]) continue;
-                if (!add(AS, lo, hi, S.sender, lo_s, sA, S.receivers[(size_t)j], org[(size_t)j].data())) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
-                for (int q = 0; q < k; q++)                   // gather: part j from receiver j's shard into receiver q's
-                    if (q != j && !add(AG, lo, hi, S.receivers[(size_t)j], org[(size_t)j].data(), sB, S.receivers[(size_t)q], org[(size_t)q].data())) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
+            // all-gather over a group G of receivers: part j of the slice goes to G[j], then everybody in G copies
+            // the other parts from its peers.  Global: one group = all k receivers.  Local
+            // (PAPER.md:131): one group per receiver HOST, so the slice leaves the sender once per host.
+            auto allgather = [&](const std::vector<int> &G, OpTables &scatter, OpTables &gather) -> bool {
+                const int g = (int)G.size();
+                int cd = 0;                                    // cut the outermost dim that has >= g rows (else the longest)
+                for (int d = 0; d < N; d++) if (S.hi[d] - S.lo[d] > S.hi[cd] - S.lo[cd]) cd = d;
+                for (int d = N - 1; d >= 0; d--) if (S.hi[d] - S.lo[d] >= g) cd = d;
+                const int64_t ext = S.hi[cd] - S.lo[cd], step = (ext + g - 1) / g;
+                for (int j = 0; j < g; j++) {
+                    int64_t lo[RS_MAX_NDIM], hi[RS_MAX_NDIM];
+                    for (int d = 0; d < N; d++) { lo[d] = S.lo[d]; hi[d] = S.hi[d]; }
+                    lo[cd] = std::min(S.lo[cd] + j * step, S.hi[cd]);
+                    hi[cd] = std::min(S.lo[cd] + (j + 1) * step, S.hi[cd]);
+                    if (lo[cd] >= hi[cd]) continue;
+                    const int rj = G[(size_t)j];
+                    if (!add(scatter, lo, hi, S.sender, lo_s, sA, S.receivers[(size_t)rj], org[(size_t)rj].data())) return false;
+                    for (int q : G)                            // gather: part j from G[j]'s shard into every other member's
+                        if (q != rj && !add(gather, lo, hi, S.receivers[(size_t)rj], org[(size_t)rj].data(), sB, S.receivers[(size_t)q], org[(size_t)q].data())) return false;
+                }
+                return true;
+            };
+            std::vector<int> all((size_t)k);
+            for (int j = 0; j < k; j++) all[(size_t)j] = j;
+            bool ok = allgather(all, AS, AG);
+            for (int j = 0; j < k && ok;) {                    // receivers are ascending, so a host's receivers are adjacent
+                std::vector<int> G;
+                const int host = S.receivers[(size_t)j] / P->sched.dst_dph;
+                while (j < k && S.receivers[(size_t)j] / P->sched.dst_dph == host) G.push_back(j++);
+                ok = allgather(G, LS, LG);
             }
+            if (!ok) { set_error("slice extent exceeds 32 bits"); return RS_EUNSUPPORTED; }
         }
     }
     rs_status st;
@@ -459,6 +478,11 @@ rs_status build_tables(Plan *P) {
         if ((st = finish_op(P, &SR, tensor_bytes * P->r_B, tensor_bytes * P->r_B)) != RS_OK) return st;
         if ((st = finish_op(P, &AS, tensor_bytes, tensor_bytes)) != RS_OK) return st;
         if ((st = finish_op(P, &AG, tensor_bytes * (P->r_B - 1), tensor_bytes * (P->r_B - 1))) != RS_OK) return st;
+        int64_t ls = 0, lg = 0;                                // local variant: bytes depend on how receivers fall on hosts
+        for (const RsTask &T : LS.tasks) ls += T.run_bytes * task_rows(T);
+        for (const RsTask &T : LG.tasks) lg += T.run_bytes * task_rows(T);
+        if ((st = finish_op(P, &LS, ls, ls)) != RS_OK) return st;
+        if ((st = finish_op(P, &LG, lg, lg)) != RS_OK) return st;
     }
     if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
     if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;

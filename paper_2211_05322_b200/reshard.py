@@ -20,8 +20,8 @@ RS_PATH_AUTO, RS_PATH_LSU, RS_PATH_BULK, RS_PATH_BULK_SHIFT = 0x00, 0x10, 0x20, 
 RS_HOST_ONLY = 0x100
 RS_EVEN_ONLY = 0x200
 RS_WITH_STRATEGIES = 0x400
-RS_OP_SENDRECV, RS_OP_AG_SCATTER, RS_OP_AG_GATHER = 4, 5, 6
-RS_STRATEGY_BROADCAST, RS_STRATEGY_SENDRECV, RS_STRATEGY_ALLGATHER = 0, 1, 2
+RS_OP_SENDRECV, RS_OP_AG_SCATTER, RS_OP_AG_GATHER, RS_OP_AGL_SCATTER, RS_OP_AGL_GATHER = 4, 5, 6, 7, 8
+RS_STRATEGY_BROADCAST, RS_STRATEGY_SENDRECV, RS_STRATEGY_ALLGATHER, RS_STRATEGY_ALLGATHER_LOCAL = 0, 1, 2, 3
 RS_OP_EXECUTE, RS_OP_PACK, RS_OP_UNPACK, RS_OP_EXECUTE_SLABS = 0, 1, 2, 3
 RS_SRC, RS_DST = 0, 1
 RS_SCHED_NONE, RS_SCHED_NAIVE, RS_SCHED_LOAD_BALANCE, RS_SCHED_DFS, RS_SCHED_GREEDY, RS_SCHED_ENSEMBLE = range(6)

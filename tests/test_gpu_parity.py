@@ -328,7 +328,8 @@ def test_execute_host_pipeline_cases(case):
             g.fill_(0x5A5A)
 
 
-@pytest.mark.parametrize("strategy", [rs.RS_STRATEGY_BROADCAST, rs.RS_STRATEGY_SENDRECV, rs.RS_STRATEGY_ALLGATHER])
+@pytest.mark.parametrize("strategy", [rs.RS_STRATEGY_BROADCAST, rs.RS_STRATEGY_SENDRECV, rs.RS_STRATEGY_ALLGATHER,
+                                      rs.RS_STRATEGY_ALLGATHER_LOCAL])
 @pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])
 @pytest.mark.parametrize("case", [SMALL[i] for i in (0, 3, 4, 7, 9, 10, 13, 17, 20, 23, 24)])
 def test_strategies_reach_the_oracle_result(case, path, strategy):
@@ -338,14 +339,14 @@ def test_strategies_reach_the_oracle_result(case, path, strategy):
     D = rng.integers(-2 ** 15, 2 ** 15, size=shape).astype(np.int16)
     src = do.shards_from_global(D, sm, ss)
     want = do.reshard(shape, sm, ss, dm, ds, src, fill=0xA5)
-    p = rs.Plan(shape, 2, sm, ss, dm, ds, path | rs.RS_WITH_STRATEGIES)
+    p = rs.Plan(shape, 2, sm, ss, dm, ds, path | rs.RS_WITH_STRATEGIES, dict(dst_devices_per_host=2))
     src_d = [gu.to_dev(s) for s in src]
     dst_d = [torch.full((w.nbytes,), 0xA5, dtype=torch.uint8, device=gu.dev()) for w in want]
     n0 = rs.launch_count()
     p.execute_strategy(strategy, gu.ptrs(src_d), gu.ptrs(dst_d), gu.stream())
     torch.cuda.synchronize()
-    r_B = p.info.write_bytes // p.info.tensor_bytes
-    assert rs.launch_count() - n0 == (1 if strategy != rs.RS_STRATEGY_ALLGATHER or r_B == 1 else 2)
+    gather = {rs.RS_STRATEGY_ALLGATHER: rs.RS_OP_AG_GATHER, rs.RS_STRATEGY_ALLGATHER_LOCAL: rs.RS_OP_AGL_GATHER}.get(strategy)
+    assert rs.launch_count() - n0 == (2 if gather is not None and p.op_info(gather).n_tiles else 1)
     for q, w in enumerate(want):
         assert dst_d[q].cpu().numpy().tobytes() == w.tobytes(), "device %d differs" % q
 
@@ -354,9 +355,9 @@ def test_strategies_full_size_multicast_and_refusal():
     w = inputs.sweep_workload("P5", "m8", 256 << 20)               # 1 read + 8 writes at 256 MiB
     e = inputs.elem_bytes(w.dtype)
     D, src = gu.workload_on_device(w)
-    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, rs.RS_WITH_STRATEGIES)
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, rs.RS_WITH_STRATEGIES, dict(dst_devices_per_host=4))
     idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
-    for strategy in (rs.RS_STRATEGY_SENDRECV, rs.RS_STRATEGY_ALLGATHER):
+    for strategy in (rs.RS_STRATEGY_SENDRECV, rs.RS_STRATEGY_ALLGATHER, rs.RS_STRATEGY_ALLGATHER_LOCAL):
         dst = [torch.zeros(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
         p.execute_strategy(strategy, gu.ptrs(src), gu.ptrs(dst), gu.stream())
         torch.cuda.synchronize()

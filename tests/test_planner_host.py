@@ -430,6 +430,21 @@ def test_strategy_tables_replay_equals_oracle(shape, sm, ss, dm, ds):
     a, g = p.op_info(rs.RS_OP_AG_SCATTER), p.op_info(rs.RS_OP_AG_GATHER)
     assert a.read_bytes == a.write_bytes == p.info.tensor_bytes
     assert g.read_bytes == g.write_bytes == p.info.tensor_bytes * (r_B - 1)
+    # local all-gather: per receiver host; with one device per host it degenerates to send/recv bytes
+    for dph in (1, 2, 4):
+        pl = _plan(shape, e, sm, ss, dm, ds, rs.RS_WITH_STRATEGIES, dict(dst_devices_per_host=dph))
+        dst = [np.zeros(want[0].nbytes, np.uint8) for _ in range(n_dst)]
+        cnt = [np.zeros(want[0].nbytes, np.int32) for _ in range(n_dst)]
+        ti.replay(pl, rs.RS_OP_AGL_SCATTER, [_bytes(s) for s in src], dst, cnt)
+        hosts_per_slice = [len({r // dph for r in sl["receivers"]}) for sl in pl.slices()]
+        slice_bytes = [int(np.prod([h - l for l, h in zip(sl["lo"], sl["hi"])])) * e for sl in pl.slices()]
+        assert sum(int(c.sum()) for c in cnt) == sum(h * b for h, b in zip(hosts_per_slice, slice_bytes))   # one copy per HOST
+        assert pl.op_info(rs.RS_OP_AGL_SCATTER).read_bytes == sum(h * b for h, b in zip(hosts_per_slice, slice_bytes))
+        ti.replay(pl, rs.RS_OP_AGL_GATHER, dst, dst, cnt)
+        for q in range(n_dst):
+            assert np.array_equal(dst[q], _bytes(want[q])) and np.array_equal(cnt[q], once[q])
+        ls, lg = pl.op_info(rs.RS_OP_AGL_SCATTER), pl.op_info(rs.RS_OP_AGL_GATHER)
+        assert ls.write_bytes + lg.write_bytes == pl.info.write_bytes
     # without the flag the tables are not built
     assert _plan(shape, e, sm, ss, dm, ds).op_info(rs.RS_OP_SENDRECV).n_tasks == 0
 
