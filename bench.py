@@ -53,7 +53,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU work of the oracle sample")
     ap.add_argument("--sweep", default=None, help="time execute/pack/unpack on a list of workloads instead of the step: "
-                    "'configs' (c2,c3,c3i,c3ii,c4), 'pairs' (6 pairs x 2 mesh pairs x 1 MiB..4 GiB), 'table2', 'all', "
+                    "'configs' (c2,c3,c3i,c3ii,c4), 'pairs' (6 pairs x 2 mesh pairs x 1 MiB..4 GiB), 'table2', 'fig5' (1 sender -> n receivers), 'all', "
                     "or comma-separated workload names; one JSON line per workload")
     ap.add_argument("--strategies", action="store_true", help="with --sweep: also time RS_STRATEGY_SENDRECV and "
                     "RS_STRATEGY_ALLGATHER (PAPER.md S3.1) against the broadcast executor")
@@ -360,7 +360,8 @@ def sweep_names(what):
     pairs = ["sweep_%s_%s_%dMiB" % (p, m, b >> 20) for p in inputs.SWEEP_PAIRS for m in inputs.SWEEP_MESHES
              for b in inputs.SWEEP_BYTES]
     t2 = ["t2_%d" % c for c in (1, 2, 3, 4, 5, 6, 7, 8, 9)]
-    return {"configs": cfg, "pairs": pairs, "table2": t2, "all": cfg + pairs + t2}.get(what) or what.split(",")
+    fig5 = ["fig5_%dx%d" % ab for ab in inputs.FIG5]
+    return {"configs": cfg, "pairs": pairs, "table2": t2, "fig5": fig5, "all": cfg + pairs + t2}.get(what) or what.split(",")
 
 
 def run_sweep(args):

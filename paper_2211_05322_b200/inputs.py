@@ -176,8 +176,20 @@ def table2_workload(case, shape=(1024, 1024, 512)):
     return _w("table2_case%d" % case, shape, "bf16", sm, ss, dm, ds, "bits", 20 + case)
 
 
+def fig5_workload(nodes, gpus_per_node, shape=(1024, 1024, 512)):
+    """PAPER.md:255 (S5.1.1): one sender GPU, a receiver mesh of `nodes` x `gpus_per_node` GPUs, both fully
+    replicated, "the message size keeps 1GB" (2 B/element here)."""
+    return _w("fig5_%dx%d" % (nodes, gpus_per_node), shape, "bf16", (1,), "RRR", (nodes, gpus_per_node), "RRR", "bits", 40 + 8 * nodes + gpus_per_node)
+
+
+FIG5 = [(1, 1), (1, 2), (1, 3), (1, 4), (2, 2), (3, 2), (4, 2)]     # group 1: one node, 1-4 GPUs; group 2: 2 GPUs per node, 1-4 nodes
+
+
 def get_workload(name):
-    """'c1'..'c4', 'c1i', 'c3i', 'c3ii', 't2_<case>', 'sweep_<pair>_<m8|m4>_<MiB>'."""
+    """'c1'..'c4', 'c1i', 'c3i', 'c3ii', 'u4', 't2_<case>', 'sweep_<pair>_<m8|m4>_<MiB>', 'fig5_<nodes>x<gpus>'."""
+    if name.startswith("fig5_"):
+        a, b = name[5:].split("x")
+        return fig5_workload(int(a), int(b))
     if name in CONFIGS:
         return CONFIGS[name]
     if name.startswith("t2_"):

@@ -519,3 +519,9 @@ def test_random_layouts_alignments_and_paths(seed):
         _p, got, want = gu.run_small(shape, dtype, sm, ss, dm, ds, flags=path, seed=seed, src_offset=so, dst_offset=dofs, opts=opts)
         for q, (g, w) in enumerate(zip(got, want)):
             assert g.tobytes() == w.tobytes(), (shape, sm, ss, dm, ds, dtype, path, so, dofs, opts, q)
+
+
+@pytest.mark.parametrize("nodes,gpus", [(1, 3), (4, 2)])
+def test_fig5_single_sender_full_size(nodes, gpus):
+    """one sender, a replicated receiver mesh, 1 GiB: every receiver ends with the whole tensor"""
+    _check_full_size(inputs.fig5_workload(nodes, gpus), n_samples=256)
