@@ -31,6 +31,8 @@
 #define RS_SHIFT_WARPS       8          // u4 (6145-byte runs, 2-byte aligned): 8 x 2 x 8 KiB = 5.6-5.7 TB/s; 4 x 4 x 8 KiB a little more,
 #define RS_SHIFT_STAGES      2          // but short rows (flat walk, ~100 instructions per 512 B) need the 8 warps
 #define RS_SHIFT_TILE_BYTES  8192
+#define RS_SHIFT_WARPS_LONG  4          // rows >= 1 KiB (row-by-row stores, ~35 instructions per 512 B): fewer, deeper pipelines
+#define RS_SHIFT_STAGES_LONG 4
 
 #define RS_BULK_DESC_BYTES   4096       // per-warp descriptor ring: 64 tiles x 64 bytes
 

@@ -182,9 +182,11 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         // a caller-imposed CTA cap (rs_plan_opts.max_ctas) is made up for with more warps per CTA:
         // 64 CTAs x 4 warps move 6.0 TB/s of a 1 : 1 layout, 64 x 2 only 3.9
         const bool capped = P->max_ctas > 0 && P->max_ctas * 4 < P->sm_count * 3;
-        int warps = std::max(1, std::min(8, shift ? env_int("RS_SHIFT_WARPS", RS_SHIFT_WARPS)
+        // shifted variant: rows of >= 1 KiB are stored row by row (cheap), shorter ones window by window (ALU-heavy)
+        const bool shift_long = shift && min_run >= 1024;
+        int warps = std::max(1, std::min(8, shift ? env_int("RS_SHIFT_WARPS", shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
                                                   : env_int("RS_BULK_WARPS", short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
-        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", shift_long ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
         tile_bytes = shift ? env_int("RS_SHIFT_TILE_BYTES", RS_SHIFT_TILE_BYTES)
                            : env_int("RS_BULK_TILE_BYTES", short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
@@ -236,7 +238,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     if (bulk_family) {
         const bool shift = path == RS_PATH_BULK_SHIFT;
         int warps = I.block / 32;
-        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", min_run >= 1024 ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
         int64_t stage = tile_bytes;
         if (shift) {                                           // a row of n bytes occupies (n + 77) & ~15 bytes of a ring slot
             stage = 0;
