@@ -32,8 +32,8 @@ FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE rs_copy_* launch of reshard_execute, from the
 # `ncu --set full` capture summarised in profiles/ (null for workloads without a capture)
 NCU_TRAFFIC_BYTES = {            # profiles/r01_ncu_sweep.md (read + write, one reshard_execute launch)
-    "c4": 1615138000 + 1562324000, "c2": 134619000 + 86010000, "u4": 1542838000 + 1461254000,
-    "t2_9": 1078002000 + 4236915000,
+    "c4": 1615138000 + 1562324000, "c2": 134619000 + 86010000, "u4": 1542835000 + 1459713000,
+    "t2_9": 1078115000 + 4236157000,
     "sweep_P1_m8_1024MiB": 1076611000 + 1025437000, "sweep_P2_m8_1024MiB": 1077257000 + 4237063000,
     "sweep_P3_m8_1024MiB": 1076592000 + 1026159000, "sweep_P4_m8_1024MiB": 1076634000 + 1024245000,
     "sweep_P5_m8_1024MiB": 1076652000 + 8530394000, "sweep_P6_m8_1024MiB": 1076653000 + 1021720000,
