@@ -138,6 +138,61 @@ void emit_tiles(const RsTask &T, uint32_t task_id, int64_t tile_bytes, std::vect
     }
 }
 
+// Which kernel an operation takes (rs_op_info.path).  AUTO: runs under 512 B and small aligned operations go to the
+// register kernels (they start faster; small operations are launch-bound), 16-byte aligned layouts to the TMA
+// kernel, everything else to TMA loads + shifted stores.
+int pick_path(uint32_t forced, int64_t align, int64_t min_run, int64_t moved_bytes) {
+    const bool bulk_ok = align == 16 && min_run >= 16;
+    int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
+             : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
+             : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU
+             : bulk_ok ? (moved_bytes <= RS_SMALL_OP_BYTES ? RS_PATH_LSU : RS_PATH_BULK)
+             : RS_PATH_BULK_SHIFT;
+    if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_BULK_SHIFT;   // cp.async.bulk stores need 16-byte everything
+    return path;
+}
+
+// Launch shape of the two TMA kernels, from measurement on B200.
+struct BulkShape { int warps, stages, grid; int64_t tile_bytes; };
+
+BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes) {
+    // short runs = many bulk copies per tile: one warp issues them too slowly, so more, smaller pipelines
+    // (Table 2 case 9, 512-byte runs: 3.6 TB/s with 2 warps, 5.7 with 4)
+    const bool short_runs = min_run <= RS_BULK_SHORT_RUN;
+    // a caller-imposed CTA cap (rs_plan_opts.max_ctas) is made up for with more warps per CTA:
+    // 64 CTAs x 4 warps move 6.0 TB/s of a 1 : 1 layout, 64 x 2 only 3.9
+    const bool capped = P.max_ctas > 0 && P.max_ctas * 4 < P.sm_count * 3;
+    // shifted variant: rows of >= 1 KiB are stored row by row (cheap), shorter ones window by window (ALU-heavy)
+    const bool shift_long = shift && min_run >= 1024;
+    BulkShape sh;
+    sh.warps = std::max(1, std::min(8, shift ? env_int("RS_SHIFT_WARPS", shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
+                                             : env_int("RS_BULK_WARPS", short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
+    sh.stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", shift_long ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES)
+                                              : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
+    sh.tile_bytes = shift ? env_int("RS_SHIFT_TILE_BYTES", RS_SHIFT_TILE_BYTES)
+                          : env_int("RS_BULK_TILE_BYTES", short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
+    sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
+    while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
+    // At most one CTA per SM -- and FEWER where the memory system prefers it (148 SMs):
+    //  * write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes): 148 writers hold 5.65 TB/s
+    //    whatever the ring depth or tile size, 96 writers reach 6.1-6.2 TB/s (an SM sustains ~64 GB/s of this
+    //    mix; beyond ~104 SMs the writers contend);
+    //  * 1 : 1 operations with long runs (<= 3 bulk copies per tile): 132 CTAs are 1.5-3.7 % faster than 148;
+    //  * short runs are issue-bound per SM: write-heavy ones do best from 136 CTAs (Table 2 case 9: 5.7 -> 6.2 TB/s),
+    //    1 : 1 ones and the shifted variant from every SM;
+    //  * operations under 256 MiB are latency-bound, not contention-bound: every SM.
+    // Fractions of the SM count, so the rule survives a different part.
+    const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
+    int ctas = P.sm_count;
+    if (big && !shift) {
+        if (write_heavy) ctas = P.sm_count * (short_runs ? RS_BULK_CTAS_MCAST_SHORT_NUM : RS_BULK_CTAS_MCAST_NUM) / RS_BULK_CTAS_DEN;
+        else if (min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
+    }
+    sh.grid = std::max(1, std::min(P.sm_count, env_int(write_heavy ? "RS_BULK_CTAS_MCAST" : "RS_BULK_CTAS", std::max(1, ctas))));
+    if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
+    return sh;
+}
+
 // Alignment class, path, tile size, grid of one operation; then its tile table.
 rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes,
                     std::vector<uint32_t> *task_tile_begin = nullptr) {
@@ -161,55 +216,20 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     I.read_bytes = read_bytes;
     I.write_bytes = write_bytes;
 
-    const uint32_t forced = P->flags & RS_PATH_MASK;
-    const bool bulk_ok = align == 16 && min_run >= 16;
-    int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
-             : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
-             : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU
-             : bulk_ok ? (read_bytes + write_bytes <= RS_SMALL_OP_BYTES ? RS_PATH_LSU : RS_PATH_BULK)   // small: launch-bound, the
-             : RS_PATH_BULK_SHIFT;                                                                      // register kernel starts faster
-    if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_BULK_SHIFT;   // cp.async.bulk stores need 16-byte everything
+    const int path = pick_path(P->flags & RS_PATH_MASK, align, min_run, read_bytes + write_bytes);
     I.path = path;
     const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT;
 
     int64_t tile_bytes;
     int workers;                                               // independent tile consumers in one launch
+    int stages = 0;
     if (bulk_family) {
-        // short runs = many bulk copies per tile: one warp issues them too slowly, so use more,
-        // smaller pipelines (t2 case 9, 512-byte runs: 3.6 TB/s with 2 warps, 5.7 with 4)
-        // the shifted variant assembles every 16 bytes in registers: many warps, small tiles
-        const bool short_runs = min_run <= RS_BULK_SHORT_RUN, shift = path == RS_PATH_BULK_SHIFT;
-        // a caller-imposed CTA cap (rs_plan_opts.max_ctas) is made up for with more warps per CTA:
-        // 64 CTAs x 4 warps move 6.0 TB/s of a 1 : 1 layout, 64 x 2 only 3.9
-        const bool capped = P->max_ctas > 0 && P->max_ctas * 4 < P->sm_count * 3;
-        // shifted variant: rows of >= 1 KiB are stored row by row (cheap), shorter ones window by window (ALU-heavy)
-        const bool shift_long = shift && min_run >= 1024;
-        int warps = std::max(1, std::min(8, shift ? env_int("RS_SHIFT_WARPS", shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
-                                                  : env_int("RS_BULK_WARPS", short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
-        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", shift_long ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
-        tile_bytes = shift ? env_int("RS_SHIFT_TILE_BYTES", RS_SHIFT_TILE_BYTES)
-                           : env_int("RS_BULK_TILE_BYTES", short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
-        tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
-        while ((int64_t)warps * (stages * tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && tile_bytes > 1024) tile_bytes -= 1024;
-        I.block = warps * 32;
-        // At most one CTA per SM -- and FEWER where measurement says the memory system prefers it (B200, 148 SMs):
-        //  * write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes): 148 writers hold 5.65 TB/s
-        //    whatever the ring depth or tile size, 96 writers reach 6.1-6.2 TB/s (an SM sustains ~64 GB/s of this
-        //    mix; beyond ~104 SMs the writers contend);
-        //  * 1 : 1 operations with long runs (<= 3 bulk copies per tile): 132 CTAs are 1.5-3.7 % faster than 148;
-        //  * short runs are issue-bound per SM: write-heavy ones do best from 136 CTAs (Table 2 case 9: 5.7 -> 6.2 TB/s),
-        //    1 : 1 ones and the shifted variant from every SM.
-        // Expressed as fractions of the SM count so the rule survives a different part.
-        // Small operations are latency-bound, not contention-bound: they keep every SM.
-        const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
-        int dflt = P->sm_count;
-        if (!big) dflt = P->sm_count;
-        else if (!shift && !short_runs && write_heavy) dflt = P->sm_count * RS_BULK_CTAS_MCAST_NUM / RS_BULK_CTAS_DEN;
-        else if (!shift && short_runs && write_heavy) dflt = P->sm_count * RS_BULK_CTAS_MCAST_SHORT_NUM / RS_BULK_CTAS_DEN;
-        else if (!shift && !write_heavy && min_run >= RS_BULK_LONG_RUN) dflt = P->sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
-        I.grid = std::max(1, std::min(P->sm_count, env_int(write_heavy ? "RS_BULK_CTAS_MCAST" : "RS_BULK_CTAS", std::max(1, dflt))));
-        if (P->max_ctas > 0) I.grid = std::min(I.grid, P->max_ctas);
-        workers = I.grid * warps;
+        const BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes);
+        tile_bytes = sh.tile_bytes;
+        stages = sh.stages;
+        I.block = sh.warps * 32;
+        I.grid = sh.grid;
+        workers = sh.grid * sh.warps;
     } else {
         tile_bytes = env_int("RS_LSU_TILE_BYTES", RS_LSU_TILE_BYTES);
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
@@ -235,10 +255,10 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     for (const RsTile &t : op->tiles) mr = std::min<int64_t>(mr, t.col_bytes);
     I.min_run_bytes = op->tiles.empty() ? 0 : mr;
     op->shift_stage = 0;
+    bool lsu = !bulk_family;
     if (bulk_family) {
         const bool shift = path == RS_PATH_BULK_SHIFT;
         int warps = I.block / 32;
-        int stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", min_run >= 1024 ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES) : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
         int64_t stage = tile_bytes;
         if (shift) {                                           // a row of n bytes occupies (n + 77) & ~15 bytes of a ring slot
             stage = 0;
@@ -251,11 +271,17 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         op->lookahead = std::max(1, std::min(stages - 1, shift ? env_int("RS_SHIFT_LOOKAHEAD", stages - 1) : env_int("RS_BULK_LOOKAHEAD", RS_BULK_LOOKAHEAD)));
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
         I.smem_bytes = (int32_t)(warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024);
-        if (shift) {
-            op->shift_stage = (uint32_t)stage;
-            if (I.smem_bytes > RS_SMEM_MAX) { I.path = RS_PATH_LSU; I.smem_bytes = 0; op->shift_stage = 0; }   // rows too sparse for the ring
+        if (shift) op->shift_stage = (uint32_t)stage;
+        if (shift && I.smem_bytes > RS_SMEM_MAX) {             // rows too sparse for the ring: the register kernels take it
+            I.path = RS_PATH_LSU;
+            I.block = RS_LSU_THREADS;
+            I.grid = P->sm_count * RS_LSU_CTAS_DEFAULT;
+            if (P->max_ctas > 0) I.grid = std::min(I.grid, P->max_ctas);
+            op->shift_stage = 0;
+            lsu = true;
         }
-    } else {
+    }
+    if (lsu) {
         const int warps = RS_LSU_THREADS / 32;
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
         I.smem_bytes = 0;

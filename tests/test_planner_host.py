@@ -462,3 +462,21 @@ def test_maximum_ranks_and_device_counts(shape, sm, ss, dm, ds):
     with pytest.raises(rs.ReshardError) as ei:
         _plan(shape + (2,) * (9 - len(shape)), 2, sm, ss + ",R" * (9 - len(shape)), dm, ds + ",R" * (9 - len(shape)))
     assert ei.value.code == rs.RS_EINVAL                      # more than RS_MAX_NDIM dims
+
+
+def test_launch_shapes_follow_the_measured_rules():
+    """what AUTO picks for the benchmark workloads (148-SM part)"""
+    def shape_of(name, op=rs.RS_OP_EXECUTE, **opts):
+        w = inputs.get_workload(name)
+        p = _plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, opts or None)
+        o = p.op_info(op)
+        return o.path, o.grid, o.block
+    assert shape_of("c4") == (rs.RS_PATH_BULK, 132, 64)                           # long runs, 1 : 1
+    assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64)          # 2 KiB runs, 1 : 1
+    assert shape_of("sweep_P5_m8_1024MiB") == (rs.RS_PATH_BULK, 96, 64)           # 1 read + 8 writes
+    assert shape_of("sweep_P5_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 64)   # its unpack is a 1 : 1 copy
+    assert shape_of("t2_9") == (rs.RS_PATH_BULK, 136, 128)                        # 512-byte runs, 1 + 4
+    assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 128)                    # nothing aligned, long rows
+    assert shape_of("c2") == (rs.RS_PATH_BULK, 148, 64)                           # 256 MiB moved: below the CTA rules
+    assert shape_of("c3")[0] == shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU  # small operations: register path
+    assert shape_of("c4", max_ctas=48) == (rs.RS_PATH_BULK, 48, 128)              # capped: more warps per CTA
