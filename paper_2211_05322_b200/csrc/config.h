@@ -25,6 +25,7 @@
 #define RS_BULK_CTAS_MIN_BYTES (256ll << 20)   // operations moving less than this keep one CTA on every SM
 #define RS_SMALL_OP_BYTES    (64ll << 20)   // AUTO: aligned operations moving no more than this take the register path
                                             // (no shared-memory carve-out, no mbarriers: 16 % faster up to 8 MiB, 4 % up to 64 MiB)
+#define RS_INTERLEAVE_MAX_RUN (64 << 10)    // destination runs up to this long count as a fine interleave (tile order)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 
 // TMA loads + shifted register stores (unaligned layouts): the stores are ALU work, so more warps, smaller tiles

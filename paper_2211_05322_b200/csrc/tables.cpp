@@ -195,7 +195,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
 
 // Alignment class, path, tile size, grid of one operation; then its tile table.
 rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes,
-                    std::vector<uint32_t> *task_tile_begin = nullptr) {
+                    std::vector<uint32_t> *task_tile_begin = nullptr, bool dst_order = false) {
     int64_t align = 16, min_run = INT64_MAX, max_rows = 0;
     for (const RsTask &T : op->tasks) {
         align = std::min(align, pow2_align(T.run_bytes));
@@ -249,6 +249,33 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         emit_tiles(op->tasks[t], (uint32_t)t, tile_bytes, &op->tiles);
     }
     if (task_tile_begin) task_tile_begin->push_back((uint32_t)op->tiles.size());
+    // Tasks whose destination boxes interleave finely (a slice fills part of every destination row, another
+    // slice the rest: config 2, sweep pairs P1 / P2 / P4) are walked in DESTINATION address order, so that the
+    // pieces of one row are written close in time: +1-3 % on those layouts (P2 at 4 GiB 6.00 -> 6.18 TB/s).
+    // Only for execute (shard -> shards); not for the slab table (its tile ranges are per task) and not for coarse
+    // interleaves (config 4: 3 MiB runs).
+    bool interleaved = false;
+    for (const RsTask &T : op->tasks) interleaved = interleaved || (T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.dstride[0] > T.run_bytes);
+    if (dst_order && env_int("RS_TILE_ORDER", 1) && !task_tile_begin && interleaved && op->tasks.size() > 1) {
+        struct Key { int64_t buf, off; uint32_t idx; };
+        std::vector<Key> keys(op->tiles.size());
+        for (size_t i = 0; i < op->tiles.size(); i++) {
+            const RsTile &t = op->tiles[i];
+            const RsTask &T = op->tasks[t.task];
+            int64_t doff = 0;
+            if (t.flags & RS_TILE_FAST) doff = (int64_t)t.b;
+            else {
+                int64_t row = (int64_t)t.a;
+                for (int d = 0; d < T.nd; d++) { int64_t c = row % T.ext[d]; row /= T.ext[d]; doff += c * T.dstride[d]; }
+            }
+            const RsDst &D = op->dsts[(size_t)T.dst_first];
+            keys[i] = Key{D.buf, D.off + doff, (uint32_t)i};
+        }
+        std::stable_sort(keys.begin(), keys.end(), [](const Key &x, const Key &y) { return x.buf != y.buf ? x.buf < y.buf : x.off < y.off; });
+        std::vector<RsTile> sorted(op->tiles.size());
+        for (size_t i = 0; i < keys.size(); i++) sorted[i] = op->tiles[keys[i].idx];
+        op->tiles.swap(sorted);
+    }
     if (op->tiles.size() > 0x7FFFFFFFull) { set_error("tile table too large"); return RS_EUNSUPPORTED; }
     I.n_tiles = (int32_t)op->tiles.size();
     int64_t mr = INT64_MAX;
@@ -513,7 +540,7 @@ rs_status build_tables(Plan *P) {
         if ((st = finish_op(P, &LG, lg, lg)) != RS_OK) return st;
     }
     if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
-    if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
+    if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B, nullptr, true)) != RS_OK) return st;
     if ((st = finish_op(P, &PK, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
     if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B)) != RS_OK) return st;
     return RS_OK;
