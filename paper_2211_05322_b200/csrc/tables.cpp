@@ -252,7 +252,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     // Tasks whose destination boxes interleave finely (a slice fills part of every destination row, another
     // slice the rest: config 2, sweep pairs P1 / P2 / P4) are walked in DESTINATION address order, so that the
     // pieces of one row are written close in time: +1-3 % on those layouts (P2 at 4 GiB 6.00 -> 6.18 TB/s).
-    // Only for execute (shard -> shards); not for the slab table (its tile ranges are per task) and not for coarse
+    // Only for execute and unpack (they write shards); not for the slab table (its tile ranges are per task) and not for coarse
     // interleaves (config 4: 3 MiB runs).
     bool interleaved = false;
     for (const RsTask &T : op->tasks) interleaved = interleaved || (T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.dstride[0] > T.run_bytes);
@@ -542,7 +542,7 @@ rs_status build_tables(Plan *P) {
     if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
     if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B, nullptr, true)) != RS_OK) return st;
     if ((st = finish_op(P, &PK, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
-    if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B)) != RS_OK) return st;
+    if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B, nullptr, true)) != RS_OK) return st;
     return RS_OK;
 }
 
