@@ -519,6 +519,23 @@ def test_random_layouts_alignments_and_paths(seed):
         _p, got, want = gu.run_small(shape, dtype, sm, ss, dm, ds, flags=path, seed=seed, src_offset=so, dst_offset=dofs, opts=opts)
         for q, (g, w) in enumerate(zip(got, want)):
             assert g.tobytes() == w.tobytes(), (shape, sm, ss, dm, ds, dtype, path, so, dofs, opts, q)
+        if rng.integers(3) == 0:                                   # another route to the same layout, and pack -> unpack
+            strategy = int(rng.integers(1, 4))
+            e = np.dtype(dtype).itemsize
+            p = rs.Plan(shape, e, sm, ss, dm, ds, path | rs.RS_WITH_STRATEGIES, dict(dst_devices_per_host=int(rng.integers(1, 4))))
+            D = np.frombuffer(np.random.default_rng(seed).bytes(int(np.prod(shape)) * e), dtype=dtype).reshape(shape)
+            src_d = [gu.to_dev(x) for x in do.shards_from_global(D, sm, ss)]
+            for route in ("strategy", "pack"):
+                dst_d = [torch.full((w.nbytes,), 0xA5, dtype=torch.uint8, device=gu.dev()) for w in want]
+                if route == "strategy":
+                    p.execute_strategy(strategy, gu.ptrs(src_d), gu.ptrs(dst_d), gu.stream())
+                else:
+                    arena = torch.zeros(max(1, p.info.arena_bytes), dtype=torch.uint8, device=gu.dev())
+                    p.pack(gu.ptrs(src_d), arena.data_ptr(), gu.stream())
+                    p.unpack(arena.data_ptr(), gu.ptrs(dst_d), gu.stream())
+                torch.cuda.synchronize()
+                for q, w in enumerate(want):
+                    assert dst_d[q].cpu().numpy().tobytes() == w.tobytes(), (shape, sm, ss, dm, ds, dtype, path, route, strategy, q)
 
 
 @pytest.mark.parametrize("nodes,gpus", [(1, 3), (4, 2)])
