@@ -94,9 +94,13 @@ _LIB = None
 def _lib():
     global _LIB
     if _LIB is None:
-        if not os.path.exists(LIB_PATH):
-            raise ImportError("libreshard.so is not built: run `python -m paper_2211_05322_b200.build` "
-                              "(there is no fallback path)")
+        try:                                  # build in-tree if missing or older than its sources (nvcc, sm_100a only)
+            from . import build as _build
+            _build.build()
+        except Exception as ex:               # noqa: BLE001 -- no nvcc, or a compile error: say so, there is no fallback
+            if not os.path.exists(LIB_PATH):
+                raise ImportError("libreshard.so is not built and could not be built (%s): run "
+                                  "`python -m paper_2211_05322_b200.build` (there is no fallback path)" % ex)
         try:
             L = C.CDLL(LIB_PATH)
         except OSError:                      # libcudart not on the loader path: torch ships one
