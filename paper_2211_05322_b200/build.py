@@ -29,9 +29,15 @@ def build(force=False, verbose=False):
     if not force and not _stale():
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    tmp = "%s.%d.tmp" % (OUT, os.getpid())                  # several ranks may build at once: replace atomically
     cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          [os.path.join(CSRC, f) for f in SOURCES] + ["-o", OUT]
-    subprocess.run(cmd, check=True)
+          [os.path.join(CSRC, f) for f in SOURCES] + ["-o", tmp]
+    try:
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, OUT)
+    finally:
+        if os.path.exists(tmp):
+            os.unlink(tmp)
     return OUT
 
 
