@@ -66,8 +66,7 @@ rs_status upload(rs::Plan *P) {
     for (rs::OpTables &o : P->op) smem = std::max(smem, (int)RS_SMEM_MAX);
     e = rs::prepare_bulk(smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(rs_copy_bulk)");
-    e = rs::prepare_bulk_shift(smem);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(rs_copy_bulk_shift)");
+
     // reshard_execute_host pipeline: plan-owned upload / download streams and per-slab events
     for (int i = 0; i < 2; i++) {
         cudaStream_t st;
@@ -289,6 +288,8 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     const rs::OpTables &op = P.op[opi];
     if (op.tiles.empty()) return RS_OK;
     RsPtrTable pt;
+    const bool small = n_src <= RS_PTRS_SMALL && n_dst <= RS_PTRS_SMALL;   // then the kernels get the 256-byte table
+    for (int i = 0; i < RS_PTRS_SMALL; i++) { pt.src[i] = nullptr; pt.dst[i] = nullptr; }
     int align = op.info.vec_bytes;
     for (int i = 0; i < n_src; i++) {
         pt.src[i] = static_cast<const char *>(src[i]);
@@ -310,18 +311,18 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     const int warps = op.info.block / 32;
     if (op.info.path == RS_PATH_BULK && align == 16) {
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
-        e = rs::launch_bulk(dev, pt, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
+        e = rs::launch_bulk(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                             (uint32_t)op.info.tile_bytes, st);
     } else if (op.info.path == RS_PATH_BULK_SHIFT) {          // layout not 16-byte aligned: TMA loads, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
-        e = rs::launch_bulk_shift(dev, pt, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
+        e = rs::launch_bulk_shift(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                                   op.shift_stage, st);
     } else {                                                  // register paths (also: aligned plan, unaligned pointers)
         int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
         if (P.max_ctas > 0) cap = std::min<int64_t>(cap, P.max_ctas);
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));
-        if (align < 16) e = rs::launch_shift(dev, pt, grid, st);   // any alignment, still 16-byte accesses
-        else e = rs::launch_lsu(dev, pt, grid, st);
+        if (align < 16) e = rs::launch_shift(dev, pt, small, grid, st);   // any alignment, still 16-byte accesses
+        else e = rs::launch_lsu(dev, pt, small, grid, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
     return RS_OK;

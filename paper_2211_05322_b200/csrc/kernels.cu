@@ -51,7 +51,8 @@ static_assert(sizeof(RsDesc) == 64, "descriptor ring slot");
 #define RS_DESC_RING 64
 static_assert(RS_DESC_RING * sizeof(RsDesc) == RS_BULK_DESC_BYTES, "config.h and the ring disagree");
 
-__device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsPtrTable &ptrs, uint32_t tile_index,
+template <int NP>
+__device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsPtrTableT<NP> &ptrs, uint32_t tile_index,
                                              RsDesc *out) {
     const RsTile tile = load_tile(op.tiles, tile_index);
     const RsTask *__restrict__ T = op.tasks + tile.task;
@@ -104,9 +105,9 @@ template <> __device__ __forceinline__ void st_stream<uint4>(char *p, const uint
 // Every WARP is an independent worker (no CTA-wide synchronisation anywhere).  Inside a tile the
 // warp walks the (row, column) grid of V-sized vectors 32 at a time; (row, col) advance incrementally,
 // so the only integer division is one per tile.  U loads are issued back to back, then U x k stores.
-template <typename V, int U>
+template <typename V, int U, int NP>
 __global__ void __launch_bounds__(RS_LSU_THREADS, RS_LSU_CTAS_PER_SM)
-rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs) {
+rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
     constexpr uint32_t VB = sizeof(V);
     __shared__ RsDesc ring[RS_LSU_THREADS / 32][32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = RS_LSU_THREADS / 32;
@@ -197,9 +198,9 @@ __device__ __forceinline__ uint4 shift_window(const uint4 lo, const uint4 hi, ui
                       __funnelshift_r(y3, y4, b));
 }
 
-template <int U>
+template <int U, int NP>
 __global__ void __launch_bounds__(RS_LSU_THREADS, RS_LSU_CTAS_DEFAULT)
-rs_copy_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs) {
+rs_copy_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
     __shared__ RsDesc ring[RS_LSU_THREADS / 32][32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = RS_LSU_THREADS / 32;
     RsDesc *descs = ring[warp];
@@ -327,8 +328,9 @@ __device__ __forceinline__ void bulk_wait_read(int pending) {  // immediate oper
     }
 }
 
+template <int NP>
 __global__ void __launch_bounds__(256, 1)
-rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const int stages, const int lookahead,
+rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
              const uint32_t stage_bytes) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
@@ -497,8 +499,9 @@ __device__ __forceinline__ void slot_store(const ShiftSlot &t, char *dr, uint32_
     }
 }
 
+template <int NP>
 __global__ void __launch_bounds__(256, 1)
-rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, const int stages, const int lookahead,
+rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
                    const uint32_t stage_bytes) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
@@ -603,42 +606,52 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTable ptrs, co
 static thread_local int64_t g_launches = 0;
 int64_t launch_count() { return g_launches; }
 
-cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st) {
-    rs_copy_lsu<uint4, RS_LSU_UNROLL / 2><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);   // 64 B in flight per thread
+// the first n pointers of each side in a 256-byte parameter
+static RsPtrTableT<RS_PTRS_SMALL> small_table(const RsPtrTable &ptrs) {
+    RsPtrTableT<RS_PTRS_SMALL> t;
+    for (int i = 0; i < RS_PTRS_SMALL; i++) { t.src[i] = ptrs.src[i]; t.dst[i] = ptrs.dst[i]; }
+    return t;
+}
+
+static cudaError_t launched() {
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) ++g_launches;
     return e;
 }
 
-cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, int grid, cudaStream_t st) {
-    rs_copy_shift<4><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) ++g_launches;
-    return e;
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, cudaStream_t st) {
+    constexpr int U = RS_LSU_UNROLL / 2;                       // 64 B in flight per thread
+    if (small) rs_copy_lsu<uint4, U, RS_PTRS_SMALL><<<grid, RS_LSU_THREADS, 0, st>>>(op, small_table(ptrs));
+    else rs_copy_lsu<uint4, U, 128><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
+    return launched();
+}
+
+cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, cudaStream_t st) {
+    if (small) rs_copy_shift<4, RS_PTRS_SMALL><<<grid, RS_LSU_THREADS, 0, st>>>(op, small_table(ptrs));
+    else rs_copy_shift<4, 128><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
+    return launched();
 }
 
 cudaError_t prepare_bulk(int smem_bytes) {
-    return cudaFuncSetAttribute(rs_copy_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-}
-
-cudaError_t prepare_bulk_shift(int smem_bytes) {
-    return cudaFuncSetAttribute(rs_copy_bulk_shift, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-}
-
-cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
-                              int lookahead, uint32_t stage_bytes, cudaStream_t st) {
-    rs_copy_bulk_shift<<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) ++g_launches;
+    cudaError_t e = cudaFuncSetAttribute(rs_copy_bulk<RS_PTRS_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rs_copy_bulk<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rs_copy_bulk_shift<RS_PTRS_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rs_copy_bulk_shift<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
     return e;
 }
 
-cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, int grid, int block, int smem_bytes, int stages,
+cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
+                              int stages, int lookahead, uint32_t stage_bytes, cudaStream_t st) {
+    if (small) rs_copy_bulk_shift<RS_PTRS_SMALL><<<grid, block, smem_bytes, st>>>(op, small_table(ptrs), stages, lookahead, stage_bytes);
+    else rs_copy_bulk_shift<128><<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
+    return launched();
+}
+
+cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes, int stages,
                         int lookahead, uint32_t stage_bytes, cudaStream_t st) {
-    rs_copy_bulk<<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) ++g_launches;
-    return e;
+    if (small) rs_copy_bulk<RS_PTRS_SMALL><<<grid, block, smem_bytes, st>>>(op, small_table(ptrs), stages, lookahead, stage_bytes);
+    else rs_copy_bulk<128><<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
+    return launched();
 }
 
 }  // namespace rs

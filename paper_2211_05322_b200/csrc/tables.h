@@ -47,10 +47,14 @@ struct alignas(16) RsTile {
     uint64_t a, b;
 };
 
-struct RsPtrTable {                      // kernel parameter: shard base pointers of one launch
-    const char *src[128];
-    char *dst[128];
+template <int NP>
+struct RsPtrTableT {                     // kernel parameter: shard base pointers of one launch
+    const char *src[NP];
+    char *dst[NP];
 };
+typedef RsPtrTableT<128> RsPtrTable;     // RS_MAX_DEVICES per side: what the launch glue fills
+#define RS_PTRS_SMALL 16                 // meshes of up to 16 devices per side get a 256-byte parameter instead of 2 KiB:
+                                         // ~1 us less launch time, which is 10 % of a 1 MiB operation
 
 struct RsOpDev {                         // one operation's tables in device memory
     const RsTask *tasks;
