@@ -59,6 +59,8 @@ def parse_args():
                     "RS_STRATEGY_ALLGATHER (PAPER.md S3.1) against the broadcast executor")
     ap.add_argument("--overlap", action="store_true", help="resharding beside compute (PAPER.md S4, on chip): reshard_execute "
                     "on a high-priority stream limited to max_ctas CTAs while torch.matmul (cuBLAS) runs on another stream")
+    ap.add_argument("--group", action="store_true", help="many tensors across one stage boundary (PAPER.md:100): n copies of "
+                    "--workload resharded by n launches against ONE launch of a reshard_plan_group")
     ap.add_argument("--sweep-md", default=None, help="also write the sweep as a markdown table to this file")
     return ap.parse_args()
 
@@ -557,8 +559,75 @@ def run_overlap(args):
     return 0
 
 
+def run_group(args):
+    """n tensors of the same layout pair: n x reshard_execute back to back against one grouped launch (CUDA events,
+    L2 flushed before every timed region, median of --steps)."""
+    import torch
+    from paper_2211_05322_b200 import harness, inputs
+    from paper_2211_05322_b200 import reshard as rs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream()
+    sh = stream.cuda_stream
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    K = max(5, min(args.steps, 40))
+    rows = []
+    for name in args.workload.split(","):
+        w = inputs.get_workload(name)
+        for n in (1, 2, 4, 8):
+            plans = [harness.make_plan(w) for _ in range(n)]
+            info = plans[0].info
+            if n * max(info.n_src, info.n_dst) > rs.RS_MAX_DEVICES:
+                break
+            src = [[torch.empty(info.src_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_src)] for _ in range(n)]
+            dst = [[torch.empty(info.dst_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_dst)] for _ in range(n)]
+            g = rs.Plan.group(plans)
+            sp, dp = [harness.ptrs(x) for x in src], [harness.ptrs(x) for x in dst]
+            gsp, gdp = [a for x in sp for a in x], [a for x in dp for a in x]
+
+            def separate():
+                for i in range(n):
+                    plans[i].execute(sp[i], dp[i], sh)
+
+            def grouped():
+                g.execute(gsp, gdp, sh)
+
+            res = {}
+            for label, fn in (("separate", separate), ("grouped", grouped)):
+                for _ in range(3):
+                    fn()
+                ts = []
+                for _ in range(K):
+                    flush.fill_(1)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream); fn(); e1.record(stream)
+                    e1.synchronize()
+                    ts.append(e0.elapsed_time(e1))
+                res[label] = statistics.median(ts)
+            nbytes = n * (info.unique_read_bytes + info.write_bytes)
+            row = {"workload": name, "tensors": n, "bytes": nbytes, "separate_us": res["separate"] * 1e3, "grouped_us": res["grouped"] * 1e3,
+                   "separate_GBs": nbytes / res["separate"] / 1e6, "grouped_GBs": nbytes / res["grouped"] / 1e6,
+                   "speedup": res["separate"] / res["grouped"]}
+            rows.append(row)
+            print(json.dumps(row), flush=True)
+            g.close()
+            for p in plans:
+                p.close()
+    if args.sweep_md:
+        with open(args.sweep_md, "w") as f:
+            f.write("| workload | tensors | bytes moved | n launches: us (GB/s) | one grouped launch: us (GB/s) | speedup |\n|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %s | %d | %.1f MiB | %.1f (%.0f) | %.1f (%.0f) | %.2f |\n" % (r["workload"], r["tensors"], r["bytes"] / 2**20,
+                        r["separate_us"], r["separate_GBs"], r["grouped_us"], r["grouped_GBs"], r["speedup"]))
+    return 0
+
+
 def main():
     args = parse_args()
+    if args.group:
+        return run_group(args)
     if args.overlap:
         return run_overlap(args)
     if args.sweep:

@@ -209,6 +209,15 @@ RS_API rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int3
 RS_API rs_status reshard_plan_schedule(const rs_plan *plan, rs_schedule_info *info, int32_t *sender_host,
                                 int64_t *start, int32_t *order);
 
+/* reshard_plan_group: ONE plan that runs the reshard_execute of several plans in a single launch -- every tensor
+ * that crosses a stage boundary at once; for small tensors the launch, not HBM, is the cost.
+ * The group's src_shards array is the concatenation of the members' source arrays in the order given, its
+ * dst_shards array likewise (at most RS_MAX_DEVICES pointers on each side in total, else RS_EUNSUPPORTED).
+ * The members may be destroyed afterwards.  A group supports reshard_execute, reshard_plan_info (counts and
+ * byte totals), reshard_op_info / reshard_op_tables of RS_OP_EXECUTE, and reshard_plan_destroy; everything
+ * else returns RS_EINVAL.  flags: RS_PATH_*, RS_HOST_ONLY.  plans [HOST array of n_plans plans, none a group]. */
+RS_API rs_status reshard_plan_group(const rs_plan *const *plans, int32_t n_plans, uint32_t flags, rs_plan **out_plan);
+
 RS_API void reshard_plan_destroy(rs_plan *plan);      /* NULL is allowed */
 
 /* ---- queries (all host-side, no CUDA) ------------------------------------------------------ */

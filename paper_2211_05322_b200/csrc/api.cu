@@ -35,6 +35,7 @@ rs_status upload(rs::Plan *P) {
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
     if (sms != P->sm_count) {                                 // grids are sized in multiples of the SM count
+        if (P->group_src) { rs::set_error("groups are built for a 148-SM part"); return RS_EUNSUPPORTED; }
         P->sm_count = sms;
         rs_status st = rs::build_tables(P);
         if (st != RS_OK) return st;
@@ -146,6 +147,32 @@ rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int32_t ele
     return RS_OK;
 }
 
+rs_status reshard_plan_group(const rs_plan *const *plans, int32_t n_plans, uint32_t flags, rs_plan **out_plan) {
+    rs::set_error("");
+    if (!plans || !out_plan || n_plans < 1) { rs::set_error("null argument or empty group"); return RS_EINVAL; }
+    std::vector<const rs::Plan *> members;
+    for (int32_t i = 0; i < n_plans; i++) {
+        if (!plans[i] || plans[i]->p.group_src) { rs::set_error("a member is null or is itself a group"); return RS_EINVAL; }
+        members.push_back(&plans[i]->p);
+    }
+    rs_plan *h = new (std::nothrow) rs_plan();
+    if (!h) return RS_ENOMEM;
+    rs::Plan *G = &h->p;
+    G->flags = flags;
+    G->elem_bytes = members[0]->elem_bytes;
+    G->A.ndim = G->B.ndim = 0;
+    rs_status st;
+    try {
+        st = rs::build_group(G, members);
+        if (st == RS_OK && !(flags & RS_HOST_ONLY)) st = upload(G);
+    } catch (const std::bad_alloc &) {
+        st = RS_ENOMEM;
+    }
+    if (st != RS_OK) { reshard_plan_destroy(h); return st; }
+    *out_plan = h;
+    return RS_OK;
+}
+
 void reshard_plan_destroy(rs_plan *plan) {
     if (!plan) return;
     for (void *ev : plan->p.events) cudaEventDestroy(static_cast<cudaEvent_t>(ev));
@@ -164,6 +191,15 @@ rs_status reshard_plan_info(const rs_plan *plan, rs_plan_info *out) {
     out->n_dst = P.B.n_dev;
     out->n_slices = (int32_t)P.slices.size();
     out->n_messages = (int32_t)P.messages.size();
+    if (P.group_src) {                                        // a group: counts and byte totals only
+        out->ndim = 0;
+        out->n_slices = P.op[RS_OP_EXECUTE].info.n_tasks;
+        out->n_messages = 0;
+        out->tensor_bytes = out->unique_read_bytes = P.op[RS_OP_EXECUTE].info.read_bytes;
+        out->write_bytes = P.op[RS_OP_EXECUTE].info.write_bytes;
+        out->device = P.device;
+        return RS_OK;
+    }
     int64_t tb = P.elem_bytes;
     for (int d = 0; d < P.A.ndim; d++) tb *= P.A.shape[d];
     out->tensor_bytes = tb;
@@ -194,6 +230,7 @@ rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *
 }
 
 rs_status reshard_plan_local_shape(const rs_plan *plan, int32_t side, int64_t *out) {
+    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
     if (!plan || !out || (side != RS_SRC && side != RS_DST)) return RS_EINVAL;
     const rs::Layout &L = side == RS_SRC ? plan->p.A : plan->p.B;
     for (int d = 0; d < L.ndim; d++) out[d] = L.local[d];
@@ -201,6 +238,7 @@ rs_status reshard_plan_local_shape(const rs_plan *plan, int32_t side, int64_t *o
 }
 
 rs_status reshard_plan_device_box(const rs_plan *plan, int32_t side, int32_t dev, int64_t *lo, int64_t *hi) {
+    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
     if (!plan || !lo || !hi || (side != RS_SRC && side != RS_DST)) return RS_EINVAL;
     const rs::Layout &L = side == RS_SRC ? plan->p.A : plan->p.B;
     if (dev < 0 || dev >= L.n_dev) return RS_EINVAL;
@@ -246,6 +284,7 @@ rs_status reshard_plan_schedule(const rs_plan *plan, rs_schedule_info *info, int
 }
 
 rs_status reshard_plan_sender_bytes(const rs_plan *plan, int64_t *out) {
+    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
     if (!plan || !out) return RS_EINVAL;
     std::copy(plan->p.sender_bytes.begin(), plan->p.sender_bytes.end(), out);
     return RS_OK;
@@ -356,18 +395,21 @@ rs_status reshard_execute_strategy(const rs_plan *plan, int32_t strategy, const 
 }
 
 rs_status reshard_pack(const rs_plan *plan, const void *const *src_shards, void *msg_arena, void *cuda_stream) {
+    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
     if (!plan) return RS_EINVAL;
     void *dst[1] = {msg_arena};
     return run_op(plan, RS_OP_PACK, src_shards, plan->p.A.n_dev, dst, 1, plan->p.used_src.data(), cuda_stream);
 }
 
 rs_status reshard_unpack(const rs_plan *plan, const void *msg_arena, void *const *dst_shards, void *cuda_stream) {
+    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
     if (!plan) return RS_EINVAL;
     const void *src[1] = {msg_arena};
     return run_op(plan, RS_OP_UNPACK, src, 1, dst_shards, plan->p.B.n_dev, nullptr, cuda_stream);
 }
 
 int64_t reshard_host_workspace_bytes(const rs_plan *plan) {
+    if (plan && plan->p.group_src) return -1;
     if (!plan) return -1;
     const rs::Plan &P = plan->p;
     int64_t n_used = 0;
@@ -378,6 +420,7 @@ int64_t reshard_host_workspace_bytes(const rs_plan *plan) {
 
 rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shards_host, void *const *dst_shards_host,
                                void *workspace, void *cuda_stream, int64_t *h2d_bytes, int64_t *d2h_bytes) {
+    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
     rs::set_error("");
     if (!plan || !src_shards_host || !dst_shards_host || !workspace) { rs::set_error("null argument"); return RS_EINVAL; }
     const rs::Plan &P = plan->p;

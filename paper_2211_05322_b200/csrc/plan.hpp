@@ -99,6 +99,7 @@ struct Plan {
     std::vector<char> used_src;          // [n_src] 1 if some task reads that shard
     int device = -1;
     int sm_count = 148;
+    int group_src = 0, group_dst = 0;    // > 0: this plan is a GROUP (reshard_plan_group): only its execute table exists
     int max_ctas = 0;                    // rs_plan_opts.max_ctas: cap on CTAs per launch (0: none)
     void *dev_blob = nullptr;            // the ONE device allocation
 };
@@ -114,6 +115,7 @@ void choose_senders(Plan *P);                          // a4
 rs_status schedule_plan(Plan *P);                      // S3.2: senders + order at host level, schedule.cpp
 rs_status build_messages(Plan *P);                     // message layout
 rs_status build_tables(Plan *P);                       // a5 (host side), tables.cpp
+rs_status build_group(Plan *G, const std::vector<const Plan *> &members);   // merged execute table, tables.cpp
 rs_status pipeline_simulate(const rs_pipeline_opts &o, rs_pipeline_result *res, int32_t *op_kind, int32_t *op_micro,
                             int64_t *op_start, int64_t *op_end);                    // S4, pipeline.cpp
 int pipeline_least_delay(int schedule, int S, int stage, int M, int64_t f, int64_t b, int64_t b_act, int64_t c_bwd);

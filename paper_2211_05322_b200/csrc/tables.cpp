@@ -391,6 +391,31 @@ rs_status build_slabs(Plan *P, const int64_t *sA, const int64_t *sB, int64_t ten
 
 }  // namespace
 
+// A GROUP: the execute tables of several plans merged into one, so that all the cross-mesh resharding
+// tasks of a stage boundary ("many cross-mesh resharding tasks for each tensor exchanged at the
+// boundary of two pipeline stages") run in ONE launch.  Buffer ids are shifted so that the group's pointer
+// arrays are the concatenation of the members' arrays.
+rs_status build_group(Plan *G, const std::vector<const Plan *> &members) {
+    OpTables &X = G->op[RS_OP_EXECUTE];
+    for (OpTables &o : G->op) { o.tasks.clear(); o.dsts.clear(); o.tiles.clear(); o.info = rs_op_info{}; }
+    int n_src = 0, n_dst = 0;
+    int64_t rd = 0, wr = 0;
+    G->used_src.clear();
+    for (const Plan *M : members) {
+        const OpTables &mx = M->op[RS_OP_EXECUTE];
+        if (n_src + M->A.n_dev > RS_MAX_DEVICES || n_dst + M->B.n_dev > RS_MAX_DEVICES) { set_error("a group holds at most RS_MAX_DEVICES source and RS_MAX_DEVICES destination shards"); return RS_EUNSUPPORTED; }
+        const int32_t d0 = (int32_t)X.dsts.size();
+        for (RsTask T : mx.tasks) { T.src_buf += n_src; T.dst_first += d0; X.tasks.push_back(T); }
+        for (RsDst D : mx.dsts) { D.buf += n_dst; X.dsts.push_back(D); }
+        G->used_src.insert(G->used_src.end(), M->used_src.begin(), M->used_src.end());
+        n_src += M->A.n_dev; n_dst += M->B.n_dev;
+        rd += mx.info.read_bytes; wr += mx.info.write_bytes;
+    }
+    G->A.n_dev = n_src; G->B.n_dev = n_dst;
+    G->group_src = n_src; G->group_dst = n_dst;
+    return finish_op(G, &X, rd, wr, nullptr, true);
+}
+
 rs_status build_tables(Plan *P) {
     const Layout &A = P->A, &B = P->B;
     const int N = A.ndim;

@@ -29,7 +29,7 @@ RS_MAX_NDIM, RS_MAX_MESH_NDIM, RS_MAX_DEVICES = 8, 4, 128
 
 # every symbol include/reshard.h declares (tests check the library exports exactly these)
 SYMBOLS = [
-    "reshard_plan", "reshard_plan_ex", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
+    "reshard_plan", "reshard_plan_ex", "reshard_plan_group", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
     "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
     "reshard_plan_message", "reshard_execute", "reshard_execute_strategy", "reshard_pack", "reshard_unpack", "reshard_execute_host",
     "reshard_host_workspace_bytes", "reshard_pipeline_simulate", "reshard_pipeline_least_delay", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
@@ -162,6 +162,19 @@ class Plan:
         self.info = PlanInfo()
         _chk(_lib().reshard_plan_info(self._h, C.byref(self.info)))
         self.ndim = self.info.ndim
+
+    @classmethod
+    def group(cls, plans, flags=0):
+        """reshard_plan_group: one plan whose execute() runs all of `plans` in a single launch; its pointer lists
+        are the concatenations of the members' lists"""
+        self = cls.__new__(cls)
+        self._h = C.c_void_p()
+        arr = (C.c_void_p * len(plans))(*[p._h for p in plans])
+        _chk(_lib().reshard_plan_group(arr, len(plans), C.c_uint32(flags), C.byref(self._h)))
+        self.info = PlanInfo()
+        _chk(_lib().reshard_plan_info(self._h, C.byref(self.info)))
+        self.ndim = 0
+        return self
 
     def close(self):
         if getattr(self, "_h", None):

@@ -542,3 +542,27 @@ def test_random_layouts_alignments_and_paths(seed):
 def test_fig5_single_sender_full_size(nodes, gpus):
     """one sender, a replicated receiver mesh, 1 GiB: every receiver ends with the whole tensor"""
     _check_full_size(inputs.fig5_workload(nodes, gpus), n_samples=256)
+
+
+@pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU, rs.RS_PATH_BULK_SHIFT])
+def test_plan_group_runs_every_member_in_one_launch(path):
+    """reshard_plan_group (many resharding tasks per stage boundary): one launch, every member bit-exact"""
+    members = [SMALL[i] for i in (2, 4, 9, 10, 17, 21, 25)]
+    plans, src_d, want = [], [], []
+    rng = np.random.default_rng(3)
+    for shape, sm, ss, dm, ds in members:
+        D = rng.integers(-2 ** 15, 2 ** 15, size=shape).astype(np.int16)
+        src = do.shards_from_global(D, sm, ss)
+        want += do.reshard(shape, sm, ss, dm, ds, src, fill=0xA5)
+        src_d += [gu.to_dev(s) for s in src]
+        plans.append(rs.Plan(shape, 2, sm, ss, dm, ds, path))
+    g = rs.Plan.group(plans, path)
+    for p in plans:
+        p.close()                                                  # the group owns its own tables
+    dst_d = [torch.full((w.nbytes,), 0xA5, dtype=torch.uint8, device=gu.dev()) for w in want]
+    n0 = rs.launch_count()
+    g.execute(gu.ptrs(src_d), gu.ptrs(dst_d), gu.stream())
+    torch.cuda.synchronize()
+    assert rs.launch_count() == n0 + 1
+    for q, w in enumerate(want):
+        assert dst_d[q].cpu().numpy().tobytes() == w.tobytes(), "group buffer %d" % q

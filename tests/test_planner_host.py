@@ -480,3 +480,34 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("c2") == (rs.RS_PATH_BULK, 148, 64)                           # 256 MiB moved: below the CTA rules
     assert shape_of("c3")[0] == shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU  # small operations: register path
     assert shape_of("c4", max_ctas=48) == (rs.RS_PATH_BULK, 48, 128)              # capped: more warps per CTA
+
+
+def test_plan_group_merges_execute_tables():
+    """reshard_plan_group: the members' execute tables in one table, buffer ids shifted; replay equals every member's oracle result"""
+    members = [((4, 8, 16), np.int16, (2, 4), "S0,R,S1", (2, 4), "S0,S1,R"),
+               ((8, 8, 8), np.int16, (2, 4), "S0,R,R", (2, 4), "R,R,R"),
+               ((7, 9), np.int16, (2, 4), "S1,S0", (4, 2), "S0,S1"),
+               ((16, 7), np.int16, (4,), "S0,R", (2,), "R,R")]
+    plans, srcs, wants = [], [], []
+    for shape, dt, sm, ss, dm, ds in members:
+        plans.append(_plan(shape, 2, sm, ss, dm, ds))
+        D = (np.arange(int(np.prod(shape)), dtype=np.int64) * 2654435761 % 251 + len(plans)).astype(dt).reshape(shape)
+        src = do.shards_from_global(D, sm, ss)
+        srcs += [_bytes(x) for x in src]
+        wants += [_bytes(w) for w in do.reshard(shape, sm, ss, dm, ds, src)]
+    g = rs.Plan.group(plans, HOST)
+    assert g.info.n_src == len(srcs) == 28 and g.info.n_dst == len(wants) == 26
+    assert g.info.unique_read_bytes == sum(p.info.tensor_bytes for p in plans)
+    assert g.info.write_bytes == sum(p.info.write_bytes for p in plans)
+    assert g.op_info(rs.RS_OP_EXECUTE).n_tasks == sum(p.info.n_slices for p in plans)
+    dst = [np.zeros(w.size, np.uint8) for w in wants]
+    ti.replay(g, rs.RS_OP_EXECUTE, srcs, dst)
+    for q, w in enumerate(wants):
+        assert np.array_equal(dst[q], w), "group buffer %d" % q
+    for call in (lambda: g.pack([1] * 28, 1), lambda: g.local_shape(rs.RS_SRC), lambda: g.schedule(), lambda: rs.Plan.group([g], HOST)):
+        with pytest.raises(rs.ReshardError):
+            call()
+    big = [_plan((256, 2), 4, (1,), "R,R", (128,), "R,R")] * 2          # 256 destination shards: too many for one launch
+    with pytest.raises(rs.ReshardError) as ei:
+        rs.Plan.group(big, HOST)
+    assert ei.value.code == rs.RS_EUNSUPPORTED
