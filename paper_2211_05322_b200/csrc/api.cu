@@ -356,7 +356,12 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                                   op.shift_stage, st);
-    } else {                                                  // register paths (also: aligned plan, unaligned pointers)
+    } else if (op.info.path == RS_PATH_BULK && op.alt_stage) { // aligned plan, under-aligned pointers: same tiles, shifted stores
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(P.max_ctas > 0 ? std::min(P.sm_count, P.max_ctas) : P.sm_count,
+                                                                     (n_tiles + op.alt_warps - 1) / op.alt_warps));
+        e = rs::launch_bulk_shift(dev, pt, small, grid, op.alt_warps * 32, op.alt_smem, op.alt_stages, op.alt_stages - 1,
+                                  op.alt_stage, st);
+    } else {                                                  // register paths
         int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
         if (P.max_ctas > 0) cap = std::min<int64_t>(cap, P.max_ctas);
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));

@@ -51,6 +51,8 @@ struct OpTables {                        // one operation (execute / pack / unpa
     rs_op_info info{};
     int stages = 0, lookahead = 0;       // TMA path: ring slots per warp, loads in flight
     uint32_t shift_stage = 0;            // rs_copy_bulk_shift: bytes per ring slot (rows padded), 0 if the path is not used
+    uint32_t alt_stage = 0;              // TMA plans handed under-aligned pointers: shape of rs_copy_bulk_shift on the same tiles
+    int alt_warps = 0, alt_stages = 0, alt_smem = 0;
     RsOpDev dev{};                       // device copies (null for a host-only plan)
 };
 

@@ -282,6 +282,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     for (const RsTile &t : op->tiles) mr = std::min<int64_t>(mr, t.col_bytes);
     I.min_run_bytes = op->tiles.empty() ? 0 : mr;
     op->shift_stage = 0;
+    op->alt_stage = 0;
     bool lsu = !bulk_family;
     if (bulk_family) {
         const bool shift = path == RS_PATH_BULK_SHIFT;
@@ -299,6 +300,20 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
         I.smem_bytes = (int32_t)(warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024);
         if (shift) op->shift_stage = (uint32_t)stage;
+        if (!shift) {
+            // An aligned plan may be handed under-aligned pointers at execute time: keep a launch shape of the
+            // shifted TMA kernel for the SAME tile table (rows padded in the ring, so fewer warps or slots fit).
+            int64_t pad = 0;
+            for (const RsTile &t : op->tiles) pad = std::max<int64_t>(pad, (int64_t)t.n_rows * (((int64_t)t.col_bytes + 77) & ~15ll));
+            const bool long_rows = min_run >= 1024;
+            int aw = long_rows ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS, as = long_rows ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES;
+            while (as > 2 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) as--;
+            while (aw > 1 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) aw--;
+            if ((int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 <= RS_SMEM_MAX && !op->tiles.empty()) {
+                op->alt_stage = (uint32_t)pad; op->alt_warps = aw; op->alt_stages = as;
+                op->alt_smem = (int)(aw * (as * pad + RS_BULK_DESC_BYTES) + 1024);
+            }
+        }
         if (shift && I.smem_bytes > RS_SMEM_MAX) {             // rows too sparse for the ring: the register kernels take it
             I.path = RS_PATH_LSU;
             I.block = RS_LSU_THREADS;
