@@ -177,8 +177,8 @@ class Plan:
         return self
 
     def close(self):
-        if getattr(self, "_h", None):
-            _lib().reshard_plan_destroy(self._h)
+        if getattr(self, "_h", None) and _LIB is not None:     # _LIB is None again while the interpreter shuts down
+            _LIB.reshard_plan_destroy(self._h)
             self._h = None
 
     __del__ = close
