@@ -77,8 +77,9 @@ enum {
                                to the lightest candidate; groups of <= 16 tasks are finished by an
                                exact branch-and-bound (R9).  Default.                  */
     RS_LB_NAIVE    = 0x1,   /* always the lowest-indexed candidate                  */
-    RS_PATH_AUTO   = 0x00,  /* executor chosen per operation from alignment and run length        */
-    RS_PATH_LSU    = 0x10,  /* force the register path: 128-bit ld.global -> st.global x k        */
+    RS_PATH_AUTO   = 0x00,  /* executor chosen per operation from alignment, run length and size  */
+    RS_PATH_LSU    = 0x10,  /* force the register paths: 128-bit ld.global -> st.global x k (AUTO:
+                               runs < 512 B and operations moving <= 64 MiB)                     */
     RS_PATH_BULK   = 0x20,  /* force the TMA path: cp.async.bulk global->smem ring->global x k    */
     RS_PATH_BULK_SHIFT = 0x30, /* force TMA loads + byte-shifted 128-bit register stores (any alignment;
                                what AUTO picks for runs >= 512 B that are not 16-byte aligned)     */
