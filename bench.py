@@ -575,14 +575,14 @@ def run_group(args):
     K = max(5, min(args.steps, 40))
     rows = []
     for name in args.workload.split(","):
-        w = inputs.get_workload(name)
-        for n in (1, 2, 4, 8):
-            plans = [harness.make_plan(w) for _ in range(n)]
-            info = plans[0].info
-            if n * max(info.n_src, info.n_dst) > rs.RS_MAX_DEVICES:
+        mixed = "+" in name                                  # a+b+c: ONE group of different workloads
+        for n in ((len(name.split("+")),) if mixed else (1, 2, 4, 8)):
+            ws = [inputs.get_workload(x) for x in name.split("+")] if mixed else [inputs.get_workload(name)] * n
+            plans = [harness.make_plan(w) for w in ws]
+            if sum(p.info.n_src for p in plans) > rs.RS_MAX_DEVICES or sum(p.info.n_dst for p in plans) > rs.RS_MAX_DEVICES:
                 break
-            src = [[torch.empty(info.src_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_src)] for _ in range(n)]
-            dst = [[torch.empty(info.dst_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_dst)] for _ in range(n)]
+            src = [[torch.empty(p.info.src_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(p.info.n_src)] for p in plans]
+            dst = [[torch.empty(p.info.dst_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(p.info.n_dst)] for p in plans]
             g = rs.Plan.group(plans)
             sp, dp = [harness.ptrs(x) for x in src], [harness.ptrs(x) for x in dst]
             gsp, gdp = [a for x in sp for a in x], [a for x in dp for a in x]
@@ -606,7 +606,7 @@ def run_group(args):
                     e1.synchronize()
                     ts.append(e0.elapsed_time(e1))
                 res[label] = statistics.median(ts)
-            nbytes = n * (info.unique_read_bytes + info.write_bytes)
+            nbytes = sum(p.info.unique_read_bytes + p.info.write_bytes for p in plans)
             row = {"workload": name, "tensors": n, "bytes": nbytes, "separate_us": res["separate"] * 1e3, "grouped_us": res["grouped"] * 1e3,
                    "separate_GBs": nbytes / res["separate"] / 1e6, "grouped_GBs": nbytes / res["grouped"] / 1e6,
                    "speedup": res["separate"] / res["grouped"]}

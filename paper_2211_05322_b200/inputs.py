@@ -185,8 +185,21 @@ def fig5_workload(nodes, gpus_per_node, shape=(1024, 1024, 512)):
 FIG5 = [(1, 1), (1, 2), (1, 3), (1, 4), (2, 2), (3, 2), (4, 2)]     # group 1: one node, 1-4 GPUs; group 2: 2 GPUs per node, 1-4 nodes
 
 
+# The skip connections of a U-shaped network put several feature maps of different resolution on one stage
+# boundary.  The paper gives no shapes; these four follow config 3's [8, 320, 64, 64] down a
+# 2x-per-level U (channels x2, resolution /2), same layout pair as c3ii.  Synthetic stand-ins.
+UNET_LEVELS = [(320, 64), (640, 32), (1280, 16), (1280, 8)]
+
+
+def unet_workload(level):
+    c, hw = UNET_LEVELS[level]
+    return _w("unet_l%d" % level, (8, c, hw, hw), "fp16", (1, 4), "S1,R,R,R", (2, 2), "R,S0,R,R", "bits", 60 + level)
+
+
 def get_workload(name):
     """'c1'..'c4', 'c1i', 'c3i', 'c3ii', 'u4', 't2_<case>', 'sweep_<pair>_<m8|m4>_<MiB>', 'fig5_<nodes>x<gpus>'."""
+    if name.startswith("unet_l"):
+        return unet_workload(int(name[6:]))
     if name.startswith("fig5_"):
         a, b = name[5:].split("x")
         return fig5_workload(int(a), int(b))

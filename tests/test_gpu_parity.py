@@ -566,3 +566,23 @@ def test_plan_group_runs_every_member_in_one_launch(path):
     assert rs.launch_count() == n0 + 1
     for q, w in enumerate(want):
         assert dst_d[q].cpu().numpy().tobytes() == w.tobytes(), "group buffer %d" % q
+
+
+def test_unet_boundary_group_full_size():
+    """four feature maps of a U-shaped network on one stage boundary, one launch"""
+    ws = [inputs.unet_workload(l) for l in range(4)]
+    plans, src, dst, expect = [], [], [], []
+    for w in ws:
+        D, s = gu.workload_on_device(w)
+        p = rs.Plan(w.shape, 2, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+        plans.append(p)
+        src += s
+        dst += [torch.zeros(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+        expect += [D[idx] for idx in gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)]
+    g = rs.Plan.group(plans)
+    n0 = rs.launch_count()
+    g.execute(gu.ptrs(src), gu.ptrs(dst), gu.stream())
+    torch.cuda.synchronize()
+    assert rs.launch_count() == n0 + 1
+    for got, want in zip(dst, expect):
+        assert torch.equal(got, want)
