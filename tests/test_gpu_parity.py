@@ -510,9 +510,11 @@ def test_random_layouts_alignments_and_paths(seed):
     shard pointers at random byte offsets, every executor, with and without a schedule -- bit-exact, guard bands intact"""
     rng = np.random.default_rng(2211_05322 + seed)
     dtypes = [np.uint8, np.int16, np.float32, np.int64, np.dtype("V16")]
+    members = []                                                   # the same layouts once more, as ONE group launch
     for _ in range(12):
         shape, sm, ss, dm, ds = _random_layout(rng)
         dtype = dtypes[int(rng.integers(len(dtypes)))]
+        members.append((shape, dtype, sm, ss, dm, ds))
         path = PATHS[int(rng.integers(len(PATHS)))]
         so, dofs = (int(rng.integers(0, 16)), int(rng.integers(0, 16))) if rng.integers(2) else (0, 0)
         opts = dict(schedule=int(rng.integers(1, 6)), src_devices_per_host=int(rng.integers(1, 3)), node_budget=2000) if rng.integers(3) == 0 else None
@@ -536,6 +538,22 @@ def test_random_layouts_alignments_and_paths(seed):
                 torch.cuda.synchronize()
                 for q, w in enumerate(want):
                     assert dst_d[q].cpu().numpy().tobytes() == w.tobytes(), (shape, sm, ss, dm, ds, dtype, path, route, strategy, q)
+    plans, src_d, wants = [], [], []
+    for shape, dtype, sm, ss, dm, ds in members:
+        e = np.dtype(dtype).itemsize
+        if len(src_d) + do.num_devices(sm) > 128 or len(wants) + do.num_devices(dm) > 128:
+            break
+        D = np.frombuffer(np.random.default_rng(seed + len(plans)).bytes(int(np.prod(shape)) * e), dtype=dtype).reshape(shape)
+        src = do.shards_from_global(D, sm, ss)
+        wants += do.reshard(shape, sm, ss, dm, ds, src, fill=0xA5)
+        src_d += [gu.to_dev(x) for x in src]
+        plans.append(rs.Plan(shape, e, sm, ss, dm, ds))
+    g = rs.Plan.group(plans, PATHS[seed % len(PATHS)])
+    dst_d = [torch.full((w.nbytes,), 0xA5, dtype=torch.uint8, device=gu.dev()) for w in wants]
+    g.execute(gu.ptrs(src_d), gu.ptrs(dst_d), gu.stream())
+    torch.cuda.synchronize()
+    for q, w in enumerate(wants):
+        assert dst_d[q].cpu().numpy().tobytes() == w.tobytes(), ("group", seed, q)
 
 
 @pytest.mark.parametrize("nodes,gpus", [(1, 3), (4, 2)])
