@@ -120,7 +120,9 @@ typedef struct rs_schedule_info {
     int32_t winner;                  /* ensemble: RS_SCHED_DFS or RS_SCHED_GREEDY; else = algorithm         */
     int32_t n_tasks, n_rounds;       /* unit tasks; rounds of the greedy search (0 if it did not run)       */
     int32_t n_src_hosts, n_dst_hosts;
-    int32_t dfs_finished, reserved;  /* 1 if the search ended before the node budget (its result is optimal)*/
+    int32_t dfs_finished, reserved;  /* 1 if the DFS ran and ended before the node budget (its result is optimal);
+                                        0 if it hit the budget, was skipped (more than 4096 unit tasks,
+                                        PAPER.md:179) or the algorithm runs no DFS                          */
     int64_t dfs_nodes;
     int64_t makespan;                /* Eq. 1 with T_i = slice bytes (R7)                         */
     int64_t busiest_host_bytes;      /* max over hosts of the bytes it sends or receives: no schedule of

@@ -170,17 +170,75 @@ def test_sweep_1gib_full_size(pair, meshes):
     _check_full_size(inputs.sweep_workload(pair, meshes, 1 << 30))
 
 
-@pytest.mark.parametrize("pair,meshes", [("P1", "m8"), ("P5", "m8"), ("P2", "m4"), ("P6", "m8")])
+@pytest.mark.parametrize("pair", sorted(inputs.SWEEP_PAIRS))
+@pytest.mark.parametrize("meshes", ["m8", "m4"])
 def test_sweep_4gib_maximum_size(pair, meshes):
-    """2^31 elements: byte offsets beyond 2^32"""
+    """2^31 elements: byte offsets beyond 2^32 (all 12 pair x mesh combinations of BASELINE config 5)"""
     _check_full_size(inputs.sweep_workload(pair, meshes, 4 << 30), n_samples=1024)
     torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("mib", [1, 4, 16, 64, 256])
-@pytest.mark.parametrize("pair", ["P1", "P2", "P5"])
-def test_sweep_small_sizes(pair, mib):
-    _check_full_size(inputs.sweep_workload(pair, "m8", mib << 20), n_samples=512)
+@pytest.mark.parametrize("meshes", ["m8", "m4"])
+@pytest.mark.parametrize("pair", sorted(inputs.SWEEP_PAIRS))
+def test_sweep_small_sizes(pair, meshes, mib):
+    """every point of BASELINE config 5 below 1 GiB: AUTO changes kernel and launch shape inside this range"""
+    _check_full_size(inputs.sweep_workload(pair, meshes, mib << 20), n_samples=512)
+
+
+@pytest.mark.parametrize("name", ["c4", "sweep_P5_m8_1024MiB"])
+def test_full_size_every_byte_against_the_oracles_own_output(name):
+    """the headline config (and one 1 GiB multicast point) against reshard_oracle ITSELF: the oracle computes
+    every destination shard from host source shards, the GPU shards are copied back and compared byte
+    for byte; execute and pack -> unpack"""
+    w = inputs.get_workload(name)
+    e = inputs.elem_bytes(w.dtype)
+    D = inputs.global_tensor(w)
+    src = do.shards_from_global(D, w.src_mesh, w.src_spec)
+    del D
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    src_d = [torch.from_numpy(s).to(gu.dev()) for s in src]
+    dst_d = [torch.full((p.info.dst_shard_bytes,), 0x5A, dtype=torch.uint8, device=gu.dev()) for _ in range(p.info.n_dst)]
+    dst2_d = [torch.full((p.info.dst_shard_bytes,), 0xA5, dtype=torch.uint8, device=gu.dev()) for _ in range(p.info.n_dst)]
+    arena = torch.empty(p.info.arena_bytes, dtype=torch.uint8, device=gu.dev())
+    p.execute(gu.ptrs(src_d), gu.ptrs(dst_d), gu.stream())
+    p.pack(gu.ptrs(src_d), arena.data_ptr(), gu.stream())
+    p.unpack(arena.data_ptr(), gu.ptrs(dst2_d), gu.stream())
+    torch.cuda.synchronize()
+    n_thr = do.max_threads()
+    want = np.empty(do.local_shape(w.shape, w.dst_mesh, w.dst_spec), dtype=src[0].dtype)
+    for q in range(p.info.n_dst):
+        do.reshard_device(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, src, q, src[0].dtype, n_threads=n_thr, out=want)
+        wb = want.view(np.uint8).reshape(-1)
+        assert np.array_equal(dst_d[q].cpu().numpy(), wb), "%s: execute, device %d differs from the oracle" % (name, q)
+        assert np.array_equal(dst2_d[q].cpu().numpy(), wb), "%s: pack -> unpack, device %d differs from the oracle" % (name, q)
+
+
+def test_pack_arena_contents_full_size_c4():
+    """config 4: every message of the arena equals the concatenation, in slice-id order, of the sender's boxes
+    (plan oracle's message table and tile boxes; the slicing itself is torch basic slicing on the device)"""
+    w = inputs.get_workload("c4")
+    e = inputs.elem_bytes(w.dtype)
+    _D, src = gu.workload_on_device(w)
+    del _D
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    arena = torch.full((p.info.arena_bytes,), 0x77, dtype=torch.uint8, device=gu.dev())
+    p.pack(gu.ptrs(src), arena.data_ptr(), gu.stream())
+    torch.cuda.synchronize()
+    tasks = po.unit_tasks(w.shape, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    senders = [s["sender"] for s in p.slices()]
+    table = po.message_table(tasks, senders)
+    msgs = p.messages()
+    assert len(msgs) == len(table)
+    used = torch.zeros(p.info.arena_bytes, dtype=torch.bool, device=gu.dev())
+    for m, (s, r, ids, n_elems) in zip(msgs, table):
+        assert (m["sender"], m["receiver"], m["slice_ids"], m["bytes"]) == (s, r, ids, n_elems * e)
+        lo, _hi = po.tile_box(w.shape, w.src_mesh, w.src_spec, s)
+        parts = [src[s][tuple(slice(a - l, b - l) for a, b, l in zip(tasks[i]["lo"], tasks[i]["hi"], lo))].reshape(-1) for i in ids]
+        payload = torch.cat(parts).view(torch.uint8)
+        assert torch.equal(arena[m["offset"]:m["offset"] + m["bytes"]], payload), "message (%d, %d)" % (s, r)
+        used[m["offset"]:m["offset"] + m["bytes"]] = True
+    assert bool((arena[~used] == 0x77).all())                           # padding between messages untouched
 
 
 @pytest.mark.parametrize("case", [1, 2, 3, 4, 5, 6, 7, 8, 9])
