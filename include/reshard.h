@@ -102,6 +102,22 @@ enum {
     RS_SCHED_ENSEMBLE = 5       /* DFS and greedy, the better one (ties: DFS)                 */
 };
 
+/* Launch-shape overrides for tests and tuning sweeps (rs_plan_opts.tuning).  Every field: 0 = the library's
+ * choice.  They change how an operation is tiled and launched, never its result.  The plan copies the struct. */
+typedef struct rs_tuning {
+    int32_t bulk_warps, bulk_stages, bulk_lookahead;   /* rs_copy_bulk: warps (pipelines) per CTA, ring slots per warp,
+                                                          loads in flight per warp                                   */
+    int32_t bulk_tile_bytes;                           /* bytes per ring slot = tile size (multiple of 128)          */
+    int32_t bulk_ctas, bulk_ctas_mcast;                /* CTAs for 1 : 1 / for write-heavy (multicast) operations    */
+    int32_t shift_warps, shift_stages, shift_lookahead, shift_tile_bytes;   /* the same for rs_copy_bulk_shift       */
+    int32_t lsu_tile_bytes, lsu_ctas_per_sm;           /* register kernels                                           */
+    int32_t task_order;                                /* 1: walk tiles task by task even where slices share
+                                                          destination rows (default: destination address order)     */
+    int32_t small_op_bytes_mib;                        /* AUTO takes the register path for aligned operations moving
+                                                          at most this many MiB (-1: never); 0 = library default     */
+    int32_t reserved[2];
+} rs_tuning;
+
 typedef struct rs_plan_opts {
     uint32_t flags;                  /* as reshard_plan; RS_LB_* is ignored when schedule != RS_SCHED_NONE  */
     int32_t schedule;                /* RS_SCHED_*                                                          */
@@ -113,6 +129,7 @@ typedef struct rs_plan_opts {
                                         streams -- overlapping a resharding with compute (PAPER.md S4) on chip  */
     int64_t node_budget;             /* DFS nodes before giving up with the best found; 0 = 200000          */
     uint64_t seed;                   /* of the counter-based generator the greedy search draws from         */
+    const rs_tuning *tuning;         /* [HOST] may be NULL: launch shapes chosen by the library             */
 } rs_plan_opts;
 
 typedef struct rs_schedule_info {
@@ -174,12 +191,16 @@ typedef struct rs_op_info {
     int32_t n_tasks;                 /* copy tasks (execute/pack: one per slice; unpack: per
                                         (slice, receiver))                                         */
     int32_t n_dsts;                  /* (task, destination) entries                                */
-    int32_t n_tiles;                 /* entries of the flat tile table                             */
+    int32_t n_tiles;                 /* tiles one launch walks (units of GPU work; decoded, never stored)  */
     int32_t tile_bytes;              /* target bytes read per tile                                 */
     int32_t grid, block;             /* launch configuration                                       */
     int32_t smem_bytes;              /* dynamic shared memory per CTA                              */
     int64_t read_bytes, write_bytes; /* algorithmic bytes of one launch                            */
     int64_t min_run_bytes;           /* shortest contiguous run any tile copies                    */
+    int32_t n_segs;                  /* segments: groups of tasks whose tiles are walked round-robin       */
+    int32_t table_bytes;             /* bytes of this operation's tables in device memory: O(unit tasks),
+                                        independent of the tensor size (the plan is the
+                                        slice list)                                                        */
 } rs_op_info;
 
 /*
@@ -244,9 +265,14 @@ RS_API rs_status reshard_plan_message(const rs_plan *plan, int32_t m, int32_t *s
                                int64_t *offset, int64_t *bytes, int32_t *n_slice_ids, int32_t *slice_ids);
 
 /* Raw copy of operation `op`'s flat tables (inspection and host-side tests; the layouts are the
- * structs RsTask / RsDst / RsTile of paper_2211_05322_b200/csrc/tables.h: 192, 16 and 32 bytes).
- * tasks [HOST, n_tasks*192], dsts [HOST, n_dsts*16], tiles [HOST, n_tiles*32]; each may be NULL. */
-RS_API rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *dsts, void *tiles);
+ * structs RsTask / RsDst / RsSeg of paper_2211_05322_b200/csrc/tables.h: 224, 16 and 16 bytes).
+ * tasks [HOST, n_tasks*224], dsts [HOST, n_dsts*16], segs [HOST, n_segs*16]; each may be NULL. */
+RS_API rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *dsts, void *segs);
+/* Tiles first_tile .. first_tile + n_tiles - 1 of operation `op`, decoded on the host by the same routine the
+ * kernels run on the device (tables.h rs_tile_locate / rs_tile_decode), as 32-byte RsTile records
+ * {u32 task, n_rows, col_bytes, flags; u64 a, b}.  tiles [HOST, n_tiles*32].  RS_EINVAL if the range leaves
+ * [0, rs_op_info.n_tiles). */
+RS_API rs_status reshard_op_tiles(const rs_plan *plan, int32_t op, int64_t first_tile, int64_t n_tiles, void *tiles);
 
 /* ---- the data path (steps a6..a8): asynchronous, allocate nothing, never synchronise -------- */
 /*
@@ -281,10 +307,11 @@ RS_API rs_status reshard_unpack(const rs_plan *plan, const void *msg_arena, void
  * plan-owned upload stream, resharded by one kernel launch on `cuda_stream`, and its destination
  * byte ranges are copied device->host on a plan-owned download stream while slab c+1 uploads.
  * All work is ordered after prior work on `cuda_stream`, and `cuda_stream` waits for the last
- * download; returns without synchronising.  Not reentrant per plan (the plan owns the side streams).
+ * download; returns without synchronising.  Calls on one plan from several host threads are serialised
+ * while they enqueue (the plan owns the side streams, created on first use).
  *   src_shards_host [HOST array of n_src HOST pointers]  (pinned memory makes the copies async)
  *   dst_shards_host [HOST array of n_dst HOST pointers]
- *   workspace [DEVICE]  at least reshard_host_workspace_bytes(plan) bytes, 256-byte aligned
+ *   workspace [DEVICE]  at least reshard_host_workspace_bytes(plan) bytes, 256-byte aligned (else RS_EINVAL)
  *   h2d_bytes, d2h_bytes [HOST, may be NULL]  receive the bytes copied in each direction
  */
 RS_API rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shards_host,

@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -12,7 +13,7 @@
 #include "kernels.h"
 #include "plan.hpp"
 
-static_assert(sizeof(RsTask) == 192 && sizeof(RsDst) == 16 && sizeof(RsTile) == 32, "table layouts are part of reshard_op_tables");
+static_assert(sizeof(RsTask) == 224 && sizeof(RsDst) == 16 && sizeof(RsSeg) == 16 && sizeof(RsTile) == 32, "table layouts are part of reshard_op_tables / reshard_op_tiles");
 
 struct rs_plan {
     rs::Plan p;
@@ -27,25 +28,26 @@ rs_status cuda_fail(cudaError_t e, const char *what) {
 
 size_t round256(size_t x) { return (x + 255) / 256 * 256; }
 
-// one device allocation holding the three operations' task / destination / tile tables
-rs_status upload(rs::Plan *P) {
+// SM count of the current device: grids are sized from it, so it is read BEFORE the tables are built
+rs_status query_device(rs::Plan *P) {
     cudaError_t e = cudaGetDevice(&P->device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
     int sms = 0;
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
-    if (sms != P->sm_count) {                                 // grids are sized in multiples of the SM count
-        if (P->group_src) { rs::set_error("groups are built for a 148-SM part"); return RS_EUNSUPPORTED; }
-        P->sm_count = sms;
-        rs_status st = rs::build_tables(P);
-        if (st != RS_OK) return st;
-    }
+    P->sm_count = sms;
+    return RS_OK;
+}
+
+// One device allocation holding every operation's task / destination / segment tables: O(unit tasks) bytes
+// (tiles are decoded by the kernels, tables.h), one cudaMalloc + one cudaMemcpy.
+rs_status upload(rs::Plan *P) {
     size_t total = 0;
     for (rs::OpTables &o : P->op)
         total += round256(o.tasks.size() * sizeof(RsTask)) + round256(o.dsts.size() * sizeof(RsDst)) +
-                 round256(o.tiles.size() * sizeof(RsTile));
+                 round256(o.segs.size() * sizeof(RsSeg));
     std::vector<char> host(total, 0);
-    e = cudaMalloc(&P->dev_blob, std::max<size_t>(total, 256));
+    cudaError_t e = cudaMalloc(&P->dev_blob, std::max<size_t>(total, 256));
     if (e != cudaSuccess) { P->dev_blob = nullptr; return e == cudaErrorMemoryAllocation ? RS_ENOMEM : cuda_fail(e, "cudaMalloc"); }
     size_t off = 0;
     char *base = static_cast<char *>(P->dev_blob);
@@ -56,30 +58,36 @@ rs_status upload(rs::Plan *P) {
         o.dev.dsts = reinterpret_cast<const RsDst *>(base + off);
         std::memcpy(host.data() + off, o.dsts.data(), o.dsts.size() * sizeof(RsDst));
         off += round256(o.dsts.size() * sizeof(RsDst));
-        o.dev.tiles = reinterpret_cast<const RsTile *>(base + off);
-        std::memcpy(host.data() + off, o.tiles.data(), o.tiles.size() * sizeof(RsTile));
-        off += round256(o.tiles.size() * sizeof(RsTile));
-        o.dev.n_tiles = (uint32_t)o.tiles.size();
+        o.dev.segs = reinterpret_cast<const RsSeg *>(base + off);
+        std::memcpy(host.data() + off, o.segs.data(), o.segs.size() * sizeof(RsSeg));
+        off += round256(o.segs.size() * sizeof(RsSeg));
+        o.dev.n_segs = (uint32_t)o.segs.size();
+        o.dev.tile_base = 0;
+        o.dev.n_tiles = (uint32_t)o.info.n_tiles;
     }
     e = cudaMemcpy(P->dev_blob, host.data(), total, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpy(tables)");
-    int smem = 0;
-    for (rs::OpTables &o : P->op) smem = std::max(smem, (int)RS_SMEM_MAX);
-    e = rs::prepare_bulk(smem);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(rs_copy_bulk)");
+    static std::once_flag smem_once;                           // once per process: the four TMA kernels may use all of shared memory
+    static cudaError_t smem_err = cudaSuccess;
+    std::call_once(smem_once, [] { smem_err = rs::prepare_bulk(RS_SMEM_MAX); });
+    if (smem_err != cudaSuccess) return cuda_fail(smem_err, "cudaFuncSetAttribute(rs_copy_bulk)");
+    return RS_OK;
+}
 
-    // reshard_execute_host pipeline: plan-owned upload / download streams and per-slab events
+// reshard_execute_host: plan-owned upload / download streams and per-slab events, created on first use
+rs_status host_streams(const rs::Plan &P) {
+    if (P.streams[0]) return RS_OK;
     for (int i = 0; i < 2; i++) {
         cudaStream_t st;
-        e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+        cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
         if (e != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
-        P->streams[i] = st;
+        P.streams[i] = st;
     }
-    for (size_t i = 0; i < 2 * P->slabs.size() + 2; i++) {
+    for (size_t i = 0; i < 2 * P.slabs.size() + 2; i++) {
         cudaEvent_t ev;
-        e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+        cudaError_t e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
         if (e != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
-        P->events.push_back(ev);
+        P.events.push_back(ev);
     }
     return RS_OK;
 }
@@ -125,9 +133,11 @@ rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int32_t ele
     P->sched.node_budget = opts->node_budget;
     P->sched.seed = opts->seed;
     P->max_ctas = std::max(0, opts->max_ctas);
+    if (opts->tuning) P->tune = *opts->tuning;
     rs_status st;
     try {
-        st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, (flags & RS_EVEN_ONLY) != 0, &P->A);
+        st = (flags & RS_HOST_ONLY) ? RS_OK : query_device(P);
+        if (st == RS_OK) st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, (flags & RS_EVEN_ONLY) != 0, &P->A);
         if (st == RS_OK) st = rs::make_layout(global_shape, ndim, dst_mesh_shape, dst_mesh_ndim, dst_spec, (flags & RS_EVEN_ONLY) != 0, &P->B);
         if (st == RS_OK) st = rs::build_slices(P);
         if (st == RS_OK) {
@@ -160,10 +170,12 @@ rs_status reshard_plan_group(const rs_plan *const *plans, int32_t n_plans, uint3
     rs::Plan *G = &h->p;
     G->flags = flags;
     G->elem_bytes = members[0]->elem_bytes;
+    G->tune = members[0]->tune;
     G->A.ndim = G->B.ndim = 0;
     rs_status st;
     try {
-        st = rs::build_group(G, members);
+        st = (flags & RS_HOST_ONLY) ? RS_OK : query_device(G);
+        if (st == RS_OK) st = rs::build_group(G, members);
         if (st == RS_OK && !(flags & RS_HOST_ONLY)) st = upload(G);
     } catch (const std::bad_alloc &) {
         st = RS_ENOMEM;
@@ -220,12 +232,25 @@ rs_status reshard_op_info(const rs_plan *plan, int32_t op, rs_op_info *out) {
     return RS_OK;
 }
 
-rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *dsts, void *tiles) {
+rs_status reshard_op_tables(const rs_plan *plan, int32_t op, void *tasks, void *dsts, void *segs) {
     if (!plan || op < 0 || op >= rs::RS_N_OPS) return RS_EINVAL;
     const rs::OpTables &o = plan->p.op[op];
     if (tasks) std::memcpy(tasks, o.tasks.data(), o.tasks.size() * sizeof(RsTask));
     if (dsts) std::memcpy(dsts, o.dsts.data(), o.dsts.size() * sizeof(RsDst));
-    if (tiles) std::memcpy(tiles, o.tiles.data(), o.tiles.size() * sizeof(RsTile));
+    if (segs) std::memcpy(segs, o.segs.data(), o.segs.size() * sizeof(RsSeg));
+    return RS_OK;
+}
+
+rs_status reshard_op_tiles(const rs_plan *plan, int32_t op, int64_t first_tile, int64_t n_tiles, void *tiles) {
+    if (!plan || !tiles || op < 0 || op >= rs::RS_N_OPS) return RS_EINVAL;
+    const rs::OpTables &o = plan->p.op[op];
+    if (first_tile < 0 || n_tiles < 0 || first_tile + n_tiles > o.info.n_tiles) { rs::set_error("tile range out of bounds"); return RS_EINVAL; }
+    RsTile *out = static_cast<RsTile *>(tiles);
+    for (int64_t i = 0; i < n_tiles; i++) {                   // the routine the kernels run (tables.h), on the host
+        uint32_t task, u;
+        rs_tile_locate(o.segs.data(), (uint32_t)o.segs.size(), (uint32_t)(first_tile + i), &task, &u);
+        out[i] = rs_tile_decode(o.tasks[task], task, u);
+    }
     return RS_OK;
 }
 
@@ -325,7 +350,7 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     const rs::Plan &P = plan->p;
     if (!P.dev_blob) { rs::set_error("plan was built with RS_HOST_ONLY"); return RS_EINVAL; }
     const rs::OpTables &op = P.op[opi];
-    if (op.tiles.empty()) return RS_OK;
+    if (op.info.n_tiles == 0) return RS_OK;
     RsPtrTable pt;
     const bool small = n_src <= RS_PTRS_SMALL && n_dst <= RS_PTRS_SMALL;   // then the kernels get the 256-byte table
     for (int i = 0; i < RS_PTRS_SMALL; i++) { pt.src[i] = nullptr; pt.dst[i] = nullptr; }
@@ -344,7 +369,7 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaError_t e;
     RsOpDev dev = op.dev;
-    if (tile_end > tile_begin) { dev.tiles += tile_begin; dev.n_tiles = tile_end - tile_begin; }   // one slab
+    if (tile_end > tile_begin) { dev.tile_base = tile_begin; dev.n_tiles = tile_end - tile_begin; }   // one slab
     const int64_t n_tiles = dev.n_tiles;
     const bool bulk_family = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_BULK_SHIFT;
     const int warps = op.info.block / 32;
@@ -430,7 +455,9 @@ rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shard
     if (!plan || !src_shards_host || !dst_shards_host || !workspace) { rs::set_error("null argument"); return RS_EINVAL; }
     const rs::Plan &P = plan->p;
     if (!P.dev_blob) { rs::set_error("plan was built with RS_HOST_ONLY"); return RS_EINVAL; }
-    if (ptr_align(workspace) < 16) { rs::set_error("workspace must be 256-byte aligned"); return RS_EINVAL; }
+    if (reinterpret_cast<uintptr_t>(workspace) % 256) { rs::set_error("workspace must be 256-byte aligned"); return RS_EINVAL; }
+    std::lock_guard<std::mutex> lock(P.host_mu);               // the side streams and events are the plan's
+    { rs_status hs = host_streams(P); if (hs != RS_OK) return hs; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     cudaStream_t up_st = static_cast<cudaStream_t>(P.streams[0]), down_st = static_cast<cudaStream_t>(P.streams[1]);
     const size_t sb = (size_t)(P.A.shard_elems() * P.elem_bytes), db = (size_t)(P.B.shard_elems() * P.elem_bytes);

@@ -27,19 +27,10 @@ namespace rs {
 // ------------------------------------------------------------------------------------------------
 // shared device helpers
 
-__device__ __forceinline__ RsTile load_tile(const RsTile *tiles, uint32_t t) {
-    const uint4 *p = reinterpret_cast<const uint4 *>(tiles + t);
-    uint4 x = __ldg(p), y = __ldg(p + 1);
-    RsTile r;
-    r.task = x.x; r.n_rows = x.y; r.col_bytes = x.z; r.flags = x.w;
-    r.a = (uint64_t)y.x | ((uint64_t)y.y << 32);
-    r.b = (uint64_t)y.z | ((uint64_t)y.w << 32);
-    return r;
-}
-
 // Per-warp descriptor ring: everything one tile needs, resolved 32 tiles at a time (lane i resolves
-// the warp's tile it+i: tile record -> task -> base pointers), so the per-tile critical path has
-// no dependent global load -- one shared-memory broadcast read instead.
+// the warp's tile it+i: segment search -> task -> procedural tile decode (tables.h) -> base pointers),
+// so the per-tile critical path has no dependent global load and no division -- one shared-memory
+// broadcast read instead.  The plan holds no per-tile record: its size is O(unit tasks).
 struct alignas(16) RsDesc {
     const char *src;                     // FAST: address of the tile's first source byte; GENERIC: box origin
     int64_t dst_rel;                     // FAST: tile.b; GENERIC: byte offset inside the run
@@ -54,8 +45,10 @@ static_assert(RS_DESC_RING * sizeof(RsDesc) == RS_BULK_DESC_BYTES, "config.h and
 template <int NP>
 __device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsPtrTableT<NP> &ptrs, uint32_t tile_index,
                                              RsDesc *out) {
-    const RsTile tile = load_tile(op.tiles, tile_index);
-    const RsTask *__restrict__ T = op.tasks + tile.task;
+    uint32_t task, u;
+    rs_tile_locate(op.segs, op.n_segs, op.tile_base + tile_index, &task, &u);
+    const RsTask *__restrict__ T = op.tasks + task;
+    const RsTile tile = rs_tile_decode(*T, task, u);
     RsDesc d;
     const char *base = ptrs.src[T->src_buf] + T->src_off;
     d.src = (tile.flags & RS_TILE_FAST) ? base + tile.a : base;
@@ -67,19 +60,9 @@ __device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsPtrTable
     *out = d;
 }
 
-// GENERIC tiles: byte offsets of linear row `lin` of a task's box, relative to the box origin on each side
+// GENERIC tiles: byte offsets of linear row `lin` (< 2^31) of a task's box, relative to the box origin on each side
 __device__ __forceinline__ void generic_row(const RsTask *__restrict__ T, uint64_t lin, int64_t *so, int64_t *doff) {
-    int64_t s = 0, d = 0;
-    const int nd = T->nd;
-    for (int i = 0; i < nd; i++) {
-        uint32_t e = T->ext[i];
-        uint64_t q = lin / e;
-        uint32_t c = (uint32_t)(lin - q * e);
-        lin = q;
-        s += (int64_t)c * T->sstride[i];
-        d += (int64_t)c * T->dstride[i];
-    }
-    *so = s; *doff = d;
+    rs_row_offsets(*T, 0, (uint32_t)lin, so, doff);
 }
 
 // ------------------------------------------------------------------------------------------------

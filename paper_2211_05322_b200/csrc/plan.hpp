@@ -7,6 +7,7 @@
 //   a5 flat task / tile tables, message layout north_star items (1), (3)
 #pragma once
 #include <stdint.h>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -47,7 +48,7 @@ struct Message {                         // wire model: everything sender s ship
 struct OpTables {                        // one operation (execute / pack / unpack)
     std::vector<RsTask> tasks;
     std::vector<RsDst> dsts;
-    std::vector<RsTile> tiles;
+    std::vector<RsSeg> segs;             // tiles are never stored: decoded from (segs, tasks), tables.h
     rs_op_info info{};
     int stages = 0, lookahead = 0;       // TMA path: ring slots per warp, loads in flight
     uint32_t shift_stage = 0;            // rs_copy_bulk_shift: bytes per ring slot (rows padded), 0 if the path is not used
@@ -62,7 +63,7 @@ struct HostCopy {                        // one contiguous host<->device copy of
 };
 
 struct HostSlab {                        // one stage of the reshard_execute_host pipeline: a slab of tensor dim 0
-    uint32_t tile_begin = 0, tile_end = 0;       // range in op[RS_OP_SLABS].tiles
+    uint32_t tile_begin = 0, tile_end = 0;       // tile range of op[RS_OP_SLABS] (its tasks are consecutive)
     std::vector<HostCopy> up, down;      // source ranges to upload before, destination ranges to download after
 };
 
@@ -96,13 +97,17 @@ struct Plan {
     int64_t r_B = 1;                     // destination replication factor
     OpTables op[RS_N_OPS];
     std::vector<HostSlab> slabs;         // reshard_execute_host pipeline (PAPER.md:137's chunked pipelining, over PCIe)
-    void *streams[2] = {nullptr, nullptr};   // plan-owned upload / download streams (cudaStream_t)
-    std::vector<void *> events;          // plan-owned cudaEvent_t: 2 per slab + 2
+    // reshard_execute_host: plan-owned upload / download streams (cudaStream_t) and cudaEvent_t (2 per slab + 2),
+    // created on first use; host_mu serialises the enqueue of concurrent calls
+    mutable std::mutex host_mu;
+    mutable void *streams[2] = {nullptr, nullptr};
+    mutable std::vector<void *> events;
     std::vector<char> used_src;          // [n_src] 1 if some task reads that shard
     int device = -1;
     int sm_count = 148;
     int group_src = 0, group_dst = 0;    // > 0: this plan is a GROUP (reshard_plan_group): only its execute table exists
     int max_ctas = 0;                    // rs_plan_opts.max_ctas: cap on CTAs per launch (0: none)
+    rs_tuning tune{};                    // rs_plan_opts.tuning (all zero: the library's launch shapes)
     void *dev_blob = nullptr;            // the ONE device allocation
 };
 

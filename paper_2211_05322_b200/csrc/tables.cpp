@@ -1,10 +1,13 @@
-// tables.cpp -- step a5: unit tasks -> collapsed copy tasks -> flat tile tables for the three
-// operations (execute / pack / unpack), plus the per-operation launch configuration.
+// tables.cpp -- step a5: unit tasks -> collapsed copy tasks -> flat task tables for the three
+// operations (execute / pack / unpack), the shape of every task's tile grid (tiles themselves are
+// never stored: tables.h), plus the per-operation launch configuration.  O(unit tasks) work and
+// memory, whatever the tensor size (the plan is the slice list).
 // Paper analogue: "choose the better result as the schedule to launch broadcasts";
-// north_star item (1): "emits a flat task table".  No CUDA here.
+// north_star item (1): "emits a flat task table".  No CUDA here, no environment variables: launch
+// shapes are overridden only through rs_plan_opts.tuning.
 #include <algorithm>
-#include <cstdlib>
 #include <cstring>
+#include <map>
 
 #include "config.h"
 #include "plan.hpp"
@@ -76,77 +79,70 @@ int64_t pow2_align(int64_t x) {                               // largest power o
     return a;
 }
 
-int env_int(const char *name, int dflt) {
-    const char *v = std::getenv(name);
-    if (!v || !*v) return dflt;
-    return std::atoi(v);
-}
+int pick(int override_value, int dflt) { return override_value > 0 ? override_value : dflt; }
 
-// Emit the tiles of one task.  tile_bytes is a multiple of 128.
-void emit_tiles(const RsTask &T, uint32_t task_id, int64_t tile_bytes, std::vector<RsTile> *out) {
-    const int64_t R = task_rows(T), B = T.run_bytes;
-    auto row_offsets = [&](int64_t row, int64_t *so, int64_t *doff) {
-        int64_t s = 0, d = 0;
-        for (int i = 0; i < T.nd; i++) {
-            int64_t c = row % T.ext[i];
-            row /= T.ext[i];
-            s += c * T.sstride[i];
-            d += c * T.dstride[i];
-        }
-        *so = s; *doff = d;
-    };
+// Shape of one task's tile grid (tables.h): nothing per tile is stored, the kernels decode tile u from
+// these few numbers.  tile_bytes is a multiple of 128.
+void set_tiling(RsTask *T, int64_t tile_bytes) {
+    const int64_t R = task_rows(*T), B = T->run_bytes;
+    T->n_rows = (uint32_t)R;
+    T->pad = 0;
+    T->chunk_bytes = (uint32_t)std::min<int64_t>(B, 0xFFFFFF80ll);
+    T->n_chunks = 1; T->rows_per_tile = 1; T->tiles_per_span = 1;
     if (B > tile_bytes) {                                     // long runs: split every row into column chunks
-        int64_t n = (B + tile_bytes - 1) / tile_bytes;
-        int64_t chunk = ((B + n - 1) / n + 127) / 128 * 128;
-        for (int64_t r = 0; r < R; r++) {
-            int64_t so, doff;
-            row_offsets(r, &so, &doff);
-            for (int64_t c = 0; c < B; c += chunk) {
-                RsTile t{};
-                t.task = task_id; t.n_rows = 1; t.col_bytes = (uint32_t)std::min(chunk, B - c);
-                t.flags = RS_TILE_FAST;
-                t.a = (uint64_t)(so + c); t.b = (uint64_t)(doff + c);
-                out->push_back(t);
-            }
-        }
+        const int64_t n = (B + tile_bytes - 1) / tile_bytes;
+        const int64_t chunk = ((B + n - 1) / n + 127) / 128 * 128;
+        T->kind = RS_TILING_SPLIT;
+        T->chunk_bytes = (uint32_t)chunk;
+        T->n_chunks = (uint32_t)((B + chunk - 1) / chunk);
+        T->n_tiles = (uint32_t)std::min<int64_t>(R * T->n_chunks, 0xFFFFFFFFll);
         return;
     }
     const int64_t rpt = std::max<int64_t>(1, tile_bytes / B);  // rows per tile
-    const int64_t ext0 = T.nd > 0 ? T.ext[0] : 1;
-    if (T.nd <= 1 || ext0 >= rpt) {                           // FAST tiles inside one span of row dim 0
-        int64_t n = (ext0 + rpt - 1) / rpt, sz = (ext0 + n - 1) / n;
-        for (int64_t span = 0; span < R / ext0; span++) {
-            int64_t so, doff;
-            row_offsets(span * ext0, &so, &doff);
-            for (int64_t r0 = 0; r0 < ext0; r0 += sz) {
-                RsTile t{};
-                t.task = task_id; t.n_rows = (uint32_t)std::min(sz, ext0 - r0); t.col_bytes = (uint32_t)B;
-                t.flags = RS_TILE_FAST;
-                t.a = (uint64_t)(so + r0 * T.sstride[0]); t.b = (uint64_t)(doff + r0 * T.dstride[0]);
-                out->push_back(t);
-            }
-        }
+    const int64_t ext0 = T->nd > 0 ? T->ext[0] : 1;
+    if (T->nd <= 1 || ext0 >= rpt) {                          // FAST tiles inside one span of row dim 0
+        const int64_t n = (ext0 + rpt - 1) / rpt, sz = (ext0 + n - 1) / n;
+        T->kind = RS_TILING_FAST;
+        T->rows_per_tile = (uint32_t)sz;
+        T->tiles_per_span = (uint32_t)((ext0 + sz - 1) / sz);
+        T->n_tiles = (uint32_t)std::min<int64_t>(R / ext0 * T->tiles_per_span, 0xFFFFFFFFll);
         return;
     }
-    int64_t n = (R + rpt - 1) / rpt, sz = (R + n - 1) / n;     // GENERIC tiles: any run of linear rows
-    for (int64_t r0 = 0; r0 < R; r0 += sz) {
-        RsTile t{};
-        t.task = task_id; t.n_rows = (uint32_t)std::min(sz, R - r0); t.col_bytes = (uint32_t)B;
-        t.flags = 0;
-        t.a = (uint64_t)r0; t.b = 0;
-        out->push_back(t);
-    }
+    const int64_t n = (R + rpt - 1) / rpt, sz = (R + n - 1) / n;   // GENERIC tiles: any run of linear rows
+    T->kind = RS_TILING_GENERIC;
+    T->rows_per_tile = (uint32_t)sz;
+    T->n_tiles = (uint32_t)((R + sz - 1) / sz);
+}
+
+int64_t task_tiles_exact(const RsTask &T) {                   // n_tiles before the 32-bit clamp
+    const int64_t R = task_rows(T);
+    if (T.kind == RS_TILING_SPLIT) return R * T.n_chunks;
+    if (T.kind == RS_TILING_FAST) return R / std::max<int64_t>(1, T.nd > 0 ? T.ext[0] : 1) * T.tiles_per_span;
+    return (R + T.rows_per_tile - 1) / T.rows_per_tile;
+}
+
+int64_t task_min_col(const RsTask &T) {                       // shortest contiguous run any of its tiles copies
+    if (T.kind != RS_TILING_SPLIT) return T.run_bytes;
+    return std::min<int64_t>(T.chunk_bytes, T.run_bytes - (int64_t)(T.n_chunks - 1) * T.chunk_bytes);
+}
+
+int64_t task_shift_stage(const RsTask &T) {                   // ring-slot bytes its largest tile needs in rs_copy_bulk_shift
+    const int64_t col = T.kind == RS_TILING_SPLIT ? T.chunk_bytes : T.run_bytes;
+    const int64_t rows = T.kind == RS_TILING_SPLIT ? 1 : std::min<int64_t>(T.rows_per_tile, T.n_rows);
+    return rows * ((col + 77) & ~15ll);                       // a row of n bytes occupies (n + 77) & ~15 bytes of a slot
 }
 
 // Which kernel an operation takes (rs_op_info.path).  AUTO: runs under 512 B and small aligned operations go to the
 // register kernels (they start faster; small operations are launch-bound), 16-byte aligned layouts to the TMA
 // kernel, everything else to TMA loads + shifted stores.
-int pick_path(uint32_t forced, int64_t align, int64_t min_run, int64_t moved_bytes) {
+int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t moved_bytes) {
+    const uint32_t forced = P.flags & RS_PATH_MASK;
+    const int64_t small_op = P.tune.small_op_bytes_mib < 0 ? -1 : P.tune.small_op_bytes_mib > 0 ? ((int64_t)P.tune.small_op_bytes_mib << 20) : RS_SMALL_OP_BYTES;
     const bool bulk_ok = align == 16 && min_run >= 16;
     int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
              : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
              : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU
-             : bulk_ok ? (moved_bytes <= RS_SMALL_OP_BYTES ? RS_PATH_LSU : RS_PATH_BULK)
+             : bulk_ok ? (moved_bytes <= small_op ? RS_PATH_LSU : RS_PATH_BULK)
              : RS_PATH_BULK_SHIFT;
     if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_BULK_SHIFT;   // cp.async.bulk stores need 16-byte everything
     return path;
@@ -156,6 +152,7 @@ int pick_path(uint32_t forced, int64_t align, int64_t min_run, int64_t moved_byt
 struct BulkShape { int warps, stages, grid; int64_t tile_bytes; };
 
 BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes) {
+    const rs_tuning &U = P.tune;
     // short runs = many bulk copies per tile: one warp issues them too slowly, so more, smaller pipelines
     // (Table 2 case 9, 512-byte runs: 3.6 TB/s with 2 warps, 5.7 with 4)
     const bool short_runs = min_run <= RS_BULK_SHORT_RUN;
@@ -165,12 +162,12 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     // shifted variant: rows of >= 1 KiB are stored row by row (cheap), shorter ones window by window (ALU-heavy)
     const bool shift_long = shift && min_run >= 1024;
     BulkShape sh;
-    sh.warps = std::max(1, std::min(8, shift ? env_int("RS_SHIFT_WARPS", shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
-                                             : env_int("RS_BULK_WARPS", short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
-    sh.stages = std::max(2, std::min(8, shift ? env_int("RS_SHIFT_STAGES", shift_long ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES)
-                                              : env_int("RS_BULK_STAGES", RS_BULK_STAGES)));
-    sh.tile_bytes = shift ? env_int("RS_SHIFT_TILE_BYTES", RS_SHIFT_TILE_BYTES)
-                          : env_int("RS_BULK_TILE_BYTES", short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
+    sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
+                                             : pick(U.bulk_warps, short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
+    sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES)
+                                              : pick(U.bulk_stages, RS_BULK_STAGES)));
+    sh.tile_bytes = shift ? pick(U.shift_tile_bytes, RS_SHIFT_TILE_BYTES)
+                          : pick(U.bulk_tile_bytes, short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
     sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
     while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
     // At most one CTA per SM -- and FEWER where the memory system prefers it (148 SMs):
@@ -188,15 +185,59 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
         if (write_heavy) ctas = P.sm_count * (short_runs ? RS_BULK_CTAS_MCAST_SHORT_NUM : RS_BULK_CTAS_MCAST_NUM) / RS_BULK_CTAS_DEN;
         else if (min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
     }
-    sh.grid = std::max(1, std::min(P.sm_count, env_int(write_heavy ? "RS_BULK_CTAS_MCAST" : "RS_BULK_CTAS", std::max(1, ctas))));
+    sh.grid = std::max(1, std::min(P.sm_count, pick(write_heavy ? U.bulk_ctas_mcast : U.bulk_ctas, std::max(1, ctas))));
     if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
     return sh;
 }
 
-// Alignment class, path, tile size, grid of one operation; then its tile table.
-rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes,
-                    std::vector<uint32_t> *task_tile_begin = nullptr, bool dst_order = false) {
-    int64_t align = 16, min_run = INT64_MAX, max_rows = 0;
+// Slices that share destination rows (one slice fills part of every destination row, another slice the rest:
+// config 2, sweep pairs P1 / P2 / P4) become ONE segment whose tiles are walked round-robin, i.e. in DESTINATION
+// address order, so that the pieces of one row are written close in time: +1-3 % on those layouts (P2 at 4 GiB
+// 6.00 -> 6.18 TB/s).  Members must have identical tile grids and destination buffers, and start in the same
+// destination row.  Reorders op->tasks so that the members of a segment are consecutive (ascending destination
+// offset); the order of the segments follows their first member.
+void group_interleaved(OpTables *op) {
+    const size_t n = op->tasks.size();
+    std::map<std::vector<int64_t>, std::vector<uint32_t>> buckets;
+    std::vector<std::vector<int64_t>> key_of(n);
+    for (size_t i = 0; i < n; i++) {
+        const RsTask &T = op->tasks[i];
+        std::vector<int64_t> key;
+        if (T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.dstride[0] > T.run_bytes && T.kind != RS_TILING_GENERIC) {
+            const RsDst &D0 = op->dsts[(size_t)T.dst_first];
+            key = {T.k, T.nd, T.run_bytes, (int64_t)T.kind, T.chunk_bytes, T.n_chunks, T.rows_per_tile, T.tiles_per_span, T.n_tiles,
+                   D0.off / T.dstride[0]};
+            for (int d = 0; d < T.nd; d++) { key.push_back(T.ext[d]); key.push_back(T.dstride[d]); }
+            for (int j = 0; j < T.k; j++) {                   // the same receivers, at the same distance from the first one
+                const RsDst &D = op->dsts[(size_t)T.dst_first + j];
+                key.push_back(D.buf); key.push_back(D.off - D0.off);
+            }
+        } else {
+            key = {-1, (int64_t)i};                           // not a candidate: alone
+        }
+        buckets[key].push_back((uint32_t)i);
+        key_of[i] = std::move(key);
+    }
+    std::vector<RsTask> ordered;
+    ordered.reserve(n);
+    std::vector<char> done(n, 0);
+    op->segs.clear();
+    for (size_t i = 0; i < n; i++) {
+        if (done[i]) continue;
+        std::vector<uint32_t> &members = buckets[key_of[i]];
+        std::stable_sort(members.begin(), members.end(), [&](uint32_t a, uint32_t b) {
+            return op->dsts[(size_t)op->tasks[a].dst_first].off < op->dsts[(size_t)op->tasks[b].dst_first].off;
+        });
+        op->segs.push_back(RsSeg{0, (uint32_t)ordered.size(), (uint32_t)members.size(), op->tasks[i].n_tiles});
+        for (uint32_t m : members) { ordered.push_back(op->tasks[m]); done[m] = 1; }
+    }
+    op->tasks.swap(ordered);
+}
+
+// Alignment class, path, tile size, grid of one operation; then the shape of every task's tile grid and the
+// segments.  per_task: one segment per task, in task order (the slab table: its tile ranges are per task).
+rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes, bool per_task = false, bool dst_order = false) {
+    int64_t align = 16, min_run = INT64_MAX;
     for (const RsTask &T : op->tasks) {
         align = std::min(align, pow2_align(T.run_bytes));
         align = std::min(align, pow2_align(T.src_off));
@@ -206,7 +247,6 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         }
         for (int j = 0; j < T.k; j++) align = std::min(align, pow2_align(op->dsts[(size_t)T.dst_first + j].off));
         min_run = std::min(min_run, T.run_bytes);
-        max_rows = std::max(max_rows, task_rows(T));
         if (task_rows(T) > 0x7FFFFFFFll) { set_error("more than 2^31-1 rows in one slice"); return RS_EUNSUPPORTED; }
     }
     rs_op_info &I = op->info;
@@ -216,7 +256,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     I.read_bytes = read_bytes;
     I.write_bytes = write_bytes;
 
-    const int path = pick_path(P->flags & RS_PATH_MASK, align, min_run, read_bytes + write_bytes);
+    const int path = pick_path(*P, align, min_run, read_bytes + write_bytes);
     I.path = path;
     const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT;
 
@@ -231,10 +271,10 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         I.grid = sh.grid;
         workers = sh.grid * sh.warps;
     } else {
-        tile_bytes = env_int("RS_LSU_TILE_BYTES", RS_LSU_TILE_BYTES);
+        tile_bytes = pick(P->tune.lsu_tile_bytes, RS_LSU_TILE_BYTES);
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
         I.block = RS_LSU_THREADS;
-        I.grid = P->sm_count * std::max(1, std::min(RS_LSU_CTAS_PER_SM, env_int("RS_LSU_CTAS_PER_SM", RS_LSU_CTAS_DEFAULT)));
+        I.grid = P->sm_count * std::max(1, std::min(RS_LSU_CTAS_PER_SM, pick(P->tune.lsu_ctas_per_sm, RS_LSU_CTAS_DEFAULT)));
         if (P->max_ctas > 0) I.grid = std::min(I.grid, P->max_ctas);
         workers = I.grid * (RS_LSU_THREADS / 32);
     }
@@ -243,44 +283,28 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     tile_bytes = std::max<int64_t>(tile_bytes, 128);
     I.tile_bytes = (int32_t)tile_bytes;
 
-    op->tiles.clear();
-    for (size_t t = 0; t < op->tasks.size(); t++) {
-        if (task_tile_begin) task_tile_begin->push_back((uint32_t)op->tiles.size());
-        emit_tiles(op->tasks[t], (uint32_t)t, tile_bytes, &op->tiles);
-    }
-    if (task_tile_begin) task_tile_begin->push_back((uint32_t)op->tiles.size());
-    // Tasks whose destination boxes interleave finely (a slice fills part of every destination row, another
-    // slice the rest: config 2, sweep pairs P1 / P2 / P4) are walked in DESTINATION address order, so that the
-    // pieces of one row are written close in time: +1-3 % on those layouts (P2 at 4 GiB 6.00 -> 6.18 TB/s).
-    // Only for execute and unpack (they write shards); not for the slab table (its tile ranges are per task) and not for coarse
-    // interleaves (config 4: 3 MiB runs).
+    int64_t total_tiles = 0;
+    for (RsTask &T : op->tasks) { set_tiling(&T, tile_bytes); total_tiles += task_tiles_exact(T); }
+    if (total_tiles > 0x7FFFFFFFll) { set_error("more than 2^31-1 tiles in one operation"); return RS_EUNSUPPORTED; }
+    // Destination-address order only for execute and unpack (they write shards), only where slices share
+    // destination rows at a fine grain (not config 4: 3 MiB runs), and not under a schedule: there the tables list
+    // the unit tasks in order of S_i and the tiles follow them.
     bool interleaved = false;
     for (const RsTask &T : op->tasks) interleaved = interleaved || (T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.dstride[0] > T.run_bytes);
-    if (dst_order && env_int("RS_TILE_ORDER", 1) && !task_tile_begin && interleaved && op->tasks.size() > 1) {
-        struct Key { int64_t buf, off; uint32_t idx; };
-        std::vector<Key> keys(op->tiles.size());
-        for (size_t i = 0; i < op->tiles.size(); i++) {
-            const RsTile &t = op->tiles[i];
-            const RsTask &T = op->tasks[t.task];
-            int64_t doff = 0;
-            if (t.flags & RS_TILE_FAST) doff = (int64_t)t.b;
-            else {
-                int64_t row = (int64_t)t.a;
-                for (int d = 0; d < T.nd; d++) { int64_t c = row % T.ext[d]; row /= T.ext[d]; doff += c * T.dstride[d]; }
-            }
-            const RsDst &D = op->dsts[(size_t)T.dst_first];
-            keys[i] = Key{D.buf, D.off + doff, (uint32_t)i};
-        }
-        std::stable_sort(keys.begin(), keys.end(), [](const Key &x, const Key &y) { return x.buf != y.buf ? x.buf < y.buf : x.off < y.off; });
-        std::vector<RsTile> sorted(op->tiles.size());
-        for (size_t i = 0; i < keys.size(); i++) sorted[i] = op->tiles[keys[i].idx];
-        op->tiles.swap(sorted);
+    if (dst_order && !per_task && !P->tune.task_order && P->sched.algorithm == RS_SCHED_NONE && interleaved && op->tasks.size() > 1) {
+        group_interleaved(op);
+    } else {
+        op->segs.resize(op->tasks.size());
+        for (size_t t = 0; t < op->tasks.size(); t++) op->segs[t] = RsSeg{0, (uint32_t)t, 1, op->tasks[t].n_tiles};
     }
-    if (op->tiles.size() > 0x7FFFFFFFull) { set_error("tile table too large"); return RS_EUNSUPPORTED; }
-    I.n_tiles = (int32_t)op->tiles.size();
-    int64_t mr = INT64_MAX;
-    for (const RsTile &t : op->tiles) mr = std::min<int64_t>(mr, t.col_bytes);
-    I.min_run_bytes = op->tiles.empty() ? 0 : mr;
+    uint32_t begin = 0;
+    for (RsSeg &s : op->segs) { s.tile_begin = begin; begin += s.n_members * s.tiles_each; }
+    I.n_tiles = (int32_t)begin;
+    I.n_segs = (int32_t)op->segs.size();
+    I.table_bytes = (int32_t)(op->tasks.size() * sizeof(RsTask) + op->dsts.size() * sizeof(RsDst) + op->segs.size() * sizeof(RsSeg));
+    int64_t mr = INT64_MAX, pad = 0;
+    for (const RsTask &T : op->tasks) { mr = std::min(mr, task_min_col(T)); pad = std::max(pad, task_shift_stage(T)); }
+    I.min_run_bytes = op->tasks.empty() ? 0 : mr;
     op->shift_stage = 0;
     op->alt_stage = 0;
     bool lsu = !bulk_family;
@@ -288,28 +312,25 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         const bool shift = path == RS_PATH_BULK_SHIFT;
         int warps = I.block / 32;
         int64_t stage = tile_bytes;
-        if (shift) {                                           // a row of n bytes occupies (n + 77) & ~15 bytes of a ring slot
-            stage = 0;
-            for (const RsTile &t : op->tiles) stage = std::max<int64_t>(stage, (int64_t)t.n_rows * (((int64_t)t.col_bytes + 77) & ~15ll));
+        if (shift) {
+            stage = pad;
             while (stages > 2 && (int64_t)warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) stages--;
             while (warps > 1 && (int64_t)warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) warps--;
             I.block = warps * 32;
         }
         op->stages = stages;
-        op->lookahead = std::max(1, std::min(stages - 1, shift ? env_int("RS_SHIFT_LOOKAHEAD", stages - 1) : env_int("RS_BULK_LOOKAHEAD", RS_BULK_LOOKAHEAD)));
+        op->lookahead = std::max(1, std::min(stages - 1, shift ? pick(P->tune.shift_lookahead, stages - 1) : pick(P->tune.bulk_lookahead, RS_BULK_LOOKAHEAD)));
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
         I.smem_bytes = (int32_t)(warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024);
         if (shift) op->shift_stage = (uint32_t)stage;
         if (!shift) {
             // An aligned plan may be handed under-aligned pointers at execute time: keep a launch shape of the
-            // shifted TMA kernel for the SAME tile table (rows padded in the ring, so fewer warps or slots fit).
-            int64_t pad = 0;
-            for (const RsTile &t : op->tiles) pad = std::max<int64_t>(pad, (int64_t)t.n_rows * (((int64_t)t.col_bytes + 77) & ~15ll));
+            // shifted TMA kernel for the SAME tiles (rows padded in the ring, so fewer warps or slots fit).
             const bool long_rows = min_run >= 1024;
             int aw = long_rows ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS, as = long_rows ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES;
             while (as > 2 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) as--;
             while (aw > 1 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) aw--;
-            if ((int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 <= RS_SMEM_MAX && !op->tiles.empty()) {
+            if ((int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 <= RS_SMEM_MAX && I.n_tiles > 0) {
                 op->alt_stage = (uint32_t)pad; op->alt_warps = aw; op->alt_stages = as;
                 op->alt_smem = (int)(aw * (as * pad + RS_BULK_DESC_BYTES) + 1024);
             }
@@ -340,7 +361,7 @@ rs_status build_slabs(Plan *P, const int64_t *sA, const int64_t *sB, int64_t ten
     const int N = A.ndim;
     const int64_t e = P->elem_bytes, l0 = A.shape[0];
     OpTables &H = P->op[RS_OP_SLABS];
-    H.tasks.clear(); H.dsts.clear(); H.tiles.clear();
+    H.tasks.clear(); H.dsts.clear(); H.segs.clear();
     P->slabs.clear();
     int64_t C = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(l0, RS_HOST_SLABS_MAX),
                                                        tensor_bytes / RS_HOST_SLAB_MIN_BYTES));
@@ -392,14 +413,13 @@ rs_status build_slabs(Plan *P, const int64_t *sA, const int64_t *sB, int64_t ten
         }
         P->slabs.push_back(std::move(S));
     }
-    std::vector<uint32_t> ttb;
-    rs_status st = finish_op(P, &H, tensor_bytes, tensor_bytes * P->r_B, &ttb);
+    rs_status st = finish_op(P, &H, tensor_bytes, tensor_bytes * P->r_B, /*per_task=*/true);
     if (st != RS_OK) return st;
     for (HostSlab &S : P->slabs) { S.tile_begin = 0xFFFFFFFFu; S.tile_end = 0; }
-    for (size_t t = 0; t < task_slab.size(); t++) {
+    for (size_t t = 0; t < task_slab.size(); t++) {           // one segment per task, in task order
         HostSlab &S = P->slabs[task_slab[t]];
-        S.tile_begin = std::min(S.tile_begin, ttb[t]);
-        S.tile_end = std::max(S.tile_end, ttb[t + 1]);
+        S.tile_begin = std::min(S.tile_begin, H.segs[t].tile_begin);
+        S.tile_end = std::max(S.tile_end, H.segs[t].tile_begin + H.segs[t].tiles_each);
     }
     return RS_OK;
 }
@@ -412,7 +432,7 @@ rs_status build_slabs(Plan *P, const int64_t *sA, const int64_t *sB, int64_t ten
 // arrays are the concatenation of the members' arrays.
 rs_status build_group(Plan *G, const std::vector<const Plan *> &members) {
     OpTables &X = G->op[RS_OP_EXECUTE];
-    for (OpTables &o : G->op) { o.tasks.clear(); o.dsts.clear(); o.tiles.clear(); o.info = rs_op_info{}; }
+    for (OpTables &o : G->op) { o.tasks.clear(); o.dsts.clear(); o.segs.clear(); o.info = rs_op_info{}; }
     int n_src = 0, n_dst = 0;
     int64_t rd = 0, wr = 0;
     G->used_src.clear();
@@ -428,7 +448,7 @@ rs_status build_group(Plan *G, const std::vector<const Plan *> &members) {
     }
     G->A.n_dev = n_src; G->B.n_dev = n_dst;
     G->group_src = n_src; G->group_dst = n_dst;
-    return finish_op(G, &X, rd, wr, nullptr, true);
+    return finish_op(G, &X, rd, wr, false, true);
 }
 
 rs_status build_tables(Plan *P) {
@@ -451,7 +471,7 @@ rs_status build_tables(Plan *P) {
         }
 
     OpTables &X = P->op[RS_OP_EXECUTE], &PK = P->op[RS_OP_PACK], &UP = P->op[RS_OP_UNPACK];
-    for (OpTables *o : {&X, &PK, &UP}) { o->tasks.clear(); o->dsts.clear(); o->tiles.clear(); }
+    for (OpTables *o : {&X, &PK, &UP}) { o->tasks.clear(); o->dsts.clear(); o->segs.clear(); }
 
     for (int i : P->exec_order) {                              // slice-id order, or the schedule's (S3.2)
         const Slice &S = P->slices[(size_t)i];
@@ -510,7 +530,7 @@ rs_status build_tables(Plan *P) {
     // its peers' shards (k - 1 reads + k - 1 writes): again 2k, in two dependent launches.
     OpTables &SR = P->op[RS_OP_SENDRECV], &AS = P->op[RS_OP_AG_SCATTER], &AG = P->op[RS_OP_AG_GATHER];
     OpTables &LS = P->op[RS_OP_AGL_SCATTER], &LG = P->op[RS_OP_AGL_GATHER];
-    for (OpTables *o : {&SR, &AS, &AG, &LS, &LG}) { o->tasks.clear(); o->dsts.clear(); o->tiles.clear(); o->info = rs_op_info{}; }
+    for (OpTables *o : {&SR, &AS, &AG, &LS, &LG}) { o->tasks.clear(); o->dsts.clear(); o->segs.clear(); o->info = rs_op_info{}; }
     if (P->flags & RS_WITH_STRATEGIES) {
         auto add = [&](OpTables &O, const int64_t *lo, const int64_t *hi, int src_buf, const int64_t *src_origin,
                        const int64_t *sstr, int dst_buf, const int64_t *dst_origin) -> bool {
@@ -580,9 +600,9 @@ rs_status build_tables(Plan *P) {
         if ((st = finish_op(P, &LG, lg, lg)) != RS_OK) return st;
     }
     if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
-    if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B, nullptr, true)) != RS_OK) return st;
+    if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B, false, true)) != RS_OK) return st;
     if ((st = finish_op(P, &PK, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
-    if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B, nullptr, true)) != RS_OK) return st;
+    if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B, false, true)) != RS_OK) return st;
     return RS_OK;
 }
 

@@ -29,7 +29,7 @@ RS_MAX_NDIM, RS_MAX_MESH_NDIM, RS_MAX_DEVICES = 8, 4, 128
 
 # every symbol include/reshard.h declares (tests check the library exports exactly these)
 SYMBOLS = [
-    "reshard_plan", "reshard_plan_ex", "reshard_plan_group", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables",
+    "reshard_plan", "reshard_plan_ex", "reshard_plan_group", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables", "reshard_op_tiles",
     "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
     "reshard_plan_message", "reshard_execute", "reshard_execute_strategy", "reshard_pack", "reshard_unpack", "reshard_execute_host",
     "reshard_host_workspace_bytes", "reshard_pipeline_simulate", "reshard_pipeline_least_delay", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
@@ -49,13 +49,22 @@ class OpInfo(C.Structure):
     _fields_ = [("path", C.c_int32), ("vec_bytes", C.c_int32), ("n_tasks", C.c_int32), ("n_dsts", C.c_int32),
                 ("n_tiles", C.c_int32), ("tile_bytes", C.c_int32), ("grid", C.c_int32), ("block", C.c_int32),
                 ("smem_bytes", C.c_int32), ("read_bytes", C.c_int64), ("write_bytes", C.c_int64),
-                ("min_run_bytes", C.c_int64)]
+                ("min_run_bytes", C.c_int64), ("n_segs", C.c_int32), ("table_bytes", C.c_int32)]
+
+
+class Tuning(C.Structure):
+    """rs_tuning: launch-shape overrides for tests and sweeps (0 = the library's choice)"""
+    _fields_ = [("bulk_warps", C.c_int32), ("bulk_stages", C.c_int32), ("bulk_lookahead", C.c_int32),
+                ("bulk_tile_bytes", C.c_int32), ("bulk_ctas", C.c_int32), ("bulk_ctas_mcast", C.c_int32),
+                ("shift_warps", C.c_int32), ("shift_stages", C.c_int32), ("shift_lookahead", C.c_int32),
+                ("shift_tile_bytes", C.c_int32), ("lsu_tile_bytes", C.c_int32), ("lsu_ctas_per_sm", C.c_int32),
+                ("task_order", C.c_int32), ("small_op_bytes_mib", C.c_int32), ("reserved", C.c_int32 * 2)]
 
 
 class PlanOpts(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("schedule", C.c_int32), ("src_devices_per_host", C.c_int32),
                 ("dst_devices_per_host", C.c_int32), ("trials", C.c_int32), ("max_ctas", C.c_int32),
-                ("node_budget", C.c_int64), ("seed", C.c_uint64)]
+                ("node_budget", C.c_int64), ("seed", C.c_uint64), ("tuning", C.POINTER(Tuning))]
 
 
 class ScheduleInfo(C.Structure):
@@ -98,8 +107,8 @@ def _lib():
             from . import build as _build
             _build.build()
         except Exception as ex:               # noqa: BLE001 -- no nvcc, or a compile error: say so, there is no fallback
-            if not os.path.exists(LIB_PATH):
-                raise ImportError("libreshard.so is not built and could not be built (%s): run "
+            if not os.path.exists(LIB_PATH) or _build._stale():      # an up-to-date library needs no compiler
+                raise ImportError("libreshard.so is missing or older than its sources and could not be built (%s): run "
                                   "`python -m paper_2211_05322_b200.build` (there is no fallback path)" % ex)
         try:
             L = C.CDLL(LIB_PATH)
@@ -146,7 +155,8 @@ class Plan:
     """reshard_plan(...) handle.  See include/reshard.h for the contract of every call."""
 
     def __init__(self, global_shape, elem_bytes, src_mesh, src_spec, dst_mesh, dst_spec, flags=0, opts=None):
-        """opts: dict of rs_plan_opts fields (schedule, src_devices_per_host, ...) -> reshard_plan_ex"""
+        """opts: dict of rs_plan_opts fields (schedule, src_devices_per_host, ..., tuning=dict of rs_tuning
+        fields) -> reshard_plan_ex"""
         self._h = C.c_void_p()
         if opts is None:
             _chk(_lib().reshard_plan(_i64(global_shape), len(global_shape), int(elem_bytes),
@@ -154,7 +164,12 @@ class Plan:
                                      _i32(dst_mesh), len(dst_mesh), dst_spec.encode(),
                                      C.c_uint32(flags), C.byref(self._h)))
         else:
+            opts = dict(opts)
+            tune = opts.pop("tuning", None)
             o = PlanOpts(flags=flags, **opts)
+            if tune:
+                t = Tuning(**tune)                                   # the plan copies it
+                o.tuning = C.pointer(t)
             _chk(_lib().reshard_plan_ex(_i64(global_shape), len(global_shape), int(elem_bytes),
                                         _i32(src_mesh), len(src_mesh), src_spec.encode(),
                                         _i32(dst_mesh), len(dst_mesh), dst_spec.encode(),
@@ -190,12 +205,20 @@ class Plan:
         return out
 
     def op_tables(self, op):
-        """raw bytes of (tasks, dsts, tiles); layouts in csrc/tables.h"""
+        """raw bytes of (tasks, dsts, segs); layouts in csrc/tables.h"""
         oi = self.op_info(op)
-        t, d, l = (C.create_string_buffer(max(1, oi.n_tasks * 192)), C.create_string_buffer(max(1, oi.n_dsts * 16)),
-                   C.create_string_buffer(max(1, oi.n_tiles * 32)))
-        _chk(_lib().reshard_op_tables(self._h, op, t, d, l))
-        return t.raw[:oi.n_tasks * 192], d.raw[:oi.n_dsts * 16], l.raw[:oi.n_tiles * 32]
+        t, d, g = (C.create_string_buffer(max(1, oi.n_tasks * 224)), C.create_string_buffer(max(1, oi.n_dsts * 16)),
+                   C.create_string_buffer(max(1, oi.n_segs * 16)))
+        _chk(_lib().reshard_op_tables(self._h, op, t, d, g))
+        return t.raw[:oi.n_tasks * 224], d.raw[:oi.n_dsts * 16], g.raw[:oi.n_segs * 16]
+
+    def op_tiles(self, op, first=0, count=None):
+        """raw bytes of tiles first .. first + count - 1 as the LIBRARY decodes them (32-byte RsTile records)"""
+        if count is None:
+            count = self.op_info(op).n_tiles - first
+        buf = C.create_string_buffer(max(1, count * 32))
+        _chk(_lib().reshard_op_tiles(self._h, op, C.c_int64(first), C.c_int64(count), buf))
+        return buf.raw[:count * 32]
 
     def local_shape(self, side):
         out = (C.c_int64 * self.ndim)()

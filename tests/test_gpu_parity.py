@@ -80,16 +80,15 @@ def test_under_aligned_shard_pointers(off, path):
 
 @pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK, rs.RS_PATH_BULK_SHIFT])
 @pytest.mark.parametrize("tile", [128, 1024, 4096])
-def test_tile_sizes_and_ring_depths(tile, path, monkeypatch):
-    monkeypatch.setenv("RS_LSU_TILE_BYTES", str(tile))
-    monkeypatch.setenv("RS_BULK_TILE_BYTES", str(tile))
+def test_tile_sizes_and_ring_depths(tile, path):
+    """rs_plan_opts.tuning: other tile sizes, ring depths and warp counts, same bytes"""
     for stages, look, warps in [(2, 1, 1), (3, 2, 4), (8, 4, 2), (6, 5, 8)]:
-        monkeypatch.setenv("RS_BULK_STAGES", str(stages))
-        monkeypatch.setenv("RS_BULK_LOOKAHEAD", str(look))
-        monkeypatch.setenv("RS_BULK_WARPS", str(warps))
+        tuning = dict(lsu_tile_bytes=tile, bulk_tile_bytes=tile, shift_tile_bytes=tile, bulk_stages=stages, bulk_lookahead=look,
+                      bulk_warps=warps, shift_stages=stages, shift_lookahead=look, shift_warps=warps)
         for case in (SMALL[2], SMALL[15], SMALL[17], SMALL[18]):
             shape, sm, ss, dm, ds = case
-            _p, got, want = gu.run_small(shape, np.int32, sm, ss, dm, ds, flags=path)
+            p, got, want = gu.run_small(shape, np.int32, sm, ss, dm, ds, flags=path, opts=dict(tuning=tuning))
+            assert p.op_info(rs.RS_OP_EXECUTE).tile_bytes <= max(tile, 128)
             for g, w in zip(got, want):
                 assert g.tobytes() == w.tobytes()
         if path == rs.RS_PATH_LSU:

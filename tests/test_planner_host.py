@@ -222,21 +222,15 @@ def _valid_bytes(shape, mesh, spec, e):
     return out
 
 
-def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, env=None, opts=None):
+def _check_tables(shape, dtype, sm, ss, dm, ds, flags=0, tuning=None, opts=None):
     e = np.dtype(dtype).itemsize
     once = _valid_bytes(shape, dm, ds, e)
-    old = {}
-    for k, v in (env or {}).items():
-        old[k] = os.environ.get(k)
-        os.environ[k] = str(v)
-    try:
-        p = _plan(shape, e, sm, ss, dm, ds, flags, opts)
-    finally:
-        for k, v in old.items():
-            if v is None:
-                os.environ.pop(k)
-            else:
-                os.environ[k] = v
+    if tuning:
+        opts = dict(opts or {}, tuning=tuning)
+    p = _plan(shape, e, sm, ss, dm, ds, flags, opts)
+    for op in (rs.RS_OP_EXECUTE, rs.RS_OP_PACK, rs.RS_OP_UNPACK, rs.RS_OP_EXECUTE_SLABS):
+        mine, theirs = ti.tiles(p, op), ti.lib_tiles(p, op)       # the decode restated here vs the routine the kernels run
+        assert mine.tobytes() == theirs.tobytes(), "tile decode of op %d differs" % op
     D = (np.arange(int(np.prod(shape)), dtype=np.int64) * 2654435761 % 251 + 1).astype(dtype).reshape(shape)
     src = do.shards_from_global(D, sm, ss)
     want = do.reshard(shape, sm, ss, dm, ds, src)
@@ -289,14 +283,14 @@ def test_tables_replay_equals_oracle(shape, sm, ss, dm, ds, dtype):
 @pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK])
 def test_tables_with_tiny_tiles_cover_every_tile_kind(tile, path):
     """small tile sizes force column-split rows, FAST row groups and GENERIC tiles at test sizes"""
-    env = {"RS_LSU_TILE_BYTES": tile, "RS_BULK_TILE_BYTES": tile}
+    tuning = {"lsu_tile_bytes": tile, "bulk_tile_bytes": tile}
     kinds = set()
     for shape, sm, ss, dm, ds in [((4, 6, 64), (2, 2), "S0,S1,R", (2, 2), "S1,S0,R"),      # long runs -> column split
                                   ((8, 16, 16), (2, 4), "S0,R,S1", (2, 4), "S0,S1,R"),     # short runs, wide ext0
                                   ((8, 6, 2, 16), (2, 2), "S0,R,R,S1", (2, 2), "R,S0,R,S1"),  # ext0 = 2 -> GENERIC
                                   ((6, 4, 2, 3, 8), (2,), "R,R,R,R,S0", (2,), "S0,R,R,R,R")]:
-        p = _check_tables(shape, np.int32, sm, ss, dm, ds, flags=path, env=env)
-        _t, _d, tiles = ti.tables(p, rs.RS_OP_EXECUTE)
+        p = _check_tables(shape, np.int32, sm, ss, dm, ds, flags=path, tuning=tuning)
+        tiles = ti.tiles(p, rs.RS_OP_EXECUTE)
         for t in tiles:
             kinds.add("split" if t["n_rows"] == 1 and t["flags"] & 1 else "fast" if t["flags"] & 1 else "generic")
         assert p.op_info(rs.RS_OP_EXECUTE).tile_bytes <= max(tile, 128)
@@ -330,8 +324,11 @@ def test_full_size_tables_cover_every_byte_once(name):
     w = inputs.get_workload(name)
     p = _plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
     for op in (rs.RS_OP_EXECUTE, rs.RS_OP_PACK, rs.RS_OP_UNPACK):
-        tasks, dsts, tiles = ti.tables(p, op)
+        tasks, dsts, _segs = ti.tables(p, op)
+        tiles = ti.tiles(p, op)
+        assert tiles.tobytes() == ti.lib_tiles(p, op).tobytes()
         oi = p.op_info(op)
+        assert oi.n_tiles == len(tiles) and oi.table_bytes == 224 * oi.n_tasks + 16 * oi.n_dsts + 16 * oi.n_segs
         T = tasks[tiles["task"]]
         nbytes = tiles["n_rows"].astype(np.int64) * tiles["col_bytes"].astype(np.int64)
         assert int(nbytes.sum()) == oi.read_bytes
@@ -384,7 +381,7 @@ def test_random_layouts_tables_equal_oracle(layout):
         with pytest.raises(rs.ReshardError) as ei:
             _plan(shape, 1, sm, ss, dm, ds, rs.RS_EVEN_ONLY)
         assert ei.value.code == rs.RS_EDIVIS
-    _check_tables(shape, dtype, sm, ss, dm, ds, env={"RS_LSU_TILE_BYTES": tile, "RS_BULK_TILE_BYTES": tile})
+    _check_tables(shape, dtype, sm, ss, dm, ds, tuning={"lsu_tile_bytes": tile, "bulk_tile_bytes": tile})
 
 
 def test_slab_table_cuts_dim0_when_large():
@@ -392,7 +389,7 @@ def test_slab_table_cuts_dim0_when_large():
     p = _plan((32, 2048, 12288), 2, (2, 4), "S0,S1,R", (4, 2), "S1,R,S0")
     assert p.op_info(rs.RS_OP_EXECUTE_SLABS).n_tasks == 16 * 32 // 2      # 16 slabs x the 16 slices each slab meets
     p = _plan((6, 1024, 2048), 2, (2, 2), "S0,R,S1", (3,), "S0,R,R")       # 24 MiB -> 3 slabs over l_0 = 6
-    tasks, _d, tiles = ti.tables(p, rs.RS_OP_EXECUTE_SLABS)
+    tiles = ti.tiles(p, rs.RS_OP_EXECUTE_SLABS)
     assert p.op_info(rs.RS_OP_EXECUTE_SLABS).read_bytes == p.info.tensor_bytes
     assert int((tiles["n_rows"].astype(np.int64) * tiles["col_bytes"]).sum()) == p.info.tensor_bytes
     p = _plan((8, 16), 4, (1, 2), "S1,R", (1, 2), "R,S1")                  # tiny: one slab == the execute table
@@ -511,3 +508,47 @@ def test_plan_group_merges_execute_tables():
     with pytest.raises(rs.ReshardError) as ei:
         rs.Plan.group(big, HOST)
     assert ei.value.code == rs.RS_EUNSUPPORTED
+
+
+def test_plan_is_o_slices_not_o_bytes():
+    """PAPER.md:482-492 (App. B.2): the plan is the slice list, nothing finer.  Table bytes and plan time do not
+    grow with the tensor: tiles are decoded on the device (csrc/tables.h), never stored."""
+    import time
+    sizes = {}
+    for mib in (1, 64, 1024, 4096):
+        w = inputs.sweep_workload("P1", "m8", mib << 20)
+        p = _plan(w.shape, 2, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+        sizes[mib] = [p.op_info(op).table_bytes for op in (rs.RS_OP_EXECUTE, rs.RS_OP_PACK, rs.RS_OP_UNPACK)]
+        assert p.op_info(rs.RS_OP_EXECUTE).n_tiles >= (mib << 20) // 16384
+    assert sizes[1] == sizes[64] == sizes[1024] == sizes[4096]
+    for name in ("c1", "c2", "c3", "c3i", "c3ii", "c4", "sweep_P5_m8_4096MiB", "sweep_P1_m8_4096MiB", "t2_4"):
+        w = inputs.get_workload(name)
+        e = inputs.elem_bytes(w.dtype)
+        _plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)                    # warm
+        t0 = time.perf_counter()
+        p = _plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+        dt = time.perf_counter() - t0
+        for op in (rs.RS_OP_EXECUTE, rs.RS_OP_PACK, rs.RS_OP_UNPACK):
+            assert p.op_info(op).table_bytes < 64 << 10, (name, op)
+        assert dt < 0.02, "%s: host plan took %.1f ms" % (name, dt * 1e3)                      # round 1: 18-225 ms
+
+
+def test_destination_order_segments():
+    """slices that share destination rows (config 2: four slices fill a quarter of every row of a receiver's
+    shard) form one segment walked round-robin = in destination address order; rs_tuning.task_order and a
+    schedule (tables in order of S_i) switch it off"""
+    w = inputs.get_workload("c2")
+    p = _plan(w.shape, 2, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    tasks, dsts, segs = ti.tables(p, rs.RS_OP_EXECUTE)
+    assert len(tasks) == 32 and len(segs) == 8 and (segs["n_members"] == 4).all()
+    tiles = ti.tiles(p, rs.RS_OP_EXECUTE)
+    T = tasks[tiles["task"]]
+    key = dsts[T["dst_first"]]["buf"].astype(np.int64) * (1 << 40) + dsts[T["dst_first"]]["off"] + tiles["b"].astype(np.int64)
+    assert (np.diff(key) > 0).all()                                   # ascending (buffer, address)
+    for opts in (dict(tuning=dict(task_order=1)), dict(schedule=rs.RS_SCHED_LOAD_BALANCE)):
+        q = _plan(w.shape, 2, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, opts)
+        _t, _d, segs = ti.tables(q, rs.RS_OP_EXECUTE)
+        assert len(segs) == 32 and (segs["n_members"] == 1).all()
+        assert (np.diff(ti.tiles(q, rs.RS_OP_EXECUTE)["task"].astype(np.int64)) >= 0).all()   # task by task
+    _t, _d, segs = ti.tables(p, rs.RS_OP_PACK)                        # pack writes dense messages: nothing to interleave
+    assert (segs["n_members"] == 1).all()

@@ -126,3 +126,23 @@ def test_unscheduled_plan_has_no_schedule_and_bad_options_fail():
         p.schedule()
     with pytest.raises(rs.ReshardError):
         _plan((8, 8), 2, (2,), "S0,R", (2,), "R,S0", 0, dict(schedule=9))
+
+
+@pytest.mark.parametrize("n", [96, 128])
+@pytest.mark.parametrize("alg", [rs.RS_SCHED_DFS, rs.RS_SCHED_ENSEMBLE])
+def test_thousands_of_unit_tasks_do_not_overflow_the_stack(n, alg):
+    """n x n unit tasks (9216 / 16384) on 128-device meshes: the DFS is iterative and skipped above 4096 tasks
+    (useless beyond ~20); the schedule is still valid (makespan >= the busiest host's bytes)"""
+    p = rs.Plan((4 * n, 4 * n), 2, (n,), "S0,R", (n,), "R,S0", rs.RS_HOST_ONLY, dict(schedule=alg))
+    info = p.schedule()["info"]
+    assert p.info.n_slices == n * n and info.dfs_finished == 0 and info.dfs_nodes == 0
+    assert info.makespan >= info.busiest_host_bytes > 0
+    if alg == rs.RS_SCHED_ENSEMBLE:
+        assert info.winner == rs.RS_SCHED_GREEDY
+
+
+def test_deep_dfs_runs_inside_its_node_budget():
+    """2500 unit tasks: the search descends 2500 levels on the heap and stops at the node budget"""
+    p = rs.Plan((200, 200), 2, (50,), "S0,R", (50,), "R,S0", rs.RS_HOST_ONLY, dict(schedule=rs.RS_SCHED_DFS, node_budget=6000))
+    info = p.schedule()["info"]
+    assert info.dfs_finished == 0 and info.dfs_nodes == 6000 and info.makespan >= info.busiest_host_bytes
