@@ -130,6 +130,15 @@ typedef struct rs_plan_opts {
     int64_t node_budget;             /* DFS nodes before giving up with the best found; 0 = 200000          */
     uint64_t seed;                   /* of the counter-based generator the greedy search draws from         */
     const rs_tuning *tuning;         /* [HOST] may be NULL: launch shapes chosen by the library             */
+    const int32_t *src_owner;        /* [HOST, n_src] may be NULL.  Multi-process executor (one process per GPU): the
+                                        rank that holds source shard r.  With it the plan's execute table lists only
+                                        the unit tasks whose chosen sender `rank` holds (unit tasks are independent,
+                                        PAPER.md:90, 100); every rank builds the same plan with its own `rank`, and the
+                                        union of their launches is the whole task.  Such a plan supports
+                                        reshard_execute and the queries; pack / unpack / execute_host / strategies /
+                                        groups return RS_EINVAL                                             */
+    int32_t rank;                    /* this process, with src_owner                                        */
+    int32_t reserved;
 } rs_plan_opts;
 
 typedef struct rs_schedule_info {
@@ -284,6 +293,10 @@ RS_API rs_status reshard_op_tiles(const rs_plan *plan, int32_t op, int64_t first
  * Preconditions (undefined behaviour otherwise, not checked): replicas on the source side hold
  * identical bytes; no destination shard overlaps any other shard (Mesh_A and Mesh_B are
  * disjoint).  Pointers of source shards that no task reads may be NULL.
+ * A plan built with rs_plan_opts.src_owner runs this rank's unit tasks only: source pointers of shards other
+ * ranks hold may be NULL, destination pointers may be NULL for shards this rank never writes, and the others may
+ * be peer memory (another GPU's shard mapped through CUDA IPC or peer access: the slice is moved by the kernel's
+ * stores, "the sender's GPU issues the writes").
  * One kernel launch.  Returns RS_ECUDA if the launch fails, RS_EINVAL for a host-only plan.
  */
 RS_API rs_status reshard_execute(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
@@ -318,6 +331,20 @@ RS_API rs_status reshard_execute_host(const rs_plan *plan, const void *const *sr
                                void *const *dst_shards_host, void *workspace, void *cuda_stream,
                                int64_t *h2d_bytes, int64_t *d2h_bytes);
 RS_API int64_t reshard_host_workspace_bytes(const rs_plan *plan);
+
+/* ---- multi-process executor plumbing: CUDA IPC -------------------------------------------------
+ * One process per GPU; every rank exports the destination shards it holds, the senders' ranks import them and
+ * pass the mapped pointers to reshard_execute.  These three calls only wrap cudaIpcGetMemHandle /
+ * cudaIpcOpenMemHandle / cudaIpcCloseMemHandle and deal with sub-allocated pointers (a caching allocator hands out
+ * pieces of one cudaMalloc block: the handle names the block, the offset the piece). */
+#define RS_IPC_HANDLE_BYTES 80
+/* dev_ptr [DEVICE, from cudaMalloc in THIS process] -> handle_out [HOST, RS_IPC_HANDLE_BYTES], to be sent to peers */
+RS_API rs_status reshard_ipc_export(const void *dev_ptr, void *handle_out);
+/* handle [HOST, RS_IPC_HANDLE_BYTES, exported by ANOTHER process] -> *dev_ptr_out [DEVICE pointer valid in this
+ * process].  Every exporting allocation is mapped once per process and kept until reshard_ipc_release_all. */
+RS_API rs_status reshard_ipc_import(const void *handle, void **dev_ptr_out);
+/* unmap everything reshard_ipc_import mapped (before the exporters free their memory) */
+RS_API rs_status reshard_ipc_release_all(void);
 
 /* ---- S4: pipeline schedules around the resharding tasks (host only, no CUDA) ------------------- */
 #define RS_PIPE_MAX_STAGES 64
@@ -356,7 +383,8 @@ typedef struct rs_pipeline_result {
 RS_API rs_status reshard_pipeline_simulate(const rs_pipeline_opts *opts, rs_pipeline_result *result, int32_t *op_kind,
                                     int32_t *op_micro_batch, int64_t *op_start, int64_t *op_end);
 /* PAPER.md:217 "delay the least to cover all communications": the smallest bw_delay for which the compute a
- * stage (1-based) runs between an activation-gradient op and its weight-gradient op covers comm_bwd. */
+ * stage (1-based) runs between an activation-gradient op and its weight-gradient op covers comm_bwd.
+ * Returns -1 for bad arguments and when no delay up to 2 * n_micro_batches covers it. */
 RS_API int32_t reshard_pipeline_least_delay(int32_t schedule, int32_t n_stages, int32_t stage, int32_t n_micro_batches,
                                      int64_t fwd, int64_t bwd, int64_t bwd_act, int64_t comm_bwd);
 

@@ -27,7 +27,7 @@ seed + counter; Fisher-Yates from the top); R25 the DFS explores (next task, sen
 ascending (task id, host id) and stops after a node budget instead of a time budget.
 
 Pins: tests/test_schedule_oracle_pins.py (hand-computed timelines of Table 2 cases 1, 2, 3, 8 as
-the paper describes them at PAPER.md:306, 320; brute force over all orders x senders; the
+the paper describes them at PAPER.md:282, 320; brute force over all orders x senders; the
 independent pairwise Eq. 3 checker; Eq. 4 lower bound).
 """
 import itertools

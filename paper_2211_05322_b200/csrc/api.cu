@@ -137,6 +137,15 @@ rs_status reshard_plan_ex(const int64_t *global_shape, int32_t ndim, int32_t ele
     rs_status st;
     try {
         st = (flags & RS_HOST_ONLY) ? RS_OK : query_device(P);
+        if (st == RS_OK && opts->src_owner) {                  // multi-process executor: this rank's share of the unit tasks
+            int64_t n_src = 1;
+            for (int32_t a = 0; src_mesh_shape && a < src_mesh_ndim && a < RS_MAX_MESH_NDIM; a++) n_src *= std::max(1, src_mesh_shape[a]);
+            if (n_src > RS_MAX_DEVICES) n_src = 0;             // make_layout reports the real error
+            if (flags & RS_WITH_STRATEGIES) { rs::set_error("RS_WITH_STRATEGIES is not available with src_owner"); st = RS_EINVAL; }
+            if (opts->rank < 0) { rs::set_error("rank < 0 with src_owner"); st = RS_EINVAL; }
+            P->src_owner.assign(opts->src_owner, opts->src_owner + n_src);
+            P->rank = opts->rank;
+        }
         if (st == RS_OK) st = rs::make_layout(global_shape, ndim, src_mesh_shape, src_mesh_ndim, src_spec, (flags & RS_EVEN_ONLY) != 0, &P->A);
         if (st == RS_OK) st = rs::make_layout(global_shape, ndim, dst_mesh_shape, dst_mesh_ndim, dst_spec, (flags & RS_EVEN_ONLY) != 0, &P->B);
         if (st == RS_OK) st = rs::build_slices(P);
@@ -162,7 +171,7 @@ rs_status reshard_plan_group(const rs_plan *const *plans, int32_t n_plans, uint3
     if (!plans || !out_plan || n_plans < 1) { rs::set_error("null argument or empty group"); return RS_EINVAL; }
     std::vector<const rs::Plan *> members;
     for (int32_t i = 0; i < n_plans; i++) {
-        if (!plans[i] || plans[i]->p.group_src) { rs::set_error("a member is null or is itself a group"); return RS_EINVAL; }
+        if (!plans[i] || plans[i]->p.group_src || !plans[i]->p.src_owner.empty()) { rs::set_error("a member is null, is itself a group or was built with src_owner"); return RS_EINVAL; }
         members.push_back(&plans[i]->p);
     }
     rs_plan *h = new (std::nothrow) rs_plan();
@@ -344,7 +353,8 @@ int ptr_align(const void *p) {
 
 // one launch of operation `opi` on the given buffers
 rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src, void *const *dst, int n_dst,
-                 const char *used_src, void *stream, uint32_t tile_begin = 0, uint32_t tile_end = 0) {
+                 const char *used_src, void *stream, uint32_t tile_begin = 0, uint32_t tile_end = 0,
+                 const char *used_dst = nullptr) {
     rs::set_error("");
     if (!plan || !src || !dst) { rs::set_error("null argument"); return RS_EINVAL; }
     const rs::Plan &P = plan->p;
@@ -362,8 +372,9 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         align = std::min(align, ptr_align(src[i]));
     }
     for (int i = 0; i < n_dst; i++) {
-        if (!dst[i]) { rs::set_error("a destination pointer is null"); return RS_EINVAL; }
         pt.dst[i] = static_cast<char *>(dst[i]);
+        if (used_dst && !used_dst[i]) continue;                // a rank of the multi-process executor: shards it never writes
+        if (!dst[i]) { rs::set_error("a destination pointer is null"); return RS_EINVAL; }
         align = std::min(align, ptr_align(dst[i]));
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -404,8 +415,9 @@ extern "C" {
 rs_status reshard_execute(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
                           void *cuda_stream) {
     if (!plan) return RS_EINVAL;
-    return run_op(plan, RS_OP_EXECUTE, src_shards, plan->p.A.n_dev, dst_shards, plan->p.B.n_dev,
-                  plan->p.used_src.data(), cuda_stream);
+    const rs::Plan &P = plan->p;
+    return run_op(plan, RS_OP_EXECUTE, src_shards, P.A.n_dev, dst_shards, P.B.n_dev, P.used_src.data(), cuda_stream, 0, 0,
+                  P.src_owner.empty() ? nullptr : P.used_dst.data());
 }
 
 rs_status reshard_execute_strategy(const rs_plan *plan, int32_t strategy, const void *const *src_shards,
@@ -413,6 +425,7 @@ rs_status reshard_execute_strategy(const rs_plan *plan, int32_t strategy, const 
     if (!plan) return RS_EINVAL;
     const rs::Plan &P = plan->p;
     if (strategy == RS_STRATEGY_BROADCAST) return reshard_execute(plan, src_shards, dst_shards, cuda_stream);
+    if (!P.src_owner.empty()) { rs::set_error("not available for a plan built with src_owner"); return RS_EINVAL; }
     if (!(P.flags & RS_WITH_STRATEGIES)) { rs::set_error("plan was built without RS_WITH_STRATEGIES"); return RS_EINVAL; }
     if (strategy == RS_STRATEGY_SENDRECV)
         return run_op(plan, RS_OP_SENDRECV, src_shards, P.A.n_dev, dst_shards, P.B.n_dev, P.used_src.data(), cuda_stream);
@@ -425,21 +438,21 @@ rs_status reshard_execute_strategy(const rs_plan *plan, int32_t strategy, const 
 }
 
 rs_status reshard_pack(const rs_plan *plan, const void *const *src_shards, void *msg_arena, void *cuda_stream) {
-    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
+    if (plan && (plan->p.group_src || !plan->p.src_owner.empty())) { rs::set_error("not available for a plan group or a plan built with src_owner"); return RS_EINVAL; }
     if (!plan) return RS_EINVAL;
     void *dst[1] = {msg_arena};
     return run_op(plan, RS_OP_PACK, src_shards, plan->p.A.n_dev, dst, 1, plan->p.used_src.data(), cuda_stream);
 }
 
 rs_status reshard_unpack(const rs_plan *plan, const void *msg_arena, void *const *dst_shards, void *cuda_stream) {
-    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
+    if (plan && (plan->p.group_src || !plan->p.src_owner.empty())) { rs::set_error("not available for a plan group or a plan built with src_owner"); return RS_EINVAL; }
     if (!plan) return RS_EINVAL;
     const void *src[1] = {msg_arena};
     return run_op(plan, RS_OP_UNPACK, src, 1, dst_shards, plan->p.B.n_dev, nullptr, cuda_stream);
 }
 
 int64_t reshard_host_workspace_bytes(const rs_plan *plan) {
-    if (plan && plan->p.group_src) return -1;
+    if (plan && (plan->p.group_src || !plan->p.src_owner.empty())) return -1;
     if (!plan) return -1;
     const rs::Plan &P = plan->p;
     int64_t n_used = 0;
@@ -450,7 +463,7 @@ int64_t reshard_host_workspace_bytes(const rs_plan *plan) {
 
 rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shards_host, void *const *dst_shards_host,
                                void *workspace, void *cuda_stream, int64_t *h2d_bytes, int64_t *d2h_bytes) {
-    if (plan && plan->p.group_src) { rs::set_error("not available for a plan group"); return RS_EINVAL; }
+    if (plan && (plan->p.group_src || !plan->p.src_owner.empty())) { rs::set_error("not available for a plan group or a plan built with src_owner"); return RS_EINVAL; }
     rs::set_error("");
     if (!plan || !src_shards_host || !dst_shards_host || !workspace) { rs::set_error("null argument"); return RS_EINVAL; }
     const rs::Plan &P = plan->p;
@@ -521,6 +534,69 @@ rs_status reshard_execute_host(const rs_plan *plan, const void *const *src_shard
     if (h2d_bytes) *h2d_bytes = up;
     if (d2h_bytes) *d2h_bytes = down;
     return RS_OK;
+}
+
+// ---- CUDA IPC plumbing of the multi-process executor ------------------------------------------
+
+namespace {
+struct IpcWire {                                               // RS_IPC_HANDLE_BYTES on the wire
+    cudaIpcMemHandle_t handle;                                 // 64 bytes: the exporting ALLOCATION
+    int64_t offset;                                            // of the exported pointer inside it
+    int64_t reserved;
+};
+static_assert(sizeof(IpcWire) == RS_IPC_HANDLE_BYTES, "rs ipc handle layout");
+std::mutex g_ipc_mu;
+std::vector<std::pair<cudaIpcMemHandle_t, void *>> g_ipc_open;  // one mapping per exporting allocation and process
+}  // namespace
+
+rs_status reshard_ipc_export(const void *dev_ptr, void *handle_out) {
+    rs::set_error("");
+    if (!dev_ptr || !handle_out) { rs::set_error("null argument"); return RS_EINVAL; }
+    typedef int (*range_fn)(unsigned long long *, size_t *, unsigned long long);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &q);
+    if (e != cudaSuccess || !fn) return cuda_fail(e, "cudaGetDriverEntryPoint(cuMemGetAddressRange)");
+    unsigned long long base = 0;
+    size_t size = 0;
+    if (reinterpret_cast<range_fn>(fn)(&base, &size, (unsigned long long)reinterpret_cast<uintptr_t>(dev_ptr)) != 0) {
+        rs::set_error("cuMemGetAddressRange failed: not a device allocation");
+        return RS_ECUDA;
+    }
+    IpcWire w;
+    std::memset(&w, 0, sizeof(w));
+    e = cudaIpcGetMemHandle(&w.handle, reinterpret_cast<void *>(static_cast<uintptr_t>(base)));
+    if (e != cudaSuccess) return cuda_fail(e, "cudaIpcGetMemHandle");
+    w.offset = (int64_t)(reinterpret_cast<uintptr_t>(dev_ptr) - (uintptr_t)base);
+    std::memcpy(handle_out, &w, sizeof(w));
+    return RS_OK;
+}
+
+rs_status reshard_ipc_import(const void *handle, void **dev_ptr_out) {
+    rs::set_error("");
+    if (!handle || !dev_ptr_out) { rs::set_error("null argument"); return RS_EINVAL; }
+    IpcWire w;
+    std::memcpy(&w, handle, sizeof(w));
+    std::lock_guard<std::mutex> lock(g_ipc_mu);
+    for (auto &m : g_ipc_open)
+        if (std::memcmp(&m.first, &w.handle, sizeof(w.handle)) == 0) { *dev_ptr_out = static_cast<char *>(m.second) + w.offset; return RS_OK; }
+    void *base = nullptr;
+    cudaError_t e = cudaIpcOpenMemHandle(&base, w.handle, cudaIpcMemLazyEnablePeerAccess);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaIpcOpenMemHandle");
+    g_ipc_open.emplace_back(w.handle, base);
+    *dev_ptr_out = static_cast<char *>(base) + w.offset;
+    return RS_OK;
+}
+
+rs_status reshard_ipc_release_all(void) {
+    std::lock_guard<std::mutex> lock(g_ipc_mu);
+    cudaError_t first = cudaSuccess;
+    for (auto &m : g_ipc_open) {
+        cudaError_t e = cudaIpcCloseMemHandle(m.second);
+        if (e != cudaSuccess && first == cudaSuccess) first = e;
+    }
+    g_ipc_open.clear();
+    return first == cudaSuccess ? RS_OK : cuda_fail(first, "cudaIpcCloseMemHandle");
 }
 
 rs_status reshard_pipeline_simulate(const rs_pipeline_opts *opts, rs_pipeline_result *result, int32_t *op_kind,

@@ -145,7 +145,7 @@ rs_status pipeline_simulate(const rs_pipeline_opts &o, rs_pipeline_result *res, 
 }
 
 // PAPER.md:217 cost model: the least delay whose intervening compute (the ops a stage runs between BA(m)
-// and its BW(m), BW included) covers the backward transfer
+// and its BW(m), BW included) covers the backward transfer; -1 if none up to 2 M does
 int pipeline_least_delay(int schedule, int S, int stage, int M, int64_t f, int64_t b, int64_t b_act, int64_t c_bwd) {
     for (int delay = 0; delay <= 2 * M; delay++) {
         const std::vector<Op> ops = stage_ops(schedule, S, stage, M, true, delay);
@@ -159,7 +159,7 @@ int pipeline_least_delay(int schedule, int S, int stage, int M, int64_t f, int64
         }
         if (covered >= c_bwd) return delay;
     }
-    return 2 * M;
+    return -1;                                                 // no delay up to 2 M covers the transfer
 }
 
 }  // namespace rs

@@ -108,6 +108,11 @@ struct Plan {
     int group_src = 0, group_dst = 0;    // > 0: this plan is a GROUP (reshard_plan_group): only its execute table exists
     int max_ctas = 0;                    // rs_plan_opts.max_ctas: cap on CTAs per launch (0: none)
     rs_tuning tune{};                    // rs_plan_opts.tuning (all zero: the library's launch shapes)
+    // multi-process executor (rs_plan_opts.src_owner / rank): the tables list only the unit tasks whose chosen sender
+    // this rank holds; the other ranks run the rest (unit tasks are independent)
+    std::vector<int> src_owner;          // [n_src] rank holding source shard r; empty: single-process plan
+    int rank = -1;
+    std::vector<char> used_dst;          // [n_dst] 1 if some task of the execute table writes that shard
     void *dev_blob = nullptr;            // the ONE device allocation
 };
 

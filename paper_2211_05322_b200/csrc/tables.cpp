@@ -473,8 +473,13 @@ rs_status build_tables(Plan *P) {
     OpTables &X = P->op[RS_OP_EXECUTE], &PK = P->op[RS_OP_PACK], &UP = P->op[RS_OP_UNPACK];
     for (OpTables *o : {&X, &PK, &UP}) { o->tasks.clear(); o->dsts.clear(); o->segs.clear(); }
 
+    const bool sharded = !P->src_owner.empty();               // multi-process executor: only this rank's unit tasks
+    int64_t my_read = 0, my_write = 0;
     for (int i : P->exec_order) {                              // slice-id order, or the schedule's (S3.2)
         const Slice &S = P->slices[(size_t)i];
+        if (sharded && P->src_owner[(size_t)S.sender] != P->rank) continue;
+        my_read += S.elems * e;
+        my_write += S.elems * e * (int64_t)S.receivers.size();
         int64_t lo_s[RS_MAX_NDIM], hi_s[RS_MAX_NDIM], ext[RS_MAX_NDIM], dense[RS_MAX_NDIM];
         device_box(A, S.sender, lo_s, hi_s);
         for (int d = 0; d < N; d++) ext[d] = S.hi[d] - S.lo[d];
@@ -598,6 +603,21 @@ rs_status build_tables(Plan *P) {
         for (const RsTask &T : LG.tasks) lg += T.run_bytes * task_rows(T);
         if ((st = finish_op(P, &LS, ls, ls)) != RS_OK) return st;
         if ((st = finish_op(P, &LG, lg, lg)) != RS_OK) return st;
+    }
+    P->used_dst.assign((size_t)B.n_dev, 0);
+    for (const RsDst &D : X.dsts) P->used_dst[(size_t)D.buf] = 1;
+    if (sharded) {
+        // A rank of the multi-process executor runs reshard_execute only: its share of the unit tasks, written to
+        // local and peer-mapped destination shards.  pack / unpack / the host pipeline belong to single-process plans.
+        PK.tasks.clear(); PK.dsts.clear(); UP.tasks.clear(); UP.dsts.clear();
+        OpTables &H = P->op[RS_OP_SLABS];
+        H.tasks.clear(); H.dsts.clear(); H.segs.clear(); H.info = rs_op_info{};
+        P->slabs.clear();
+        P->used_src.assign((size_t)A.n_dev, 0);
+        for (const RsTask &T : X.tasks) P->used_src[(size_t)T.src_buf] = 1;
+        if ((st = finish_op(P, &X, my_read, my_write, false, true)) != RS_OK) return st;
+        if ((st = finish_op(P, &PK, 0, 0)) != RS_OK) return st;
+        return finish_op(P, &UP, 0, 0);
     }
     if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
     if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B, false, true)) != RS_OK) return st;

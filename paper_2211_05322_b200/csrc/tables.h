@@ -114,6 +114,9 @@ RS_HD uint32_t rs_find_seg(const RsSeg *segs, uint32_t n_segs, uint32_t t) {
 // byte offsets of linear row `row` of a task's box over row dims first..nd-1 (row counted in those dims only)
 RS_HD void rs_row_offsets(const RsTask &T, int first, uint32_t row, int64_t *so, int64_t *doff) {
     int64_t s = 0, d = 0;
+#if defined(__CUDA_ARCH__)
+#pragma unroll 1                         // off the critical path (once per tile, 32 tiles at a time): keep the code small
+#endif
     for (int i = first; i < T.nd; i++) {
         const uint32_t e = T.ext[i], q = row / e, c = row - q * e;
         row = q;

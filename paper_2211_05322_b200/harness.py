@@ -7,8 +7,10 @@ from . import inputs
 from . import reshard as rs
 
 
-def make_plan(w, flags=0):
-    return rs.Plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, flags)
+def make_plan(w, flags=0, tuning=None):
+    """tuning: dict of rs_tuning fields (A/B runs of bench.py), None = the library's launch shapes"""
+    return rs.Plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, flags,
+                   dict(tuning=tuning) if tuning else None)
 
 
 def device_inputs(w, plan, device):

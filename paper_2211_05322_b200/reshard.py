@@ -32,6 +32,7 @@ SYMBOLS = [
     "reshard_plan", "reshard_plan_ex", "reshard_plan_group", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables", "reshard_op_tiles",
     "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
     "reshard_plan_message", "reshard_execute", "reshard_execute_strategy", "reshard_pack", "reshard_unpack", "reshard_execute_host",
+    "reshard_ipc_export", "reshard_ipc_import", "reshard_ipc_release_all",
     "reshard_host_workspace_bytes", "reshard_pipeline_simulate", "reshard_pipeline_least_delay", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
     "reshard_version",
 ]
@@ -64,7 +65,8 @@ class Tuning(C.Structure):
 class PlanOpts(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("schedule", C.c_int32), ("src_devices_per_host", C.c_int32),
                 ("dst_devices_per_host", C.c_int32), ("trials", C.c_int32), ("max_ctas", C.c_int32),
-                ("node_budget", C.c_int64), ("seed", C.c_uint64), ("tuning", C.POINTER(Tuning))]
+                ("node_budget", C.c_int64), ("seed", C.c_uint64), ("tuning", C.POINTER(Tuning)),
+                ("src_owner", C.POINTER(C.c_int32)), ("rank", C.c_int32), ("reserved", C.c_int32)]
 
 
 class ScheduleInfo(C.Structure):
@@ -143,6 +145,27 @@ def _ptrs(addrs):
     return (C.c_void_p * len(addrs))(*[C.c_void_p(int(a) if a else None) for a in addrs])
 
 
+RS_IPC_HANDLE_BYTES = 80
+
+
+def ipc_export(dev_ptr):
+    """reshard_ipc_export: bytes to send to the peers for a device pointer of this process"""
+    buf = C.create_string_buffer(RS_IPC_HANDLE_BYTES)
+    _chk(_lib().reshard_ipc_export(C.c_void_p(int(dev_ptr)), buf))
+    return buf.raw
+
+
+def ipc_import(handle):
+    """reshard_ipc_import: device pointer, valid in this process, of another process's exported pointer"""
+    out = C.c_void_p()
+    _chk(_lib().reshard_ipc_import(C.create_string_buffer(bytes(handle), RS_IPC_HANDLE_BYTES), C.byref(out)))
+    return int(out.value)
+
+
+def ipc_release_all():
+    _chk(_lib().reshard_ipc_release_all())
+
+
 def version():
     return _lib().reshard_version().decode()
 
@@ -166,7 +189,11 @@ class Plan:
         else:
             opts = dict(opts)
             tune = opts.pop("tuning", None)
+            owner = opts.pop("src_owner", None)
             o = PlanOpts(flags=flags, **opts)
+            if owner is not None:                                    # multi-process executor: rank = opts["rank"]
+                arr = _i32(owner)
+                o.src_owner = C.cast(arr, C.POINTER(C.c_int32))
             if tune:
                 t = Tuning(**tune)                                   # the plan copies it
                 o.tuning = C.pointer(t)

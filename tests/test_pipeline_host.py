@@ -52,6 +52,9 @@ def test_least_delay_and_bad_arguments():
     for stage in (1, 2, 3):
         for c in (0, 1, 2, 3, 5, 9):
             assert rs.pipeline_least_delay(rs.RS_PIPE_EAGER_1F1B, 4, stage, 16, 2, 4, 2, c) == pp.least_delay("eager", 4, stage, 16, 2, 4, 2, c)
+    # a transfer no delay can cover: the oracle answers with its search limit 2 M, the library says so with -1
+    assert pp.least_delay("eager", 4, 1, 4, 2, 4, 2, 10 ** 6) == 8
+    assert rs.pipeline_least_delay(rs.RS_PIPE_EAGER_1F1B, 4, 1, 4, 2, 4, 2, 10 ** 6) == -1
     with pytest.raises(rs.ReshardError):
         rs.pipeline_simulate(rs.RS_PIPE_1F1B, 0, 4, 1, 2, 0, 0)
     with pytest.raises(rs.ReshardError):

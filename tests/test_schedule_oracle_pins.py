@@ -76,7 +76,7 @@ def test_paper_narrative_cases_1_2_8():
 
 @pytest.mark.parametrize("case", [3, 4, 5, 9])
 def test_paper_narrative_congested_cases(case):
-    """PAPER.md:306, 320: naive and load-balance-only are congested, the ensemble leaves no host idle."""
+    """PAPER.md:282, 320: naive and load-balance-only are congested, the ensemble leaves no host idle."""
     ht = table2_hosts(case)
     T = ht[0]["T"]
     opt = G["case%d_optimum" % case][0] * T
