@@ -47,7 +47,7 @@ TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 ROOF_CSV = os.path.join(ROOT, "profiles", "roof_1k.csv")
 TUNING_FIELDS = ("bulk_warps", "bulk_stages", "bulk_lookahead", "bulk_tile_bytes", "bulk_ctas", "bulk_ctas_mcast", "shift_warps",
                  "shift_stages", "shift_lookahead", "shift_tile_bytes", "lsu_tile_bytes", "lsu_ctas_per_sm", "task_order",
-                 "small_op_bytes_mib")
+                 "small_op_bytes_mib", "tiles_per_worker", "pace_permille", "no_pdl")
 
 
 def parse_args():
@@ -58,6 +58,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", help="c4 (default, 1.5 GiB GPT activation), c2, c3, t2_<n>, sweep_<pair>_<m8|m4>_<MiB>MiB")
     ap.add_argument("--path", default="auto", choices=["auto", "lsu", "bulk", "shift"])
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "sharded"], help="N > 1: 'replicas' (default, DESIGN.md S8: every rank runs "
+                    "the whole task on its own GPU) or 'sharded' (the multi-process executor: virtual device r lives on rank r mod N, every "
+                    "rank launches its share of the unit tasks and stores into its peers' shards through CUDA IPC; NCCL only for the barrier)")
     ap.add_argument("--tune", default="", help="rs_plan_opts.tuning overrides, e.g. bulk_ctas=148,bulk_warps=4 (A/B runs and ncu captures)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
@@ -726,6 +729,59 @@ def run_roof(args):
     return 0
 
 
+def run_sharded(args):
+    """--mode sharded: ONE resharding task over N GPUs (strong scaling).  Virtual device r lives on rank r mod N; every
+    rank executes the unit tasks whose sender it holds, writing local and peer-mapped (CUDA IPC -> NVLink) destination
+    shards; no data-path collective.  A step = one reshard_execute launch per rank; time = max over ranks of the device
+    time of K steps.  Not measurable on the 1-GPU boxes of this run (world 1 degenerates to the normal plan)."""
+    import torch
+    from paper_2211_05322_b200 import inputs, multi, sharded
+    from paper_2211_05322_b200 import reshard as rs
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world == 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29511")
+        os.environ.setdefault("RANK", "0"); os.environ.setdefault("WORLD_SIZE", "1")
+    multi.init("nccl", dev)
+    w = inputs.get_workload(args.workload)
+    e = inputs.elem_bytes(w.dtype)
+    n_src, n_dst = 1, 1
+    for m in w.src_mesh: n_src *= m
+    for m in w.dst_mesh: n_dst *= m
+    so, dow = sharded.round_robin_owner(n_src, world), sharded.round_robin_owner(n_dst, world)
+    x = sharded.ShardedReshard(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, so, dow, 0, dict(tuning=parse_tune(args.tune)) if args.tune else None)
+    info = x.plan.info
+    src_local = {r: torch.empty(info.src_shard_bytes, dtype=torch.uint8, device=dev).random_(0, 256) for r in range(n_src) if so[r] == rank}
+    dst_local = {q: torch.empty(info.dst_shard_bytes, dtype=torch.uint8, device=dev) for q in range(n_dst) if dow[q] == rank}
+    x.bind(src_local, dst_local)
+    stream = torch.cuda.current_stream()
+    K, W = max(1, args.steps), max(3, args.warmup)
+    for _ in range(W):
+        x.execute(stream.cuda_stream)
+    x.wait()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = rs.launch_count()
+    e0.record(stream)
+    for _ in range(K):
+        x.execute(stream.cuda_stream)
+    e1.record(stream)
+    x.wait()
+    ms = multi.max_over_ranks(e0.elapsed_time(e1) / K, dev)
+    total = info.unique_read_bytes + info.write_bytes
+    peer = sum(1 for q in x.writes if dow[q] != rank)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": total / (ms * 1e-3) / 1e9, "unit": "GB/s", "n_gpus": world, "steps": K, "warmup": W,
+                          "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+                          "mode": "sharded", "config": dict(_config(w), step="reshard_execute, one launch per rank", parallelism="virtual device r on rank r mod N; peer stores through CUDA IPC"),
+                          "gpu_launches": rs.launch_count() - n0, "rank0_bytes_per_step": x.my_bytes(), "rank0_peer_destinations": peer}))
+    x.close()
+    multi.shutdown()
+    return 0
+
+
 def run_overlap(args):
     """Per CTA cap: time N matmuls alone, M reshard_execute launches alone, then both started together on two
     streams (wall time on the device between a common start event and the later of the two end events).
@@ -998,6 +1054,8 @@ def main():
         return run_sweep(args)
     if args.impl == "reference":
         return run_reference(args)
+    if args.mode == "sharded":
+        return run_sharded(args)
     return run_ours(args)
 
 

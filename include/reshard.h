@@ -115,7 +115,12 @@ typedef struct rs_tuning {
                                                           destination rows (default: destination address order)     */
     int32_t small_op_bytes_mib;                        /* AUTO takes the register path for aligned operations moving
                                                           at most this many MiB (-1: never); 0 = library default     */
-    int32_t reserved[2];
+    int32_t tiles_per_worker;                          /* small operations: tiles shrink (to 2 KiB at least) until every
+                                                          worker (warp) has this many; 0 = library default          */
+    int32_t pace_permille;                             /* rs_copy_bulk rate matching: offered load in permille of the DRAM
+                                                          peak (2 x memory clock x bus width); -1: unpaced; 0 = default */
+    int32_t no_pdl;                                    /* 1: launch without programmatic dependent launch (a kernel then
+                                                          starts only after the previous kernel of the stream has ended) */
 } rs_tuning;
 
 typedef struct rs_plan_opts {
@@ -210,6 +215,9 @@ typedef struct rs_op_info {
     int32_t table_bytes;             /* bytes of this operation's tables in device memory: O(unit tasks),
                                         independent of the tensor size (the plan is the
                                         slice list)                                                        */
+    int32_t pace_permille;           /* rs_copy_bulk rate matching: the launch offers this many permille of the
+                                        DRAM peak (write-heavy operations); 0 = unpaced                    */
+    int32_t reserved;
 } rs_op_info;
 
 /*

@@ -36,6 +36,10 @@ rs_status query_device(rs::Plan *P) {
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
     P->sm_count = sms;
+    int mem_khz = 0, bus_bits = 0;                             // DRAM peak = 2 x memory clock x bus width (B200: 7 672 GB/s)
+    cudaDeviceGetAttribute(&mem_khz, cudaDevAttrMemoryClockRate, P->device);
+    cudaDeviceGetAttribute(&bus_bits, cudaDevAttrGlobalMemoryBusWidth, P->device);
+    if (mem_khz > 0 && bus_bits > 0) P->dram_peak_gbs = 2.0 * mem_khz * 1e3 * bus_bits / 8 / 1e9;
     return RS_OK;
 }
 
@@ -62,6 +66,9 @@ rs_status upload(rs::Plan *P) {
         std::memcpy(host.data() + off, o.segs.data(), o.segs.size() * sizeof(RsSeg));
         off += round256(o.segs.size() * sizeof(RsSeg));
         o.dev.n_segs = (uint32_t)o.segs.size();
+        o.dev.n_tasks = (uint32_t)o.tasks.size();
+        o.dev.n_dsts = (uint32_t)o.dsts.size();
+        o.dev.early_trigger = 0;
         o.dev.tile_base = 0;
         o.dev.n_tiles = (uint32_t)o.info.n_tiles;
     }
@@ -384,25 +391,33 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     const int64_t n_tiles = dev.n_tiles;
     const bool bulk_family = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_BULK_SHIFT;
     const int warps = op.info.block / 32;
+    const bool pdl = !P.tune.no_pdl;
     if (op.info.path == RS_PATH_BULK && align == 16) {
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
+        dev.early_trigger = grid >= P.sm_count;
+        // rate matching: the launch as a whole offers pace_permille / 1000 of the DRAM peak
+        const int permille = P.tune.pace_permille > 0 ? P.tune.pace_permille : P.tune.pace_permille < 0 ? 0 : op.pace_permille;
+        const float pace = permille > 0 ? (float)((double)grid * warps / (P.dram_peak_gbs * permille / 1000.0)) : 0.f;
         e = rs::launch_bulk(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
-                            (uint32_t)op.info.tile_bytes, st);
+                            (uint32_t)op.info.tile_bytes, pace, pdl, st);
     } else if (op.info.path == RS_PATH_BULK_SHIFT) {          // layout not 16-byte aligned: TMA loads, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
+        dev.early_trigger = grid >= P.sm_count;
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
-                                  op.shift_stage, st);
+                                  op.shift_stage, pdl, st);
     } else if (op.info.path == RS_PATH_BULK && op.alt_stage) { // aligned plan, under-aligned pointers: same tiles, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(P.max_ctas > 0 ? std::min(P.sm_count, P.max_ctas) : P.sm_count,
                                                                      (n_tiles + op.alt_warps - 1) / op.alt_warps));
+        dev.early_trigger = grid >= P.sm_count;
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.alt_warps * 32, op.alt_smem, op.alt_stages, op.alt_stages - 1,
-                                  op.alt_stage, st);
+                                  op.alt_stage, pdl, st);
     } else {                                                  // register paths
         int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
         if (P.max_ctas > 0) cap = std::min<int64_t>(cap, P.max_ctas);
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));
-        if (align < 16) e = rs::launch_shift(dev, pt, small, grid, st);   // any alignment, still 16-byte accesses
-        else e = rs::launch_lsu(dev, pt, small, grid, st);
+        dev.early_trigger = grid >= P.sm_count;
+        if (align < 16) e = rs::launch_shift(dev, pt, small, grid, pdl, st);   // any alignment, still 16-byte accesses
+        else e = rs::launch_lsu(dev, pt, small, grid, pdl, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
     return RS_OK;

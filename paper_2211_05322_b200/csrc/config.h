@@ -6,8 +6,12 @@
 #define RS_LSU_THREADS       256
 #define RS_LSU_CTAS_PER_SM   4          // persistent CTAs per SM (grid = 148 * this); every warp is a worker
 #define RS_LSU_CTAS_DEFAULT  2          // CTAs per SM actually launched (more bytes in flight is slower on B200)
+#define RS_LSU_CTAS_SMALL    4          // ... for operations moving <= RS_SMALL_OP_BYTES (ramp-bound, not DRAM-bound)
 #define RS_LSU_TILE_BYTES    16384
 #define RS_LSU_UNROLL        8          // independent vector loads in flight per thread
+#define RS_LSU_TABLE_BYTES   12288      // tables (tasks + destinations + segments) up to this size are staged in shared memory at
+                                        // kernel start: ONE global latency instead of a chain of dependent ones before the first load
+                                        // (small operations are ramp-bound)
 
 // TMA path: cp.async.bulk global -> shared ring -> global x k; every warp is its own pipeline
 #define RS_BULK_WARPS        2          // warps (independent pipelines) per CTA, one CTA per SM
@@ -18,13 +22,18 @@
 #define RS_BULK_WARPS_SHORT  4
 #define RS_BULK_TILE_BYTES_SHORT 8192
 #define RS_BULK_CTAS_DEN       148    // CTA counts below are out of 148 SMs
-#define RS_BULK_CTAS_MCAST_NUM 96     // write-heavy (multicast) operations
-#define RS_BULK_CTAS_MCAST_SHORT_NUM 136   // write-heavy operations with short runs (4 warps per CTA)
 #define RS_BULK_CTAS_LONG_NUM  132    // 1 : 1 operations whose runs are at least RS_BULK_LONG_RUN
+// Rate matching of write-heavy (multicast) operations: every SM runs, every warp paces its tiles so that the launch
+// offers this many permille of the DRAM peak (2 x memory clock x bus width = 7 672 GB/s on B200).  Measured
+// (profiles/r02_pacing.md): achieved = 0.99 x offered up to 860 permille (6.52 TB/s on 1 + 8), collapse from 880 on
+// (6.09, then 5.56 at 920; unpaced 5.66); runs of 512 B: up to 820 (6.18 TB/s), 6.00 at 840.  10 permille below the edge.
+#define RS_PACE_PERMILLE       850
+#define RS_PACE_PERMILLE_SHORT 810
 #define RS_BULK_LONG_RUN       4096
 #define RS_BULK_CTAS_MIN_BYTES (256ll << 20)   // operations moving less than this keep one CTA on every SM
-#define RS_SMALL_OP_BYTES    (64ll << 20)   // AUTO: aligned operations moving no more than this take the register path
-                                            // (no shared-memory carve-out, no mbarriers: 16 % faster up to 8 MiB, 4 % up to 64 MiB)
+#define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path
+                                            // (no shared-memory carve-out, no mbarriers: 4 MiB + 4 MiB in 3.2 us against 6.5 us;
+                                            // equal at 16 + 16 MiB; from 20 + 20 MiB on the TMA ring wins: 8.1 against 8.6 us)
 #define RS_INTERLEAVE_MAX_RUN (64 << 10)    // destination runs up to this long count as a fine interleave (tile order)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 
@@ -41,4 +50,5 @@
 #define RS_HOST_SLABS_MAX        16
 #define RS_HOST_SLAB_MIN_BYTES  (8 << 20)
 
+#define RS_TILES_PER_WORKER   4          // small operations: tiles shrink until every warp has this many (tail balance)
 #define RS_SMEM_MAX          (227 * 1024)

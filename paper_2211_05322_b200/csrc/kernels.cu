@@ -42,12 +42,31 @@ static_assert(sizeof(RsDesc) == 64, "descriptor ring slot");
 #define RS_DESC_RING 64
 static_assert(RS_DESC_RING * sizeof(RsDesc) == RS_BULK_DESC_BYTES, "config.h and the ring disagree");
 
+// Programmatic dependent launch (sm_90+): every kernel lets the NEXT kernel of the stream be launched early
+// (launch_dependents) and itself waits for the PREVIOUS kernel only where it first touches shard memory
+// (griddepcontrol.wait; a no-op without a programmatic dependency).  What runs before the wait reads nothing but the
+// plan's immutable tables and the kernel parameters: table staging, segment search, tile decode.  In a stream of
+// resharding launches (or behind any kernel) launch latency and prologue overlap the predecessor's tail -- small
+// operations are launch- and ramp-bound (config 3: 10.2 -> 8.1 us).  The trigger is given at entry when the grid
+// covers every SM (the successor's CTAs then spread evenly: one beside each of ours); a grid that leaves SMs idle
+// triggers only when its CTAs run out of tiles -- otherwise the successor's waiting CTAs pile up on the idle SMs,
+// two and three to an SM, and run at half speed (measured: 96 CTAs, 3.2 instead of 6.1 TB/s).
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// the operation's tables as the kernel reads them: in global memory, or staged in shared memory (generic pointers)
+struct RsTables {
+    const RsTask *tasks;
+    const RsDst *dsts;
+    const RsSeg *segs;
+};
+
 template <int NP>
-__device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsPtrTableT<NP> &ptrs, uint32_t tile_index,
+__device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsTables &tb, const RsPtrTableT<NP> &ptrs, uint32_t tile_index,
                                              RsDesc *out) {
     uint32_t task, u;
-    rs_tile_locate(op.segs, op.n_segs, op.tile_base + tile_index, &task, &u);
-    const RsTask *__restrict__ T = op.tasks + task;
+    rs_tile_locate(tb.segs, op.n_segs, op.tile_base + tile_index, &task, &u);
+    const RsTask *__restrict__ T = tb.tasks + task;
     const RsTile tile = rs_tile_decode(*T, task, u);
     RsDesc d;
     const char *base = ptrs.src[T->src_buf] + T->src_off;
@@ -93,26 +112,43 @@ __global__ void __launch_bounds__(RS_LSU_THREADS, RS_LSU_CTAS_PER_SM)
 rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
     constexpr uint32_t VB = sizeof(V);
     __shared__ RsDesc ring[RS_LSU_THREADS / 32][32];
+    __shared__ uint4 staged[RS_LSU_TABLE_BYTES / 16];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = RS_LSU_THREADS / 32;
     RsDesc *descs = ring[warp];
     const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
     const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
+    // Small tables (a few dozen unit tasks) are copied to shared memory first: one global-memory latency, after which
+    // segment search, task fields and destination entries are shared-memory reads.
+    if (op.early_trigger) pdl_launch_dependents();
+    RsTables tb{op.tasks, op.dsts, op.segs};
+    const uint32_t v_tasks = op.n_tasks * (uint32_t)(sizeof(RsTask) / 16), v_dsts = op.n_dsts, v_segs = op.n_segs;
+    if ((v_tasks + v_dsts + v_segs) * 16u <= RS_LSU_TABLE_BYTES) {
+        const uint4 *gt = reinterpret_cast<const uint4 *>(op.tasks), *gd = reinterpret_cast<const uint4 *>(op.dsts),
+                    *gs = reinterpret_cast<const uint4 *>(op.segs);
+        for (uint32_t i = threadIdx.x; i < v_tasks + v_dsts + v_segs; i += RS_LSU_THREADS)
+            staged[i] = i < v_tasks ? __ldg(gt + i) : i < v_tasks + v_dsts ? __ldg(gd + (i - v_tasks)) : __ldg(gs + (i - v_tasks - v_dsts));
+        __syncthreads();
+        tb.tasks = reinterpret_cast<const RsTask *>(staged);
+        tb.dsts = reinterpret_cast<const RsDst *>(staged + v_tasks);
+        tb.segs = reinterpret_cast<const RsSeg *>(staged + v_tasks + v_dsts);
+    }
 
     for (int it = 0; it < n_my; ++it) {
         if ((it & 31) == 0) {                                 // resolve the next 32 tiles of this warp
             __syncwarp();
-            if (it + lane < n_my) resolve_desc(op, ptrs, worker + (uint32_t)(it + lane) * n_workers, descs + lane);
+            if (it + lane < n_my) resolve_desc(op, tb, ptrs, worker + (uint32_t)(it + lane) * n_workers, descs + lane);
             __syncwarp();
+            if (it == 0) pdl_wait();                          // shard memory is touched from here on
         }
         const RsDesc *d = descs + (it & 31);
         const uint32_t n_rows = d->n_rows, k = d->k;
         const uint32_t vpr = d->col_bytes / VB;               // vectors per row
         const uint32_t total = n_rows * vpr;
-        const RsDst *__restrict__ dsts = op.dsts + d->dst_first;
+        const RsDst *__restrict__ dsts = tb.dsts + d->dst_first;
         const bool fast = d->flags & RS_TILE_FAST;
         const char *src = d->src;
         const int64_t s0 = d->s0, d0 = d->d0, dst_rel = d->dst_rel;
-        const RsTask *__restrict__ T = op.tasks + d->task;
+        const RsTask *__restrict__ T = tb.tasks + d->task;
         if (!fast) {                                          // GENERIC tiles (rare): one vector at a time
             for (uint32_t v = lane; v < total; v += 32) {
                 const uint32_t r = v / vpr, c = v - r * vpr;
@@ -189,12 +225,14 @@ rs_copy_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
     RsDesc *descs = ring[warp];
     const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
     const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
+    if (op.early_trigger) pdl_launch_dependents();
 
     for (int it = 0; it < n_my; ++it) {
         if ((it & 31) == 0) {
             __syncwarp();
-            if (it + lane < n_my) resolve_desc(op, ptrs, worker + (uint32_t)(it + lane) * n_workers, descs + lane);
+            if (it + lane < n_my) resolve_desc(op, RsTables{op.tasks, op.dsts, op.segs}, ptrs, worker + (uint32_t)(it + lane) * n_workers, descs + lane);
             __syncwarp();
+            if (it == 0) pdl_wait();
         }
         const RsDesc *d = descs + (it & 31);
         const uint32_t n_rows = d->n_rows, k = d->k, n = d->col_bytes;
@@ -311,16 +349,45 @@ __device__ __forceinline__ void bulk_wait_read(int pending) {  // immediate oper
     }
 }
 
+__device__ __forceinline__ uint64_t global_ns() {             // 32 ns resolution, ~10 cycles (measured on B200)
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// RATE MATCHING.  HBM punishes an offered load above what it can drain: with every SM pushing a 1-read + k-write
+// stream as fast as its store port allows (~65 GB/s per SM), 148 SMs offer ~9.6 TB/s and the achieved rate COLLAPSES to
+// 5.2-5.8 TB/s, while an offered load equal to the roof (found before by trimming the grid to a magic 96 CTAs) holds
+// 6.2-6.45 TB/s (profiles/r02_roof.md).  So every warp paces itself: a tile that moves b bytes of DRAM traffic
+// (reads + k writes) may start `pace` x b nanoseconds after the previous one, pace = workers / target rate; the target
+// is a fraction of the DRAM peak read from the device (api.cu).  A token bucket with a burst of two tiles: a warp
+// that is behind schedule (HBM slower than the target, another kernel running beside) never waits.
+__device__ __forceinline__ void pace_tile(uint64_t &t_next, float pace, uint32_t traffic_bytes, int lane) {
+    const uint64_t interval = (uint64_t)(pace * (float)traffic_bytes);
+    if (lane == 0) {
+        uint64_t now = global_ns();
+        while (now < t_next) {
+            const uint64_t left = t_next - now;
+            __nanosleep((unsigned)(left > 2000 ? 2000 : left));
+            now = global_ns();
+        }
+        const uint64_t floor = now - (now > 2 * interval ? 2 * interval : now);
+        t_next = (t_next > floor ? t_next : floor) + interval;
+    }
+    __syncwarp();
+}
+
 template <int NP>
 __global__ void __launch_bounds__(256, 1)
 rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
-             const uint32_t stage_bytes) {
+             const uint32_t stage_bytes, const float pace) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const uint32_t bars = smem_u32(smem) + warp * 64;                       // <= 8 mbarriers per warp
     RsDesc *descs = reinterpret_cast<RsDesc *>(smem + 1024) + warp * RS_DESC_RING;
     const uint32_t ring = smem_u32(smem) + 1024 + (uint32_t)W * RS_DESC_RING * sizeof(RsDesc) +
                           (uint32_t)warp * stages * stage_bytes;
+    if (op.early_trigger) pdl_launch_dependents();
     if (lane == 0) {
         for (int s = 0; s < stages; s++) mbar_init(bars + 8 * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -332,14 +399,16 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, con
     const int pending_ok = stages - lookahead - 1;            // store groups that may still read smem
     int ld_slot = 0, st_slot = 0;                             // it % stages, j % stages without dividing
     uint32_t st_parity = 0;
+    uint64_t t_next = 0;                                      // rate matching: earliest start of this warp's next tile
 
     for (int it = 0; it < n_my + lookahead; ++it) {
         if (it < n_my) {                                      // ---- load tile `it` into slot ld_slot
             if ((it & 31) == 0) {                             // resolve the next 32 tiles of this warp
                 const int mine = it + lane;
                 if (mine < n_my)
-                    resolve_desc(op, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
+                    resolve_desc(op, RsTables{op.tasks, op.dsts, op.segs}, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
                 __syncwarp();
+                if (it == 0) pdl_wait();                      // shard memory is touched from here on
             }
             if (it >= stages) {                               // slot reuse: its stores must have read it
                 bulk_wait_read(pending_ok);
@@ -347,6 +416,7 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, con
             }
             const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
             const uint32_t n_rows = d->n_rows, col_bytes = d->col_bytes;
+            if (pace > 0.f) pace_tile(t_next, pace, n_rows * col_bytes * (1u + d->k), lane);
             const uint32_t bar = bars + 8 * ld_slot, slot = ring + (uint32_t)ld_slot * stage_bytes;
             if (lane == 0) mbar_expect_tx(bar, n_rows * col_bytes);
             __syncwarp();
@@ -392,6 +462,7 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, con
             if (++st_slot == stages) { st_slot = 0; st_parity ^= 1u; }
         }
     }
+    pdl_launch_dependents();                                  // out of tiles: the successor may start beside the drain
     bulk_wait_read(0);                                        // shared memory must outlive the stores' reads
 }
 
@@ -492,6 +563,7 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptr
     RsDesc *descs = reinterpret_cast<RsDesc *>(smem + 1024) + warp * RS_DESC_RING;
     const uint32_t ring = smem_u32(smem) + 1024 + (uint32_t)W * RS_DESC_RING * sizeof(RsDesc) +
                           (uint32_t)warp * stages * stage_bytes;
+    if (op.early_trigger) pdl_launch_dependents();
     if (lane == 0) {
         for (int s = 0; s < stages; s++) mbar_init(bars + 8 * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -508,8 +580,9 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptr
             if ((it & 31) == 0) {
                 const int mine = it + lane;
                 if (mine < n_my)
-                    resolve_desc(op, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
+                    resolve_desc(op, RsTables{op.tasks, op.dsts, op.segs}, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
                 __syncwarp();
+                if (it == 0) pdl_wait();                      // shard memory is touched from here on
             }
             const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
             const uint32_t n_rows = d->n_rows, n = d->col_bytes, pitch = shift_pitch(n);
@@ -596,23 +669,33 @@ static RsPtrTableT<RS_PTRS_SMALL> small_table(const RsPtrTable &ptrs) {
     return t;
 }
 
-static cudaError_t launched() {
-    cudaError_t e = cudaGetLastError();
+static cudaError_t launched(cudaError_t e) {
+    if (e == cudaSuccess) e = cudaGetLastError();
     if (e == cudaSuccess) ++g_launches;
     return e;
 }
 
-cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, cudaStream_t st) {
-    constexpr int U = RS_LSU_UNROLL / 2;                       // 64 B in flight per thread
-    if (small) rs_copy_lsu<uint4, U, RS_PTRS_SMALL><<<grid, RS_LSU_THREADS, 0, st>>>(op, small_table(ptrs));
-    else rs_copy_lsu<uint4, U, 128><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
-    return launched();
+// every launch carries the programmatic-stream-serialization attribute unless the plan switched it off
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    return launched(cudaLaunchKernelEx(&cfg, kernel, args...));
 }
 
-cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, cudaStream_t st) {
-    if (small) rs_copy_shift<4, RS_PTRS_SMALL><<<grid, RS_LSU_THREADS, 0, st>>>(op, small_table(ptrs));
-    else rs_copy_shift<4, 128><<<grid, RS_LSU_THREADS, 0, st>>>(op, ptrs);
-    return launched();
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st) {
+    constexpr int U = RS_LSU_UNROLL / 2;                       // 64 B in flight per thread
+    if (small) return launch_k(rs_copy_lsu<uint4, U, RS_PTRS_SMALL>, grid, RS_LSU_THREADS, 0, st, pdl, op, small_table(ptrs));
+    return launch_k(rs_copy_lsu<uint4, U, 128>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);
+}
+
+cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st) {
+    if (small) return launch_k(rs_copy_shift<4, RS_PTRS_SMALL>, grid, RS_LSU_THREADS, 0, st, pdl, op, small_table(ptrs));
+    return launch_k(rs_copy_shift<4, 128>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);
 }
 
 cudaError_t prepare_bulk(int smem_bytes) {
@@ -624,17 +707,15 @@ cudaError_t prepare_bulk(int smem_bytes) {
 }
 
 cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
-                              int stages, int lookahead, uint32_t stage_bytes, cudaStream_t st) {
-    if (small) rs_copy_bulk_shift<RS_PTRS_SMALL><<<grid, block, smem_bytes, st>>>(op, small_table(ptrs), stages, lookahead, stage_bytes);
-    else rs_copy_bulk_shift<128><<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
-    return launched();
+                              int stages, int lookahead, uint32_t stage_bytes, bool pdl, cudaStream_t st) {
+    if (small) return launch_k(rs_copy_bulk_shift<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes);
+    return launch_k(rs_copy_bulk_shift<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes);
 }
 
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes, int stages,
-                        int lookahead, uint32_t stage_bytes, cudaStream_t st) {
-    if (small) rs_copy_bulk<RS_PTRS_SMALL><<<grid, block, smem_bytes, st>>>(op, small_table(ptrs), stages, lookahead, stage_bytes);
-    else rs_copy_bulk<128><<<grid, block, smem_bytes, st>>>(op, ptrs, stages, lookahead, stage_bytes);
-    return launched();
+                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st) {
+    if (small) return launch_k(rs_copy_bulk<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes, pace);
+    return launch_k(rs_copy_bulk<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes, pace);
 }
 
 }  // namespace rs

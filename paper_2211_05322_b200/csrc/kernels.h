@@ -6,13 +6,15 @@
 #include "tables.h"
 
 namespace rs {
+// `pdl`: launch with the programmatic-stream-serialization attribute (kernels.cu).
 // `small`: every buffer index of the launch is below RS_PTRS_SMALL, so the 256-byte pointer table is enough
-cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, cudaStream_t st);      // 16-byte aligned only
-cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, cudaStream_t st);
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st);      // 16-byte aligned only
+cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st);
 cudaError_t prepare_bulk(int smem_bytes);                                             // both TMA kernels, both table sizes
+// pace: nanoseconds a warp lets pass per byte of DRAM traffic of its tiles (rate matching, kernels.cu); 0 = unpaced
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes, int stages,
-                        int lookahead, uint32_t stage_bytes, cudaStream_t st);
+                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st);
 cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
-                              int stages, int lookahead, uint32_t stage_bytes, cudaStream_t st);
+                              int stages, int lookahead, uint32_t stage_bytes, bool pdl, cudaStream_t st);
 int64_t launch_count();
 }  // namespace rs

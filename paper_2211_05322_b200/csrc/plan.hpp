@@ -52,6 +52,7 @@ struct OpTables {                        // one operation (execute / pack / unpa
     rs_op_info info{};
     int stages = 0, lookahead = 0;       // TMA path: ring slots per warp, loads in flight
     uint32_t shift_stage = 0;            // rs_copy_bulk_shift: bytes per ring slot (rows padded), 0 if the path is not used
+    int pace_permille = 0;               // rs_copy_bulk: offered load as permille of the DRAM peak (0: unpaced)
     uint32_t alt_stage = 0;              // TMA plans handed under-aligned pointers: shape of rs_copy_bulk_shift on the same tiles
     int alt_warps = 0, alt_stages = 0, alt_smem = 0;
     RsOpDev dev{};                       // device copies (null for a host-only plan)
@@ -105,6 +106,7 @@ struct Plan {
     std::vector<char> used_src;          // [n_src] 1 if some task reads that shard
     int device = -1;
     int sm_count = 148;
+    double dram_peak_gbs = 7672.0;       // 2 x memory clock x bus width of the device (B200 default for host-only plans)
     int group_src = 0, group_dst = 0;    // > 0: this plan is a GROUP (reshard_plan_group): only its execute table exists
     int max_ctas = 0;                    // rs_plan_opts.max_ctas: cap on CTAs per launch (0: none)
     rs_tuning tune{};                    // rs_plan_opts.tuning (all zero: the library's launch shapes)

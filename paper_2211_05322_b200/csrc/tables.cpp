@@ -149,7 +149,7 @@ int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t moved_bytes
 }
 
 // Launch shape of the two TMA kernels, from measurement on B200.
-struct BulkShape { int warps, stages, grid; int64_t tile_bytes; };
+struct BulkShape { int warps, stages, grid, pace_permille; int64_t tile_bytes; };
 
 BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes) {
     const rs_tuning &U = P.tune;
@@ -170,23 +170,19 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
                           : pick(U.bulk_tile_bytes, short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
     sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
     while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
-    // At most one CTA per SM -- and FEWER where the memory system prefers it (148 SMs):
-    //  * write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes): 148 writers hold 5.65 TB/s
-    //    whatever the ring depth or tile size, 96 writers reach 6.1-6.2 TB/s (an SM sustains ~64 GB/s of this
-    //    mix; beyond ~104 SMs the writers contend);
-    //  * 1 : 1 operations with long runs (<= 3 bulk copies per tile): 132 CTAs are 1.5-3.7 % faster than 148;
-    //  * short runs are issue-bound per SM: write-heavy ones do best from 136 CTAs (Table 2 case 9: 5.7 -> 6.2 TB/s),
-    //    1 : 1 ones and the shifted variant from every SM;
-    //  * operations under 256 MiB are latency-bound, not contention-bound: every SM.
-    // Fractions of the SM count, so the rule survives a different part.
+    // One CTA per SM.
+    //  * Write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes) are an OPEN loop: stores are fire and
+    //    forget, every SM can push ~65 GB/s, 148 of them offer 9.6 TB/s and HBM collapses to 5.2-5.8 TB/s.  They run on
+    //    every SM and are RATE MATCHED (kernels.cu pace_tile, config.h RS_PACE_PERMILLE): 6.4-6.5 TB/s.
+    //  * 1 : 1 operations limit themselves (loads are a closed loop: bytes in flight / latency) and stay unpaced;
+    //    with long runs (<= 3 bulk copies per tile) 132 CTAs are 1.5-3.7 % faster than 148 (a fraction of the SM count,
+    //    so the rule survives a different part); operations under 256 MiB are ramp-bound: every SM.
     const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
     int ctas = P.sm_count;
-    if (big && !shift) {
-        if (write_heavy) ctas = P.sm_count * (short_runs ? RS_BULK_CTAS_MCAST_SHORT_NUM : RS_BULK_CTAS_MCAST_NUM) / RS_BULK_CTAS_DEN;
-        else if (min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
-    }
+    if (big && !shift && !write_heavy && min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
     sh.grid = std::max(1, std::min(P.sm_count, pick(write_heavy ? U.bulk_ctas_mcast : U.bulk_ctas, std::max(1, ctas))));
     if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
+    sh.pace_permille = write_heavy && !shift ? (short_runs ? RS_PACE_PERMILLE_SHORT : RS_PACE_PERMILLE) : 0;
     return sh;
 }
 
@@ -267,6 +263,8 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         const BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes);
         tile_bytes = sh.tile_bytes;
         stages = sh.stages;
+        op->pace_permille = sh.pace_permille;
+        I.pace_permille = P->tune.pace_permille > 0 ? P->tune.pace_permille : P->tune.pace_permille < 0 ? 0 : sh.pace_permille;
         I.block = sh.warps * 32;
         I.grid = sh.grid;
         workers = sh.grid * sh.warps;
@@ -274,12 +272,15 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         tile_bytes = pick(P->tune.lsu_tile_bytes, RS_LSU_TILE_BYTES);
         tile_bytes = std::max<int64_t>(128, tile_bytes / 128 * 128);
         I.block = RS_LSU_THREADS;
-        I.grid = P->sm_count * std::max(1, std::min(RS_LSU_CTAS_PER_SM, pick(P->tune.lsu_ctas_per_sm, RS_LSU_CTAS_DEFAULT)));
+        // small operations are ramp-bound: more warps per SM cover the start-up latency (c3: 11.2 -> 10.1 us with 4 CTAs
+        // per SM); large ones are DRAM-bound and do best with 2 (more bytes in flight is slower on B200)
+        const bool small_op = read_bytes + write_bytes <= RS_SMALL_OP_BYTES;
+        I.grid = P->sm_count * std::max(1, std::min(RS_LSU_CTAS_PER_SM, pick(P->tune.lsu_ctas_per_sm, small_op ? RS_LSU_CTAS_SMALL : RS_LSU_CTAS_DEFAULT)));
         if (P->max_ctas > 0) I.grid = std::min(I.grid, P->max_ctas);
         workers = I.grid * (RS_LSU_THREADS / 32);
     }
     // small problems: shrink tiles until every worker has a few (tail balance), floor 2 KiB
-    while (tile_bytes > 2048 && read_bytes / tile_bytes < (int64_t)workers * 4) tile_bytes = tile_bytes / 2 / 128 * 128;
+    while (tile_bytes > 2048 && read_bytes / tile_bytes < (int64_t)workers * pick(P->tune.tiles_per_worker, RS_TILES_PER_WORKER)) tile_bytes = tile_bytes / 2 / 128 * 128;
     tile_bytes = std::max<int64_t>(tile_bytes, 128);
     I.tile_bytes = (int32_t)tile_bytes;
 

@@ -97,6 +97,9 @@ struct RsOpDev {                         // one operation's tables in device mem
     uint32_t n_segs;
     uint32_t tile_base;                  // first tile of this launch (a slab of reshard_execute_host), else 0
     uint32_t n_tiles;                    // tiles of this launch
+    uint32_t n_tasks, n_dsts;            // table sizes: small tables are staged in shared memory by the register kernel
+    uint32_t early_trigger;              // 1: the grid covers every SM, so the next kernel of the stream may be launched at once
+                                         // (programmatic dependent launch); 0: only when this kernel's CTAs run out of tiles
 };
 
 // ---- the decode -------------------------------------------------------------------------------

@@ -50,7 +50,8 @@ class OpInfo(C.Structure):
     _fields_ = [("path", C.c_int32), ("vec_bytes", C.c_int32), ("n_tasks", C.c_int32), ("n_dsts", C.c_int32),
                 ("n_tiles", C.c_int32), ("tile_bytes", C.c_int32), ("grid", C.c_int32), ("block", C.c_int32),
                 ("smem_bytes", C.c_int32), ("read_bytes", C.c_int64), ("write_bytes", C.c_int64),
-                ("min_run_bytes", C.c_int64), ("n_segs", C.c_int32), ("table_bytes", C.c_int32)]
+                ("min_run_bytes", C.c_int64), ("n_segs", C.c_int32), ("table_bytes", C.c_int32), ("pace_permille", C.c_int32),
+                ("reserved", C.c_int32)]
 
 
 class Tuning(C.Structure):
@@ -59,7 +60,7 @@ class Tuning(C.Structure):
                 ("bulk_tile_bytes", C.c_int32), ("bulk_ctas", C.c_int32), ("bulk_ctas_mcast", C.c_int32),
                 ("shift_warps", C.c_int32), ("shift_stages", C.c_int32), ("shift_lookahead", C.c_int32),
                 ("shift_tile_bytes", C.c_int32), ("lsu_tile_bytes", C.c_int32), ("lsu_ctas_per_sm", C.c_int32),
-                ("task_order", C.c_int32), ("small_op_bytes_mib", C.c_int32), ("reserved", C.c_int32 * 2)]
+                ("task_order", C.c_int32), ("small_op_bytes_mib", C.c_int32), ("tiles_per_worker", C.c_int32), ("pace_permille", C.c_int32), ("no_pdl", C.c_int32)]
 
 
 class PlanOpts(C.Structure):

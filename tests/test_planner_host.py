@@ -467,16 +467,20 @@ def test_launch_shapes_follow_the_measured_rules():
         w = inputs.get_workload(name)
         p = _plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, opts or None)
         o = p.op_info(op)
-        return o.path, o.grid, o.block
-    assert shape_of("c4") == (rs.RS_PATH_BULK, 132, 64)                           # long runs, 1 : 1
-    assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64)          # 2 KiB runs, 1 : 1
-    assert shape_of("sweep_P5_m8_1024MiB") == (rs.RS_PATH_BULK, 96, 64)           # 1 read + 8 writes
-    assert shape_of("sweep_P5_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 64)   # its unpack is a 1 : 1 copy
-    assert shape_of("t2_9") == (rs.RS_PATH_BULK, 136, 128)                        # 512-byte runs, 1 + 4
-    assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 128)                    # nothing aligned, long rows
-    assert shape_of("c2") == (rs.RS_PATH_BULK, 148, 64)                           # 256 MiB moved: below the CTA rules
-    assert shape_of("c3")[0] == shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU  # small operations: register path
-    assert shape_of("c4", max_ctas=48) == (rs.RS_PATH_BULK, 48, 128)              # capped: more warps per CTA
+        return o.path, o.grid, o.block, o.pace_permille
+    assert shape_of("c4") == (rs.RS_PATH_BULK, 132, 64, 0)                        # long runs, 1 : 1: closed loop, unpaced
+    assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64, 0)       # 2 KiB runs, 1 : 1
+    assert shape_of("sweep_P5_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64, 850)     # 1 read + 8 writes: every SM, rate matched
+    assert shape_of("sweep_P5_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 64, 0)   # its unpack is a 1 : 1 copy
+    assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 64, 850)       # write-heavy at any size
+    assert shape_of("t2_9") == (rs.RS_PATH_BULK, 148, 128, 810)                   # 512-byte runs, 1 + 4: 4 warps, lower roof
+    assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 128, 0)                 # nothing aligned, long rows
+    assert shape_of("c2") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 256 MiB moved: below the CTA rule
+    assert shape_of("c3") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 20 + 20 MiB: the TMA ring from 32 MiB moved on
+    assert shape_of("sweep_P1_m8_16MiB")[:2] == (rs.RS_PATH_LSU, 4 * 148)         # small operations: register path, 4 CTAs per SM
+    assert shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU
+    assert shape_of("c4", max_ctas=48) == (rs.RS_PATH_BULK, 48, 128, 0)           # capped: more warps per CTA
+    assert shape_of("sweep_P5_m8_1024MiB", tuning=dict(pace_permille=-1))[3] == 0  # rate matching can be switched off
 
 
 def test_plan_group_merges_execute_tables():
