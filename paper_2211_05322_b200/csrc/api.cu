@@ -28,18 +28,27 @@ rs_status cuda_fail(cudaError_t e, const char *what) {
 
 size_t round256(size_t x) { return (x + 255) / 256 * 256; }
 
-// SM count of the current device: grids are sized from it, so it is read BEFORE the tables are built
+// SM count and DRAM peak of the current device: grids and pacing are sized from them, so they are read BEFORE the
+// tables are built.  Queried once per device and process (the clock-rate attributes take milliseconds).
 rs_status query_device(rs::Plan *P) {
+    struct Info { int sms = 0; double peak = 0; };
+    static std::mutex mu;
+    static Info cache[64];
     cudaError_t e = cudaGetDevice(&P->device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
-    int sms = 0;
-    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->device);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
-    P->sm_count = sms;
-    int mem_khz = 0, bus_bits = 0;                             // DRAM peak = 2 x memory clock x bus width (B200: 7 672 GB/s)
-    cudaDeviceGetAttribute(&mem_khz, cudaDevAttrMemoryClockRate, P->device);
-    cudaDeviceGetAttribute(&bus_bits, cudaDevAttrGlobalMemoryBusWidth, P->device);
-    if (mem_khz > 0 && bus_bits > 0) P->dram_peak_gbs = 2.0 * mem_khz * 1e3 * bus_bits / 8 / 1e9;
+    std::lock_guard<std::mutex> lock(mu);
+    Info local;
+    Info &I = P->device >= 0 && P->device < 64 ? cache[P->device] : local;
+    if (I.sms == 0) {
+        e = cudaDeviceGetAttribute(&I.sms, cudaDevAttrMultiProcessorCount, P->device);
+        if (e != cudaSuccess) { I.sms = 0; return cuda_fail(e, "cudaDeviceGetAttribute"); }
+        int mem_khz = 0, bus_bits = 0;                         // DRAM peak = 2 x memory clock x bus width (B200: 7 672 GB/s)
+        cudaDeviceGetAttribute(&mem_khz, cudaDevAttrMemoryClockRate, P->device);
+        cudaDeviceGetAttribute(&bus_bits, cudaDevAttrGlobalMemoryBusWidth, P->device);
+        if (mem_khz > 0 && bus_bits > 0) I.peak = 2.0 * mem_khz * 1e3 * bus_bits / 8 / 1e9;
+    }
+    P->sm_count = I.sms;
+    if (I.peak > 0) P->dram_peak_gbs = I.peak;
     return RS_OK;
 }
 

@@ -29,6 +29,7 @@
 // (6.09, then 5.56 at 920; unpaced 5.66); runs of 512 B: up to 820 (6.18 TB/s), 6.00 at 840.  10 permille below the edge.
 #define RS_PACE_PERMILLE       850
 #define RS_PACE_PERMILLE_SHORT 810
+#define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
 #define RS_BULK_LONG_RUN       4096
 #define RS_BULK_CTAS_MIN_BYTES (256ll << 20)   // operations moving less than this keep one CTA on every SM
 #define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path

@@ -182,7 +182,8 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     if (big && !shift && !write_heavy && min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
     sh.grid = std::max(1, std::min(P.sm_count, pick(write_heavy ? U.bulk_ctas_mcast : U.bulk_ctas, std::max(1, ctas))));
     if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
-    sh.pace_permille = write_heavy && !shift ? (short_runs ? RS_PACE_PERMILLE_SHORT : RS_PACE_PERMILLE) : 0;
+    // (operations under 64 MiB are over before the pacing has anything to hold back: they keep the unpaced ramp)
+    sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? RS_PACE_PERMILLE_SHORT : RS_PACE_PERMILLE) : 0;
     return sh;
 }
 
