@@ -57,7 +57,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", help="c4 (default, 1.5 GiB GPT activation), c2, c3, t2_<n>, sweep_<pair>_<m8|m4>_<MiB>MiB")
-    ap.add_argument("--path", default="auto", choices=["auto", "lsu", "bulk", "shift"])
+    ap.add_argument("--path", default="auto", choices=["auto", "lsu", "bulk", "shift", "tmap"])
     ap.add_argument("--mode", default="replicas", choices=["replicas", "sharded"], help="N > 1: 'replicas' (default, DESIGN.md S8: every rank runs "
                     "the whole task on its own GPU) or 'sharded' (the multi-process executor: virtual device r lives on rank r mod N, every "
                     "rank launches its share of the unit tasks and stores into its peers' shards through CUDA IPC; NCCL only for the barrier)")
@@ -362,7 +362,7 @@ def run_ours(args):
         multi.barrier(torch.cuda.synchronize)
 
     w = inputs.get_workload(args.workload)
-    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK, "shift": rs.RS_PATH_BULK_SHIFT}[args.path]
+    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK, "shift": rs.RS_PATH_BULK_SHIFT, "tmap": rs.RS_PATH_TMAP}[args.path]
     tune = parse_tune(args.tune)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -467,7 +467,7 @@ def run_ours(args):
 
     peak, peak_src = peak_hbm()
     names = ["reshard_execute", "reshard_pack", "reshard_unpack"]
-    pname = {rs.RS_PATH_LSU: "rs_copy_lsu", rs.RS_PATH_BULK: "rs_copy_bulk", rs.RS_PATH_BULK_SHIFT: "rs_copy_bulk_shift"}
+    pname = {rs.RS_PATH_LSU: "rs_copy_lsu", rs.RS_PATH_BULK: "rs_copy_bulk", rs.RS_PATH_BULK_SHIFT: "rs_copy_bulk_shift", rs.RS_PATH_TMAP: "rs_copy_tmap"}
     kernels = {n: {"kernel": pname[o.path], "ms": k_ms[j], "best_ms": k_best[j], "bytes": op_bytes[j],
                    "GB/s": op_bytes[j] / (k_ms[j] * 1e-3) / 1e9, "grid": o.grid, "block": o.block,
                    "smem": o.smem_bytes, "tiles": o.n_tiles, "tile_bytes": o.tile_bytes, "table_bytes": o.table_bytes}
@@ -538,7 +538,7 @@ def run_sweep(args):
     stream = torch.cuda.current_stream()
     sh = stream.cuda_stream
     peak, _ = peak_hbm()
-    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK, "shift": rs.RS_PATH_BULK_SHIFT}[args.path]
+    flags = {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK, "shift": rs.RS_PATH_BULK_SHIFT, "tmap": rs.RS_PATH_TMAP}[args.path]
     tune = parse_tune(args.tune)
     K = max(3, min(args.steps, 30))
     want_ops = args.ops.split(",")
@@ -588,7 +588,12 @@ def run_sweep(args):
                 med, best = time_rotating([(lambda st, s=s, call=call: call(s, st)) for s in sets], max(50, 2 * n_sets))
             else:
                 med, best = time_each(lambda call=call: call(sets[0], sh), stream, K)
-            row[opname] = {"kernel": {rs.RS_PATH_BULK: "rs_copy_bulk", rs.RS_PATH_BULK_SHIFT: "rs_copy_bulk_shift"}.get(o.path, "rs_copy_lsu"), "bytes": nbytes,
+            t0 = time.perf_counter()                          # host cost of one call (marshalling + launch, no synchronisation)
+            for _ in range(100):
+                call(sets[0], sh)
+            host_us = (time.perf_counter() - t0) / 100 * 1e6
+            torch.cuda.synchronize()
+            row[opname] = {"host_us_per_call": host_us, "kernel": {rs.RS_PATH_BULK: "rs_copy_bulk", rs.RS_PATH_BULK_SHIFT: "rs_copy_bulk_shift", rs.RS_PATH_TMAP: "rs_copy_tmap"}.get(o.path, "rs_copy_lsu"), "bytes": nbytes,
                            "ms": med, "best_ms": best, "GB/s": nbytes / med / 1e6, "frac_of_copy_peak": nbytes / med / 1e6 / peak,
                            "tiles": o.n_tiles, "tile_bytes": o.tile_bytes, "grid": o.grid, "block": o.block, "table_bytes": o.table_bytes}
         roof = roof_1k(r_B)
@@ -939,7 +944,7 @@ def run_ncu_summary(args):
     """`ncu -i <report> --page raw --csv` of one-launch reports -> CSV rows on stdout (header first).  Append them to
     profiles/ncu_traffic.csv; bench.py reads roofline.traffic from there."""
     cols = ["workload", "op", "kernel", "grid", "block", "duration_us", "dram_read_bytes", "dram_write_bytes", "dram_throughput_pct",
-            "lts_sectors_read", "lts_sectors_write", "warp_inst_executed", "commit", "report"]
+            "dram_active_min_pct", "dram_active_max_pct", "warp_inst_executed", "commit", "report"]
     print(",".join(cols))
     for item in args.ncu_summary:
         key, path = item.split("=", 1)
@@ -963,7 +968,8 @@ def run_ncu_summary(args):
             workload, op, v[hdr.index("Kernel Name")].split("(")[0], dims(v[hdr.index("Grid Size")]), dims(v[hdr.index("Block Size")]),
             "%.3f" % get("gpu__time_duration.sum"), int(get("dram__bytes_read.sum")), int(get("dram__bytes_write.sum")),
             "%.2f" % get("gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", False),
-            int(get("lts__t_sectors_op_read.sum", False) or 0), int(get("lts__t_sectors_op_write.sum", False) or 0),
+            "%.2f" % get("dram__cycles_active.min.pct_of_peak_sustained_elapsed", False),      # least / most busy DRAM channel
+            "%.2f" % get("dram__cycles_active.max.pct_of_peak_sustained_elapsed", False),
             int(get("smsp__inst_executed.sum", False) or 0), git_commit(), os.path.basename(path)]))
     return 0
 

@@ -83,6 +83,12 @@ enum {
     RS_PATH_BULK   = 0x20,  /* force the TMA path: cp.async.bulk global->smem ring->global x k    */
     RS_PATH_BULK_SHIFT = 0x30, /* force TMA loads + byte-shifted 128-bit register stores (any alignment;
                                what AUTO picks for runs >= 512 B that are not 16-byte aligned)     */
+    RS_PATH_TMAP   = 0x40,  /* force the tensor-map TMA path: like RS_PATH_BULK, but a tile of several short rows
+                               (<= 2 KiB each) moves with ONE cp.async.bulk.tensor load and one store per receiver
+                               instead of one bulk copy per row; tensor maps are encoded at execute time from the
+                               caller's pointers.  Needs <= 16 shards per side and 16-byte aligned layouts, else it is
+                               RS_PATH_BULK.  AUTO picks it for operations of 32-320 MiB whose rows are at most 2 KiB
+                               long (profiles/r02_tmap.md)                                                    */
     RS_HOST_ONLY   = 0x100, /* build host tables only: no CUDA call, execute/pack/unpack refuse   */
     RS_WITH_STRATEGIES = 0x400, /* also build the tables of RS_STRATEGY_SENDRECV / RS_STRATEGY_ALLGATHER
                                (reshard_execute_strategy): the comparison of PAPER.md S3.1, S5.1         */
@@ -200,7 +206,7 @@ typedef struct rs_plan_info {
 } rs_plan_info;
 
 typedef struct rs_op_info {
-    int32_t path;                    /* RS_PATH_LSU, RS_PATH_BULK or RS_PATH_BULK_SHIFT selected   */
+    int32_t path;                    /* RS_PATH_LSU, RS_PATH_BULK, RS_PATH_BULK_SHIFT or RS_PATH_TMAP selected */
     int32_t vec_bytes;               /* widest access every offset/stride/run of the op allows     */
     int32_t n_tasks;                 /* copy tasks (execute/pack: one per slice; unpack: per
                                         (slice, receiver))                                         */

@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/reshard.h: plan creation / upload / queries and the launch glue of
 // execute, pack, unpack and the host-buffer entry point.
+#include <cuda.h>                         // CUtensorMap and its enums only; the encoder is fetched through the runtime
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -367,6 +368,41 @@ int ptr_align(const void *p) {
     return a;
 }
 
+// RS_PATH_TMAP: one CUtensorMap per buffer that has a geometry, from the pointers of THIS call (plans are pointer
+// agnostic).  cuTensorMapEncodeTiled is a host-side routine of the driver, reached through cudaGetDriverEntryPoint so
+// that the library links against the runtime only.
+typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                              const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+rs_status encode_tmaps(const rs::OpTables &op, const RsPtrTable &pt, unsigned char *out /* RS_TMAP_TABLE_BYTES */) {
+    static encode_fn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess) fn = reinterpret_cast<encode_fn>(p);
+    });
+    if (!fn) { rs::set_error("cuTensorMapEncodeTiled is not available"); return RS_ECUDA; }
+    static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap size");
+    std::memset(out, 0, RS_TMAP_TABLE_BYTES);
+    for (int side = 0; side < 2; side++)
+        for (int b = 0; b < RS_TMAP_BUFS; b++) {
+            const RsTmapGeom &G = side == 0 ? op.tmap_src[b] : op.tmap_dst[b];
+            void *base = side == 0 ? const_cast<char *>(pt.src[b]) : pt.dst[b];
+            if (!G.valid || !base) continue;
+            const int64_t cap = side == 0 ? op.src_cap : op.dst_cap;
+            const cuuint64_t dims[2] = {(cuuint64_t)(G.pitch / RS_TMAP_ELEM), (cuuint64_t)((cap + G.pitch - 1) / G.pitch)};
+            const cuuint64_t strides[1] = {(cuuint64_t)G.pitch};
+            const cuuint32_t box[2] = {G.box_cols / RS_TMAP_ELEM, G.box_rows}, estr[2] = {1, 1};
+            CUtensorMap *m = reinterpret_cast<CUtensorMap *>(out + (size_t)(side * RS_TMAP_BUFS + b) * 128);
+            const CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) { rs::set_error("cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"); return RS_ECUDA; }
+        }
+    return RS_OK;
+}
+
 // one launch of operation `opi` on the given buffers
 rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src, void *const *dst, int n_dst,
                  const char *used_src, void *stream, uint32_t tile_begin = 0, uint32_t tile_end = 0,
@@ -398,15 +434,23 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     RsOpDev dev = op.dev;
     if (tile_end > tile_begin) { dev.tile_base = tile_begin; dev.n_tiles = tile_end - tile_begin; }   // one slab
     const int64_t n_tiles = dev.n_tiles;
-    const bool bulk_family = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_BULK_SHIFT;
+    const bool bulk_family = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_BULK_SHIFT || op.info.path == RS_PATH_TMAP;
+    const bool as_bulk = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_TMAP;   // aligned TMA plans
     const int warps = op.info.block / 32;
     const bool pdl = !P.tune.no_pdl;
-    if (op.info.path == RS_PATH_BULK && align == 16) {
+    if (as_bulk && align == 16) {
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         dev.early_trigger = grid >= P.sm_count;
         // rate matching: the launch as a whole offers pace_permille / 1000 of the DRAM peak
         const int permille = P.tune.pace_permille > 0 ? P.tune.pace_permille : P.tune.pace_permille < 0 ? 0 : op.pace_permille;
         const float pace = permille > 0 ? (float)((double)grid * warps / (P.dram_peak_gbs * permille / 1000.0)) : 0.f;
+        if (op.info.path == RS_PATH_TMAP && small) {          // tensor maps of this call's pointers, then the same ring kernel
+            alignas(64) unsigned char tm[RS_TMAP_TABLE_BYTES];
+            rs_status ts = encode_tmaps(op, pt, tm);
+            if (ts != RS_OK) return ts;
+            e = rs::launch_tmap(dev, pt, tm, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
+                                (uint32_t)op.info.tile_bytes, pace, pdl, st);
+        } else
         e = rs::launch_bulk(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                             (uint32_t)op.info.tile_bytes, pace, pdl, st);
     } else if (op.info.path == RS_PATH_BULK_SHIFT) {          // layout not 16-byte aligned: TMA loads, shifted stores
@@ -414,7 +458,7 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         dev.early_trigger = grid >= P.sm_count;
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
                                   op.shift_stage, pdl, st);
-    } else if (op.info.path == RS_PATH_BULK && op.alt_stage) { // aligned plan, under-aligned pointers: same tiles, shifted stores
+    } else if (as_bulk && op.alt_stage) {                     // aligned plan, under-aligned pointers: same tiles, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(P.max_ctas > 0 ? std::min(P.sm_count, P.max_ctas) : P.sm_count,
                                                                      (n_tiles + op.alt_warps - 1) / op.alt_warps));
         dev.early_trigger = grid >= P.sm_count;

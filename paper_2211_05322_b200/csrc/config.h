@@ -37,6 +37,7 @@
                                             // equal at 16 + 16 MiB; from 20 + 20 MiB on the TMA ring wins: 8.1 against 8.6 us)
 #define RS_INTERLEAVE_MAX_RUN (64 << 10)    // destination runs up to this long count as a fine interleave (tile order)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
+#define RS_TMAP_MAX_BYTES    (320ll << 20)  // AUTO: tensor-map copies for short-row operations moving up to this much
 
 // TMA loads + shifted register stores (unaligned layouts): the stores are ALU work, so more warps, smaller tiles
 #define RS_SHIFT_WARPS       8          // u4 (6145-byte runs, 2-byte aligned): 8 x 2 x 8 KiB = 5.6-5.7 TB/s; 4 x 4 x 8 KiB a little more,

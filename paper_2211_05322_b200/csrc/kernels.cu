@@ -17,6 +17,7 @@
 //                 of the stores.  Needs 16-byte alignment of every address and length.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "config.h"
 #include "kernels.h"
@@ -377,10 +378,26 @@ __device__ __forceinline__ void pace_tile(uint64_t &t_next, float pace, uint32_t
     __syncwarp();
 }
 
-template <int NP>
-__global__ void __launch_bounds__(256, 1)
-rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
-             const uint32_t stage_bytes, const float pace) {
+// Tensor-map TMA (RS_PATH_TMAP): the shard of every buffer is described once per launch as a 2-D byte matrix
+// [rows][pitch] with a box of box_rows x box_cols bytes (CUtensorMap, encoded on the host from the caller's pointers,
+// passed as a __grid_constant__ parameter).  A full tile is then ONE cp.async.bulk.tensor.2d load (SASS UTMALDG) and
+// one store per receiver (UTMASTG) instead of one bulk copy per row and receiver.  The box lands in shared memory
+// densely, row after row -- the layout the per-row copies use -- so the two kinds of tile share the ring.
+struct alignas(64) RsTmap { unsigned char opaque[128]; };      // CUtensorMap
+struct RsTmapTable { RsTmap src[RS_TMAP_BUFS], dst[RS_TMAP_BUFS]; };
+
+__device__ __forceinline__ void tmap_g2s(uint32_t smem_dst, const RsTmap *map, uint32_t x, uint32_t y, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 :: "r"(smem_dst), "l"(map), "r"(x), "r"(y), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmap_s2g(const RsTmap *map, uint32_t x, uint32_t y, uint32_t smem_src) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];"
+                 :: "l"(map), "r"(x), "r"(y), "r"(smem_src) : "memory");
+}
+
+template <int NP, bool TMAP>
+__device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<NP> &ptrs, const RsTmapTable *tm, const int stages,
+                                          const int lookahead, const uint32_t stage_bytes, const float pace) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const uint32_t bars = smem_u32(smem) + warp * 64;                       // <= 8 mbarriers per warp
@@ -405,8 +422,20 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, con
         if (it < n_my) {                                      // ---- load tile `it` into slot ld_slot
             if ((it & 31) == 0) {                             // resolve the next 32 tiles of this warp
                 const int mine = it + lane;
-                if (mine < n_my)
-                    resolve_desc(op, RsTables{op.tasks, op.dsts, op.segs}, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
+                if (mine < n_my) {
+                    RsDesc *dd = descs + (mine & (RS_DESC_RING - 1));
+                    resolve_desc(op, RsTables{op.tasks, op.dsts, op.segs}, ptrs, worker + (uint32_t)mine * n_workers, dd);
+                    if (TMAP) {                               // a full tile of a task whose buffers have tensor maps
+                        const RsTask *__restrict__ T = op.tasks + dd->task;
+                        if (T->tmap_ok && dd->n_rows == T->rows_per_tile) {
+                            const uint64_t addr = (uint64_t)(dd->src - ptrs.src[T->src_buf]);   // byte offset inside the source buffer
+                            const uint64_t y = addr / (uint64_t)dd->s0;
+                            dd->lin = (y << 32) | (uint64_t)((addr - y * (uint64_t)dd->s0) / RS_TMAP_ELEM);
+                            dd->task = (uint32_t)T->src_buf;
+                            dd->flags |= RS_TILE_TMAP;
+                        }
+                    }
+                }
                 __syncwarp();
                 if (it == 0) pdl_wait();                      // shard memory is touched from here on
             }
@@ -420,7 +449,9 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, con
             const uint32_t bar = bars + 8 * ld_slot, slot = ring + (uint32_t)ld_slot * stage_bytes;
             if (lane == 0) mbar_expect_tx(bar, n_rows * col_bytes);
             __syncwarp();
-            if (d->flags & RS_TILE_FAST) {
+            if (TMAP && (d->flags & RS_TILE_TMAP)) {
+                if (lane == 0) tmap_g2s(slot, tm->src + d->task, (uint32_t)d->lin, (uint32_t)(d->lin >> 32), bar);
+            } else if (d->flags & RS_TILE_FAST) {
                 const char *src = d->src;
                 const int64_t s0 = d->s0;
                 for (uint32_t r = lane; r < n_rows; r += 32)
@@ -442,20 +473,28 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, con
             const RsDst *__restrict__ dsts = op.dsts + d->dst_first;
             const uint32_t slot = ring + (uint32_t)st_slot * stage_bytes;
             const bool fast = d->flags & RS_TILE_FAST;
-            const RsTask *__restrict__ T = op.tasks + d->task;
             mbar_wait(bars + 8 * st_slot, st_parity);
-            for (uint32_t r = lane; r < n_rows; r += 32) {
-                int64_t doff;
-                if (fast) {
-                    doff = d->dst_rel + (int64_t)r * d->d0;
-                } else {
-                    int64_t so;
-                    generic_row(T, d->lin + r, &so, &doff);
-                    doff += d->dst_rel;
-                }
-                for (uint32_t q = 0; q < k; q++) {            // read once, write k times
+            if (TMAP && (d->flags & RS_TILE_TMAP)) {          // lane q stores the whole box to receiver q
+                for (uint32_t q = lane; q < k; q += 32) {
                     const RsDst dd = dsts[q];
-                    bulk_s2g(ptrs.dst[dd.buf] + dd.off + doff, slot + r * col_bytes, col_bytes);
+                    const uint64_t addr = (uint64_t)(dd.off + d->dst_rel), y = addr / (uint64_t)d->d0;
+                    tmap_s2g(tm->dst + dd.buf, (uint32_t)((addr - y * (uint64_t)d->d0) / RS_TMAP_ELEM), (uint32_t)y, slot);
+                }
+            } else {
+                const RsTask *__restrict__ T = op.tasks + d->task;
+                for (uint32_t r = lane; r < n_rows; r += 32) {
+                    int64_t doff;
+                    if (fast) {
+                        doff = d->dst_rel + (int64_t)r * d->d0;
+                    } else {
+                        int64_t so;
+                        generic_row(T, d->lin + r, &so, &doff);
+                        doff += d->dst_rel;
+                    }
+                    for (uint32_t q = 0; q < k; q++) {        // read once, write k times
+                        const RsDst dd = dsts[q];
+                        bulk_s2g(ptrs.dst[dd.buf] + dd.off + doff, slot + r * col_bytes, col_bytes);
+                    }
                 }
             }
             bulk_commit();
@@ -464,6 +503,19 @@ rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, con
     }
     pdl_launch_dependents();                                  // out of tiles: the successor may start beside the drain
     bulk_wait_read(0);                                        // shared memory must outlive the stores' reads
+}
+
+template <int NP>
+__global__ void __launch_bounds__(256, 1)
+rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
+             const uint32_t stage_bytes, const float pace) {
+    bulk_body<NP, false>(op, ptrs, nullptr, stages, lookahead, stage_bytes, pace);
+}
+
+__global__ void __launch_bounds__(256, 1)
+rs_copy_tmap(const RsOpDev op, const __grid_constant__ RsPtrTableT<RS_PTRS_SMALL> ptrs, const __grid_constant__ RsTmapTable tm,
+             const int stages, const int lookahead, const uint32_t stage_bytes, const float pace) {
+    bulk_body<RS_PTRS_SMALL, true>(op, ptrs, &tm, stages, lookahead, stage_bytes, pace);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -701,6 +753,7 @@ cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, 
 cudaError_t prepare_bulk(int smem_bytes) {
     cudaError_t e = cudaFuncSetAttribute(rs_copy_bulk<RS_PTRS_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(rs_copy_bulk<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rs_copy_tmap, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(rs_copy_bulk_shift<RS_PTRS_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(rs_copy_bulk_shift<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
     return e;
@@ -710,6 +763,14 @@ cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool sm
                               int stages, int lookahead, uint32_t stage_bytes, bool pdl, cudaStream_t st) {
     if (small) return launch_k(rs_copy_bulk_shift<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes);
     return launch_k(rs_copy_bulk_shift<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes);
+}
+
+cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,
+                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st) {
+    static_assert(sizeof(RsTmapTable) == RS_TMAP_TABLE_BYTES, "kernels.h and the tensor-map table disagree");
+    RsTmapTable tm;
+    memcpy(&tm, tmaps, sizeof(tm));
+    return launch_k(rs_copy_tmap, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), tm, stages, lookahead, stage_bytes, pace);
 }
 
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes, int stages,

@@ -16,5 +16,9 @@ cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, i
                         int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st);
 cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
                               int stages, int lookahead, uint32_t stage_bytes, bool pdl, cudaStream_t st);
+// tensor-map TMA path: tmaps = RS_TMAP_TABLE_BYTES bytes, RS_TMAP_BUFS CUtensorMap per side (api.cu encodes them)
+#define RS_TMAP_TABLE_BYTES (2 * RS_TMAP_BUFS * 128)
+cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,
+                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st);
 int64_t launch_count();
 }  // namespace rs

@@ -86,7 +86,7 @@ int pick(int override_value, int dflt) { return override_value > 0 ? override_va
 void set_tiling(RsTask *T, int64_t tile_bytes) {
     const int64_t R = task_rows(*T), B = T->run_bytes;
     T->n_rows = (uint32_t)R;
-    T->pad = 0;
+    T->tmap_ok = 0;
     T->chunk_bytes = (uint32_t)std::min<int64_t>(B, 0xFFFFFF80ll);
     T->n_chunks = 1; T->rows_per_tile = 1; T->tiles_per_span = 1;
     if (B > tile_bytes) {                                     // long runs: split every row into column chunks
@@ -135,15 +135,22 @@ int64_t task_shift_stage(const RsTask &T) {                   // ring-slot bytes
 // Which kernel an operation takes (rs_op_info.path).  AUTO: runs under 512 B and small aligned operations go to the
 // register kernels (they start faster; small operations are launch-bound), 16-byte aligned layouts to the TMA
 // kernel, everything else to TMA loads + shifted stores.
-int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t moved_bytes) {
+int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, int64_t moved_bytes) {
     const uint32_t forced = P.flags & RS_PATH_MASK;
     const int64_t small_op = P.tune.small_op_bytes_mib < 0 ? -1 : P.tune.small_op_bytes_mib > 0 ? ((int64_t)P.tune.small_op_bytes_mib << 20) : RS_SMALL_OP_BYTES;
     const bool bulk_ok = align == 16 && min_run >= 16;
     int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
+             : forced == RS_PATH_TMAP ? (bulk_ok ? RS_PATH_TMAP : RS_PATH_BULK_SHIFT)
              : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
              : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU
              : bulk_ok ? (moved_bytes <= small_op ? RS_PATH_LSU : RS_PATH_BULK)
              : RS_PATH_BULK_SHIFT;
+    // Mid-size operations made of short rows (config 2: 2 KiB destination runs, 128 + 128 MiB) are the one place
+    // where tensor-map copies beat one bulk copy per row: +3-5 % at 64-256 MiB moved; from 512 MiB on they lose 1-2 %,
+    // 512-byte rows with 4 warps are a tie (profiles/r02_tmap.md).  Not for groups (buffers of different sizes).
+    if (!forced && path == RS_PATH_BULK && max_run <= 256 * RS_TMAP_ELEM && moved_bytes <= RS_TMAP_MAX_BYTES && !P.group_src &&
+        P.A.n_dev <= RS_TMAP_BUFS && P.B.n_dev <= RS_TMAP_BUFS)
+        path = RS_PATH_TMAP;
     if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_BULK_SHIFT;   // cp.async.bulk stores need 16-byte everything
     return path;
 }
@@ -234,7 +241,7 @@ void group_interleaved(OpTables *op) {
 // Alignment class, path, tile size, grid of one operation; then the shape of every task's tile grid and the
 // segments.  per_task: one segment per task, in task order (the slab table: its tile ranges are per task).
 rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes, bool per_task = false, bool dst_order = false) {
-    int64_t align = 16, min_run = INT64_MAX;
+    int64_t align = 16, min_run = INT64_MAX, max_run = 0;
     for (const RsTask &T : op->tasks) {
         align = std::min(align, pow2_align(T.run_bytes));
         align = std::min(align, pow2_align(T.src_off));
@@ -244,6 +251,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         }
         for (int j = 0; j < T.k; j++) align = std::min(align, pow2_align(op->dsts[(size_t)T.dst_first + j].off));
         min_run = std::min(min_run, T.run_bytes);
+        max_run = std::max(max_run, T.run_bytes);
         if (task_rows(T) > 0x7FFFFFFFll) { set_error("more than 2^31-1 rows in one slice"); return RS_EUNSUPPORTED; }
     }
     rs_op_info &I = op->info;
@@ -253,9 +261,9 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     I.read_bytes = read_bytes;
     I.write_bytes = write_bytes;
 
-    const int path = pick_path(*P, align, min_run, read_bytes + write_bytes);
+    const int path = pick_path(*P, align, min_run, max_run, read_bytes + write_bytes);
     I.path = path;
-    const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT;
+    const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT || path == RS_PATH_TMAP;
 
     int64_t tile_bytes;
     int workers;                                               // independent tile consumers in one launch
@@ -307,6 +315,35 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     int64_t mr = INT64_MAX, pad = 0;
     for (const RsTask &T : op->tasks) { mr = std::min(mr, task_min_col(T)); pad = std::max(pad, task_shift_stage(T)); }
     I.min_run_bytes = op->tasks.empty() ? 0 : mr;
+    // RS_PATH_TMAP: every buffer is seen as ONE 2-D byte matrix [rows][pitch] with ONE box shape; a task whose full
+    // tiles fit the matrices of its source and of all its destinations moves them with tensor-map copies, everything
+    // else (ragged last tiles, long or odd rows, other pitches) with the per-row bulk copies of rs_copy_bulk.
+    for (int b = 0; b < RS_TMAP_BUFS; b++) { op->tmap_src[b] = RsTmapGeom{}; op->tmap_dst[b] = RsTmapGeom{}; }
+    for (RsTask &T : op->tasks) T.tmap_ok = 0;
+    if (path == RS_PATH_TMAP && op->src_cap > 0 && op->dst_cap > 0) {
+        auto fits = [](RsTmapGeom &G, int64_t pitch, uint32_t cols, uint32_t rows, int64_t origin) {
+            if (pitch <= 0 || pitch % 16 || pitch / RS_TMAP_ELEM > 0xFFFFFFFFll || origin % pitch + cols > pitch) return false;
+            if (!G.valid) { G = RsTmapGeom{pitch, cols, rows, 1, 0}; return true; }
+            return G.pitch == pitch && G.box_cols == cols && G.box_rows == rows;
+        };
+        for (RsTask &T : op->tasks) {
+            if (T.kind != RS_TILING_FAST || T.rows_per_tile < 2 || T.rows_per_tile > 256 || T.run_bytes > 256 * RS_TMAP_ELEM || T.run_bytes % 16 ||
+                T.src_buf >= RS_TMAP_BUFS) continue;
+            RsTmapGeom src_try = op->tmap_src[T.src_buf];
+            if (!fits(src_try, T.sstride[0], (uint32_t)T.run_bytes, T.rows_per_tile, T.src_off)) continue;
+            RsTmapGeom dst_try[RS_TMAP_BUFS];
+            for (int b = 0; b < RS_TMAP_BUFS; b++) dst_try[b] = op->tmap_dst[b];
+            bool ok = true;
+            for (int j = 0; j < T.k && ok; j++) {
+                const RsDst &D = op->dsts[(size_t)T.dst_first + j];
+                ok = D.buf < RS_TMAP_BUFS && fits(dst_try[D.buf], T.dstride[0], (uint32_t)T.run_bytes, T.rows_per_tile, D.off);
+            }
+            if (!ok) continue;
+            op->tmap_src[T.src_buf] = src_try;
+            for (int b = 0; b < RS_TMAP_BUFS; b++) op->tmap_dst[b] = dst_try[b];
+            T.tmap_ok = 1;
+        }
+    }
     op->shift_stage = 0;
     op->alt_stage = 0;
     bool lsu = !bulk_family;
@@ -622,6 +659,8 @@ rs_status build_tables(Plan *P) {
         return finish_op(P, &UP, 0, 0);
     }
     if ((st = build_slabs(P, sA, sB, tensor_bytes)) != RS_OK) return st;
+    const int64_t cap_a = A.shard_elems() * e, cap_b = B.shard_elems() * e;
+    X.src_cap = cap_a; X.dst_cap = cap_b; PK.src_cap = cap_a; PK.dst_cap = P->arena_bytes; UP.src_cap = P->arena_bytes; UP.dst_cap = cap_b;
     if ((st = finish_op(P, &X, tensor_bytes, tensor_bytes * P->r_B, false, true)) != RS_OK) return st;
     if ((st = finish_op(P, &PK, tensor_bytes, tensor_bytes * P->r_B)) != RS_OK) return st;
     if ((st = finish_op(P, &UP, tensor_bytes * P->r_B, tensor_bytes * P->r_B, false, true)) != RS_OK) return st;

@@ -50,7 +50,7 @@ struct alignas(16) RsTask {
     uint32_t tiles_per_span;             // FAST: tiles per span of row dim 0 = ceil(ext[0] / rows_per_tile)
     uint32_t n_tiles;                    // tiles of this task
     uint32_t n_rows;                     // rows of the box = prod ext[i] (< 2^31)
-    uint32_t pad;
+    uint32_t tmap_ok;                    // RS_PATH_TMAP: 1 if the full tiles of this task match the tensor maps of its buffers
     uint32_t ext[RS_ROW_DIMS + 1];       // ext[0] = innermost row dim ... ; unused = 1
     int64_t sstride[RS_ROW_DIMS + 1];    // byte strides, source side
     int64_t dstride[RS_ROW_DIMS + 1];    // byte strides, destination side (same for all k)
@@ -69,7 +69,15 @@ struct alignas(16) RsSeg {
     uint32_t tiles_each;                 // tiles per member
 };
 
-enum : uint32_t { RS_TILE_FAST = 1u };
+enum : uint32_t { RS_TILE_FAST = 1u, RS_TILE_TMAP = 2u };
+
+#define RS_TMAP_BUFS 16                  // tensor maps per side in the kernel parameter
+#define RS_TMAP_ELEM 8                   // tensor-map element: UINT64 (the widest): boxes of up to 256 x 8 = 2048 bytes per row
+struct RsTmapGeom {                      // one buffer seen as a 2-D byte matrix [rows][pitch]; boxes of box_rows x box_cols bytes
+    int64_t pitch;
+    uint32_t box_cols, box_rows;
+    uint32_t valid, pad;
+};
 
 struct alignas(16) RsTile {              // a DECODED tile (never stored in a plan)
     uint32_t task;

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libreshard.so")
 
 RS_OK, RS_EINVAL, RS_ESPEC, RS_EDIVIS, RS_EUNSUPPORTED, RS_ENOMEM, RS_ECUDA = range(7)
 RS_LB_GREEDY, RS_LB_NAIVE = 0x0, 0x1
-RS_PATH_AUTO, RS_PATH_LSU, RS_PATH_BULK, RS_PATH_BULK_SHIFT = 0x00, 0x10, 0x20, 0x30
+RS_PATH_AUTO, RS_PATH_LSU, RS_PATH_BULK, RS_PATH_BULK_SHIFT, RS_PATH_TMAP = 0x00, 0x10, 0x20, 0x30, 0x40
 RS_HOST_ONLY = 0x100
 RS_EVEN_ONLY = 0x200
 RS_WITH_STRATEGIES = 0x400

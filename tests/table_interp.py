@@ -11,7 +11,7 @@ import numpy as np
 
 TASK = np.dtype([("src_off", "<i8"), ("run_bytes", "<i8"), ("src_buf", "<i4"), ("k", "<i4"), ("dst_first", "<i4"), ("nd", "<i4"),
                  ("kind", "<u4"), ("chunk_bytes", "<u4"), ("n_chunks", "<u4"), ("rows_per_tile", "<u4"),
-                 ("tiles_per_span", "<u4"), ("n_tiles", "<u4"), ("n_rows", "<u4"), ("pad", "<u4"),
+                 ("tiles_per_span", "<u4"), ("n_tiles", "<u4"), ("n_rows", "<u4"), ("tmap_ok", "<u4"),
                  ("ext", "<u4", 8), ("sstride", "<i8", 8), ("dstride", "<i8", 8)])
 DST = np.dtype([("off", "<i8"), ("buf", "<i4"), ("pad", "<i4")])
 SEG = np.dtype([("tile_begin", "<u4"), ("first_task", "<u4"), ("n_members", "<u4"), ("tiles_each", "<u4")])

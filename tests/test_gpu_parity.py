@@ -12,7 +12,7 @@ from paper_2211_05322_b200 import reshard as rs
 
 pytestmark = pytest.mark.gpu
 
-PATHS = [rs.RS_PATH_AUTO, rs.RS_PATH_LSU, rs.RS_PATH_BULK, rs.RS_PATH_BULK_SHIFT]
+PATHS = [rs.RS_PATH_AUTO, rs.RS_PATH_LSU, rs.RS_PATH_BULK, rs.RS_PATH_BULK_SHIFT, rs.RS_PATH_TMAP]
 
 SMALL = [
     ((8, 16), (1, 2), "S0,R", (1, 2), "R,S0"),                      # config 1 literal
@@ -153,6 +153,29 @@ def _check_full_size(w, path=rs.RS_PATH_AUTO, n_samples=4096):
 @pytest.mark.parametrize("path", PATHS)
 def test_config4_full_size(path):
     _check_full_size(inputs.get_workload("c4"), path)
+
+
+@pytest.mark.parametrize("name", ["c2", "t2_9", "sweep_P1_m8_1024MiB", "sweep_P2_m8_256MiB", "sweep_P4_m4_64MiB", "c3ii"])
+def test_tensor_map_path_full_size(name):
+    """RS_PATH_TMAP on the short-run layouts it is meant for: full tiles move by cp.async.bulk.tensor (one load, one store
+    per receiver), ragged tiles by per-row bulk copies, in one launch; execute, pack and unpack"""
+    import table_interp as ti
+    w = inputs.get_workload(name)
+    p = _check_full_size(w, rs.RS_PATH_TMAP, n_samples=512)
+    assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_TMAP
+    tasks, _d, _s = ti.tables(p, rs.RS_OP_EXECUTE)
+    if name in ("c2", "t2_9", "sweep_P1_m8_1024MiB", "sweep_P4_m4_64MiB"):   # runs of 512 B .. 2 KiB; the others (4 KiB, 1.25 MiB
+        assert tasks["tmap_ok"].all(), "no task of %s takes the tensor-map copies" % name   # runs) keep the per-row copies
+    e = inputs.elem_bytes(w.dtype)
+    D, src = gu.workload_on_device(w)
+    arena = torch.empty(p.info.arena_bytes, dtype=torch.uint8, device=gu.dev())
+    dst = [torch.zeros(p.local_shape(rs.RS_DST), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+    p.pack(gu.ptrs(src), arena.data_ptr(), gu.stream())
+    p.unpack(arena.data_ptr(), gu.ptrs(dst), gu.stream())
+    torch.cuda.synchronize()
+    idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
+    for q in range(p.info.n_dst):
+        assert torch.equal(dst[q], D[idx[q]])
 
 
 @pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])

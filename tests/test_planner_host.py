@@ -301,7 +301,7 @@ def test_tables_with_tiny_tiles_cover_every_tile_kind(tile, path):
 def test_alignment_class_and_path_choice():
     p = _plan((16, 1024, 4096), 2, (2, 4), "S0,R,S1", (2, 4), "S0,S1,R")
     oi = p.op_info(rs.RS_OP_EXECUTE)
-    assert oi.vec_bytes == 16 and oi.path == rs.RS_PATH_BULK and oi.min_run_bytes == 2048
+    assert oi.vec_bytes == 16 and oi.path == rs.RS_PATH_TMAP and oi.min_run_bytes == 2048     # config 2: 2 KiB rows, 256 MiB moved
     assert oi.read_bytes == p.info.tensor_bytes and oi.write_bytes == p.info.tensor_bytes
     p = _plan((4, 6, 5, 3), 2, (2, 2), "S0,S1,R,R", (2, 2), "S1,R,R,R")          # runs of 15 elements = 30 B
     oi = p.op_info(rs.RS_OP_EXECUTE)
@@ -475,7 +475,8 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 64, 850)       # write-heavy at any size
     assert shape_of("t2_9") == (rs.RS_PATH_BULK, 148, 128, 810)                   # 512-byte runs, 1 + 4: 4 warps, lower roof
     assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 128, 0)                 # nothing aligned, long rows
-    assert shape_of("c2") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 256 MiB moved: below the CTA rule
+    assert shape_of("c2") == (rs.RS_PATH_TMAP, 148, 64, 0)                        # 256 MiB moved in 2 KiB rows: tensor-map copies
+    assert shape_of("sweep_P1_m8_1024MiB")[0] == shape_of("sweep_P2_m8_64MiB")[0] == rs.RS_PATH_BULK   # too large / rows of 4 KiB
     assert shape_of("c3") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 20 + 20 MiB: the TMA ring from 32 MiB moved on
     assert shape_of("sweep_P1_m8_16MiB")[:2] == (rs.RS_PATH_LSU, 4 * 148)         # small operations: register path, 4 CTAs per SM
     assert shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU
