@@ -945,9 +945,10 @@ def run_ncu_summary(args):
     profiles/ncu_traffic.csv; bench.py reads roofline.traffic from there."""
     cols = ["workload", "op", "kernel", "grid", "block", "duration_us", "dram_read_bytes", "dram_write_bytes", "dram_throughput_pct",
             "dram_active_min_pct", "dram_active_max_pct", "warp_inst_executed", "commit", "report"]
-    print(",".join(cols))
+    out_csv = csv.writer(sys.stdout, lineterminator="\n")
+    out_csv.writerow(cols)
     for item in args.ncu_summary:
-        key, path = item.split("=", 1)
+        key, path = item.rsplit("=", 1)
         workload, op = key.split(":") if ":" in key else (key, "execute")
         out = subprocess.run(["ncu", "-i", path, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
         rows = list(csv.reader(io.StringIO(out)))
@@ -964,19 +965,20 @@ def run_ncu_summary(args):
             x = float(v[i].replace(",", ""))
             return x * _UNIT.get(units[i], 1.0) if scale else x
         dims = lambda s: int(re.findall(r"\d+", s)[0])
-        print(",".join(str(x) for x in [
+        out_csv.writerow([
             workload, op, v[hdr.index("Kernel Name")].split("(")[0], dims(v[hdr.index("Grid Size")]), dims(v[hdr.index("Block Size")]),
             "%.3f" % get("gpu__time_duration.sum"), int(get("dram__bytes_read.sum")), int(get("dram__bytes_write.sum")),
             "%.2f" % get("gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", False),
             "%.2f" % get("dram__cycles_active.min.pct_of_peak_sustained_elapsed", False),      # least / most busy DRAM channel
             "%.2f" % get("dram__cycles_active.max.pct_of_peak_sustained_elapsed", False),
-            int(get("smsp__inst_executed.sum", False) or 0), git_commit(), os.path.basename(path)]))
+            int(get("smsp__inst_executed.sum", False) or 0), git_commit(), os.path.basename(path)])
     return 0
 
 
 def run_sass(_args):
     """cuobjdump -sass libreshard.so -> per kernel: instruction count and the opcodes that prove (or disprove) the
-    Blackwell copy engines: UBLKCP (cp.async.bulk), UTMALDG / UTMASTG (tensor-map TMA), SYNCS (mbarrier), LDG / STG."""
+    Blackwell copy engines: UBLKCP (cp.async.bulk), UTMALDG / UTMASTG (tensor-map TMA), SYNCS (mbarrier), PREEXIT / ACQBULK
+    (griddepcontrol.launch_dependents / .wait: programmatic dependent launch), NANOSLEEP (rate matching), LDG / STG."""
     from paper_2211_05322_b200 import reshard as rs
     rs._lib()
     out = subprocess.run(["cuobjdump", "-sass", rs.LIB_PATH], capture_output=True, text=True, check=True).stdout
@@ -990,7 +992,7 @@ def run_sass(_args):
         m = re.match(r"\s*/\*[0-9a-f]{4}\*/\s+(?:@!?U?P\d+\s+)?([A-Z][A-Z0-9_.]*)", line)
         if m and cur:
             kernels[cur][m.group(1)] = kernels[cur].get(m.group(1), 0) + 1
-    watch = ["UBLKCP", "UTMALDG", "UTMASTG", "UTMAPF", "SYNCS", "LDG", "STG", "LDS", "STS", "SHF", "IMAD", "BAR", "LDC", "UTC", "HMMA"]
+    watch = ["UBLKCP", "UTMALDG", "UTMASTG", "SYNCS", "PREEXIT", "ACQBULK", "NANOSLEEP", "LDG", "STG", "LDS", "STS", "SHF", "IMAD", "BAR", "LDC", "UTC", "HMMA"]
     print("Command: `python bench.py --sass` (= `cuobjdump -sass paper_2211_05322_b200/libreshard.so`, opcode prefixes counted per kernel), commit %s.\n" % git_commit())
     print("| kernel | instructions | " + " | ".join(watch) + " |")
     print("|---|---|" + "---|" * len(watch))
