@@ -1,10 +1,11 @@
-// config.h -- launch-shape defaults of the two executors.  Each can be overridden at plan time by
-// an environment variable of the same name (tuning sweeps on the GPU box without a rebuild).
+// config.h -- launch-shape defaults of the executors, every one from a measurement on B200 (S3, profiles/).
+// Tests and sweeps override them per plan through rs_plan_opts.tuning (include/reshard.h rs_tuning); the library reads
+// no environment variable.
 #pragma once
 
 // register path: 128-bit ld.global -> st.global x k
 #define RS_LSU_THREADS       256
-#define RS_LSU_CTAS_PER_SM   4          // persistent CTAs per SM (grid = 148 * this); every warp is a worker
+#define RS_LSU_CTAS_PER_SM   4          // most persistent CTAs per SM (grid = SMs * CTAs per SM); every warp is a worker
 #define RS_LSU_CTAS_DEFAULT  2          // CTAs per SM actually launched (more bytes in flight is slower on B200)
 #define RS_LSU_CTAS_SMALL    4          // ... for operations moving <= RS_SMALL_OP_BYTES (ramp-bound, not DRAM-bound)
 #define RS_LSU_TILE_BYTES    16384

@@ -4,8 +4,9 @@
 // box is read ONCE from its source buffer and written to each of its k destination buffers.
 // reshard_execute / reshard_pack / reshard_unpack differ only in the task table they run.
 //
-// Four kernels (a TMA and a register design, each with a variant for unaligned layouts), all sm_100a,
-// no tensor cores (pure data movement, HBM-bound):
+// Five kernels (a TMA and a register design, each with a variant for unaligned layouts, and the tensor-map variant of
+// the TMA ring), all sm_100a, no tensor cores (pure data movement, HBM-bound).  All of them: tiles decoded
+// procedurally 32 at a time (tables.h), programmatic dependent launch (pdl_* below):
 //   rs_copy_lsu   register path for 16-byte aligned layouts with short runs.  Every thread keeps 4
 //                 independent 128-bit loads (ld.global.nc) in flight and stores each value k times.
 //   rs_copy_shift / rs_copy_bulk_shift   the same two designs for layouts (or pointers) that are NOT
@@ -14,7 +15,10 @@
 //                 issues cp.async.bulk global->shared for row r of the tile (mbarrier complete_tx),
 //                 and once the tile has landed, cp.async.bulk shared->global to each of the k
 //                 destinations (bulk_group).  No register staging, loads run LOOKAHEAD tiles ahead
-//                 of the stores.  Needs 16-byte alignment of every address and length.
+//                 of the stores.  Needs 16-byte alignment of every address and length.  Write-heavy
+//                 (multicast) launches are RATE MATCHED: every warp paces its tiles (pace_tile).
+//   rs_copy_tmap  the same ring; full tiles of short rows move with cp.async.bulk.tensor.2d (SASS: UTMALDG /
+//                 UTMASTG) through tensor maps encoded per call from the caller's pointers.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string.h>

@@ -46,3 +46,15 @@ def test_our_arm_line():
     assert r["e2e"]["h2d_bytes_per_step"] == r["e2e"]["d2h_bytes_per_step"] == 3 * 2 ** 29 and 0 < r["e2e"]["value"] < r["value"]
     assert r["cpu_baseline"]["kind"] == "oracle" and 0 < r["cpu_baseline"]["value"] < r["value"]
     assert not set(r["clocks"]["reasons"]) & {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+
+
+@pytest.mark.gpu
+def test_sharded_mode_degenerates_to_one_rank():
+    """bench.py --mode sharded on one GPU: the multi-process executor with a world of 1 (every virtual device on rank 0)"""
+    env = dict(os.environ, RANK="0", WORLD_SIZE="1", LOCAL_RANK="0", MASTER_ADDR="127.0.0.1", MASTER_PORT="29533")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--mode", "sharded", "--workload", "c2", "--steps", "5"],
+                         capture_output=True, text=True, cwd=ROOT, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    r = json.loads([l for l in out.stdout.splitlines() if l.strip()][-1])
+    assert r["mode"] == "sharded" and r["n_gpus"] == 1 and r["gpu_launches"] == 5 and r["scaling"] == "strong"
+    assert r["rank0_bytes_per_step"] == 2 * 128 * 2 ** 20 and r["rank0_peer_destinations"] == 0 and r["value"] > 1000

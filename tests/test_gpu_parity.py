@@ -525,6 +525,35 @@ def test_maximum_ranks_and_device_counts(case, path):
         assert g.tobytes() == w.tobytes()
 
 
+@pytest.mark.parametrize("tuning", [dict(pace_permille=5), dict(pace_permille=850), dict(pace_permille=-1), dict(no_pdl=1),
+                                    dict(pace_permille=300, no_pdl=1, bulk_warps=4, bulk_tile_bytes=2048), dict(task_order=1),
+                                    dict(tiles_per_worker=1), dict(small_op_bytes_mib=-1), dict(lsu_ctas_per_sm=1)])
+def test_rate_matching_and_launch_switches_change_no_byte(tuning):
+    """rs_plan_opts.tuning: pacing (down to a crawl), programmatic dependent launch off, task order, other shapes -- same bytes;
+    back-to-back dependent launches (B reads what A wrote) stay ordered with PDL on and off"""
+    for path in (rs.RS_PATH_AUTO, rs.RS_PATH_BULK, rs.RS_PATH_TMAP):
+        for case in (SMALL[9], SMALL[10], SMALL[17], SMALL[18]):          # 1 + 4, 1 + 8 multicast, several tiles per warp
+            shape, sm, ss, dm, ds = case
+            p, got, want = gu.run_small(shape, np.int32, sm, ss, dm, ds, flags=path, opts=dict(tuning=tuning))
+            for g, w in zip(got, want):
+                assert g.tobytes() == w.tobytes()
+    w = inputs.get_workload("sweep_P5_m8_16MiB")                            # 1 + 8 at 144 MiB moved: paced by default
+    e = inputs.elem_bytes(w.dtype)
+    D, src = gu.workload_on_device(w)
+    fwd = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, dict(tuning=tuning))
+    bwd = rs.Plan(w.shape, e, w.dst_mesh, w.dst_spec, w.src_mesh, w.src_spec, 0, dict(tuning=tuning))
+    if not tuning.get("pace_permille"):
+        assert fwd.op_info(rs.RS_OP_EXECUTE).pace_permille == 850
+    mid = [torch.zeros(fwd.info.dst_shard_bytes, dtype=torch.uint8, device=gu.dev()) for _ in range(fwd.info.n_dst)]
+    back = [torch.zeros_like(s) for s in src]
+    for _ in range(3):                                                      # a chain of dependent launches, no host sync in between
+        fwd.execute(gu.ptrs(src), gu.ptrs(mid), gu.stream())
+        bwd.execute(gu.ptrs(mid), gu.ptrs(back), gu.stream())
+    torch.cuda.synchronize()
+    for a, b in zip(src, back):
+        assert torch.equal(a, b)
+
+
 @pytest.mark.parametrize("cap", [1, 7, 64])
 def test_max_ctas_caps_the_grid_not_the_result(cap):
     """rs_plan_opts.max_ctas: fewer CTAs (SMs left to other streams), same bytes"""
