@@ -438,6 +438,8 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     const bool as_bulk = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_TMAP;   // aligned TMA plans
     const int warps = op.info.block / 32;
     const bool pdl = !P.tune.no_pdl;
+    const int shift_mode = P.tune.shift_mode == rs::RS_SHIFT_REG || P.tune.shift_mode == rs::RS_SHIFT_BULK ? P.tune.shift_mode
+                         : op.info.min_run_bytes >= RS_SHIFT_LONG_RUN ? rs::RS_SHIFT_BULK : rs::RS_SHIFT_REG;
     if (as_bulk && align == 16) {
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         dev.early_trigger = grid >= P.sm_count;
@@ -457,17 +459,21 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         dev.early_trigger = grid >= P.sm_count;
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
-                                  op.shift_stage, pdl, st);
+                                  op.shift_stage, shift_mode, pdl, st);
     } else if (as_bulk && op.alt_stage) {                     // aligned plan, under-aligned pointers: same tiles, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(P.max_ctas > 0 ? std::min(P.sm_count, P.max_ctas) : P.sm_count,
                                                                      (n_tiles + op.alt_warps - 1) / op.alt_warps));
         dev.early_trigger = grid >= P.sm_count;
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.alt_warps * 32, op.alt_smem, op.alt_stages, op.alt_stages - 1,
-                                  op.alt_stage, pdl, st);
+                                  op.alt_stage, shift_mode, pdl, st);
     } else {                                                  // register paths
         int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
         if (P.max_ctas > 0) cap = std::min<int64_t>(cap, P.max_ctas);
-        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_tiles + 7) / 8, cap));
+        // 8 warps per CTA, every warp a worker (warp-major over the grid); an operation with fewer tiles than that still
+        // gets one CTA on every SM while it has a tile for each: its dependents may then be launched at entry
+        int64_t want = (n_tiles + 7) / 8;
+        if (want < P.sm_count) want = std::min<int64_t>(n_tiles, P.sm_count);
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, cap));
         dev.early_trigger = grid >= P.sm_count;
         if (align < 16) e = rs::launch_shift(dev, pt, small, grid, pdl, st);   // any alignment, still 16-byte accesses
         else e = rs::launch_lsu(dev, pt, small, grid, pdl, st);

@@ -20,6 +20,7 @@
 #define RS_BULK_LOOKAHEAD    2          // loads in flight per warp before the first store is issued
 #define RS_BULK_TILE_BYTES   12288      // bytes per ring slot
 #define RS_BULK_SHORT_RUN    1024       // runs up to this long: many copies per tile, use the SHORT shape
+#define RS_BULK_MIN_FILL     0.7        // slots less full than this on average: the SHORT shape too
 #define RS_BULK_WARPS_SHORT  4
 #define RS_BULK_TILE_BYTES_SHORT 8192
 #define RS_BULK_CTAS_DEN       148    // CTA counts below are out of 148 SMs
@@ -44,8 +45,11 @@
 #define RS_SHIFT_WARPS       8          // u4 (6145-byte runs, 2-byte aligned): 8 x 2 x 8 KiB = 5.6-5.7 TB/s; 4 x 4 x 8 KiB a little more,
 #define RS_SHIFT_STAGES      2          // but short rows (flat walk, ~100 instructions per 512 B) need the 8 warps
 #define RS_SHIFT_TILE_BYTES  8192
-#define RS_SHIFT_WARPS_LONG  4          // rows >= 1 KiB (row-by-row stores, ~35 instructions per 512 B): fewer, deeper pipelines
-#define RS_SHIFT_STAGES_LONG 4
+#define RS_SHIFT_LONG_RUN    4096       // rows at least this long: bulk stores (u4, 6 KiB rows: 6.12 TB/s against 5.65 from registers);
+                                        // shorter: register stores, 8 warps (u1, 2 KiB rows: 5.8 against 4.1 with bulk stores)
+#define RS_SHIFT_WARPS_LONG  6          // rows >= 1 KiB: bodies realigned in the ring and stored with bulk copies.  One warp per
+#define RS_SHIFT_STAGES_LONG 3          // scheduler hides no latency (~520 instructions per tile at ~6 cycles each), so 6 warps:
+                                        // u4 4 x 4: 4.4 TB/s, 5 x 4: 5.4, 6 x 3: 6.12, 7 x 3: 6.05, 8 x 3: 5.75 (register stores, 4 x 4: 5.79)
 
 #define RS_BULK_DESC_BYTES   4096       // per-warp descriptor ring: 64 tiles x 64 bytes
 

@@ -120,7 +120,9 @@ rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
     __shared__ uint4 staged[RS_LSU_TABLE_BYTES / 16];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = RS_LSU_THREADS / 32;
     RsDesc *descs = ring[warp];
-    const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
+    // worker = warp-major over the grid: consecutive tiles go to different CTAs, so an operation of a few hundred tiles
+    // still spreads over every SM (and may give its launch_dependents trigger at entry)
+    const uint32_t worker = warp * gridDim.x + blockIdx.x, n_workers = gridDim.x * W;
     const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
     // Small tables (a few dozen unit tasks) are copied to shared memory first: one global-memory latency, after which
     // segment search, task fields and destination entries are shared-memory reads.
@@ -228,7 +230,7 @@ rs_copy_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
     __shared__ RsDesc ring[RS_LSU_THREADS / 32][32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = RS_LSU_THREADS / 32;
     RsDesc *descs = ring[warp];
-    const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
+    const uint32_t worker = warp * gridDim.x + blockIdx.x, n_workers = gridDim.x * W;
     const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
     if (op.early_trigger) pdl_launch_dependents();
 
@@ -458,8 +460,12 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
             } else if (d->flags & RS_TILE_FAST) {
                 const char *src = d->src;
                 const int64_t s0 = d->s0;
-                for (uint32_t r = lane; r < n_rows; r += 32)
-                    bulk_g2s(slot + r * col_bytes, src + (int64_t)r * s0, col_bytes, bar);
+                if (s0 == (int64_t)col_bytes || n_rows == 1) { // rows adjacent in the source: the tile is ONE run there
+                    if (lane == 0) bulk_g2s(slot, src, n_rows * col_bytes, bar);
+                } else {
+                    for (uint32_t r = lane; r < n_rows; r += 32)
+                        bulk_g2s(slot + r * col_bytes, src + (int64_t)r * s0, col_bytes, bar);
+                }
             } else {
                 const RsTask *__restrict__ T = op.tasks + d->task;
                 for (uint32_t r = lane; r < n_rows; r += 32) {
@@ -483,6 +489,13 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
                     const RsDst dd = dsts[q];
                     const uint64_t addr = (uint64_t)(dd.off + d->dst_rel), y = addr / (uint64_t)d->d0;
                     tmap_s2g(tm->dst + dd.buf, (uint32_t)((addr - y * (uint64_t)d->d0) / RS_TMAP_ELEM), (uint32_t)y, slot);
+                }
+            } else if (fast && (d->d0 == (int64_t)col_bytes || n_rows == 1)) {
+                // rows adjacent in the destinations (a message, or a shard whose rows the slice covers whole): lane q
+                // stores the tile to receiver q with ONE bulk copy
+                for (uint32_t q = lane; q < k; q += 32) {
+                    const RsDst dd = dsts[q];
+                    bulk_s2g(ptrs.dst[dd.buf] + dd.off + d->dst_rel, slot, n_rows * col_bytes);
                 }
             } else {
                 const RsTask *__restrict__ T = op.tasks + d->task;
@@ -583,6 +596,63 @@ __device__ __forceinline__ void store_row(char *dr, uint32_t sm, uint32_t n, uin
     }
 }
 
+// TMA STORES for unaligned rows.  cp.async.bulk needs 16-byte aligned addresses and sizes on both sides, and the
+// 16-byte aligned BODY of a destination row (everything but < 16 head and < 16 tail bytes) has them in global memory.
+// So the body is first realigned INSIDE the ring slot: window c of the body (row bytes [head + 16c, head + 16c + 16),
+// which sit at q0 + 16c with q0 = base + delta) is assembled from the aligned words c and c + 1 and written back over
+// word c.  32 windows at a time, all loads before all stores: a group overwrites words c0 .. c0 + 31 and has read words
+// c0 .. c0 + 32; the next group starts at word c0 + 32, which is still intact.  Afterwards one bulk copy per row and
+// receiver stores the body from `base` (st.global from registers tops out ~6 % below TMA stores on B200: DESIGN.md S3).
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4 &v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" :: "r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+template <int W>
+__device__ __forceinline__ uint4 funnel_window(const uint4 &lo, const uint4 &hi, uint32_t b) {
+    const uint32_t w[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+    return make_uint4(__funnelshift_r(w[W], w[W + 1], b), __funnelshift_r(w[W + 1], w[W + 2], b),
+                      __funnelshift_r(w[W + 2], w[W + 3], b), __funnelshift_r(w[W + 3], w[W + 4], b));
+}
+
+// (one warp per scheduler hides no latency: what counts is the instruction count, so 128 windows per trip, four per lane)
+template <int W>
+__device__ __forceinline__ void row_realign(uint32_t base, uint32_t full, uint32_t b, uint32_t lane) {
+    uint32_t c0 = 0;
+    for (; c0 + 128u <= full; c0 += 128u) {                                 // whole trips: no predicates
+        const uint32_t p = base + 16u * (c0 + lane);
+        const uint4 l0 = lds128(p), h0 = lds128(p + 16u), l1 = lds128(p + 512u), h1 = lds128(p + 528u),
+                    l2 = lds128(p + 1024u), h2 = lds128(p + 1040u), l3 = lds128(p + 1536u), h3 = lds128(p + 1552u);
+        __syncwarp();
+        sts128(p, funnel_window<W>(l0, h0, b));
+        sts128(p + 512u, funnel_window<W>(l1, h1, b));
+        sts128(p + 1024u, funnel_window<W>(l2, h2, b));
+        sts128(p + 1536u, funnel_window<W>(l3, h3, b));
+        __syncwarp();
+    }
+    for (; c0 < full; c0 += 32u) {                                          // the ragged rest, 32 windows per trip
+        const uint32_t c = c0 + lane, p = base + 16u * c;
+        uint4 lo, hi;
+        if (c < full) { lo = lds128(p); hi = lds128(p + 16u); }
+        __syncwarp();
+        if (c < full) sts128(p, funnel_window<W>(lo, hi, b));
+        __syncwarp();
+    }
+}
+
+// where the pieces of one destination row are: n bytes in shared memory from `sm`, going to global address `dr`
+struct RowCut { uint32_t head, full, tail, base, delta; };
+__device__ __forceinline__ RowCut cut_row(uintptr_t dr, uint32_t sm, uint32_t n) {
+    RowCut c;
+    c.head = (16u - (uint32_t)(dr & 15u)) & 15u;
+    if (c.head > n) c.head = n;
+    c.full = (n - c.head) >> 4;
+    c.tail = n - c.head - (c.full << 4);
+    const uint32_t q0 = sm + c.head;
+    c.delta = q0 & 15u;
+    c.base = q0 - c.delta;
+    return c;
+}
+
 // One 16-byte aligned window of a destination row, in two steps so that several windows' shared-memory
 // loads can be in flight: n bytes of the row sit in shared memory from byte address `sm`.
 struct ShiftSlot { uint4 lo, hi; int32_t X; uint32_t delta; };
@@ -612,7 +682,7 @@ __device__ __forceinline__ void slot_store(const ShiftSlot &t, char *dr, uint32_
 template <int NP>
 __global__ void __launch_bounds__(256, 1)
 rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
-                   const uint32_t stage_bytes) {
+                   const uint32_t stage_bytes, const int mode) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const uint32_t bars = smem_u32(smem) + warp * 64;
@@ -628,17 +698,22 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptr
 
     const uint32_t worker = blockIdx.x * W + warp, n_workers = gridDim.x * W;
     const int n_my = worker < op.n_tiles ? (int)((op.n_tiles - worker + n_workers - 1) / n_workers) : 0;
+    const int pending_ok = stages - lookahead - 1;            // store groups that may still read the ring (>= 0)
     int ld_slot = 0, st_slot = 0;
     uint32_t st_parity = 0;
 
     for (int it = 0; it < n_my + lookahead; ++it) {
-        if (it < n_my) {                                      // ---- load tile `it` (its slot was drained in program order)
+        if (it < n_my) {                                      // ---- load tile `it`
             if ((it & 31) == 0) {
                 const int mine = it + lane;
                 if (mine < n_my)
                     resolve_desc(op, RsTables{op.tasks, op.dsts, op.segs}, ptrs, worker + (uint32_t)mine * n_workers, descs + (mine & (RS_DESC_RING - 1)));
                 __syncwarp();
                 if (it == 0) pdl_wait();                      // shard memory is touched from here on
+            }
+            if (it >= stages) {                               // slot reuse: the bulk stores of its last tile must have read it
+                bulk_wait_read(pending_ok);                   // (register stores drained it in program order)
+                __syncwarp();
             }
             const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
             const uint32_t n_rows = d->n_rows, n = d->col_bytes, pitch = shift_pitch(n);
@@ -674,6 +749,54 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptr
             const RsTask *__restrict__ T = op.tasks + d->task;
             const uint32_t SL = (n + 30u) >> 4;               // destination windows per row, at most
             mbar_wait(bars + 8 * st_slot, st_parity);
+            // Long rows whose k destinations are congruent modulo 16 (always, for k = 1): realign the body of every row in
+            // place, then one bulk store per row and receiver; head and tail bytes go out as byte stores.
+            bool tma_stores = mode == RS_SHIFT_BULK && fast && SL >= 64u && n_rows <= 32u;
+            if (tma_stores && k > 1) {
+                const uint32_t a0 = (uint32_t)((uintptr_t)(ptrs.dst[dsts[0].buf] + dsts[0].off) & 15u);
+                bool same = true;
+                for (uint32_t q = lane; q < k; q += 32) same = same && ((uint32_t)((uintptr_t)(ptrs.dst[dsts[q].buf] + dsts[q].off) & 15u) == a0);
+                tma_stores = __all_sync(0xffffffffu, same);
+            }
+            if (tma_stores) {
+                const RsDst d0q = dsts[0];
+                const uintptr_t dp0 = (uintptr_t)(ptrs.dst[d0q.buf] + d0q.off + d->dst_rel);
+                for (uint32_t r = 0; r < n_rows; r++) {
+                    const uint32_t sm = slot + r * pitch + 16u + (uint32_t)((uintptr_t)(d->src + (int64_t)r * d->s0) & 15u);
+                    const RowCut c = cut_row(dp0 + (uintptr_t)((int64_t)r * d->d0), sm, n);
+                    uint32_t edge = 0;                        // this lane's head or tail byte, read before the body moves
+                    const bool is_head = (uint32_t)lane < c.head, is_tail = lane >= 16 && (uint32_t)lane - 16u < c.tail;
+                    const uint32_t edge_off = is_head ? (uint32_t)lane : c.head + (c.full << 4) + (uint32_t)lane - 16u;
+                    if (is_head || is_tail) edge = lds_u8(sm + edge_off);
+                    __syncwarp();
+                    if (c.delta) {
+                        const uint32_t b = (c.delta & 3u) * 8u;
+                        switch (c.delta >> 2) {               // warp-uniform
+                            case 0: row_realign<0>(c.base, c.full, b, (uint32_t)lane); break;
+                            case 1: row_realign<1>(c.base, c.full, b, (uint32_t)lane); break;
+                            case 2: row_realign<2>(c.base, c.full, b, (uint32_t)lane); break;
+                            default: row_realign<3>(c.base, c.full, b, (uint32_t)lane); break;
+                        }
+                    }
+                    if (is_head || is_tail)
+                        for (uint32_t q = 0; q < k; q++) {
+                            const RsDst dd = dsts[q];
+                            (ptrs.dst[dd.buf] + dd.off + d->dst_rel + (int64_t)r * d->d0)[edge_off] = (char)edge;
+                        }
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the realigned bodies, before the copy engine reads them
+                __syncwarp();
+                if ((uint32_t)lane < n_rows) {                // lane r: the body of row r to every receiver
+                    const uint32_t r = (uint32_t)lane;
+                    const uint32_t sm = slot + r * pitch + 16u + (uint32_t)((uintptr_t)(d->src + (int64_t)r * d->s0) & 15u);
+                    const RowCut c = cut_row(dp0 + (uintptr_t)((int64_t)r * d->d0), sm, n);
+                    if (c.full)
+                        for (uint32_t q = 0; q < k; q++) {
+                            const RsDst dd = dsts[q];
+                            bulk_s2g(ptrs.dst[dd.buf] + dd.off + d->dst_rel + (int64_t)r * d->d0 + c.head, c.base, c.full << 4);
+                        }
+                }
+            } else
             for (uint32_t q = 0; q < k; q++) {                // read once (from HBM), write k times
                 const RsDst dd = dsts[q];
                 char *dp = ptrs.dst[dd.buf] + dd.off + d->dst_rel;
@@ -705,11 +828,14 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptr
                     }
                 }
             }
+            bulk_commit();                                    // one group per tile, empty when registers stored it
             __syncwarp();                                     // every lane has read the slot ...
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // ... before the copy engine may overwrite it
             if (++st_slot == stages) { st_slot = 0; st_parity ^= 1u; }
         }
     }
+    pdl_launch_dependents();
+    bulk_wait_read(0);                                        // shared memory must outlive the stores' reads
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -764,9 +890,9 @@ cudaError_t prepare_bulk(int smem_bytes) {
 }
 
 cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
-                              int stages, int lookahead, uint32_t stage_bytes, bool pdl, cudaStream_t st) {
-    if (small) return launch_k(rs_copy_bulk_shift<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes);
-    return launch_k(rs_copy_bulk_shift<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes);
+                              int stages, int lookahead, uint32_t stage_bytes, int mode, bool pdl, cudaStream_t st) {
+    if (small) return launch_k(rs_copy_bulk_shift<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes, mode);
+    return launch_k(rs_copy_bulk_shift<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes, mode);
 }
 
 cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,

@@ -158,16 +158,19 @@ int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, in
 // Launch shape of the two TMA kernels, from measurement on B200.
 struct BulkShape { int warps, stages, grid, pace_permille; int64_t tile_bytes; };
 
-BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes) {
+BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes, bool dst_dense, bool underfilled) {
     const rs_tuning &U = P.tune;
     // short runs = many bulk copies per tile: one warp issues them too slowly, so more, smaller pipelines
     // (Table 2 case 9, 512-byte runs: 3.6 TB/s with 2 warps, 5.7 with 4)
-    const bool short_runs = min_run <= RS_BULK_SHORT_RUN;
+    // ... and so do tiles that would fill little of a 12 KiB slot (a run of 6160 bytes: one row per tile): a warp spends
+    // ~220 instructions per tile at ~6 cycles each with nothing to overlap them, so 2 warps x half-empty tiles are
+    // issue-bound (a4: 4.55 TB/s; 4 warps x 8 KiB slots: 6.33)
+    const bool short_runs = min_run <= RS_BULK_SHORT_RUN || underfilled;
     // a caller-imposed CTA cap (rs_plan_opts.max_ctas) is made up for with more warps per CTA:
     // 64 CTAs x 4 warps move 6.0 TB/s of a 1 : 1 layout, 64 x 2 only 3.9
     const bool capped = P.max_ctas > 0 && P.max_ctas * 4 < P.sm_count * 3;
-    // shifted variant: rows of >= 1 KiB are stored row by row (cheap), shorter ones window by window (ALU-heavy)
-    const bool shift_long = shift && min_run >= 1024;
+    // shifted variant: rows of >= 4 KiB leave through bulk stores (config.h RS_SHIFT_LONG_RUN), shorter ones through registers
+    const bool shift_long = shift && min_run >= RS_SHIFT_LONG_RUN;
     BulkShape sh;
     sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
                                              : pick(U.bulk_warps, short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
@@ -190,7 +193,9 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     sh.grid = std::max(1, std::min(P.sm_count, pick(write_heavy ? U.bulk_ctas_mcast : U.bulk_ctas, std::max(1, ctas))));
     if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
     // (operations under 64 MiB are over before the pacing has anything to hold back: they keep the unpaced ramp)
-    sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? RS_PACE_PERMILLE_SHORT : RS_PACE_PERMILLE) : 0;
+    // short rows that are adjacent in every destination are stored with one bulk copy per tile and receiver (kernels.cu):
+    // they pace like long rows (Table 2 case 9: 6.12 TB/s at 810, 6.35 at 850); stored row by row they peak at 820
+    sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs && !dst_dense ? RS_PACE_PERMILLE_SHORT : RS_PACE_PERMILLE) : 0;
     return sh;
 }
 
@@ -269,7 +274,18 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     int workers;                                               // independent tile consumers in one launch
     int stages = 0;
     if (bulk_family) {
-        const BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes);
+        bool dst_dense = true;                                 // rows of every task adjacent in its destinations
+        for (const RsTask &T : op->tasks) dst_dense = dst_dense && (T.nd == 0 || T.dstride[0] == T.run_bytes);
+        // how full the default 12 KiB slots would be, averaged over the bytes moved
+        const int64_t tb0 = std::max<int64_t>(128, pick(P->tune.bulk_tile_bytes, RS_BULK_TILE_BYTES) / 128 * 128);
+        double filled = 0, total = 0;
+        for (RsTask T : op->tasks) {
+            set_tiling(&T, tb0);
+            const double bytes = (double)task_rows(T) * (double)T.run_bytes, tiles = (double)task_tiles_exact(T);
+            if (tiles > 0) { filled += bytes; total += tiles * (double)tb0; }
+        }
+        const bool underfilled = total > 0 && filled < RS_BULK_MIN_FILL * total;
+        const BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled);
         tile_bytes = sh.tile_bytes;
         stages = sh.stages;
         op->pace_permille = sh.pace_permille;
@@ -365,7 +381,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         if (!shift) {
             // An aligned plan may be handed under-aligned pointers at execute time: keep a launch shape of the
             // shifted TMA kernel for the SAME tiles (rows padded in the ring, so fewer warps or slots fit).
-            const bool long_rows = min_run >= 1024;
+            const bool long_rows = min_run >= RS_SHIFT_LONG_RUN;
             int aw = long_rows ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS, as = long_rows ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES;
             while (as > 2 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) as--;
             while (aw > 1 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) aw--;
@@ -385,7 +401,9 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     }
     if (lsu) {
         const int warps = RS_LSU_THREADS / 32;
-        I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
+        int64_t want = (I.n_tiles + warps - 1) / warps;
+        if (want < P->sm_count) want = std::min<int64_t>(I.n_tiles, P->sm_count);   // few tiles: still one CTA on every SM (api.cu)
+        I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, want));
         I.smem_bytes = 0;
     }
     return RS_OK;

@@ -122,6 +122,10 @@ CONFIGS = {
     # 6145 B at 2-byte alignment (the "tiling, padding" case of PAPER.md:259 at GPT-activation size)
     "u4":   _w("u4", (30, 2047, 12290), "bf16", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 6),
     "u4b":  _w("u4b", (30, 2047, 24579), "u8", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 7),
+    # sweep pair P1 at 1 GiB on extents that divide nothing: 2050-byte destination rows at 2-byte alignment
+    "u1":   _w("u1", (64, 2046, 4100), "bf16", (2, 4), "S0,R,S1", (2, 4), "S0,S1,R", "bits", 9),
+    # the same pair with rows that are 16-byte aligned and nothing more (6160-byte runs): the least the TMA path accepts
+    "a4":   _w("a4", (32, 2048, 12320), "bf16", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 8),
 }
 
 # config 5: six layout pairs (BASELINE.json configs[4]) on two mesh pairs.
