@@ -37,6 +37,11 @@
 #define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path
                                             // (no shared-memory carve-out, no mbarriers: 4 MiB + 4 MiB in 3.2 us against 6.5 us;
                                             // equal at 16 + 16 MiB; from 20 + 20 MiB on the TMA ring wins: 8.1 against 8.6 us)
+#define RS_SMALL_OP_BYTES_MCAST (10ll << 20)   // ... write-heavy ones (a slice with k >= 2 receivers): up to 1 + 8 MiB
+#define RS_SMALL_MCAST_BYTES   (40ll << 20)    // write-heavy operations moving up to this much: 8 warps x 3 slots x 4 KiB per SM
+#define RS_BULK_WARPS_SMALL_MCAST      8       // (4 + 16 MiB: 4.8 us against 6.7 us with 2 x 4 x 12 KiB and 6.4 us in registers;
+#define RS_BULK_STAGES_SMALL_MCAST     3       //  4 + 32 MiB: 7.5 us either way; from 16 + 64 MiB on the default shape)
+#define RS_BULK_TILE_BYTES_SMALL_MCAST 4096
 #define RS_INTERLEAVE_MAX_RUN (64 << 10)    // destination runs up to this long count as a fine interleave (tile order)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 #define RS_TMAP_MAX_BYTES    (320ll << 20)  // AUTO: tensor-map copies for short-row operations moving up to this much

@@ -135,9 +135,12 @@ int64_t task_shift_stage(const RsTask &T) {                   // ring-slot bytes
 // Which kernel an operation takes (rs_op_info.path).  AUTO: runs under 512 B and small aligned operations go to the
 // register kernels (they start faster; small operations are launch-bound), 16-byte aligned layouts to the TMA
 // kernel, everything else to TMA loads + shifted stores.
-int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, int64_t moved_bytes) {
+int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, int64_t moved_bytes, bool write_heavy) {
     const uint32_t forced = P.flags & RS_PATH_MASK;
-    const int64_t small_op = P.tune.small_op_bytes_mib < 0 ? -1 : P.tune.small_op_bytes_mib > 0 ? ((int64_t)P.tune.small_op_bytes_mib << 20) : RS_SMALL_OP_BYTES;
+    // (write-heavy operations leave the register path earlier: k stores per load keep a thread busy, the ring's stores are
+    // fire and forget -- 4 + 16 MiB: 6.4 us in registers, 4.8 us on the ring; 1 + 8 MiB: 3.1 against 4.5 us)
+    const int64_t small_op = P.tune.small_op_bytes_mib < 0 ? -1 : P.tune.small_op_bytes_mib > 0 ? ((int64_t)P.tune.small_op_bytes_mib << 20)
+                           : write_heavy ? RS_SMALL_OP_BYTES_MCAST : RS_SMALL_OP_BYTES;
     const bool bulk_ok = align == 16 && min_run >= 16;
     int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
              : forced == RS_PATH_TMAP ? (bulk_ok ? RS_PATH_TMAP : RS_PATH_BULK_SHIFT)
@@ -171,13 +174,15 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     const bool capped = P.max_ctas > 0 && P.max_ctas * 4 < P.sm_count * 3;
     // shifted variant: rows of >= 4 KiB leave through bulk stores (config.h RS_SHIFT_LONG_RUN), shorter ones through registers
     const bool shift_long = shift && min_run >= RS_SHIFT_LONG_RUN;
+    // small write-heavy operations (4 MiB to 8 receivers) are over in 5-8 us: many short pipelines ramp up faster
+    const bool small_mcast = !shift && write_bytes >= 2 * read_bytes && read_bytes + write_bytes <= RS_SMALL_MCAST_BYTES && !capped;
     BulkShape sh;
     sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
-                                             : pick(U.bulk_warps, short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
+                                             : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
     sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES)
-                                              : pick(U.bulk_stages, RS_BULK_STAGES)));
+                                              : pick(U.bulk_stages, small_mcast ? RS_BULK_STAGES_SMALL_MCAST : RS_BULK_STAGES)));
     sh.tile_bytes = shift ? pick(U.shift_tile_bytes, RS_SHIFT_TILE_BYTES)
-                          : pick(U.bulk_tile_bytes, short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
+                          : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
     sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
     while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
     // One CTA per SM.
@@ -266,7 +271,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     I.read_bytes = read_bytes;
     I.write_bytes = write_bytes;
 
-    const int path = pick_path(*P, align, min_run, max_run, read_bytes + write_bytes);
+    const int path = pick_path(*P, align, min_run, max_run, read_bytes + write_bytes, write_bytes >= 2 * read_bytes);
     I.path = path;
     const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT || path == RS_PATH_TMAP;
 
