@@ -55,7 +55,8 @@ def device_shards_from_global(D, mesh, spec, fill=0):
 
 
 def run_small(shape, np_dtype, sm, ss, dm, ds, flags=0, seed=1, src_offset=0, dst_offset=0, opts=None):
-    """execute on the GPU and return (plan, got dst shards as numpy, oracle dst shards as numpy)."""
+    """execute on the GPU and return (plan, got dst shards as numpy, oracle dst shards as numpy).
+    src_offset / dst_offset: bytes every shard pointer is moved by (an int, or a function of the device index, < 64)"""
     e = np.dtype(np_dtype).itemsize
     rng = np.random.default_rng(seed)
     D = np.frombuffer(rng.bytes(int(np.prod(shape)) * e), dtype=np_dtype).reshape(shape)
@@ -63,16 +64,18 @@ def run_small(shape, np_dtype, sm, ss, dm, ds, flags=0, seed=1, src_offset=0, ds
     want = do.reshard(shape, sm, ss, dm, ds, src, fill=0xA5)      # padding (R5) must come back untouched
     p = rs.Plan(shape, e, sm, ss, dm, ds, flags, opts)
     src_d = [torch.zeros(s.nbytes + 64, dtype=torch.uint8, device=dev()) for s in src]
-    for t, s in zip(src_d, src):
-        t[src_offset:src_offset + s.nbytes] = to_dev(s)
+    so = [src_offset(r) if callable(src_offset) else src_offset for r in range(len(src))]
+    do_ = [dst_offset(q) if callable(dst_offset) else dst_offset for q in range(len(want))]
+    for t, s, o in zip(src_d, src, so):
+        t[o:o + s.nbytes] = to_dev(s)
     dst_d = [torch.full((want[0].nbytes + 64,), 0xA5, dtype=torch.uint8, device=dev()) for _ in want]
-    p.execute([t.data_ptr() + src_offset for t in src_d], [t.data_ptr() + dst_offset for t in dst_d], stream())
+    p.execute([t.data_ptr() + o for t, o in zip(src_d, so)], [t.data_ptr() + o for t, o in zip(dst_d, do_)], stream())
     torch.cuda.synchronize()
     got = []
-    for t, w in zip(dst_d, want):
+    for t, w, o in zip(dst_d, want, do_):
         raw = t.cpu().numpy()
-        assert (raw[:dst_offset] == 0xA5).all() and (raw[dst_offset + w.nbytes:] == 0xA5).all(), "wrote outside the shard"
-        got.append(raw[dst_offset:dst_offset + w.nbytes].view(np_dtype).reshape(w.shape))
+        assert (raw[:o] == 0xA5).all() and (raw[o + w.nbytes:] == 0xA5).all(), "wrote outside the shard"
+        got.append(raw[o:o + w.nbytes].view(np_dtype).reshape(w.shape))
     return p, got, want
 
 

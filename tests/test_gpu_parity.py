@@ -78,6 +78,33 @@ def test_under_aligned_shard_pointers(off, path):
         assert g.tobytes() == w.tobytes()
 
 
+LONG_UNALIGNED = [
+    ((5, 9, 4099), (2,), "S0,R,R", (2, 2), "R,S0,R"),                  # 20 KiB runs cut into chunks, k = 2, uneven on two dims
+    ((4, 40, 2203), (2,), "R,R,S0", (2, 2), "S0,R,R"),                 # 1102-byte rows, several per tile, k = 2
+    ((3, 6, 9001), (1,), "R,R,R", (2, 4), "R,S0,R"),                   # 9001-byte rows, k = 4, whole rows adjacent in the receivers
+    ((2, 11, 6146), (2, 2), "S0,R,S1", (2, 2), "S1,S0,R"),             # 3073-byte rows, 1 : 1 (u4 in small)
+]
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("dtype", [np.uint8, np.int16])
+@pytest.mark.parametrize("case", LONG_UNALIGNED, ids=[str(i) for i in range(len(LONG_UNALIGNED))])
+def test_unaligned_long_rows_register_and_bulk_stores(case, dtype, mode):
+    """rs_copy_bulk_shift on rows of 1-20 KiB that are not 16-byte aligned: stores from registers (rs_tuning.shift_mode 1) and
+    bodies realigned in the ring + cp.async.bulk stores (2); receivers congruent modulo 16 (one bulk store per row and
+    receiver) and not (falls back to registers); pointers moved by odd byte counts; ring shapes from 1 to 8 warps"""
+    shape, sm, ss, dm, ds = case
+    e = np.dtype(dtype).itemsize
+    for so, dofs in [(0, 0), (e, 3 * e), (lambda r: (5 * r * e) % 16, lambda q: (7 * q * e + e) % 16), (16, lambda q: 16 if q % 2 else 0)]:
+        for warps, stages in [(0, 0), (1, 2), (8, 2), (3, 5)]:
+            tuning = dict(shift_mode=mode, shift_warps=warps, shift_stages=stages)
+            p, got, want = gu.run_small(shape, dtype, sm, ss, dm, ds, flags=rs.RS_PATH_BULK_SHIFT, src_offset=so, dst_offset=dofs,
+                                        opts=dict(tuning=tuning))
+            assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_BULK_SHIFT
+            for q, (g, w) in enumerate(zip(got, want)):
+                assert g.tobytes() == w.tobytes(), (case, dtype, mode, warps, stages, q)
+
+
 @pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK, rs.RS_PATH_BULK_SHIFT])
 @pytest.mark.parametrize("tile", [128, 1024, 4096])
 def test_tile_sizes_and_ring_depths(tile, path):
@@ -179,9 +206,14 @@ def test_tensor_map_path_full_size(name):
 
 
 @pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])
-@pytest.mark.parametrize("name", ["u4", "u4b"])
+@pytest.mark.parametrize("name", ["u4", "u4b", "u1", "a4"])
 def test_unaligned_uneven_full_size(name, path):
-    """1.4 GiB with nothing aligned: TMA loads + shifted stores (AUTO) and the register shift path (LSU)"""
+    """1-1.5 GiB with nothing aligned (a4: 16-byte aligned and nothing more): TMA loads + shifted stores (AUTO; bulk stores of
+    realigned rows for u4 / u4b, register stores for u1's 2 KiB rows, the plain TMA ring for a4) and the register path (LSU)"""
+    if name == "a4":
+        p = _check_full_size(inputs.get_workload(name), path)
+        assert p.op_info(rs.RS_OP_EXECUTE).path == (rs.RS_PATH_BULK if path == rs.RS_PATH_AUTO else rs.RS_PATH_LSU)
+        return
     p = _check_full_size(inputs.get_workload(name), path)
     assert p.op_info(rs.RS_OP_EXECUTE).path == (rs.RS_PATH_BULK_SHIFT if path == rs.RS_PATH_AUTO else rs.RS_PATH_LSU)
 
