@@ -33,7 +33,8 @@
 #define RS_PACE_PERMILLE_SHORT 810
 #define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
 #define RS_BULK_LONG_RUN       4096
-#define RS_BULK_CTAS_MIN_BYTES (256ll << 20)   // operations moving less than this keep one CTA on every SM
+#define RS_BULK_CTAS_MIN_BYTES (384ll << 20)   // operations moving less than this keep one CTA on every SM (config 2's pack, 128 + 128 MiB:
+                                               // 46.1 us on 132 CTAs, 43.3 us on 148; at 256 + 256 MiB the two are level, beyond 132 wins)
 #define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path
                                             // (no shared-memory carve-out, no mbarriers: 4 MiB + 4 MiB in 3.2 us against 6.5 us;
                                             // equal at 16 + 16 MiB; from 20 + 20 MiB on the TMA ring wins: 8.1 against 8.6 us)

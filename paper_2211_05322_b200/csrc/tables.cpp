@@ -191,7 +191,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     //    every SM and are RATE MATCHED (kernels.cu pace_tile, config.h RS_PACE_PERMILLE): 6.4-6.5 TB/s.
     //  * 1 : 1 operations limit themselves (loads are a closed loop: bytes in flight / latency) and stay unpaced;
     //    with long runs (<= 3 bulk copies per tile) 132 CTAs are 1.5-3.7 % faster than 148 (a fraction of the SM count,
-    //    so the rule survives a different part); operations under 256 MiB are ramp-bound: every SM.
+    //    so the rule survives a different part); operations moving under 384 MiB are ramp-bound: every SM.
     const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
     int ctas = P.sm_count;
     if (big && !shift && !write_heavy && min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
