@@ -53,6 +53,9 @@
 #define RS_SHIFT_TILE_BYTES  8192
 #define RS_SHIFT_LONG_RUN    4096       // rows at least this long: bulk stores (u4, 6 KiB rows: 6.12 TB/s against 5.65 from registers);
                                         // shorter: register stores, 8 warps (u1, 2 KiB rows: 5.8 against 4.1 with bulk stores)
+#define RS_SHIFT_MID_RUN     1024       // rows of 1-4 KiB (stored row by row from registers): 7 warps x 3 slots
+#define RS_SHIFT_WARPS_MID   7          // u1 (2050-byte rows): 6 x 3: 5.38 TB/s, 7 x 3: 6.08, 8 x 2: 5.85, 8 x 3: 5.65
+#define RS_SHIFT_STAGES_MID  3
 #define RS_SHIFT_WARPS_LONG  6          // rows >= 1 KiB: bodies realigned in the ring and stored with bulk copies.  One warp per
 #define RS_SHIFT_STAGES_LONG 3          // scheduler hides no latency (~520 instructions per tile at ~6 cycles each), so 6 warps:
                                         // u4 4 x 4: 4.4 TB/s, 5 x 4: 5.4, 6 x 3: 6.12, 7 x 3: 6.05, 8 x 3: 5.75 (register stores, 4 x 4: 5.79)

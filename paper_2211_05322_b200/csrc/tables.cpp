@@ -173,13 +173,13 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     // 64 CTAs x 4 warps move 6.0 TB/s of a 1 : 1 layout, 64 x 2 only 3.9
     const bool capped = P.max_ctas > 0 && P.max_ctas * 4 < P.sm_count * 3;
     // shifted variant: rows of >= 4 KiB leave through bulk stores (config.h RS_SHIFT_LONG_RUN), shorter ones through registers
-    const bool shift_long = shift && min_run >= RS_SHIFT_LONG_RUN;
+    const bool shift_long = shift && min_run >= RS_SHIFT_LONG_RUN, shift_mid = shift && !shift_long && min_run >= RS_SHIFT_MID_RUN;
     // small write-heavy operations (4 MiB to 8 receivers) are over in 5-8 us: many short pipelines ramp up faster
     const bool small_mcast = !shift && write_bytes >= 2 * read_bytes && read_bytes + write_bytes <= RS_SMALL_MCAST_BYTES && !capped;
     BulkShape sh;
-    sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS)
+    sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : shift_mid ? RS_SHIFT_WARPS_MID : RS_SHIFT_WARPS)
                                              : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
-    sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES)
+    sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : shift_mid ? RS_SHIFT_STAGES_MID : RS_SHIFT_STAGES)
                                               : pick(U.bulk_stages, small_mcast ? RS_BULK_STAGES_SMALL_MCAST : RS_BULK_STAGES)));
     sh.tile_bytes = shift ? pick(U.shift_tile_bytes, RS_SHIFT_TILE_BYTES)
                           : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
@@ -387,7 +387,9 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
             // An aligned plan may be handed under-aligned pointers at execute time: keep a launch shape of the
             // shifted TMA kernel for the SAME tiles (rows padded in the ring, so fewer warps or slots fit).
             const bool long_rows = min_run >= RS_SHIFT_LONG_RUN;
-            int aw = long_rows ? RS_SHIFT_WARPS_LONG : RS_SHIFT_WARPS, as = long_rows ? RS_SHIFT_STAGES_LONG : RS_SHIFT_STAGES;
+            const bool mid_rows = !long_rows && min_run >= RS_SHIFT_MID_RUN;
+            int aw = long_rows ? RS_SHIFT_WARPS_LONG : mid_rows ? RS_SHIFT_WARPS_MID : RS_SHIFT_WARPS;
+            int as = long_rows ? RS_SHIFT_STAGES_LONG : mid_rows ? RS_SHIFT_STAGES_MID : RS_SHIFT_STAGES;
             while (as > 2 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) as--;
             while (aw > 1 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) aw--;
             if ((int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 <= RS_SMEM_MAX && I.n_tiles > 0) {
