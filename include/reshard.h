@@ -79,10 +79,11 @@ enum {
     RS_LB_NAIVE    = 0x1,   /* always the lowest-indexed candidate                  */
     RS_PATH_AUTO   = 0x00,  /* executor chosen per operation from alignment, run length and size  */
     RS_PATH_LSU    = 0x10,  /* force the register paths: 128-bit ld.global -> st.global x k (AUTO:
-                               runs < 512 B and operations moving <= 64 MiB)                     */
+                               runs < 512 B, operations moving <= 32 MiB, write-heavy ones <= 10 MiB) */
     RS_PATH_BULK   = 0x20,  /* force the TMA path: cp.async.bulk global->smem ring->global x k    */
-    RS_PATH_BULK_SHIFT = 0x30, /* force TMA loads + byte-shifted 128-bit register stores (any alignment;
-                               what AUTO picks for runs >= 512 B that are not 16-byte aligned)     */
+    RS_PATH_BULK_SHIFT = 0x30, /* force TMA loads + byte-shifted stores (any alignment; what AUTO picks for runs
+                               >= 512 B that are not 16-byte aligned): rows >= 4 KiB are realigned in shared memory
+                               and stored with cp.async.bulk, shorter ones with 128-bit register stores        */
     RS_PATH_TMAP   = 0x40,  /* force the tensor-map TMA path: like RS_PATH_BULK, but a tile of several short rows
                                (<= 2 KiB each) moves with ONE cp.async.bulk.tensor load and one store per receiver
                                instead of one bulk copy per row; tensor maps are encoded at execute time from the
