@@ -31,7 +31,11 @@
 // (6.09, then 5.56 at 920; unpaced 5.66); runs of 512 B: up to 820 (6.18 TB/s), 6.00 at 840.  10 permille below the edge.
 #define RS_PACE_PERMILLE       850
 #define RS_PACE_PERMILLE_SHORT 810
+#define RS_PACE_PERMILLE_SHORT_DENSE 830   // short rows that are adjacent in the receivers (one bulk store per tile)
 #define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
+#define RS_PACE_PERMILLE_11    880            // 1 : 1 operations made of runs >= 1 MiB: best at 880-900, collapse from 910 (fig5_1x1 6.18 -> 6.56 TB/s,
+#define RS_PACE_11_MIN_RUN     (1ll << 20)    //   P6 at 4 GiB 6.56 -> 6.8, unpack of P2 6.59 -> 6.76; runs of 128 KiB: no change; 2-6 KiB rows: 0 to -3 %)
+#define RS_PACE_11_MIN_BYTES   (128ll << 20)
 #define RS_BULK_LONG_RUN       4096
 #define RS_BULK_CTAS_MIN_BYTES (384ll << 20)   // operations moving less than this keep one CTA on every SM (config 2's pack, 128 + 128 MiB:
                                                // 46.1 us on 132 CTAs, 43.3 us on 148; at 256 + 256 MiB the two are level, beyond 132 wins)

@@ -193,14 +193,22 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     //    with long runs (<= 3 bulk copies per tile) 132 CTAs are 1.5-3.7 % faster than 148 (a fraction of the SM count,
     //    so the rule survives a different part); operations moving under 384 MiB are ramp-bound: every SM.
     const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
+    //  * 1 : 1 operations made of VERY long runs (>= 1 MiB on both sides: whole-shard copies, unpack of a broadcast, P3 / P6)
+    //    do not limit themselves well enough either: on every SM and paced at 880 permille they reach 6.45-6.7 TB/s where the
+    //    unpaced 132-CTA launch gives 6.2-6.55 and `torch copy_` 6.4-6.6 (profiles/r02_pacing.md, second part); from 910 on
+    //    they collapse like the write-heavy ones.  Rows of a few KiB gain nothing (config 4) or lose 3 % (P1: 2 warps per SM
+    //    have no slack for a pause).
+    const bool long_11 = !shift && !write_heavy && min_run >= RS_PACE_11_MIN_RUN && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES;
     int ctas = P.sm_count;
-    if (big && !shift && !write_heavy && min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
+    if (big && !shift && !write_heavy && !long_11 && min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
     sh.grid = std::max(1, std::min(P.sm_count, pick(write_heavy ? U.bulk_ctas_mcast : U.bulk_ctas, std::max(1, ctas))));
     if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
     // (operations under 64 MiB are over before the pacing has anything to hold back: they keep the unpaced ramp)
-    // short rows that are adjacent in every destination are stored with one bulk copy per tile and receiver (kernels.cu):
-    // they pace like long rows (Table 2 case 9: 6.12 TB/s at 810, 6.35 at 850); stored row by row they peak at 820
-    sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs && !dst_dense ? RS_PACE_PERMILLE_SHORT : RS_PACE_PERMILLE) : 0;
+    // short rows that are adjacent in every destination are stored with one bulk copy per tile and receiver (kernels.cu) and
+    // take a higher rate than rows stored one by one (Table 2 case 9: 6.12 TB/s at 810, 6.26 at 830, 6.35-6.40 at 850 on two
+    // boxes but 5.98 on a third, whose edge lies lower: 830)
+    sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
+                     : long_11 ? RS_PACE_PERMILLE_11 : 0;
     return sh;
 }
 
