@@ -7,6 +7,8 @@
 #define RS_LSU_THREADS       256
 #define RS_LSU_CTAS_PER_SM   4          // most persistent CTAs per SM (grid = SMs * CTAs per SM); every warp is a worker
 #define RS_LSU_CTAS_DEFAULT  2          // CTAs per SM actually launched (more bytes in flight is slower on B200)
+#define RS_LSU_CTAS_MCAST    1          // ... for large write-heavy operations (the register path has no pacing: 128-byte rows, 1 + 4 GiB: 5.05 TB/s
+                                        // with 1 CTA per SM, 4.64 with 2, 4.59 with 4; AUTO sends them through tensor maps when it can: 6.09)
 #define RS_LSU_CTAS_SMALL    4          // ... for operations moving <= RS_SMALL_OP_BYTES (ramp-bound, not DRAM-bound)
 #define RS_LSU_TILE_BYTES    16384
 #define RS_LSU_UNROLL        8          // independent vector loads in flight per thread
@@ -49,6 +51,9 @@
 #define RS_BULK_TILE_BYTES_SMALL_MCAST 4096
 #define RS_INTERLEAVE_MAX_RUN (64 << 10)    // destination runs up to this long count as a fine interleave (tile order)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
+#define RS_TMAP_SHORT_MIN_RUN   64          // AUTO: operations made of rows of 64-511 bytes take the tensor-map kernel when they are past the
+#define RS_TMAP_SHORT_MIN_COVER 0.9        //   small-operation size and >= 90 % of their bytes move as whole boxes (else the register path)
+#define RS_PACE_PERMILLE_TMAP_SHORT 850    // ... paced when 1 : 1 (write-heavy ones: RS_PACE_PERMILLE_SHORT)
 #define RS_TMAP_MAX_BYTES    (320ll << 20)  // AUTO: tensor-map copies for short-row operations moving up to this much
 
 // TMA loads + shifted register stores (unaligned layouts): the stores are ALU work, so more warps, smaller tiles

@@ -135,24 +135,29 @@ int64_t task_shift_stage(const RsTask &T) {                   // ring-slot bytes
 // Which kernel an operation takes (rs_op_info.path).  AUTO: runs under 512 B and small aligned operations go to the
 // register kernels (they start faster; small operations are launch-bound), 16-byte aligned layouts to the TMA
 // kernel, everything else to TMA loads + shifted stores.
-int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, int64_t moved_bytes, bool write_heavy) {
+int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, int64_t moved_bytes, bool write_heavy, bool tmap_short, int n_src, int n_dst) {
     const uint32_t forced = P.flags & RS_PATH_MASK;
     // (write-heavy operations leave the register path earlier: k stores per load keep a thread busy, the ring's stores are
     // fire and forget -- 4 + 16 MiB: 6.4 us in registers, 4.8 us on the ring; 1 + 8 MiB: 3.1 against 4.5 us)
     const int64_t small_op = P.tune.small_op_bytes_mib < 0 ? -1 : P.tune.small_op_bytes_mib > 0 ? ((int64_t)P.tune.small_op_bytes_mib << 20)
                            : write_heavy ? RS_SMALL_OP_BYTES_MCAST : RS_SMALL_OP_BYTES;
     const bool bulk_ok = align == 16 && min_run >= 16;
+    // Rows shorter than 512 bytes: a tensor-map copy moves a box of up to 256 of them with one instruction, whatever their length,
+    // so a large operation made of short rows takes rs_copy_tmap (128-byte rows at 1 + 1 GiB: 6.15 TB/s against 5.53 in registers;
+    // 1 + 4 GiB: 6.09 against 4.64) -- if (nearly) all of its tiles fit the tensor maps (finish_op checks and falls back).
+    const bool short_tmap = tmap_short && bulk_ok && min_run >= RS_TMAP_SHORT_MIN_RUN && moved_bytes > small_op && !P.group_src &&
+                            n_src <= RS_TMAP_BUFS && n_dst <= RS_TMAP_BUFS;
     int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
              : forced == RS_PATH_TMAP ? (bulk_ok ? RS_PATH_TMAP : RS_PATH_BULK_SHIFT)
              : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
-             : min_run < RS_BULK_MIN_RUN ? RS_PATH_LSU
+             : min_run < RS_BULK_MIN_RUN ? (short_tmap ? RS_PATH_TMAP : RS_PATH_LSU)
              : bulk_ok ? (moved_bytes <= small_op ? RS_PATH_LSU : RS_PATH_BULK)
              : RS_PATH_BULK_SHIFT;
     // Mid-size operations made of short rows (config 2: 2 KiB destination runs, 128 + 128 MiB) are the one place
     // where tensor-map copies beat one bulk copy per row: +3-5 % at 64-256 MiB moved; from 512 MiB on they lose 1-2 %,
     // 512-byte rows with 4 warps are a tie (profiles/r02_tmap.md).  Not for groups (buffers of different sizes).
     if (!forced && path == RS_PATH_BULK && max_run <= 256 * RS_TMAP_ELEM && moved_bytes <= RS_TMAP_MAX_BYTES && !P.group_src &&
-        P.A.n_dev <= RS_TMAP_BUFS && P.B.n_dev <= RS_TMAP_BUFS)
+        n_src <= RS_TMAP_BUFS && n_dst <= RS_TMAP_BUFS)
         path = RS_PATH_TMAP;
     if (path == RS_PATH_BULK && !bulk_ok) path = RS_PATH_BULK_SHIFT;   // cp.async.bulk stores need 16-byte everything
     return path;
@@ -258,7 +263,7 @@ void group_interleaved(OpTables *op) {
 
 // Alignment class, path, tile size, grid of one operation; then the shape of every task's tile grid and the
 // segments.  per_task: one segment per task, in task order (the slab table: its tile ranges are per task).
-rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes, bool per_task = false, bool dst_order = false) {
+rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes, bool per_task, bool dst_order, bool tmap_short, double *tmap_cover) {
     int64_t align = 16, min_run = INT64_MAX, max_run = 0;
     for (const RsTask &T : op->tasks) {
         align = std::min(align, pow2_align(T.run_bytes));
@@ -279,7 +284,8 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     I.read_bytes = read_bytes;
     I.write_bytes = write_bytes;
 
-    const int path = pick_path(*P, align, min_run, max_run, read_bytes + write_bytes, write_bytes >= 2 * read_bytes);
+    const int path = pick_path(*P, align, min_run, max_run, read_bytes + write_bytes, write_bytes >= 2 * read_bytes, tmap_short, P->A.n_dev, P->B.n_dev);
+    const bool short_tmap = path == RS_PATH_TMAP && min_run < RS_BULK_MIN_RUN && !(P->flags & RS_PATH_MASK);
     I.path = path;
     const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT || path == RS_PATH_TMAP;
 
@@ -298,7 +304,9 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
             if (tiles > 0) { filled += bytes; total += tiles * (double)tb0; }
         }
         const bool underfilled = total > 0 && filled < RS_BULK_MIN_FILL * total;
-        const BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled);
+        BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled);
+        // short rows through tensor maps, 1 : 1: open loop enough to want rate matching too (128-byte rows: 5.37 TB/s unpaced, 6.15 at 850)
+        if (short_tmap && !sh.pace_permille && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES) sh.pace_permille = RS_PACE_PERMILLE_TMAP_SHORT;
         tile_bytes = sh.tile_bytes;
         stages = sh.stages;
         op->pace_permille = sh.pace_permille;
@@ -313,7 +321,7 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         // small operations are ramp-bound: more warps per SM cover the start-up latency (c3: 11.2 -> 10.1 us with 4 CTAs
         // per SM); large ones are DRAM-bound and do best with 2 (more bytes in flight is slower on B200)
         const bool small_op = read_bytes + write_bytes <= RS_SMALL_OP_BYTES;
-        I.grid = P->sm_count * std::max(1, std::min(RS_LSU_CTAS_PER_SM, pick(P->tune.lsu_ctas_per_sm, small_op ? RS_LSU_CTAS_SMALL : RS_LSU_CTAS_DEFAULT)));
+        I.grid = P->sm_count * std::max(1, std::min(RS_LSU_CTAS_PER_SM, pick(P->tune.lsu_ctas_per_sm, small_op ? RS_LSU_CTAS_SMALL : write_bytes >= 2 * read_bytes ? RS_LSU_CTAS_MCAST : RS_LSU_CTAS_DEFAULT)));
         if (P->max_ctas > 0) I.grid = std::min(I.grid, P->max_ctas);
         workers = I.grid * (RS_LSU_THREADS / 32);
     }
@@ -373,6 +381,15 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
             T.tmap_ok = 1;
         }
     }
+    if (tmap_cover) {                                          // share of the bytes that move as whole tensor-map boxes
+        double whole = 0, all = 0;
+        for (const RsTask &T : op->tasks) {
+            const double bytes = (double)task_rows(T) * (double)T.run_bytes;
+            all += bytes;
+            if (T.tmap_ok && T.nd >= 1) whole += bytes / (double)T.ext[0] * (double)(T.ext[0] / T.rows_per_tile * T.rows_per_tile);
+        }
+        *tmap_cover = path == RS_PATH_TMAP && all > 0 ? whole / all : 0.0;
+    }
     op->shift_stage = 0;
     op->alt_stage = 0;
     bool lsu = !bulk_family;
@@ -422,6 +439,19 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
         I.smem_bytes = 0;
     }
     return RS_OK;
+}
+
+// AUTO may route an operation made of short rows through the tensor-map kernel; that only pays if nearly every tile moves as a
+// whole box (a tile that does not falls back to one bulk copy per 128-byte row), so the choice is checked and undone otherwise.
+rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_bytes, bool per_task = false, bool dst_order = false) {
+    double cover = 0;
+    rs_status st = finish_op_impl(P, op, read_bytes, write_bytes, per_task, dst_order, /*tmap_short=*/!per_task, &cover);
+    if (st != RS_OK) return st;
+    int64_t min_run = INT64_MAX;
+    for (const RsTask &T : op->tasks) min_run = std::min(min_run, T.run_bytes);
+    if (op->info.path == RS_PATH_TMAP && !(P->flags & RS_PATH_MASK) && min_run < RS_BULK_MIN_RUN && cover < RS_TMAP_SHORT_MIN_COVER)
+        st = finish_op_impl(P, op, read_bytes, write_bytes, per_task, dst_order, /*tmap_short=*/false, nullptr);
+    return st;
 }
 
 // reshard_execute_host pipeline: cut tensor dim 0 into slabs.  Dim 0 is the outermost dim of every

@@ -124,6 +124,9 @@ CONFIGS = {
     "u4b":  _w("u4b", (30, 2047, 24579), "u8", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 7),
     # sweep pair P1 at 1 GiB on extents that divide nothing: 2050-byte destination rows at 2-byte alignment
     "u1":   _w("u1", (64, 2046, 4100), "bf16", (2, 4), "S0,R,S1", (2, 4), "S0,S1,R", "bits", 9),
+    # the paper's microbenchmark tensor with its LAST dim sharded 8 ways on one side: 128-byte runs (register path at full size)
+    "r128": _w("r128", (1024, 1024, 512), "bf16", (2, 4), "R,R,S01", (2, 4), "S01,R,R", "bits", 10),
+    "r128m": _w("r128m", (1024, 1024, 512), "bf16", (2, 4), "R,R,S01", (2, 4), "S0,R,R", "bits", 11),
     # the same pair with rows that are 16-byte aligned and nothing more (6160-byte runs): the least the TMA path accepts
     "a4":   _w("a4", (32, 2048, 12320), "bf16", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 8),
 }

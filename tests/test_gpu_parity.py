@@ -218,6 +218,15 @@ def test_unaligned_uneven_full_size(name, path):
     assert p.op_info(rs.RS_OP_EXECUTE).path == (rs.RS_PATH_BULK_SHIFT if path == rs.RS_PATH_AUTO else rs.RS_PATH_LSU)
 
 
+@pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])
+@pytest.mark.parametrize("name", ["r128", "r128m"])
+def test_short_rows_full_size(name, path):
+    """the paper's microbenchmark tensor with 128-byte runs (last dim sharded 8 ways), 1 : 1 and 1 + 4: tensor-map boxes of 64 rows
+    (AUTO) and the register path"""
+    p = _check_full_size(inputs.get_workload(name), path)
+    assert p.op_info(rs.RS_OP_EXECUTE).path == (rs.RS_PATH_TMAP if path == rs.RS_PATH_AUTO else rs.RS_PATH_LSU)
+
+
 @pytest.mark.parametrize("pair", sorted(inputs.SWEEP_PAIRS))
 @pytest.mark.parametrize("meshes", ["m8", "m4"])
 def test_sweep_1gib_full_size(pair, meshes):

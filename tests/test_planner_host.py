@@ -483,6 +483,11 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("c3") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 20 + 20 MiB: the TMA ring from 32 MiB moved on
     assert shape_of("sweep_P1_m8_16MiB")[:2] == (rs.RS_PATH_LSU, 4 * 148)         # small operations: register path, 4 CTAs per SM
     assert shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU
+    assert shape_of("r128") == (rs.RS_PATH_TMAP, 148, 128, 850)                   # 128-byte rows at 1 + 1 GiB: boxes of 64 rows, paced
+    assert shape_of("r128m") == (rs.RS_PATH_TMAP, 148, 128, 810)                  # ... 1 + 4 GiB
+    assert shape_of("r128", rs.RS_OP_PACK)[0] == rs.RS_PATH_BULK                  # its pack copies whole 64 KiB runs
+    p = _plan((262144, 4, 64), 2, (2,), "R,R,S0", (2,), "R,S0,R", 0)              # 64-byte rows, but only 2 per span: no box fits
+    assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_LSU                     # ... so AUTO falls back to the register path
     assert shape_of("c4", max_ctas=48) == (rs.RS_PATH_BULK, 48, 128, 0)           # capped: more warps per CTA
     assert shape_of("sweep_P5_m8_1024MiB", tuning=dict(pace_permille=-1))[3] == 0  # rate matching can be switched off
 
