@@ -23,6 +23,7 @@
 #define RS_BULK_TILE_BYTES   12288      // bytes per ring slot
 #define RS_BULK_SHORT_RUN    1024       // runs up to this long: many copies per tile, use the SHORT shape
 #define RS_BULK_MIN_FILL     0.7        // slots less full than this on average: the SHORT shape too
+#define RS_BULK_TINY_FILL    0.3        // slots less than 30 % full (tiles under ~3.5 KiB): 8 warps x 3 slots x 4 KiB
 #define RS_BULK_WARPS_SHORT  4
 #define RS_BULK_TILE_BYTES_SHORT 8192
 #define RS_BULK_CTAS_DEN       148    // CTA counts below are out of 148 SMs
@@ -53,6 +54,7 @@
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 #define RS_TMAP_SHORT_MIN_RUN   64          // AUTO: operations made of rows of 64-511 bytes take the tensor-map kernel when they are past the
 #define RS_TMAP_SHORT_MIN_COVER 0.9        //   small-operation size and >= 90 % of their bytes move as whole boxes (else the register path)
+#define RS_TMAP_SHORT_MIN_TILE  3584        //   ... and, when 1 : 1, their tiles hold at least this much
 #define RS_PACE_PERMILLE_TMAP_SHORT 850    // ... paced when 1 : 1 (write-heavy ones: RS_PACE_PERMILLE_SHORT)
 #define RS_TMAP_MAX_BYTES    (320ll << 20)  // AUTO: tensor-map copies for short-row operations moving up to this much
 
@@ -75,5 +77,6 @@
 #define RS_HOST_SLABS_MAX        16
 #define RS_HOST_SLAB_MIN_BYTES  (8 << 20)
 
+#define RS_SPAN_TILE_MIN_BYTES 1024      // spans of the innermost row dim holding at least this much become one FAST tile each
 #define RS_TILES_PER_WORKER   4          // small operations: tiles shrink until every warp has this many (tail balance)
 #define RS_SMEM_MAX          (227 * 1024)

@@ -100,7 +100,9 @@ void set_tiling(RsTask *T, int64_t tile_bytes) {
     }
     const int64_t rpt = std::max<int64_t>(1, tile_bytes / B);  // rows per tile
     const int64_t ext0 = T->nd > 0 ? T->ext[0] : 1;
-    if (T->nd <= 1 || ext0 >= rpt) {                          // FAST tiles inside one span of row dim 0
+    // (a span shorter than a tile still makes FAST tiles -- one per span -- when it holds >= RS_SPAN_TILE_MIN_BYTES: GENERIC tiles
+    // pay a division per row or vector, which cost a feature map resharded from H to W, 64-byte rows in spans of 32, 2/3 of its rate)
+    if (T->nd <= 1 || ext0 >= rpt || ext0 * B >= RS_SPAN_TILE_MIN_BYTES) {   // FAST tiles inside one span of row dim 0
         const int64_t n = (ext0 + rpt - 1) / rpt, sz = (ext0 + n - 1) / n;
         T->kind = RS_TILING_FAST;
         T->rows_per_tile = (uint32_t)sz;
@@ -166,7 +168,7 @@ int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, in
 // Launch shape of the two TMA kernels, from measurement on B200.
 struct BulkShape { int warps, stages, grid, pace_permille; int64_t tile_bytes; };
 
-BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes, bool dst_dense, bool underfilled) {
+BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes, bool dst_dense, bool underfilled, bool tiny_tiles) {
     const rs_tuning &U = P.tune;
     // short runs = many bulk copies per tile: one warp issues them too slowly, so more, smaller pipelines
     // (Table 2 case 9, 512-byte runs: 3.6 TB/s with 2 warps, 5.7 with 4)
@@ -180,7 +182,9 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     // shifted variant: rows of >= 4 KiB leave through bulk stores (config.h RS_SHIFT_LONG_RUN), shorter ones through registers
     const bool shift_long = shift && min_run >= RS_SHIFT_LONG_RUN, shift_mid = shift && !shift_long && min_run >= RS_SHIFT_MID_RUN;
     // small write-heavy operations (4 MiB to 8 receivers) are over in 5-8 us: many short pipelines ramp up faster
-    const bool small_mcast = !shift && write_bytes >= 2 * read_bytes && read_bytes + write_bytes <= RS_SMALL_MCAST_BYTES && !capped;
+    // ... and so do tiles of 1-4 KiB (a span of the innermost row dim that short: feature maps resharded across H / W): at ~1 340 cycles
+    // per tile and warp, 2 KiB tiles need 8 warps per SM (fm_hw: 2.6 TB/s with 4 warps, 4.4 with 8 before source-order segments)
+    const bool small_mcast = !shift && !capped && (tiny_tiles || (write_bytes >= 2 * read_bytes && read_bytes + write_bytes <= RS_SMALL_MCAST_BYTES));
     BulkShape sh;
     sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : shift_mid ? RS_SHIFT_WARPS_MID : RS_SHIFT_WARPS)
                                              : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
@@ -223,17 +227,21 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
 // 6.00 -> 6.18 TB/s).  Members must have identical tile grids and destination buffers, and start in the same
 // destination row.  Reorders op->tasks so that the members of a segment are consecutive (ascending destination
 // offset); the order of the segments follows their first member.
-void group_interleaved(OpTables *op) {
+void group_interleaved(OpTables *op, bool by_dst, bool by_src) {
     const size_t n = op->tasks.size();
-    std::map<std::vector<int64_t>, std::vector<uint32_t>> buckets;
-    std::vector<std::vector<int64_t>> key_of(n);
+    std::map<std::vector<int64_t>, std::vector<uint32_t>> buckets, src_buckets;
+    std::vector<std::vector<int64_t>> key_of(n), src_key_of(n);
+    auto grid_key = [](const RsTask &T) {
+        return std::vector<int64_t>{T.k, T.nd, T.run_bytes, (int64_t)T.kind, T.chunk_bytes, T.n_chunks, T.rows_per_tile, T.tiles_per_span, T.n_tiles};
+    };
     for (size_t i = 0; i < n; i++) {
         const RsTask &T = op->tasks[i];
         std::vector<int64_t> key;
-        if (T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.dstride[0] > T.run_bytes && T.kind != RS_TILING_GENERIC) {
+        const bool cand = T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.kind != RS_TILING_GENERIC;
+        if (by_dst && cand && T.dstride[0] > T.run_bytes) {
             const RsDst &D0 = op->dsts[(size_t)T.dst_first];
-            key = {T.k, T.nd, T.run_bytes, (int64_t)T.kind, T.chunk_bytes, T.n_chunks, T.rows_per_tile, T.tiles_per_span, T.n_tiles,
-                   D0.off / T.dstride[0]};
+            key = grid_key(T);
+            key.push_back(D0.off / T.dstride[0]);
             for (int d = 0; d < T.nd; d++) { key.push_back(T.ext[d]); key.push_back(T.dstride[d]); }
             for (int j = 0; j < T.k; j++) {                   // the same receivers, at the same distance from the first one
                 const RsDst &D = op->dsts[(size_t)T.dst_first + j];
@@ -244,7 +252,29 @@ void group_interleaved(OpTables *op) {
         }
         buckets[key].push_back((uint32_t)i);
         key_of[i] = std::move(key);
+        // Slices that share SOURCE rows (each reads part of every row of the sender's shard: a feature map resharded from a
+        // split of H to a split of W reads 64 of every 128 bytes) are walked together as well, so that the pieces of a row are
+        // read close in time -- only for tasks no destination group has taken.
+        std::vector<int64_t> skey = {-2, (int64_t)i};
+        if (by_src && cand && T.sstride[0] > T.run_bytes) {
+            skey = grid_key(T);
+            skey.push_back(-3); skey.push_back(T.src_buf); skey.push_back(T.src_off / T.sstride[0]);
+            for (int d = 0; d < T.nd; d++) { skey.push_back(T.ext[d]); skey.push_back(T.sstride[d]); }
+        }
+        src_key_of[i] = std::move(skey);
     }
+    for (size_t i = 0; i < n; i++)                             // tasks left alone by the destination rule: group by source
+        if (buckets[key_of[i]].size() == 1) src_buckets[src_key_of[i]].push_back((uint32_t)i);
+    for (size_t i = 0; i < n; i++) {
+        if (buckets[key_of[i]].size() != 1) continue;
+        const std::vector<uint32_t> &sb = src_buckets[src_key_of[i]];
+        if (sb.size() > 1) { key_of[i] = src_key_of[i]; }
+    }
+    for (auto &kv : src_buckets)
+        if (kv.second.size() > 1) {
+            for (uint32_t m : kv.second) buckets.erase(std::vector<int64_t>{-1, (int64_t)m});
+            buckets[kv.first] = kv.second;
+        }
     std::vector<RsTask> ordered;
     ordered.reserve(n);
     std::vector<char> done(n, 0);
@@ -252,7 +282,9 @@ void group_interleaved(OpTables *op) {
     for (size_t i = 0; i < n; i++) {
         if (done[i]) continue;
         std::vector<uint32_t> &members = buckets[key_of[i]];
+        const bool src_group = key_of[i].size() > 9 && key_of[i][9] == -3;
         std::stable_sort(members.begin(), members.end(), [&](uint32_t a, uint32_t b) {
+            if (src_group) return op->tasks[a].src_off < op->tasks[b].src_off;
             return op->dsts[(size_t)op->tasks[a].dst_first].off < op->dsts[(size_t)op->tasks[b].dst_first].off;
         });
         op->segs.push_back(RsSeg{0, (uint32_t)ordered.size(), (uint32_t)members.size(), op->tasks[i].n_tiles});
@@ -283,6 +315,8 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
     I.n_dsts = (int32_t)op->dsts.size();
     I.read_bytes = read_bytes;
     I.write_bytes = write_bytes;
+    I.pace_permille = 0;
+    op->pace_permille = 0;
 
     const int path = pick_path(*P, align, min_run, max_run, read_bytes + write_bytes, write_bytes >= 2 * read_bytes, tmap_short, P->A.n_dev, P->B.n_dev);
     const bool short_tmap = path == RS_PATH_TMAP && min_run < RS_BULK_MIN_RUN && !(P->flags & RS_PATH_MASK);
@@ -303,8 +337,8 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
             const double bytes = (double)task_rows(T) * (double)T.run_bytes, tiles = (double)task_tiles_exact(T);
             if (tiles > 0) { filled += bytes; total += tiles * (double)tb0; }
         }
-        const bool underfilled = total > 0 && filled < RS_BULK_MIN_FILL * total;
-        BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled);
+        const bool underfilled = total > 0 && filled < RS_BULK_MIN_FILL * total, tiny_tiles = total > 0 && filled < RS_BULK_TINY_FILL * total;
+        BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled, tiny_tiles);
         // short rows through tensor maps, 1 : 1: open loop enough to want rate matching too (128-byte rows: 5.37 TB/s unpaced, 6.15 at 850)
         if (short_tmap && !sh.pace_permille && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES) sh.pace_permille = RS_PACE_PERMILLE_TMAP_SHORT;
         tile_bytes = sh.tile_bytes;
@@ -337,9 +371,10 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
     // destination rows at a fine grain (not config 4: 3 MiB runs), and not under a schedule: there the tables list
     // the unit tasks in order of S_i and the tiles follow them.
     bool interleaved = false;
-    for (const RsTask &T : op->tasks) interleaved = interleaved || (T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.dstride[0] > T.run_bytes);
-    if (dst_order && !per_task && !P->tune.task_order && P->sched.algorithm == RS_SCHED_NONE && interleaved && op->tasks.size() > 1) {
-        group_interleaved(op);
+    for (const RsTask &T : op->tasks)
+        interleaved = interleaved || (T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && ((dst_order && T.dstride[0] > T.run_bytes) || T.sstride[0] > T.run_bytes));
+    if (!per_task && !P->tune.task_order && P->sched.algorithm == RS_SCHED_NONE && interleaved && op->tasks.size() > 1) {
+        group_interleaved(op, dst_order, /*by_src=*/true);
     } else {
         op->segs.resize(op->tasks.size());
         for (size_t t = 0; t < op->tasks.size(); t++) op->segs[t] = RsSeg{0, (uint32_t)t, 1, op->tasks[t].n_tiles};
@@ -449,7 +484,10 @@ rs_status finish_op(Plan *P, OpTables *op, int64_t read_bytes, int64_t write_byt
     if (st != RS_OK) return st;
     int64_t min_run = INT64_MAX;
     for (const RsTask &T : op->tasks) min_run = std::min(min_run, T.run_bytes);
-    if (op->info.path == RS_PATH_TMAP && !(P->flags & RS_PATH_MASK) && min_run < RS_BULK_MIN_RUN && cover < RS_TMAP_SHORT_MIN_COVER)
+    // (1 : 1 operations whose tiles are tiny -- spans of 1-3 KiB -- are better off in registers, 16 warps per SM: fm_hw 5.7 against
+    // 4.7 TB/s; write-heavy ones are not, the register path has no pacing: fm_hwm 4.7 against 6.0)
+    const bool tiny_11 = write_bytes < 2 * read_bytes && op->info.n_tiles > 0 && read_bytes / op->info.n_tiles < RS_TMAP_SHORT_MIN_TILE;
+    if (op->info.path == RS_PATH_TMAP && !(P->flags & RS_PATH_MASK) && min_run < RS_BULK_MIN_RUN && (cover < RS_TMAP_SHORT_MIN_COVER || tiny_11))
         st = finish_op_impl(P, op, read_bytes, write_bytes, per_task, dst_order, /*tmap_short=*/false, nullptr);
     return st;
 }

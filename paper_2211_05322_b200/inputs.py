@@ -127,6 +127,9 @@ CONFIGS = {
     # the paper's microbenchmark tensor with its LAST dim sharded 8 ways on one side: 128-byte runs (register path at full size)
     "r128": _w("r128", (1024, 1024, 512), "bf16", (2, 4), "R,R,S01", (2, 4), "S01,R,R", "bits", 10),
     "r128m": _w("r128m", (1024, 1024, 512), "bf16", (2, 4), "R,R,S01", (2, 4), "S0,R,R", "bits", 11),
+    # a feature map resharded from a split of H to a split of W: 64-byte rows, 32 of them per span (tiles cannot cross a span)
+    "fm_hw": _w("fm_hw", (64, 640, 64, 64), "fp16", (2, 2), "S0,R,S1,R", (2, 2), "S0,R,R,S1", "bits", 12),
+    "fm_hwm": _w("fm_hwm", (64, 640, 64, 64), "fp16", (1, 2), "R,R,S1,R", (2, 2), "R,R,R,S1", "bits", 13),
     # the same pair with rows that are 16-byte aligned and nothing more (6160-byte runs): the least the TMA path accepts
     "a4":   _w("a4", (32, 2048, 12320), "bf16", (2, 4), "S0,S1,R", (4, 2), "S1,R,S0", "bits", 8),
 }

@@ -219,12 +219,14 @@ def test_unaligned_uneven_full_size(name, path):
 
 
 @pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])
-@pytest.mark.parametrize("name", ["r128", "r128m"])
+@pytest.mark.parametrize("name", ["r128", "r128m", "fm_hw", "fm_hwm"])
 def test_short_rows_full_size(name, path):
     """the paper's microbenchmark tensor with 128-byte runs (last dim sharded 8 ways), 1 : 1 and 1 + 4: tensor-map boxes of 64 rows
-    (AUTO) and the register path"""
+    (AUTO) and the register path; a feature map resharded from a split of H to a split of W (64-byte rows in spans of 32: one FAST tile
+    per span, slices that share source rows walked together), 1 : 1 (AUTO: registers) and 1 + 2 (AUTO: tensor maps)"""
     p = _check_full_size(inputs.get_workload(name), path)
-    assert p.op_info(rs.RS_OP_EXECUTE).path == (rs.RS_PATH_TMAP if path == rs.RS_PATH_AUTO else rs.RS_PATH_LSU)
+    auto = rs.RS_PATH_LSU if name == "fm_hw" else rs.RS_PATH_TMAP
+    assert p.op_info(rs.RS_OP_EXECUTE).path == (auto if path == rs.RS_PATH_AUTO else rs.RS_PATH_LSU)
 
 
 @pytest.mark.parametrize("pair", sorted(inputs.SWEEP_PAIRS))

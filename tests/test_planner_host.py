@@ -533,7 +533,8 @@ def test_plan_is_o_slices_not_o_bytes():
         p = _plan(w.shape, 2, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
         sizes[mib] = [p.op_info(op).table_bytes for op in (rs.RS_OP_EXECUTE, rs.RS_OP_PACK, rs.RS_OP_UNPACK)]
         assert p.op_info(rs.RS_OP_EXECUTE).n_tiles >= (mib << 20) // 16384
-    assert sizes[1] == sizes[64] == sizes[1024] == sizes[4096]
+    assert sizes[1024] == sizes[4096] and max(max(v) for v in sizes.values()) <= 32 * (224 + 16 + 16)   # 32 unit tasks: a task, a destination
+    # and at most one segment each (slices that share rows form one segment, so a small tensor with short runs may have fewer)
     for name in ("c1", "c2", "c3", "c3i", "c3ii", "c4", "sweep_P5_m8_4096MiB", "sweep_P1_m8_4096MiB", "t2_4"):
         w = inputs.get_workload(name)
         e = inputs.elem_bytes(w.dtype)
