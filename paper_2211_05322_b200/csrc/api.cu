@@ -76,6 +76,8 @@ rs_status upload(rs::Plan *P) {
         std::memcpy(host.data() + off, o.segs.data(), o.segs.size() * sizeof(RsSeg));
         off += round256(o.segs.size() * sizeof(RsSeg));
         o.dev.n_segs = (uint32_t)o.segs.size();
+        o.dev.seg_tiles = o.segs.empty() ? 0 : o.segs[0].n_members * o.segs[0].tiles_each;
+        for (const RsSeg &sg : o.segs) if (sg.n_members * sg.tiles_each != o.dev.seg_tiles) o.dev.seg_tiles = 0;
         o.dev.n_tasks = (uint32_t)o.tasks.size();
         o.dev.n_dsts = (uint32_t)o.dsts.size();
         o.dev.early_trigger = 0;

@@ -37,6 +37,7 @@
 #define RS_PACE_PERMILLE_SHORT_DENSE 830   // short rows that are adjacent in the receivers (one bulk store per tile)
 #define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
 #define RS_PACE_PERMILLE_11    880            // 1 : 1 operations made of runs >= 1 MiB: best at 880-900, collapse from 910 (fig5_1x1 6.18 -> 6.56 TB/s,
+#define RS_PACE_PERMILLE_11_SHORT 860          // 1 : 1 operations on the 4-warp shape (rows <= 1 KiB or half-empty slots)
 #define RS_PACE_11_MIN_RUN     (1ll << 20)    //   P6 at 4 GiB 6.56 -> 6.8, unpack of P2 6.59 -> 6.76; runs of 128 KiB: no change; 2-6 KiB rows: 0 to -3 %)
 #define RS_PACE_11_MIN_BYTES   (128ll << 20)
 #define RS_BULK_LONG_RUN       4096
@@ -55,7 +56,6 @@
 #define RS_TMAP_SHORT_MIN_RUN   64          // AUTO: operations made of rows of 64-511 bytes take the tensor-map kernel when they are past the
 #define RS_TMAP_SHORT_MIN_COVER 0.9        //   small-operation size and >= 90 % of their bytes move as whole boxes (else the register path)
 #define RS_TMAP_SHORT_MIN_TILE  3584        //   ... and, when 1 : 1, their tiles hold at least this much
-#define RS_PACE_PERMILLE_TMAP_SHORT 850    // ... paced when 1 : 1 (write-heavy ones: RS_PACE_PERMILLE_SHORT)
 #define RS_TMAP_MAX_BYTES    (320ll << 20)  // AUTO: tensor-map copies for short-row operations moving up to this much
 
 // TMA loads + shifted register stores (unaligned layouts): the stores are ALU work, so more warps, smaller tiles

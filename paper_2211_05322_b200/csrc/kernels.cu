@@ -70,7 +70,7 @@ template <int NP>
 __device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsTables &tb, const RsPtrTableT<NP> &ptrs, uint32_t tile_index,
                                              RsDesc *out) {
     uint32_t task, u;
-    rs_tile_locate(tb.segs, op.n_segs, op.tile_base + tile_index, &task, &u);
+    rs_tile_locate(tb.segs, op.n_segs, op.tile_base + tile_index, &task, &u, op.seg_tiles);
     const RsTask *__restrict__ T = tb.tasks + task;
     const RsTile tile = rs_tile_decode(*T, task, u);
     RsDesc d;

@@ -217,7 +217,11 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     // take a higher rate than rows stored one by one (Table 2 case 9: 6.12 TB/s at 810, 6.26 at 830, 6.35-6.40 at 850 on two
     // boxes but 5.98 on a third, whose edge lies lower: 830)
     sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
-                     : long_11 ? RS_PACE_PERMILLE_11 : 0;
+                     : long_11 ? RS_PACE_PERMILLE_11
+                     // 1 : 1 on the 4-warp shape (rows <= 1 KiB, half-empty slots): twice the pipelines per SM make the loop open enough to want
+                     // pacing too (a4 6.09 -> 6.33-6.48 TB/s at 850-870, 1 KiB rows on 4x8 -> 8x4 meshes 5.81 -> 6.04, 128-byte rows through
+                     // tensor maps 5.37 -> 6.15-6.33; collapse at 890); the 2-warp shape loses 3 % when paced
+                     : !shift && !write_heavy && short_runs && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES ? RS_PACE_PERMILLE_11_SHORT : 0;
     return sh;
 }
 
@@ -319,7 +323,6 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
     op->pace_permille = 0;
 
     const int path = pick_path(*P, align, min_run, max_run, read_bytes + write_bytes, write_bytes >= 2 * read_bytes, tmap_short, P->A.n_dev, P->B.n_dev);
-    const bool short_tmap = path == RS_PATH_TMAP && min_run < RS_BULK_MIN_RUN && !(P->flags & RS_PATH_MASK);
     I.path = path;
     const bool bulk_family = path == RS_PATH_BULK || path == RS_PATH_BULK_SHIFT || path == RS_PATH_TMAP;
 
@@ -339,8 +342,6 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
         }
         const bool underfilled = total > 0 && filled < RS_BULK_MIN_FILL * total, tiny_tiles = total > 0 && filled < RS_BULK_TINY_FILL * total;
         BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled, tiny_tiles);
-        // short rows through tensor maps, 1 : 1: open loop enough to want rate matching too (128-byte rows: 5.37 TB/s unpaced, 6.15 at 850)
-        if (short_tmap && !sh.pace_permille && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES) sh.pace_permille = RS_PACE_PERMILLE_TMAP_SHORT;
         tile_bytes = sh.tile_bytes;
         stages = sh.stages;
         op->pace_permille = sh.pace_permille;

@@ -106,6 +106,8 @@ struct RsOpDev {                         // one operation's tables in device mem
     uint32_t tile_base;                  // first tile of this launch (a slab of reshard_execute_host), else 0
     uint32_t n_tiles;                    // tiles of this launch
     uint32_t n_tasks, n_dsts;            // table sizes: small tables are staged in shared memory by the register kernel
+    uint32_t seg_tiles;                  // > 0: every segment holds this many tiles, so tile t lies in segment t / seg_tiles (no search:
+                                         // a plan of a thousand equal unit tasks would pay ten dependent table reads per tile)
     uint32_t early_trigger;              // 1: the grid covers every SM, so the next kernel of the stream may be launched at once
                                          // (programmatic dependent launch); 0: only when this kernel's CTAs run out of tiles
 };
@@ -169,8 +171,8 @@ RS_HD RsTile rs_tile_decode(const RsTask &T, uint32_t task_id, uint32_t u) {
 }
 
 // tile t of an operation: which task, which of its tiles
-RS_HD void rs_tile_locate(const RsSeg *segs, uint32_t n_segs, uint32_t t, uint32_t *task, uint32_t *u) {
-    const RsSeg s = segs[rs_find_seg(segs, n_segs, t)];
+RS_HD void rs_tile_locate(const RsSeg *segs, uint32_t n_segs, uint32_t t, uint32_t *task, uint32_t *u, uint32_t seg_tiles = 0) {
+    const RsSeg s = segs[seg_tiles ? t / seg_tiles : rs_find_seg(segs, n_segs, t)];
     const uint32_t v = t - s.tile_begin;
     if (s.n_members == 1) { *task = s.first_task; *u = v; return; }
     const uint32_t q = v / s.n_members;

@@ -207,7 +207,13 @@ def unet_workload(level):
 
 
 def get_workload(name):
-    """'c1'..'c4', 'c1i', 'c3i', 'c3ii', 'u4', 't2_<case>', 'sweep_<pair>_<m8|m4>_<MiB>', 'fig5_<nodes>x<gpus>'."""
+    """'c1'..'c4', 'c1i', 'c3i', 'c3ii', 'u4', 't2_<case>', 'sweep_<pair>_<m8|m4>_<MiB>', 'fig5_<nodes>x<gpus>', or any task as
+    'x:<shape>:<dtype>:<src mesh>:<src spec>:<dst mesh>:<dst spec>'."""
+    if name.startswith("x:"):
+        # any task spelled out: x:<shape>:<dtype>:<src mesh>:<src spec>:<dst mesh>:<dst spec>, e.g. x:64x2048x4096:bf16:4x8:S0S1R:8x4:S1RS0 (specs without commas, so that names can be listed)
+        _x, shape, dtype, sm, ss, dm, ds = name.split(":")
+        dims = lambda s: tuple(int(v) for v in s.split("x"))
+        return _w(name, dims(shape), dtype, dims(sm), ss, dims(dm), ds, "bits", 99)
     if name.startswith("unet_l"):
         return unet_workload(int(name[6:]))
     if name.startswith("fig5_"):

@@ -483,7 +483,7 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("c3") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 20 + 20 MiB: the TMA ring from 32 MiB moved on
     assert shape_of("sweep_P1_m8_16MiB")[:2] == (rs.RS_PATH_LSU, 4 * 148)         # small operations: register path, 4 CTAs per SM
     assert shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU
-    assert shape_of("r128") == (rs.RS_PATH_TMAP, 148, 128, 850)                   # 128-byte rows at 1 + 1 GiB: boxes of 64 rows, paced
+    assert shape_of("r128") == (rs.RS_PATH_TMAP, 148, 128, 860)                   # 128-byte rows at 1 + 1 GiB: boxes of 64 rows, paced
     assert shape_of("r128m") == (rs.RS_PATH_TMAP, 148, 128, 810)                  # ... 1 + 4 GiB
     assert shape_of("r128", rs.RS_OP_PACK)[0] == rs.RS_PATH_BULK                  # its pack copies whole 64 KiB runs
     p = _plan((262144, 4, 64), 2, (2,), "R,R,S0", (2,), "R,S0,R", 0)              # 64-byte rows, but only 2 per span: no box fits
