@@ -478,7 +478,11 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, cap));
         dev.early_trigger = grid >= P.sm_count;
         if (align < 16) e = rs::launch_shift(dev, pt, small, grid, pdl, st);   // any alignment, still 16-byte accesses
-        else e = rs::launch_lsu(dev, pt, small, grid, pdl, st);
+        else {
+            bool generic = false;
+            for (const RsTask &T : op.tasks) generic = generic || T.kind == RS_TILING_GENERIC;
+            e = rs::launch_lsu(dev, pt, small, generic, grid, pdl, st);
+        }
     }
     if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
     return RS_OK;

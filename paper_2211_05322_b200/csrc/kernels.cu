@@ -109,10 +109,42 @@ template <> __device__ __forceinline__ void st_stream<uint4>(char *p, const uint
                  :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// GENERIC tiles (spans of the innermost row dim under 1 KiB): every vector decodes its own row (divisions), U loads in
+// flight per lane as in the fast walk.
+template <typename V, int U, int NP>
+__device__ __forceinline__ void lsu_generic_tile(const RsTask *__restrict__ T, const RsDst *__restrict__ dsts, const RsPtrTableT<NP> &ptrs,
+                                              const char *src, int64_t dst_rel, uint64_t lin, uint32_t total, uint32_t vpr, uint32_t k, int lane) {
+    constexpr uint32_t VB = sizeof(V);
+    for (uint32_t v0 = lane; v0 < total; v0 += 32 * U) {
+        V data[U];
+        int64_t doffs[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const uint32_t v = v0 + 32 * u;
+            if (v < total) {
+                const uint32_t r = v / vpr, c = v - r * vpr;
+                int64_t so, doff;
+                generic_row(T, lin + r, &so, &doff);
+                doffs[u] = dst_rel + doff + (int64_t)c * VB;
+                data[u] = ld_stream<V>(src + dst_rel + so + (int64_t)c * VB);
+            }
+        }
+        for (uint32_t j = 0; j < k; j++) {
+            const RsDst dd = dsts[j];
+            char *dp = ptrs.dst[dd.buf] + dd.off;
+#pragma unroll
+            for (int u = 0; u < U; u++)
+                if (v0 + 32 * u < total) st_stream<V>(dp + doffs[u], data[u]);
+        }
+    }
+}
+
 // Every WARP is an independent worker (no CTA-wide synchronisation anywhere).  Inside a tile the
 // warp walks the (row, column) grid of V-sized vectors 32 at a time; (row, col) advance incrementally,
 // so the only integer division is one per tile.  U loads are issued back to back, then U x k stores.
-template <typename V, int U, int NP>
+// GEN: the operation has GENERIC tiles.  Two instantiations, because the generic walk costs the fast one registers (64 per thread is
+// the budget of 4 CTAs per SM): operations without GENERIC tiles -- nearly all -- run the kernel that does not contain it.
+template <typename V, int U, int NP, bool GEN>
 __global__ void __launch_bounds__(RS_LSU_THREADS, RS_LSU_CTAS_PER_SM)
 rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
     constexpr uint32_t VB = sizeof(V);
@@ -156,17 +188,8 @@ rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
         const char *src = d->src;
         const int64_t s0 = d->s0, d0 = d->d0, dst_rel = d->dst_rel;
         const RsTask *__restrict__ T = tb.tasks + d->task;
-        if (!fast) {                                          // GENERIC tiles (rare): one vector at a time
-            for (uint32_t v = lane; v < total; v += 32) {
-                const uint32_t r = v / vpr, c = v - r * vpr;
-                int64_t so, doff;
-                generic_row(T, d->lin + r, &so, &doff);
-                const V x = ld_stream<V>(src + dst_rel + so + (int64_t)c * VB);
-                for (uint32_t j = 0; j < k; j++) {
-                    const RsDst dd = dsts[j];
-                    st_stream<V>(ptrs.dst[dd.buf] + dd.off + dst_rel + doff + (int64_t)c * VB, x);
-                }
-            }
+        if (GEN && !fast) {
+            lsu_generic_tile<V, U, NP>(T, dsts, ptrs, src, dst_rel, d->lin, total, vpr, k, lane);
             continue;
         }
         const uint32_t q32 = 32u / vpr, r32 = 32u - q32 * vpr;   // how (row, col) move when v += 32
@@ -869,10 +892,14 @@ static cudaError_t launch_k(void (*kernel)(KArgs...), int grid, int block, size_
     return launched(cudaLaunchKernelEx(&cfg, kernel, args...));
 }
 
-cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st) {
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, bool generic, int grid, bool pdl, cudaStream_t st) {
     constexpr int U = RS_LSU_UNROLL / 2;                       // 64 B in flight per thread
-    if (small) return launch_k(rs_copy_lsu<uint4, U, RS_PTRS_SMALL>, grid, RS_LSU_THREADS, 0, st, pdl, op, small_table(ptrs));
-    return launch_k(rs_copy_lsu<uint4, U, 128>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);
+    if (generic) {
+        if (small) return launch_k(rs_copy_lsu<uint4, U, RS_PTRS_SMALL, true>, grid, RS_LSU_THREADS, 0, st, pdl, op, small_table(ptrs));
+        return launch_k(rs_copy_lsu<uint4, U, 128, true>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);
+    }
+    if (small) return launch_k(rs_copy_lsu<uint4, U, RS_PTRS_SMALL, false>, grid, RS_LSU_THREADS, 0, st, pdl, op, small_table(ptrs));
+    return launch_k(rs_copy_lsu<uint4, U, 128, false>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);
 }
 
 cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st) {

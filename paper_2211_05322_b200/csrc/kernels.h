@@ -8,7 +8,8 @@
 namespace rs {
 // `pdl`: launch with the programmatic-stream-serialization attribute (kernels.cu).
 // `small`: every buffer index of the launch is below RS_PTRS_SMALL, so the 256-byte pointer table is enough
-cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st);      // 16-byte aligned only
+// generic: the operation has GENERIC tiles (the other instantiation does not contain their walk)
+cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, bool generic, int grid, bool pdl, cudaStream_t st);      // 16-byte aligned only
 cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st);
 cudaError_t prepare_bulk(int smem_bytes);                                             // both TMA kernels, both table sizes
 // pace: nanoseconds a warp lets pass per byte of DRAM traffic of its tiles (rate matching, kernels.cu); 0 = unpaced

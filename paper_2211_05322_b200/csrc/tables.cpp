@@ -469,6 +469,14 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
     }
     if (lsu) {
         const int warps = RS_LSU_THREADS / 32;
+        // GENERIC tiles decode every vector's row (divisions): instruction-bound, so more warps per SM than the DRAM-bound
+        // fast walk wants (spans of 128 bytes, 320 + 640 MiB: 2.8 TB/s with 1 CTA per SM, 4.2 with 2; 1 : 1: 3.3 with 2, 4.1 with 4)
+        bool generic = false;
+        for (const RsTask &T : op->tasks) generic = generic || T.kind == RS_TILING_GENERIC;
+        if (generic && !P->tune.lsu_ctas_per_sm && I.path == RS_PATH_LSU) {
+            I.grid = P->sm_count * (write_bytes >= 2 * read_bytes ? 2 : RS_LSU_CTAS_PER_SM);
+            if (P->max_ctas > 0) I.grid = std::min(I.grid, P->max_ctas);
+        }
         int64_t want = (I.n_tiles + warps - 1) / warps;
         if (want < P->sm_count) want = std::min<int64_t>(I.n_tiles, P->sm_count);   // few tiles: still one CTA on every SM (api.cu)
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, want));
