@@ -40,7 +40,9 @@ struct alignas(16) RsDesc {
     const char *src;                     // FAST: address of the tile's first source byte; GENERIC: box origin
     int64_t dst_rel;                     // FAST: tile.b; GENERIC: byte offset inside the run
     int64_t s0, d0;                      // row strides (FAST)
-    uint64_t lin;                        // GENERIC: linear index of the first row
+    uint64_t lin;                        // GENERIC: linear index of the first row; RS_TILE_K1 (FAST tile of a task with ONE receiver): the
+                                         // address of the tile's first destination byte, so that the store side of the per-tile path
+                                         // reads no table at all (a plan of a thousand unit tasks misses L1 on every tile's RsDst)
     uint32_t n_rows, col_bytes, flags, k, dst_first, task;
 };
 static_assert(sizeof(RsDesc) == 64, "descriptor ring slot");
@@ -81,6 +83,11 @@ __device__ __forceinline__ void resolve_desc(const RsOpDev &op, const RsTables &
     d.lin = tile.a;
     d.n_rows = tile.n_rows; d.col_bytes = tile.col_bytes; d.flags = tile.flags;
     d.k = (uint32_t)T->k; d.dst_first = (uint32_t)T->dst_first; d.task = tile.task;
+    if ((tile.flags & RS_TILE_FAST) && T->k == 1) {
+        const RsDst D = tb.dsts[T->dst_first];
+        d.lin = (uint64_t)(uintptr_t)(ptrs.dst[D.buf] + D.off + (int64_t)tile.b);
+        d.flags |= RS_TILE_K1;
+    }
     *out = d;
 }
 
@@ -204,8 +211,9 @@ rs_copy_lsu(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs) {
                 if (c >= vpr) { c -= vpr; r++; }
             }
             for (uint32_t j = 0; j < k; j++) {                // read once, write k times
-                const RsDst dd = dsts[j];
-                char *dp = ptrs.dst[dd.buf] + dd.off + dst_rel;
+                char *dp;
+                if (d->flags & RS_TILE_K1) dp = reinterpret_cast<char *>((uintptr_t)d->lin);
+                else { const RsDst dd = dsts[j]; dp = ptrs.dst[dd.buf] + dd.off + dst_rel; }
                 uint32_t r2 = row, c2 = col;                  // offsets are recomputed, not kept in registers
 #pragma unroll
                 for (int u = 0; u < U; u++) {
@@ -461,7 +469,7 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
                             const uint64_t y = addr / (uint64_t)dd->s0;
                             dd->lin = (y << 32) | (uint64_t)((addr - y * (uint64_t)dd->s0) / RS_TMAP_ELEM);
                             dd->task = (uint32_t)T->src_buf;
-                            dd->flags |= RS_TILE_TMAP;
+                            dd->flags = (dd->flags | RS_TILE_TMAP) & ~RS_TILE_K1;
                         }
                     }
                 }
@@ -516,10 +524,17 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
             } else if (fast && (d->d0 == (int64_t)col_bytes || n_rows == 1)) {
                 // rows adjacent in the destinations (a message, or a shard whose rows the slice covers whole): lane q
                 // stores the tile to receiver q with ONE bulk copy
+                if (d->flags & RS_TILE_K1) {
+                    if (lane == 0) bulk_s2g(reinterpret_cast<char *>((uintptr_t)d->lin), slot, n_rows * col_bytes);
+                } else
                 for (uint32_t q = lane; q < k; q += 32) {
                     const RsDst dd = dsts[q];
                     bulk_s2g(ptrs.dst[dd.buf] + dd.off + d->dst_rel, slot, n_rows * col_bytes);
                 }
+            } else if (d->flags & RS_TILE_K1) {               // one receiver, rows apart: lane r stores row r, no table read
+                char *base = reinterpret_cast<char *>((uintptr_t)d->lin);
+                const int64_t d0 = d->d0;
+                for (uint32_t r = lane; r < n_rows; r += 32) bulk_s2g(base + (int64_t)r * d0, slot + r * col_bytes, col_bytes);
             } else {
                 const RsTask *__restrict__ T = op.tasks + d->task;
                 for (uint32_t r = lane; r < n_rows; r += 32) {

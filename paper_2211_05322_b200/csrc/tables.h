@@ -69,7 +69,7 @@ struct alignas(16) RsSeg {
     uint32_t tiles_each;                 // tiles per member
 };
 
-enum : uint32_t { RS_TILE_FAST = 1u, RS_TILE_TMAP = 2u };
+enum : uint32_t { RS_TILE_FAST = 1u, RS_TILE_TMAP = 2u, RS_TILE_K1 = 4u };   // K1: kernel-side only (kernels.cu RsDesc)
 
 #define RS_TMAP_BUFS 16                  // tensor maps per side in the kernel parameter
 #define RS_TMAP_ELEM 8                   // tensor-map element: UINT64 (the widest): boxes of up to 256 x 8 = 2048 bytes per row
