@@ -531,11 +531,8 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
                     const RsDst dd = dsts[q];
                     bulk_s2g(ptrs.dst[dd.buf] + dd.off + d->dst_rel, slot, n_rows * col_bytes);
                 }
-            } else if (d->flags & RS_TILE_K1) {               // one receiver, rows apart: lane r stores row r, no table read
-                char *base = reinterpret_cast<char *>((uintptr_t)d->lin);
-                const int64_t d0 = d->d0;
-                for (uint32_t r = lane; r < n_rows; r += 32) bulk_s2g(base + (int64_t)r * d0, slot + r * col_bytes, col_bytes);
-            } else {
+            } else {                                          // (rows apart: the table read stays -- taking it out made the row stores of
+                                                              // P1 / P4 issue faster and the launch 3-6 % SLOWER, the open-loop effect again)
                 const RsTask *__restrict__ T = op.tasks + d->task;
                 for (uint32_t r = lane; r < n_rows; r += 32) {
                     int64_t doff;
