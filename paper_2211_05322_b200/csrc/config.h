@@ -52,6 +52,7 @@
 #define RS_BULK_STAGES_SMALL_MCAST     3       //  4 + 32 MiB: 7.5 us either way; from 16 + 64 MiB on the default shape)
 #define RS_BULK_TILE_BYTES_SMALL_MCAST 4096
 #define RS_INTERLEAVE_MAX_RUN (64 << 10)    // destination runs up to this long count as a fine interleave (tile order)
+#define RS_SHIFT_MIN_RUN     128        // ... unaligned layouts: rs_copy_bulk_shift from rows of 128 bytes on (large operations)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 #define RS_TMAP_SHORT_MIN_RUN   64          // AUTO: operations made of rows of 64-511 bytes take the tensor-map kernel when they are past the
 #define RS_TMAP_SHORT_MIN_COVER 0.9        //   small-operation size and >= 90 % of their bytes move as whole boxes (else the register path)

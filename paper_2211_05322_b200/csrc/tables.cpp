@@ -152,7 +152,9 @@ int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, in
     int path = forced == RS_PATH_LSU ? RS_PATH_LSU : forced == RS_PATH_BULK ? RS_PATH_BULK
              : forced == RS_PATH_TMAP ? (bulk_ok ? RS_PATH_TMAP : RS_PATH_BULK_SHIFT)
              : forced == RS_PATH_BULK_SHIFT ? RS_PATH_BULK_SHIFT
-             : min_run < RS_BULK_MIN_RUN ? (short_tmap ? RS_PATH_TMAP : RS_PATH_LSU)
+             // (rows of 128-511 bytes that are NOT 16-byte aligned: TMA loads + shifted register stores beat the register shift
+             //  kernel once the operation is large -- 130-byte rows 1.57 -> 2.05 TB/s, 257-byte rows 1.94 -> 2.92; 63-byte rows: a tie)
+             : min_run < RS_BULK_MIN_RUN ? (short_tmap ? RS_PATH_TMAP : !bulk_ok && min_run >= RS_SHIFT_MIN_RUN && moved_bytes > small_op ? RS_PATH_BULK_SHIFT : RS_PATH_LSU)
              : bulk_ok ? (moved_bytes <= small_op ? RS_PATH_LSU : RS_PATH_BULK)
              : RS_PATH_BULK_SHIFT;
     // Mid-size operations made of short rows (config 2: 2 KiB destination runs, 128 + 128 MiB) are the one place

@@ -206,7 +206,7 @@ def test_tensor_map_path_full_size(name):
 
 
 @pytest.mark.parametrize("path", [rs.RS_PATH_AUTO, rs.RS_PATH_LSU])
-@pytest.mark.parametrize("name", ["u4", "u4b", "u1", "a4"])
+@pytest.mark.parametrize("name", ["u4", "u4b", "u1", "a4", "x:1024x1024x1040:u8:2x4:RRS01:2x4:S01RR"])   # the last: 130-byte rows at 1-byte alignment
 def test_unaligned_uneven_full_size(name, path):
     """1-1.5 GiB with nothing aligned (a4: 16-byte aligned and nothing more): TMA loads + shifted stores (AUTO; bulk stores of
     realigned rows for u4 / u4b, register stores for u1's 2 KiB rows, the plain TMA ring for a4) and the register path (LSU)"""
