@@ -243,7 +243,7 @@ void group_interleaved(OpTables *op, bool by_dst, bool by_src) {
     for (size_t i = 0; i < n; i++) {
         const RsTask &T = op->tasks[i];
         std::vector<int64_t> key;
-        const bool cand = T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN && T.kind != RS_TILING_GENERIC;
+        const bool cand = T.nd >= 1 && T.run_bytes <= RS_INTERLEAVE_MAX_RUN;   // (GENERIC tiles too: equal grids cover equal rows)
         if (by_dst && cand && T.dstride[0] > T.run_bytes) {
             const RsDst &D0 = op->dsts[(size_t)T.dst_first];
             key = grid_key(T);
