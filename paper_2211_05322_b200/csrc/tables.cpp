@@ -342,7 +342,12 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
             const double bytes = (double)task_rows(T) * (double)T.run_bytes, tiles = (double)task_tiles_exact(T);
             if (tiles > 0) { filled += bytes; total += tiles * (double)tb0; }
         }
-        const bool underfilled = total > 0 && filled < RS_BULK_MIN_FILL * total, tiny_tiles = total > 0 && filled < RS_BULK_TINY_FILL * total;
+        bool underfilled = total > 0 && filled < RS_BULK_MIN_FILL * total;
+        const bool tiny_tiles = total > 0 && filled < RS_BULK_TINY_FILL * total;
+        // 1 : 1 operations in the tensor-map window (rows <= 2 KiB, 128-320 MiB moved: config 2) also take the 4-warp shape and with it the
+        // pacing of that shape: config 2 43.6 -> 41.8 us (torch copy_ 42.4), its unpack 43.1 -> 41.6, 64 + 64 MiB 22.2-22.4 -> 21.7-22.0;
+        // unpaced the 4 warps lose (45.5 us)
+        if (path == RS_PATH_TMAP && write_bytes < 2 * read_bytes && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES) underfilled = true;
         BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled, tiny_tiles);
         tile_bytes = sh.tile_bytes;
         stages = sh.stages;
