@@ -40,6 +40,7 @@
 #define RS_PACE_PERMILLE_11_SHORT 860          // 1 : 1 operations on the 4-warp shape (rows <= 1 KiB or half-empty slots)
 #define RS_PACE_11_MIN_RUN     (1ll << 20)    //   P6 at 4 GiB 6.56 -> 6.8, unpack of P2 6.59 -> 6.76; runs of 128 KiB: no change; 2-6 KiB rows: 0 to -3 %)
 #define RS_PACE_11_MIN_BYTES   (128ll << 20)
+#define RS_MID_MCAST_BYTES     (768ll << 20)  // paced write-heavy operations moving up to this much: the 4-warp shape
 #define RS_BULK_LONG_RUN       4096
 #define RS_BULK_CTAS_MIN_BYTES (384ll << 20)   // operations moving less than this keep one CTA on every SM (config 2's pack, 128 + 128 MiB:
                                                // 46.1 us on 132 CTAs, 43.3 us on 148; at 256 + 256 MiB the two are level, beyond 132 wins)

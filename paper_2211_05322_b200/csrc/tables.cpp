@@ -187,13 +187,16 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     // ... and so do tiles of 1-4 KiB (a span of the innermost row dim that short: feature maps resharded across H / W): at ~1 340 cycles
     // per tile and warp, 2 KiB tiles need 8 warps per SM (fm_hw: 2.6 TB/s with 4 warps, 4.4 with 8 before source-order segments)
     const bool small_mcast = !shift && !capped && (tiny_tiles || (write_bytes >= 2 * read_bytes && read_bytes + write_bytes <= RS_SMALL_MCAST_BYTES));
+    // paced write-heavy operations of medium size ramp faster on 4 warps x 8 KiB (16 + 128 MiB: 26.0 -> 25.3 us, 64 + 512 MiB +1.4 %; from ~1 GiB moved
+    // on the two shapes are level)
+    const bool mid_mcast = !shift && !capped && write_bytes >= 2 * read_bytes && read_bytes + write_bytes >= RS_PACE_MIN_BYTES && read_bytes + write_bytes <= RS_MID_MCAST_BYTES;
     BulkShape sh;
     sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : shift_mid ? RS_SHIFT_WARPS_MID : RS_SHIFT_WARPS)
-                                             : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : short_runs || capped ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
+                                             : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : short_runs || capped || mid_mcast ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
     sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : shift_mid ? RS_SHIFT_STAGES_MID : RS_SHIFT_STAGES)
                                               : pick(U.bulk_stages, small_mcast ? RS_BULK_STAGES_SMALL_MCAST : RS_BULK_STAGES)));
     sh.tile_bytes = shift ? pick(U.shift_tile_bytes, RS_SHIFT_TILE_BYTES)
-                          : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : short_runs ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
+                          : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : short_runs || mid_mcast ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
     sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
     while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
     // One CTA per SM.

@@ -474,7 +474,7 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("sweep_P5_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 148, 64, 880)   # its unpack is a 1 : 1 copy of 512 MiB runs: paced too
     assert shape_of("fig5_1x1") == (rs.RS_PATH_BULK, 148, 64, 880)                # one sender, one receiver, one 1 GiB run
     assert shape_of("t2_4") == (rs.RS_PATH_BULK, 132, 64, 0)                      # 128 KiB runs, 1 : 1: unpaced, trimmed grid
-    assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 64, 850)       # write-heavy at any size
+    assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 128, 850)      # write-heavy, 144 MiB moved: paced, 4 warps
     assert shape_of("t2_9") == (rs.RS_PATH_BULK, 148, 128, 830)                   # 512-byte runs, 1 + 4: 4 warps; rows adjacent in the receivers
     assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 192, 0)                 # nothing aligned, 6 KiB rows: 6 warps, bulk stores
     assert shape_of("u1") == (rs.RS_PATH_BULK_SHIFT, 148, 224, 0)                 # nothing aligned, 2 KiB rows: 7 warps, register stores
