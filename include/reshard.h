@@ -128,6 +128,7 @@ typedef struct rs_tuning {
                                                           peak (2 x memory clock x bus width); -1: unpaced; 0 = default */
     int32_t no_pdl;                                    /* 1: launch without programmatic dependent launch (a kernel then
                                                           starts only after the previous kernel of the stream has ended) */
+    int32_t pace_burst;                                /* rate matching: tiles of credit a warp that fell behind may catch up with; 0 = default (2) */
     int32_t shift_mode;                                /* rs_copy_bulk_shift, rows >= 1 KiB: 0 = library default; 1: windows
                                                           assembled in registers and stored with st.global; 2: row bodies
                                                           realigned in shared memory and stored with cp.async.bulk      */

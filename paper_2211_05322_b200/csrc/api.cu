@@ -447,16 +447,17 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         dev.early_trigger = grid >= P.sm_count;
         // rate matching: the launch as a whole offers pace_permille / 1000 of the DRAM peak
         const int permille = P.tune.pace_permille > 0 ? P.tune.pace_permille : P.tune.pace_permille < 0 ? 0 : op.pace_permille;
+        const int burst = P.tune.pace_burst > 0 ? P.tune.pace_burst : RS_PACE_BURST;
         const float pace = permille > 0 ? (float)((double)grid * warps / (P.dram_peak_gbs * permille / 1000.0)) : 0.f;
         if (op.info.path == RS_PATH_TMAP && small) {          // tensor maps of this call's pointers, then the same ring kernel
             alignas(64) unsigned char tm[RS_TMAP_TABLE_BYTES];
             rs_status ts = encode_tmaps(op, pt, tm);
             if (ts != RS_OK) return ts;
             e = rs::launch_tmap(dev, pt, tm, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
-                                (uint32_t)op.info.tile_bytes, pace, pdl, st);
+                                (uint32_t)op.info.tile_bytes, pace, burst, pdl, st);
         } else
         e = rs::launch_bulk(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
-                            (uint32_t)op.info.tile_bytes, pace, pdl, st);
+                            (uint32_t)op.info.tile_bytes, pace, burst, pdl, st);
     } else if (op.info.path == RS_PATH_BULK_SHIFT) {          // layout not 16-byte aligned: TMA loads, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         dev.early_trigger = grid >= P.sm_count;

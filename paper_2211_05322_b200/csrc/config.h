@@ -32,6 +32,7 @@
 // offers this many permille of the DRAM peak (2 x memory clock x bus width = 7 672 GB/s on B200).  Measured
 // (profiles/r02_pacing.md): achieved = 0.99 x offered up to 860 permille (6.52 TB/s on 1 + 8), collapse from 880 on
 // (6.09, then 5.56 at 920; unpaced 5.66); runs of 512 B: up to 820 (6.18 TB/s), 6.00 at 840.  10 permille below the edge.
+#define RS_PACE_BURST          2              // tiles of credit of the token bucket
 #define RS_PACE_PERMILLE       850
 #define RS_PACE_PERMILLE_SHORT 810
 #define RS_PACE_PERMILLE_SHORT_DENSE 830   // short rows that are adjacent in the receivers (one bulk store per tile)

@@ -400,7 +400,7 @@ __device__ __forceinline__ uint64_t global_ns() {             // 32 ns resolutio
 // (reads + k writes) may start `pace` x b nanoseconds after the previous one, pace = workers / target rate; the target
 // is a fraction of the DRAM peak read from the device (api.cu).  A token bucket with a burst of two tiles: a warp
 // that is behind schedule (HBM slower than the target, another kernel running beside) never waits.
-__device__ __forceinline__ void pace_tile(uint64_t &t_next, float pace, uint32_t traffic_bytes, int lane) {
+__device__ __forceinline__ void pace_tile(uint64_t &t_next, float pace, int burst, uint32_t traffic_bytes, int lane) {
     const uint64_t interval = (uint64_t)(pace * (float)traffic_bytes);
     if (lane == 0) {
         uint64_t now = global_ns();
@@ -409,7 +409,8 @@ __device__ __forceinline__ void pace_tile(uint64_t &t_next, float pace, uint32_t
             __nanosleep((unsigned)(left > 2000 ? 2000 : left));
             now = global_ns();
         }
-        const uint64_t floor = now - (now > 2 * interval ? 2 * interval : now);
+        const uint64_t credit = (uint64_t)burst * interval;   // a warp behind schedule may catch up by this much at most
+        const uint64_t floor = now - (now > credit ? credit : now);
         t_next = (t_next > floor ? t_next : floor) + interval;
     }
     __syncwarp();
@@ -434,7 +435,7 @@ __device__ __forceinline__ void tmap_s2g(const RsTmap *map, uint32_t x, uint32_t
 
 template <int NP, bool TMAP>
 __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<NP> &ptrs, const RsTmapTable *tm, const int stages,
-                                          const int lookahead, const uint32_t stage_bytes, const float pace) {
+                                          const int lookahead, const uint32_t stage_bytes, const float pace, const int burst) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const uint32_t bars = smem_u32(smem) + warp * 64;                       // <= 8 mbarriers per warp
@@ -482,7 +483,7 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
             }
             const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
             const uint32_t n_rows = d->n_rows, col_bytes = d->col_bytes;
-            if (pace > 0.f) pace_tile(t_next, pace, n_rows * col_bytes * (1u + d->k), lane);
+            if (pace > 0.f) pace_tile(t_next, pace, burst, n_rows * col_bytes * (1u + d->k), lane);
             const uint32_t bar = bars + 8 * ld_slot, slot = ring + (uint32_t)ld_slot * stage_bytes;
             if (lane == 0) mbar_expect_tx(bar, n_rows * col_bytes);
             __syncwarp();
@@ -560,14 +561,14 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
 template <int NP>
 __global__ void __launch_bounds__(256, 1)
 rs_copy_bulk(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
-             const uint32_t stage_bytes, const float pace) {
-    bulk_body<NP, false>(op, ptrs, nullptr, stages, lookahead, stage_bytes, pace);
+             const uint32_t stage_bytes, const float pace, const int burst) {
+    bulk_body<NP, false>(op, ptrs, nullptr, stages, lookahead, stage_bytes, pace, burst);
 }
 
 __global__ void __launch_bounds__(256, 1)
 rs_copy_tmap(const RsOpDev op, const __grid_constant__ RsPtrTableT<RS_PTRS_SMALL> ptrs, const __grid_constant__ RsTmapTable tm,
-             const int stages, const int lookahead, const uint32_t stage_bytes, const float pace) {
-    bulk_body<RS_PTRS_SMALL, true>(op, ptrs, &tm, stages, lookahead, stage_bytes, pace);
+             const int stages, const int lookahead, const uint32_t stage_bytes, const float pace, const int burst) {
+    bulk_body<RS_PTRS_SMALL, true>(op, ptrs, &tm, stages, lookahead, stage_bytes, pace, burst);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -935,17 +936,17 @@ cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool sm
 }
 
 cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,
-                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st) {
+                        int lookahead, uint32_t stage_bytes, float pace, int burst, bool pdl, cudaStream_t st) {
     static_assert(sizeof(RsTmapTable) == RS_TMAP_TABLE_BYTES, "kernels.h and the tensor-map table disagree");
     RsTmapTable tm;
     memcpy(&tm, tmaps, sizeof(tm));
-    return launch_k(rs_copy_tmap, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), tm, stages, lookahead, stage_bytes, pace);
+    return launch_k(rs_copy_tmap, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), tm, stages, lookahead, stage_bytes, pace, burst);
 }
 
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes, int stages,
-                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st) {
-    if (small) return launch_k(rs_copy_bulk<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes, pace);
-    return launch_k(rs_copy_bulk<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes, pace);
+                        int lookahead, uint32_t stage_bytes, float pace, int burst, bool pdl, cudaStream_t st) {
+    if (small) return launch_k(rs_copy_bulk<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes, pace, burst);
+    return launch_k(rs_copy_bulk<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes, pace, burst);
 }
 
 }  // namespace rs

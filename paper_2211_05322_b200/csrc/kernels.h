@@ -13,8 +13,9 @@ cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, bo
 cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st);
 cudaError_t prepare_bulk(int smem_bytes);                                             // both TMA kernels, both table sizes
 // pace: nanoseconds a warp lets pass per byte of DRAM traffic of its tiles (rate matching, kernels.cu); 0 = unpaced
+// burst: tiles of credit a warp that fell behind may catch up with
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes, int stages,
-                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st);
+                        int lookahead, uint32_t stage_bytes, float pace, int burst, bool pdl, cudaStream_t st);
 // mode: RS_SHIFT_REG (register stores) or RS_SHIFT_BULK (bodies of long rows realigned in the ring, bulk stores)
 enum { RS_SHIFT_REG = 1, RS_SHIFT_BULK = 2 };
 cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
@@ -22,6 +23,6 @@ cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool sm
 // tensor-map TMA path: tmaps = RS_TMAP_TABLE_BYTES bytes, RS_TMAP_BUFS CUtensorMap per side (api.cu encodes them)
 #define RS_TMAP_TABLE_BYTES (2 * RS_TMAP_BUFS * 128)
 cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,
-                        int lookahead, uint32_t stage_bytes, float pace, bool pdl, cudaStream_t st);
+                        int lookahead, uint32_t stage_bytes, float pace, int burst, bool pdl, cudaStream_t st);
 int64_t launch_count();
 }  // namespace rs
