@@ -756,3 +756,60 @@ def test_unet_boundary_group_full_size():
     assert rs.launch_count() == n0 + 1
     for got, want in zip(dst, expect):
         assert torch.equal(got, want)
+
+
+def _random_mid_size_task(rng):
+    """a seeded task of 48-320 MiB: 2-4 dims, meshes of 2-32 devices, even and uneven extents, inner dims from 16 elements to thousands"""
+    ndim = int(rng.integers(2, 5))
+    meshes = [(2, 4), (4, 2), (1, 4), (2, 2), (8,), (2,), (4, 4), (4, 8), (2, 3), (1, 1)]
+
+    def side():
+        mesh = meshes[int(rng.integers(len(meshes)))]
+        axes = list(rng.permutation(len(mesh)))
+        spec = []
+        for _ in range(ndim):
+            take = int(rng.integers(0, 3)) if axes else 0
+            mine = [axes.pop() for _ in range(min(take, len(axes)))]
+            spec.append("S" + "".join(str(a) for a in mine) if mine else "R")
+        return mesh, "".join(spec)
+    sm, ss = side()
+    dm, ds = side()
+    dtype = ["u8", "bf16", "fp32", "i64"][int(rng.integers(4))]
+    e = inputs.elem_bytes(dtype)
+    inner = int(rng.choice([16, 32, 64, 100, 256, 257, 512, 1000, 2050, 4096, 12288]))
+    mids = [int(rng.choice([4, 7, 16, 32, 33, 64, 128, 320])) for _ in range(ndim - 2)]
+    target = int(rng.integers(48, 321)) << 20
+    outer = max(1, target // (e * inner * int(np.prod(mids or [1]))))
+    shape = (outer,) + tuple(mids) + (inner,)
+    name = "x:%s:%s:%s:%s:%s:%s" % ("x".join(map(str, shape)), dtype, "x".join(map(str, sm)), ss, "x".join(map(str, dm)), ds)
+    return name
+
+
+@pytest.mark.parametrize("seed", range(96))
+def test_random_mid_size_tasks_under_auto(seed):
+    """48-320 MiB tasks under AUTO, where the launch rules switch kernels and shapes (tensor maps for short rows, span tiles, source- and
+    destination-order segments, paced shapes, both store paths of the shifted kernel): execute and pack -> unpack, every destination byte
+    against basic slicing of D with the ORACLE's boxes, padding untouched"""
+    rng = np.random.default_rng(5322_2211 + seed)
+    w = inputs.get_workload(_random_mid_size_task(rng))
+    e = inputs.elem_bytes(w.dtype)
+    D, src = gu.workload_on_device(w)
+    if D.numel() * e * (1 + do.num_devices(w.dst_mesh)) > (40 << 30):
+        pytest.skip("destination side larger than the box")
+    p = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec)
+    idx = gu.oracle_slices(w.shape, w.dst_mesh, w.dst_spec)
+    local = do.local_shape(w.shape, w.dst_mesh, w.dst_spec)
+    want = [gu.padded(D, idx[q], local, 0x5A).view(torch.uint8) for q in range(p.info.n_dst)]
+    for route in ("execute", "pack"):
+        dst = [torch.empty(tuple(local), dtype=D.dtype, device=gu.dev()) for _ in range(p.info.n_dst)]
+        for t in dst:
+            t.view(torch.uint8).fill_(0x5A)
+        if route == "execute":
+            p.execute(gu.ptrs(src), gu.ptrs(dst), gu.stream())
+        else:
+            arena = torch.empty(max(1, p.info.arena_bytes), dtype=torch.uint8, device=gu.dev())
+            p.pack(gu.ptrs(src), arena.data_ptr(), gu.stream())
+            p.unpack(arena.data_ptr(), gu.ptrs(dst), gu.stream())
+        torch.cuda.synchronize()
+        for q in range(p.info.n_dst):
+            assert torch.equal(dst[q].view(torch.uint8), want[q]), (w.name, route, q, p.op_info(rs.RS_OP_EXECUTE).path)
