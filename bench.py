@@ -47,7 +47,7 @@ TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 ROOF_CSV = os.path.join(ROOT, "profiles", "roof_1k.csv")
 TUNING_FIELDS = ("bulk_warps", "bulk_stages", "bulk_lookahead", "bulk_tile_bytes", "bulk_ctas", "bulk_ctas_mcast", "shift_warps",
                  "shift_stages", "shift_lookahead", "shift_tile_bytes", "lsu_tile_bytes", "lsu_ctas_per_sm", "task_order",
-                 "small_op_bytes_mib", "tiles_per_worker", "pace_permille", "no_pdl", "pace_burst", "shift_mode")
+                 "small_op_bytes_mib", "tiles_per_worker", "pace_permille", "no_pdl", "pace_burst", "lsu_narrow", "shift_mode")
 
 
 def parse_args():

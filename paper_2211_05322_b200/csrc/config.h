@@ -54,6 +54,8 @@
 #define RS_BULK_STAGES_SMALL_MCAST     3       //  4 + 32 MiB: 7.5 us either way; from 16 + 64 MiB on the default shape)
 #define RS_BULK_TILE_BYTES_SMALL_MCAST 4096
 #define RS_INTERLEAVE_MAX_RUN (64 << 10)    // destination runs up to this long count as a fine interleave (tile order)
+#define RS_NARROW_MAX_RUN    512        // register path, layout 8-byte aligned and no more, rows shorter than this: 8-byte vectors instead of the shift
+                                        // kernel (4-byte aligned: rows under 48 bytes; 1- and 2-byte aligned: under 8 bytes; api.cu)
 #define RS_SHIFT_MIN_RUN     128        // ... unaligned layouts: rs_copy_bulk_shift from rows of 128 bytes on (large operations)
 #define RS_BULK_MIN_RUN      512        // AUTO picks the TMA path only if every run is at least this long
 #define RS_TMAP_SHORT_MIN_RUN   64          // AUTO: operations made of rows of 64-511 bytes take the tensor-map kernel when they are past the

@@ -915,6 +915,24 @@ cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, bo
     return launch_k(rs_copy_lsu<uint4, U, 128, false>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);
 }
 
+// Layouts that are not 16-byte aligned AND made of short rows: the register kernel at the layout's own vector width (8, 4, 2 or 1 bytes)
+// instead of the shift kernel -- assembling 16-byte windows pays when rows are long; on rows of tens of bytes most windows are partial.
+template <typename V>
+static cudaError_t launch_narrow_t(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st) {
+    constexpr int U = sizeof(V) >= 8 ? 4 : 8;
+    if (small) return launch_k(rs_copy_lsu<V, U, RS_PTRS_SMALL, true>, grid, RS_LSU_THREADS, 0, st, pdl, op, small_table(ptrs));
+    return launch_k(rs_copy_lsu<V, U, 128, true>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);
+}
+
+cudaError_t launch_narrow(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int vec_bytes, int grid, bool pdl, cudaStream_t st) {
+    switch (vec_bytes) {
+        case 8: return launch_narrow_t<uint2>(op, ptrs, small, grid, pdl, st);
+        case 4: return launch_narrow_t<uint32_t>(op, ptrs, small, grid, pdl, st);
+        case 2: return launch_narrow_t<uint16_t>(op, ptrs, small, grid, pdl, st);
+        default: return launch_narrow_t<uint8_t>(op, ptrs, small, grid, pdl, st);
+    }
+}
+
 cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st) {
     if (small) return launch_k(rs_copy_shift<4, RS_PTRS_SMALL>, grid, RS_LSU_THREADS, 0, st, pdl, op, small_table(ptrs));
     return launch_k(rs_copy_shift<4, 128>, grid, RS_LSU_THREADS, 0, st, pdl, op, ptrs);

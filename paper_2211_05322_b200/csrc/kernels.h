@@ -11,6 +11,8 @@ namespace rs {
 // generic: the operation has GENERIC tiles (the other instantiation does not contain their walk)
 cudaError_t launch_lsu(const RsOpDev &op, const RsPtrTable &ptrs, bool small, bool generic, int grid, bool pdl, cudaStream_t st);      // 16-byte aligned only
 cudaError_t launch_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, bool pdl, cudaStream_t st);
+// the register kernel at vec_bytes = 8, 4, 2 or 1 (unaligned layouts made of short rows)
+cudaError_t launch_narrow(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int vec_bytes, int grid, bool pdl, cudaStream_t st);
 cudaError_t prepare_bulk(int smem_bytes);                                             // both TMA kernels, both table sizes
 // pace: nanoseconds a warp lets pass per byte of DRAM traffic of its tiles (rate matching, kernels.cu); 0 = unpaced
 // burst: tiles of credit a warp that fell behind may catch up with

@@ -53,6 +53,7 @@ struct OpTables {                        // one operation (execute / pack / unpa
     int stages = 0, lookahead = 0;       // TMA path: ring slots per warp, loads in flight
     uint32_t shift_stage = 0;            // rs_copy_bulk_shift: bytes per ring slot (rows padded), 0 if the path is not used
     int pace_permille = 0;               // rs_copy_bulk: offered load as permille of the DRAM peak (0: unpaced)
+    int64_t mean_run_bytes = 0;          // bytes moved / rows moved (register path on unaligned layouts: which vector width)
     int64_t src_cap = 0, dst_cap = 0;    // bytes of every source / destination buffer of this operation (0: they differ, groups)
     RsTmapGeom tmap_src[RS_TMAP_BUFS] = {}, tmap_dst[RS_TMAP_BUFS] = {};   // RS_PATH_TMAP: geometry of the tensor map of every buffer
     uint32_t alt_stage = 0;              // TMA plans handed under-aligned pointers: shape of rs_copy_bulk_shift on the same tiles

@@ -398,6 +398,11 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
     int64_t mr = INT64_MAX, pad = 0;
     for (const RsTask &T : op->tasks) { mr = std::min(mr, task_min_col(T)); pad = std::max(pad, task_shift_stage(T)); }
     I.min_run_bytes = op->tasks.empty() ? 0 : mr;
+    {
+        double bytes = 0, rows = 0;
+        for (const RsTask &T : op->tasks) { bytes += (double)task_rows(T) * (double)T.run_bytes; rows += (double)task_rows(T); }
+        op->mean_run_bytes = rows > 0 ? (int64_t)(bytes / rows) : 0;
+    }
     // RS_PATH_TMAP: every buffer is seen as ONE 2-D byte matrix [rows][pitch] with ONE box shape; a task whose full
     // tiles fit the matrices of its source and of all its destinations moves them with tensor-map copies, everything
     // else (ragged last tiles, long or odd rows, other pitches) with the per-row bulk copies of rs_copy_bulk.

@@ -105,6 +105,21 @@ def test_unaligned_long_rows_register_and_bulk_stores(case, dtype, mode):
                 assert g.tobytes() == w.tobytes(), (case, dtype, mode, warps, stages, q)
 
 
+@pytest.mark.parametrize("narrow", [1, -1])
+@pytest.mark.parametrize("dtype", [np.uint8, np.int16, np.float32, np.int64])
+def test_register_path_at_the_layouts_own_vector_width(dtype, narrow):
+    """layouts that are not 16-byte aligned on the register path: vectors of 8 / 4 / 2 / 1 bytes (rs_tuning.lsu_narrow = 1) and the
+    16-byte shift kernel (-1) -- FAST, SPLIT and GENERIC tiles, multicast, odd pointer offsets"""
+    e = np.dtype(dtype).itemsize
+    for i in (2, 9, 10, 13, 14, 16, 21, 24, 25):
+        shape, sm, ss, dm, ds = SMALL[i]
+        for so, dofs in [(0, 0), (e, 3 * e)]:
+            _p, got, want = gu.run_small(shape[:-1] + (shape[-1] + 1,), dtype, sm, ss, dm, ds, flags=rs.RS_PATH_LSU, src_offset=so, dst_offset=dofs,
+                                         opts=dict(tuning=dict(lsu_narrow=narrow)))
+            for q, (g, w) in enumerate(zip(got, want)):
+                assert g.tobytes() == w.tobytes(), (i, dtype, narrow, so, q)
+
+
 @pytest.mark.parametrize("path", [rs.RS_PATH_LSU, rs.RS_PATH_BULK, rs.RS_PATH_BULK_SHIFT])
 @pytest.mark.parametrize("tile", [128, 1024, 4096])
 def test_tile_sizes_and_ring_depths(tile, path):
