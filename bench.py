@@ -47,7 +47,7 @@ TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 ROOF_CSV = os.path.join(ROOT, "profiles", "roof_1k.csv")
 TUNING_FIELDS = ("bulk_warps", "bulk_stages", "bulk_lookahead", "bulk_tile_bytes", "bulk_ctas", "bulk_ctas_mcast", "shift_warps",
                  "shift_stages", "shift_lookahead", "shift_tile_bytes", "lsu_tile_bytes", "lsu_ctas_per_sm", "task_order",
-                 "small_op_bytes_mib", "tiles_per_worker", "pace_permille", "no_pdl", "pace_burst", "lsu_narrow", "shift_mode")
+                 "small_op_bytes_mib", "tiles_per_worker", "pace_permille", "no_pdl", "pace_burst", "ring_min_smem", "lsu_narrow", "shift_mode")
 
 
 def parse_args():
@@ -76,6 +76,7 @@ def parse_args():
                     "RS_STRATEGY_ALLGATHER (PAPER.md S3.1) against the broadcast executor")
     ap.add_argument("--roof", action="store_true", help="1 read + k writes on contiguous buffers, k = 1, 2, 4, 8: launch shapes swept, "
                     "beside torch copy_ / fill_ / sum and the read/write-rate model")
+    ap.add_argument("--mix", default=None, help="reshard_execute of several workloads alternating in one stream (a,b[,c]) against each back to back alone")
     ap.add_argument("--overlap", action="store_true", help="resharding beside compute (PAPER.md S4, on chip): reshard_execute "
                     "on a high-priority stream limited to max_ctas CTAs while torch.matmul (cuBLAS) runs on another stream")
     ap.add_argument("--group", action="store_true", help="many tensors across one stage boundary (PAPER.md:100): n copies of "
@@ -787,6 +788,52 @@ def run_sharded(args):
     return 0
 
 
+def run_mix(args):
+    """--mix a,b[,c]: reshard_execute of DIFFERENT workloads alternating in ONE stream (a stage boundary carries tensors of several layouts),
+    between one pair of CUDA events, against each workload launched back to back on its own.  One JSON line."""
+    import torch
+    from paper_2211_05322_b200 import harness, inputs
+    from paper_2211_05322_b200 import reshard as rs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    st = torch.cuda.current_stream().cuda_stream
+    opts = dict(tuning=parse_tune(args.tune)) if args.tune else None
+    items = []
+    for name in args.mix.split(","):
+        w = inputs.get_workload(name)
+        plan = rs.Plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec,
+                       {"auto": rs.RS_PATH_AUTO, "lsu": rs.RS_PATH_LSU, "bulk": rs.RS_PATH_BULK, "shift": rs.RS_PATH_BULK_SHIFT, "tmap": rs.RS_PATH_TMAP}[args.path], opts)
+        info = plan.info
+        src = [torch.empty(info.src_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_src)]
+        dst = [torch.empty(info.dst_shard_bytes, dtype=torch.uint8, device=dev) for _ in range(info.n_dst)]
+        o = plan.op_info(rs.RS_OP_EXECUTE)
+        items.append((name, plan, harness.ptrs(src), harness.ptrs(dst), o.read_bytes + o.write_bytes, (src, dst), o))
+
+    def rate(seq, rounds):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(rounds):
+            for it in seq:
+                it[1].execute(it[2], it[3], st)
+        e1.record()
+        torch.cuda.synchronize()
+        return sum(it[4] for it in seq) * rounds / (e0.elapsed_time(e1) * 1e-3) / 1e9
+
+    rounds = max(3, args.steps // 10)
+    for _ in range(2):
+        rate(items, 2)
+    out = {"mix": args.mix, "protocol": "%d rounds of the listed launches alternating in one stream, one pair of CUDA events" % rounds,
+           "alternating_GB/s": statistics.median(rate(items, rounds) for _ in range(5)),
+           "each_alone_GB/s": {it[0]: statistics.median(rate([it], rounds * len(items)) for _ in range(5)) for it in items},
+           "shapes": {it[0]: "%s %d x %d, %d B shared" % ({rs.RS_PATH_BULK: "rs_copy_bulk", rs.RS_PATH_BULK_SHIFT: "rs_copy_bulk_shift", rs.RS_PATH_TMAP: "rs_copy_tmap"}.get(it[6].path, "rs_copy_lsu"), it[6].grid, it[6].block, it[6].smem_bytes) for it in items},
+           "tune": args.tune}
+    print(json.dumps(out))
+    return 0
+
+
 def run_overlap(args):
     """Per CTA cap: time N matmuls alone, M reshard_execute launches alone, then both started together on two
     streams (wall time on the device between a common start event and the later of the two end events).
@@ -1056,6 +1103,8 @@ def main():
         return run_roof(args)
     if args.group:
         return run_group(args)
+    if args.mix:
+        return run_mix(args)
     if args.overlap:
         return run_overlap(args)
     if args.sweep:

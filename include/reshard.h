@@ -129,6 +129,8 @@ typedef struct rs_tuning {
     int32_t no_pdl;                                    /* 1: launch without programmatic dependent launch (a kernel then
                                                           starts only after the previous kernel of the stream has ended) */
     int32_t pace_burst;                                /* rate matching: tiles of credit a warp that fell behind may catch up with; 0 = default (2) */
+    int32_t ring_min_smem;                             /* ring kernels request at least this many bytes of shared memory (0 = default, 116 KiB:
+                                                          never two ring CTAs on one SM; 1 = only what the ring needs) */
     int32_t lsu_narrow;                                /* register path on layouts that are not 16-byte aligned: 1 = always at the layout's own vector
                                                           width, -1 = always the 16-byte shift kernel, 0 = library default (by row length) */
     int32_t shift_mode;                                /* rs_copy_bulk_shift, rows >= 1 KiB: 0 = library default; 1: windows

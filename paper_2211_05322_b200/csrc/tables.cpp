@@ -457,7 +457,13 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
         op->stages = stages;
         op->lookahead = std::max(1, std::min(stages - 1, shift ? pick(P->tune.shift_lookahead, stages - 1) : pick(P->tune.bulk_lookahead, RS_BULK_LOOKAHEAD)));
         I.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>(I.grid, (I.n_tiles + warps - 1) / warps));
-        I.smem_bytes = (int32_t)(warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024);
+        // Never two ring CTAs on one SM: with programmatic dependent launch the CTAs of the NEXT launch are placed as SMs free up, and a
+        // shape small enough to fit twice piles two of them on the SMs that finished first (a 107 KiB launch behind a 148 KiB one: 5.56
+        // instead of 6.45 TB/s for the pair).  Asking for more than half of the SM's shared memory makes the hand-over one for one.
+        // (Operations under 384 MiB keep their natural size: two of them share an SM on purpose -- the successor's prologue runs beside the
+        // predecessor, config 3: 8.0 against 8.55 us -- and a pile-up lasts microseconds.)
+        const int64_t min_smem = read_bytes + write_bytes >= RS_RING_MIN_SMEM_FROM ? pick(P->tune.ring_min_smem, RS_RING_MIN_SMEM) : 0;
+        I.smem_bytes = (int32_t)std::max<int64_t>(warps * (stages * stage + RS_BULK_DESC_BYTES) + 1024, min_smem);
         if (shift) op->shift_stage = (uint32_t)stage;
         if (!shift) {
             // An aligned plan may be handed under-aligned pointers at execute time: keep a launch shape of the
@@ -470,7 +476,7 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
             while (aw > 1 && (int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX) aw--;
             if ((int64_t)aw * (as * pad + RS_BULK_DESC_BYTES) + 1024 <= RS_SMEM_MAX && I.n_tiles > 0) {
                 op->alt_stage = (uint32_t)pad; op->alt_warps = aw; op->alt_stages = as;
-                op->alt_smem = (int)(aw * (as * pad + RS_BULK_DESC_BYTES) + 1024);
+                op->alt_smem = (int)std::max<int64_t>(aw * (as * pad + RS_BULK_DESC_BYTES) + 1024, min_smem);
             }
         }
         if (shift && I.smem_bytes > RS_SMEM_MAX) {             // rows too sparse for the ring: the register kernels take it
