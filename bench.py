@@ -47,7 +47,7 @@ TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 ROOF_CSV = os.path.join(ROOT, "profiles", "roof_1k.csv")
 TUNING_FIELDS = ("bulk_warps", "bulk_stages", "bulk_lookahead", "bulk_tile_bytes", "bulk_ctas", "bulk_ctas_mcast", "shift_warps",
                  "shift_stages", "shift_lookahead", "shift_tile_bytes", "lsu_tile_bytes", "lsu_ctas_per_sm", "task_order",
-                 "small_op_bytes_mib", "tiles_per_worker", "pace_permille", "no_pdl", "pace_burst", "ring_min_smem", "lsu_narrow", "shift_mode")
+                 "small_op_bytes_mib", "tiles_per_worker", "pace_permille", "no_pdl", "pace_burst", "pace_adapt", "ring_min_smem", "lsu_narrow", "shift_mode")
 
 
 def parse_args():
@@ -76,6 +76,8 @@ def parse_args():
                     "RS_STRATEGY_ALLGATHER (PAPER.md S3.1) against the broadcast executor")
     ap.add_argument("--roof", action="store_true", help="1 read + k writes on contiguous buffers, k = 1, 2, 4, 8: launch shapes swept, "
                     "beside torch copy_ / fill_ / sum and the read/write-rate model")
+    ap.add_argument("--hot", action="store_true", help="with --sweep (operations >= 1 GiB moved): a burst of 24 bf16 8192^3 GEMMs before every timed launch, so that "
+                    "the launch runs at the SM clock a training step leaves behind (power-limited, ~1.3-1.6 GHz) instead of the idle boost clock")
     ap.add_argument("--mix", default=None, help="reshard_execute of several workloads alternating in one stream (a,b[,c]) against each back to back alone")
     ap.add_argument("--overlap", action="store_true", help="resharding beside compute (PAPER.md S4, on chip): reshard_execute "
                     "on a high-priority stream limited to max_ctas CTAs while torch.matmul (cuBLAS) runs on another stream")
@@ -293,6 +295,24 @@ class ClockSampler:
 
 # ------------------------------------------------------------------ timing protocols
 
+_HEAT = None     # --hot: a burst of tensor-core GEMMs enqueued before every timed launch (the chip at its power-limited clocks)
+
+
+def make_heater(torch, dev, n_gemms=24):
+    n = 8192
+    a = torch.randn(n, n, device=dev, dtype=torch.bfloat16)
+    b = torch.randn(n, n, device=dev, dtype=torch.bfloat16)
+    c = torch.empty(n, n, device=dev, dtype=torch.bfloat16)
+
+    def heat():
+        for _ in range(n_gemms):
+            torch.matmul(a, b, out=c)
+    for _ in range(8):
+        heat()
+    torch.cuda.synchronize()
+    return heat
+
+
 def time_each(call, stream, n, warm=3):
     """n launches, each between its own pair of CUDA events on the launching stream (operations much larger than
     L2: nothing to flush).  Returns (median ms, best ms)."""
@@ -302,6 +322,8 @@ def time_each(call, stream, n, warm=3):
     ts = []
     for _ in range(n):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if _HEAT:
+            _HEAT()
         e0.record(stream); call(); e1.record(stream)
         e1.synchronize()
         ts.append(e0.elapsed_time(e1))
@@ -536,6 +558,9 @@ def run_sweep(args):
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
+    if args.hot:
+        global _HEAT
+        _HEAT = make_heater(torch, dev)
     stream = torch.cuda.current_stream()
     sh = stream.cuda_stream
     peak, _ = peak_hbm()

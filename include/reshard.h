@@ -129,6 +129,8 @@ typedef struct rs_tuning {
     int32_t no_pdl;                                    /* 1: launch without programmatic dependent launch (a kernel then
                                                           starts only after the previous kernel of the stream has ended) */
     int32_t pace_burst;                                /* rate matching: tiles of credit a warp that fell behind may catch up with; 0 = default (2) */
+    int32_t pace_adapt;                                /* rate matching: 1 = the interval backs off while ring slots come back late (HBM behind the
+                                                          offered load) and returns to the target afterwards; 0 = default: fixed interval */
     int32_t ring_min_smem;                             /* ring kernels request at least this many bytes of shared memory (0 = default, 116 KiB:
                                                           never two ring CTAs on one SM; 1 = only what the ring needs) */
     int32_t lsu_narrow;                                /* register path on layouts that are not 16-byte aligned: 1 = always at the layout's own vector

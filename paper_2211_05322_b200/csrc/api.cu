@@ -447,7 +447,7 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
         dev.early_trigger = grid >= P.sm_count;
         // rate matching: the launch as a whole offers pace_permille / 1000 of the DRAM peak
         const int permille = P.tune.pace_permille > 0 ? P.tune.pace_permille : P.tune.pace_permille < 0 ? 0 : op.pace_permille;
-        const int burst = P.tune.pace_burst > 0 ? P.tune.pace_burst : RS_PACE_BURST;
+        const int burst = (P.tune.pace_burst > 0 ? std::min(P.tune.pace_burst, 255) : RS_PACE_BURST) | (P.tune.pace_adapt > 0 ? 0 : 0x100);
         const float pace = permille > 0 ? (float)((double)grid * warps / (P.dram_peak_gbs * permille / 1000.0)) : 0.f;
         if (op.info.path == RS_PATH_TMAP && small) {          // tensor maps of this call's pointers, then the same ring kernel
             alignas(64) unsigned char tm[RS_TMAP_TABLE_BYTES];

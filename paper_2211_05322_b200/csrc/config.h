@@ -21,7 +21,9 @@
 #define RS_BULK_STAGES       4          // ring slots per warp
 #define RS_BULK_LOOKAHEAD    2          // loads in flight per warp before the first store is issued
 #define RS_BULK_TILE_BYTES   12288      // bytes per ring slot
-#define RS_BULK_SHORT_RUN    1024       // runs up to this long: many copies per tile, use the SHORT shape
+#define RS_BULK_SHORT_RUN    2048       // runs up to this long: many copies per tile, use the SHORT shape (4 warps; paced when 1 : 1 and >= 128 MiB).
+                                        // 2 KiB rows on 2 warps are issue-bound once the SM clock drops under power (after GEMM bursts, ~1.4 GHz):
+                                        // P1 at 1 GiB 6.35 TB/s cold but 5.2-5.3 hot; on 4 paced warps 6.30 cold, 6.24 hot (256 MiB: 6.38 -> 6.09 cold, 4.80 -> 5.63 hot)
 #define RS_BULK_MIN_FILL     0.7        // slots less full than this on average: the SHORT shape too
 #define RS_BULK_TINY_FILL    0.3        // slots less than 30 % full (tiles under ~3.5 KiB): 8 warps x 3 slots x 4 KiB
 #define RS_BULK_WARPS_SHORT  4
@@ -32,10 +34,12 @@
 // offers this many permille of the DRAM peak (2 x memory clock x bus width = 7 672 GB/s on B200).  Measured
 // (profiles/r02_pacing.md): achieved = 0.99 x offered up to 860 permille (6.52 TB/s on 1 + 8), collapse from 880 on
 // (6.09, then 5.56 at 920; unpaced 5.66); runs of 512 B: up to 820 (6.18 TB/s), 6.00 at 840.  10 permille below the edge.
+#define RS_PACE_BLOCK_NS       1500           // a ring slot still being read this long after the warp asked for it: HBM is behind, back off
 #define RS_PACE_BURST          2              // tiles of credit of the token bucket
-#define RS_PACE_PERMILLE       850
-#define RS_PACE_PERMILLE_SHORT 810
-#define RS_PACE_PERMILLE_SHORT_DENSE 830   // short rows that are adjacent in the receivers (one bulk store per tile)
+#define RS_PACE_PERMILLE       825            // (850 is the best on a cold chip: 6.45 TB/s against 6.26; after GEMM bursts -- the chip power-limited, HBM hot -- the
+                                              //  edge lies 3-5 % lower: 850 then gives an erratic 5.8-6.4, 825 a steady 6.25: profiles/r02_pacing.md part 4)
+#define RS_PACE_PERMILLE_SHORT 775            // (cold: 6.08 TB/s at 810, 5.83 at 775; hot: 4.63 at 810, 5.85 at 775)
+#define RS_PACE_PERMILLE_SHORT_DENSE 820   // short rows that are adjacent in the receivers (one bulk store per tile)
 #define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
 #define RS_PACE_PERMILLE_11    880            // 1 : 1 operations made of runs >= 1 MiB: best at 880-900, collapse from 910 (fig5_1x1 6.18 -> 6.56 TB/s,
 #define RS_PACE_PERMILLE_11_SHORT 860          // 1 : 1 operations on the 4-warp shape (rows <= 1 KiB or half-empty slots)

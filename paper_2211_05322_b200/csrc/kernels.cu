@@ -400,8 +400,18 @@ __device__ __forceinline__ uint64_t global_ns() {             // 32 ns resolutio
 // (reads + k writes) may start `pace` x b nanoseconds after the previous one, pace = workers / target rate; the target
 // is a fraction of the DRAM peak read from the device (api.cu).  A token bucket with a burst of two tiles: a warp
 // that is behind schedule (HBM slower than the target, another kernel running beside) never waits.
-__device__ __forceinline__ void pace_tile(uint64_t &t_next, float pace, int burst, uint32_t traffic_bytes, int lane) {
-    const uint64_t interval = (uint64_t)(pace * (float)traffic_bytes);
+// The target is a ceiling, not a promise: where HBM takes less than the launch offers (a hot chip -- after a burst of GEMMs the edge of the
+// collapse lies 3-5 % lower --, another kernel beside, another box) the excess shows up as ring slots that are still being read when the warp
+// wants them back (cp.async.bulk.wait_group.read blocks).  So the warp BACKS OFF: every time that wait takes longer than RS_PACE_BLOCK_NS its
+// interval grows by 1/32, after 8 tiles without blocking it shrinks by 1/128 towards the configured target (additive-increase /
+// multiplicative-decrease, per warp; all warps see the same congestion).  `mul` is that stretch factor in 1/1024.
+__device__ __forceinline__ void pace_adapt(uint32_t &mul, uint32_t &calm, bool blocked) {
+    if (blocked) { mul = mul + (mul >> 5); if (mul > 1536u) mul = 1536u; calm = 0; }
+    else if (++calm >= 8u) { calm = 0; if (mul > 1024u) { mul -= (mul >> 7); if (mul < 1024u) mul = 1024u; } }
+}
+
+__device__ __forceinline__ void pace_tile(uint64_t &t_next, float pace, int burst, uint32_t traffic_bytes, int lane, uint32_t mul = 1024u) {
+    const uint64_t interval = ((uint64_t)(pace * (float)traffic_bytes) * mul) >> 10;
     if (lane == 0) {
         uint64_t now = global_ns();
         while (now < t_next) {
@@ -455,6 +465,9 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
     int ld_slot = 0, st_slot = 0;                             // it % stages, j % stages without dividing
     uint32_t st_parity = 0;
     uint64_t t_next = 0;                                      // rate matching: earliest start of this warp's next tile
+    uint32_t pace_mul = 1024u, pace_calm = 0;                 // ... and its back-off (pace_adapt)
+    const bool adapt = pace > 0.f && !(burst & 0x100);
+    const int credit_tiles = burst & 0xff;
 
     for (int it = 0; it < n_my + lookahead; ++it) {
         if (it < n_my) {                                      // ---- load tile `it` into slot ld_slot
@@ -478,12 +491,18 @@ __device__ __forceinline__ void bulk_body(const RsOpDev &op, const RsPtrTableT<N
                 if (it == 0) pdl_wait();                      // shard memory is touched from here on
             }
             if (it >= stages) {                               // slot reuse: its stores must have read it
-                bulk_wait_read(pending_ok);
+                if (adapt) {
+                    const uint64_t t0 = global_ns();
+                    bulk_wait_read(pending_ok);
+                    pace_adapt(pace_mul, pace_calm, global_ns() - t0 > RS_PACE_BLOCK_NS);
+                } else {
+                    bulk_wait_read(pending_ok);
+                }
                 __syncwarp();
             }
             const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
             const uint32_t n_rows = d->n_rows, col_bytes = d->col_bytes;
-            if (pace > 0.f) pace_tile(t_next, pace, burst, n_rows * col_bytes * (1u + d->k), lane);
+            if (pace > 0.f) pace_tile(t_next, pace, credit_tiles, n_rows * col_bytes * (1u + d->k), lane, pace_mul);
             const uint32_t bar = bars + 8 * ld_slot, slot = ring + (uint32_t)ld_slot * stage_bytes;
             if (lane == 0) mbar_expect_tx(bar, n_rows * col_bytes);
             __syncwarp();

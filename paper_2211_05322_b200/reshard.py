@@ -61,7 +61,7 @@ class Tuning(C.Structure):
                 ("shift_warps", C.c_int32), ("shift_stages", C.c_int32), ("shift_lookahead", C.c_int32),
                 ("shift_tile_bytes", C.c_int32), ("lsu_tile_bytes", C.c_int32), ("lsu_ctas_per_sm", C.c_int32),
                 ("task_order", C.c_int32), ("small_op_bytes_mib", C.c_int32), ("tiles_per_worker", C.c_int32), ("pace_permille", C.c_int32), ("no_pdl", C.c_int32),
-                ("pace_burst", C.c_int32), ("ring_min_smem", C.c_int32), ("lsu_narrow", C.c_int32), ("shift_mode", C.c_int32)]
+                ("pace_burst", C.c_int32), ("pace_adapt", C.c_int32), ("ring_min_smem", C.c_int32), ("lsu_narrow", C.c_int32), ("shift_mode", C.c_int32)]
 
 
 class PlanOpts(C.Structure):

@@ -601,7 +601,7 @@ def test_rate_matching_and_launch_switches_change_no_byte(tuning):
     fwd = rs.Plan(w.shape, e, w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, dict(tuning=tuning))
     bwd = rs.Plan(w.shape, e, w.dst_mesh, w.dst_spec, w.src_mesh, w.src_spec, 0, dict(tuning=tuning))
     if not tuning.get("pace_permille"):
-        assert fwd.op_info(rs.RS_OP_EXECUTE).pace_permille == 850
+        assert fwd.op_info(rs.RS_OP_EXECUTE).pace_permille == 825
     mid = [torch.zeros(fwd.info.dst_shard_bytes, dtype=torch.uint8, device=gu.dev()) for _ in range(fwd.info.n_dst)]
     back = [torch.zeros_like(s) for s in src]
     for _ in range(3):                                                      # a chain of dependent launches, no host sync in between

@@ -469,13 +469,13 @@ def test_launch_shapes_follow_the_measured_rules():
         o = p.op_info(op)
         return o.path, o.grid, o.block, o.pace_permille
     assert shape_of("c4") == (rs.RS_PATH_BULK, 132, 64, 0)                        # long runs, 1 : 1: closed loop, unpaced
-    assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64, 0)       # 2 KiB runs, 1 : 1
-    assert shape_of("sweep_P5_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64, 850)     # 1 read + 8 writes: every SM, rate matched
+    assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 128, 860)    # 2 KiB runs, 1 : 1: 4 warps, paced (holds under power-limited clocks)
+    assert shape_of("sweep_P5_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64, 825)     # 1 read + 8 writes: every SM, rate matched
     assert shape_of("sweep_P5_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 148, 64, 880)   # its unpack is a 1 : 1 copy of 512 MiB runs: paced too
     assert shape_of("fig5_1x1") == (rs.RS_PATH_BULK, 148, 64, 880)                # one sender, one receiver, one 1 GiB run
     assert shape_of("t2_4") == (rs.RS_PATH_BULK, 132, 64, 0)                      # 128 KiB runs, 1 : 1: unpaced, trimmed grid
-    assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 128, 850)      # write-heavy, 144 MiB moved: paced, 4 warps
-    assert shape_of("t2_9") == (rs.RS_PATH_BULK, 148, 128, 830)                   # 512-byte runs, 1 + 4: 4 warps; rows adjacent in the receivers
+    assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 128, 825)      # write-heavy, 144 MiB moved: paced, 4 warps
+    assert shape_of("t2_9") == (rs.RS_PATH_BULK, 148, 128, 820)                   # 512-byte runs, 1 + 4: 4 warps; rows adjacent in the receivers
     assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 192, 0)                 # nothing aligned, 6 KiB rows: 6 warps, bulk stores
     assert shape_of("u1") == (rs.RS_PATH_BULK_SHIFT, 148, 224, 0)                 # nothing aligned, 2 KiB rows: 7 warps, register stores
     assert shape_of("c2") == (rs.RS_PATH_TMAP, 148, 128, 860)                     # 256 MiB moved in 2 KiB rows: tensor-map copies, 4 warps, paced
@@ -484,7 +484,7 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("sweep_P1_m8_16MiB")[:2] == (rs.RS_PATH_LSU, 4 * 148)         # small operations: register path, 4 CTAs per SM
     assert shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU
     assert shape_of("r128") == (rs.RS_PATH_TMAP, 148, 128, 860)                   # 128-byte rows at 1 + 1 GiB: boxes of 64 rows, paced
-    assert shape_of("r128m") == (rs.RS_PATH_TMAP, 148, 128, 810)                  # ... 1 + 4 GiB
+    assert shape_of("r128m") == (rs.RS_PATH_TMAP, 148, 128, 775)                  # ... 1 + 4 GiB
     assert shape_of("r128", rs.RS_OP_PACK)[0] == rs.RS_PATH_BULK                  # its pack copies whole 64 KiB runs
     p = _plan((262144, 4, 64), 2, (2,), "R,R,S0", (2,), "R,S0,R", 0)              # 64-byte rows, but only 2 per span: no box fits
     assert p.op_info(rs.RS_OP_EXECUTE).path == rs.RS_PATH_LSU                     # ... so AUTO falls back to the register path
