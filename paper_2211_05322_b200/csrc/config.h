@@ -74,11 +74,12 @@
 #define RS_SHIFT_LONG_RUN    4096       // rows at least this long: bulk stores (u4, 6 KiB rows: 6.12 TB/s against 5.65 from registers);
                                         // shorter: register stores, 8 warps (u1, 2 KiB rows: 5.8 against 4.1 with bulk stores)
 #define RS_SHIFT_MID_RUN     1024       // rows of 1-4 KiB (stored row by row from registers): 7 warps x 3 slots
-#define RS_SHIFT_WARPS_MID   7          // u1 (2050-byte rows): 6 x 3: 5.38 TB/s, 7 x 3: 6.08, 8 x 2: 5.85, 8 x 3: 5.65
-#define RS_SHIFT_STAGES_MID  3
-#define RS_SHIFT_WARPS_LONG  6          // rows >= 1 KiB: bodies realigned in the ring and stored with bulk copies.  One warp per
-#define RS_SHIFT_STAGES_LONG 3          // scheduler hides no latency (~520 instructions per tile at ~6 cycles each), so 6 warps:
-                                        // u4 4 x 4: 4.4 TB/s, 5 x 4: 5.4, 6 x 3: 6.12, 7 x 3: 6.05, 8 x 3: 5.75 (register stores, 4 x 4: 5.79)
+#define RS_SHIFT_WARPS_MID   8          // u1 (2050-byte rows): 6 x 3: 5.38 TB/s, 7 x 3: 6.08, 8 x 2: 5.85, 8 x 3: 5.65
+#define RS_SHIFT_STAGES_MID  2          // (idle chip: 7 x 3 is best, 6.08 TB/s against 5.86-5.92; after GEMM bursts 7 x 3 falls to 4.34, 8 x 2 holds 4.92-4.97)
+#define RS_SHIFT_WARPS_LONG  8          // rows >= 1 KiB: bodies realigned in the ring and stored with bulk copies.  One warp per
+#define RS_SHIFT_STAGES_LONG 2          // scheduler hides no latency (~520 instructions per tile at ~6 cycles each), so 6 warps:
+                                        // u4 4 x 4: 4.4 TB/s, 5 x 4: 5.4, 6 x 3: 6.12, 7 x 3: 6.05, 8 x 3: 5.75 (register stores, 4 x 4: 5.79) on an idle chip;
+                                        // after GEMM bursts (SM clock ~1.4 GHz) 6 x 3 falls to 4.49 while 8 x 2 holds 5.69 (idle: 5.72), so 8 x 2
 
 #define RS_BULK_DESC_BYTES   4096       // per-warp descriptor ring: 64 tiles x 64 bytes
 
