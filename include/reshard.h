@@ -326,6 +326,25 @@ RS_API rs_status reshard_op_tiles(const rs_plan *plan, int32_t op, int64_t first
  */
 RS_API rs_status reshard_execute(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
                           void *cuda_stream);
+/*
+ * reshard_execute_static: reshard_execute for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid it).  It needs no device allocation ANYWHERE: the plan may be built with
+ * RS_HOST_ONLY (reshard_plan then makes no CUDA call at all; its grids are sized for a 148-SM part), and the kernels read
+ * their task tables from a file-scope `static __device__` array of RS_STATIC_TABLE_BYTES = 256 KiB inside the library
+ * (every GPU that loads the library holds it until exit) instead of the plan's own cudaMalloc block.  The call copies the
+ * plan's execute tables into that array with cudaMemcpyAsync on `cuda_stream`, then launches the same kernels as
+ * reshard_execute on it; it calls no cudaMalloc, cudaFree or allocating library routine, and returns without synchronising.
+ *   - Limit: the execute tables (224 bytes per unit task + 16 per receiver + 16 per segment, each part rounded up to 256)
+ *     must fit the array: about 1000 unit tasks.  Larger plans return RS_EUNSUPPORTED with a message that names both
+ *     sizes; plans built with src_owner and plan groups return RS_EINVAL.
+ *   - The array is SHARED by every call on the device and keeps the last call's tables.  Every byte a launch reads is
+ *     rewritten by its own call first, so nothing has to be cleared; but calls that may overlap on the GPU (two
+ *     streams, two host threads on different streams) RACE on it: issue them on one stream, or order them with events.
+ *     Calls on one stream are ordered (these launches do not use programmatic dependent launch).
+ *   - src_shards / dst_shards as for reshard_execute; the result is byte for byte that of reshard_execute.
+ */
+RS_API rs_status reshard_execute_static(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
+                                 void *cuda_stream);
 /* reshard_execute_strategy: the same result as reshard_execute, reached with another of the paper's
  * strategies for a unit task.  The plan must have been built with RS_WITH_STRATEGIES
  * (else RS_EINVAL).  RS_STRATEGY_BROADCAST is reshard_execute; RS_STRATEGY_SENDRECV is one launch;

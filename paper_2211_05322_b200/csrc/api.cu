@@ -408,11 +408,11 @@ rs_status encode_tmaps(const rs::OpTables &op, const RsPtrTable &pt, unsigned ch
 // one launch of operation `opi` on the given buffers
 rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src, void *const *dst, int n_dst,
                  const char *used_src, void *stream, uint32_t tile_begin = 0, uint32_t tile_end = 0,
-                 const char *used_dst = nullptr) {
+                 const char *used_dst = nullptr, const RsOpDev *static_dev = nullptr /* reshard_execute_static: tables elsewhere */) {
     rs::set_error("");
     if (!plan || !src || !dst) { rs::set_error("null argument"); return RS_EINVAL; }
     const rs::Plan &P = plan->p;
-    if (!P.dev_blob) { rs::set_error("plan was built with RS_HOST_ONLY"); return RS_EINVAL; }
+    if (!P.dev_blob && !static_dev) { rs::set_error("plan was built with RS_HOST_ONLY"); return RS_EINVAL; }
     const rs::OpTables &op = P.op[opi];
     if (op.info.n_tiles == 0) return RS_OK;
     RsPtrTable pt;
@@ -433,13 +433,13 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaError_t e;
-    RsOpDev dev = op.dev;
+    RsOpDev dev = static_dev ? *static_dev : op.dev;
     if (tile_end > tile_begin) { dev.tile_base = tile_begin; dev.n_tiles = tile_end - tile_begin; }   // one slab
     const int64_t n_tiles = dev.n_tiles;
     const bool bulk_family = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_BULK_SHIFT || op.info.path == RS_PATH_TMAP;
     const bool as_bulk = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_TMAP;   // aligned TMA plans
     const int warps = op.info.block / 32;
-    const bool pdl = !P.tune.no_pdl;
+    const bool pdl = !P.tune.no_pdl && !static_dev;          // (the shared table array is rewritten between launches: full stream order)
     const int shift_mode = P.tune.shift_mode == rs::RS_SHIFT_REG || P.tune.shift_mode == rs::RS_SHIFT_BULK ? P.tune.shift_mode
                          : op.info.min_run_bytes >= RS_SHIFT_LONG_RUN ? rs::RS_SHIFT_BULK : rs::RS_SHIFT_REG;
     if (as_bulk && align == 16) {
@@ -504,6 +504,53 @@ rs_status reshard_execute(const rs_plan *plan, const void *const *src_shards, vo
     const rs::Plan &P = plan->p;
     return run_op(plan, RS_OP_EXECUTE, src_shards, P.A.n_dev, dst_shards, P.B.n_dev, P.used_src.data(), cuda_stream, 0, 0,
                   P.src_owner.empty() ? nullptr : P.used_dst.data());
+}
+
+rs_status reshard_execute_static(const rs_plan *plan, const void *const *src_shards, void *const *dst_shards,
+                                 void *cuda_stream) {
+    rs::set_error("");
+    if (!plan || !src_shards || !dst_shards) { rs::set_error("null argument"); return RS_EINVAL; }
+    const rs::Plan &P = plan->p;
+    if (!P.src_owner.empty() || P.group_src) { rs::set_error("reshard_execute_static: not for plans built with src_owner or for plan groups"); return RS_EINVAL; }
+    const rs::OpTables &o = P.op[RS_OP_EXECUTE];
+    if (o.info.n_tiles == 0) return RS_OK;
+    const size_t b_tasks = o.tasks.size() * sizeof(RsTask), b_dsts = o.dsts.size() * sizeof(RsDst), b_segs = o.segs.size() * sizeof(RsSeg);
+    const size_t off_dsts = round256(b_tasks), off_segs = off_dsts + round256(b_dsts), total = off_segs + round256(b_segs);
+    if (total > (size_t)RS_STATIC_TABLE_BYTES) {
+        rs::set_error("reshard_execute_static: the execute tables of this plan take " + std::to_string(total) + " bytes (" +
+                      std::to_string(o.tasks.size()) + " unit tasks), the static device array holds " + std::to_string(RS_STATIC_TABLE_BYTES) +
+                      "; use reshard_execute");
+        return RS_EUNSUPPORTED;
+    }
+    void *base_v = nullptr;                                    // device address of the file-scope array on the current device
+    cudaError_t e = rs::static_tables(&base_v);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(static tables)");
+    static std::once_flag smem_once;                           // a host-only plan never went through upload()
+    static cudaError_t smem_err = cudaSuccess;
+    std::call_once(smem_once, [] { smem_err = rs::prepare_bulk(RS_SMEM_MAX); });
+    if (smem_err != cudaSuccess) return cuda_fail(smem_err, "cudaFuncSetAttribute(rs_copy_bulk)");
+    char *base = static_cast<char *>(base_v);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // Three copies straight from the plan's host tables (pageable memory: staged before the call returns), in stream order
+    // before the launch.  Every byte the kernels read is written here, so nothing of the previous call's contents is used
+    // and nothing has to start at zero.
+    e = cudaMemcpyAsync(base, o.tasks.data(), b_tasks, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && b_dsts) e = cudaMemcpyAsync(base + off_dsts, o.dsts.data(), b_dsts, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && b_segs) e = cudaMemcpyAsync(base + off_segs, o.segs.data(), b_segs, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync(static tables)");
+    RsOpDev dev{};
+    dev.tasks = reinterpret_cast<const RsTask *>(base);
+    dev.dsts = reinterpret_cast<const RsDst *>(base + off_dsts);
+    dev.segs = reinterpret_cast<const RsSeg *>(base + off_segs);
+    dev.n_segs = (uint32_t)o.segs.size();
+    dev.seg_tiles = o.segs.empty() ? 0 : o.segs[0].n_members * o.segs[0].tiles_each;
+    for (const RsSeg &sg : o.segs) if (sg.n_members * sg.tiles_each != dev.seg_tiles) dev.seg_tiles = 0;
+    dev.n_tasks = (uint32_t)o.tasks.size();
+    dev.n_dsts = (uint32_t)o.dsts.size();
+    dev.early_trigger = 0;
+    dev.tile_base = 0;
+    dev.n_tiles = (uint32_t)o.info.n_tiles;
+    return run_op(plan, RS_OP_EXECUTE, src_shards, P.A.n_dev, dst_shards, P.B.n_dev, P.used_src.data(), cuda_stream, 0, 0, nullptr, &dev);
 }
 
 rs_status reshard_execute_strategy(const rs_plan *plan, int32_t strategy, const void *const *src_shards,

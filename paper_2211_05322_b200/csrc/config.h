@@ -90,5 +90,6 @@
 #define RS_SPAN_TILE_MIN_BYTES 1024      // spans of the innermost row dim holding at least this much become one FAST tile each
 #define RS_TILES_PER_WORKER   4          // small operations: tiles shrink until every warp has this many (tail balance)
 #define RS_SMEM_MAX          (227 * 1024)
+#define RS_STATIC_TABLE_BYTES (256 * 1024) // reshard_execute_static: the file-scope device array that holds one launch's tables (~1000 unit tasks)
 #define RS_RING_MIN_SMEM_FROM (384ll << 20) // ... for operations moving at least this much (below, the overlap of the prologue is worth more: 64 + 64 MiB pack 22.4 -> 23.3 us without it)
 #define RS_RING_MIN_SMEM     (116 * 1024) // ring kernels ask for at least this much: more than half an SM's shared memory, so two never share an SM

@@ -23,6 +23,8 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "config.h"
 #include "kernels.h"
 #include "tables.h"
@@ -978,6 +980,30 @@ cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *t
     RsTmapTable tm;
     memcpy(&tm, tmaps, sizeof(tm));
     return launch_k(rs_copy_tmap, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), tm, stages, lookahead, stage_bytes, pace, burst);
+}
+
+// ------------------------------------------------------------------------------------------------
+// reshard_execute_static (api.cu): the task tables of ONE launch in a file-scope array instead of the plan's cudaMalloc
+// block, for callers that cannot call cudaMalloc.  Every GPU that loads the library holds these RS_STATIC_TABLE_BYTES until
+// exit.  In host code the array's name is a host-side stand-in, NOT a device address: its device address is taken with
+// cudaGetSymbolAddress, once per device, with that device current, and handed to the kernels as their table pointer.
+static __device__ __align__(256) unsigned char g_static_tables[RS_STATIC_TABLE_BYTES];
+
+cudaError_t static_tables(void **ptr) {                       // the array on the CURRENT device
+    static std::mutex mu;
+    static void *cache[64];
+    *ptr = nullptr;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && cache[dev]) { *ptr = cache[dev]; return cudaSuccess; }
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_tables);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64) cache[dev] = p;
+    *ptr = p;
+    return cudaSuccess;
 }
 
 cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes, int stages,

@@ -26,5 +26,7 @@ cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool sm
 #define RS_TMAP_TABLE_BYTES (2 * RS_TMAP_BUFS * 128)
 cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,
                         int lookahead, uint32_t stage_bytes, float pace, int burst, bool pdl, cudaStream_t st);
+// device address, on the current device, of the file-scope table array of reshard_execute_static (RS_STATIC_TABLE_BYTES bytes, 256-byte aligned)
+cudaError_t static_tables(void **ptr);
 int64_t launch_count();
 }  // namespace rs

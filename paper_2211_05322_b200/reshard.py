@@ -31,7 +31,7 @@ RS_MAX_NDIM, RS_MAX_MESH_NDIM, RS_MAX_DEVICES = 8, 4, 128
 SYMBOLS = [
     "reshard_plan", "reshard_plan_ex", "reshard_plan_group", "reshard_plan_schedule", "reshard_plan_destroy", "reshard_plan_info", "reshard_op_info", "reshard_op_tables", "reshard_op_tiles",
     "reshard_plan_local_shape", "reshard_plan_device_box", "reshard_plan_slice", "reshard_plan_sender_bytes",
-    "reshard_plan_message", "reshard_execute", "reshard_execute_strategy", "reshard_pack", "reshard_unpack", "reshard_execute_host",
+    "reshard_plan_message", "reshard_execute", "reshard_execute_static", "reshard_execute_strategy", "reshard_pack", "reshard_unpack", "reshard_execute_host",
     "reshard_ipc_export", "reshard_ipc_import", "reshard_ipc_release_all",
     "reshard_host_workspace_bytes", "reshard_pipeline_simulate", "reshard_pipeline_least_delay", "reshard_launch_count", "reshard_strerror", "reshard_last_error",
     "reshard_version",
@@ -299,6 +299,10 @@ class Plan:
     # ---- data path (device addresses in, nothing out; asynchronous on `stream`)
     def execute(self, src_ptrs, dst_ptrs, stream=0):
         _chk(_lib().reshard_execute(self._h, _ptrs(src_ptrs), _ptrs(dst_ptrs), C.c_void_p(stream)))
+
+    def execute_static(self, src_ptrs, dst_ptrs, stream=0):
+        """reshard_execute_static: no device allocation anywhere (works on RS_HOST_ONLY plans); tables in the library's static device array"""
+        _chk(_lib().reshard_execute_static(self._h, _ptrs(src_ptrs), _ptrs(dst_ptrs), C.c_void_p(stream)))
 
     def execute_strategy(self, strategy, src_ptrs, dst_ptrs, stream=0):
         _chk(_lib().reshard_execute_strategy(self._h, int(strategy), _ptrs(src_ptrs), _ptrs(dst_ptrs), C.c_void_p(stream)))
