@@ -33,7 +33,8 @@
 // Rate matching of write-heavy (multicast) operations: every SM runs, every warp paces its tiles so that the launch
 // offers this many permille of the DRAM peak (2 x memory clock x bus width = 7 672 GB/s on B200).  Measured
 // (profiles/r02_pacing.md): achieved = 0.99 x offered up to 860 permille (6.52 TB/s on 1 + 8), collapse from 880 on
-// (6.09, then 5.56 at 920; unpaced 5.66); runs of 512 B: up to 820 (6.18 TB/s), 6.00 at 840.  10 permille below the edge.
+// (6.09, then 5.56 at 920; unpaced 5.66); runs of 512 B: up to 820 (6.18 TB/s), 6.00 at 840 -- on an IDLE chip.  The defaults below sit
+// 3-5 % lower, where a chip hot from GEMMs still holds them (profiles/r02_pacing.md part 4).
 #define RS_PACE_BLOCK_NS       1500           // a ring slot still being read this long after the warp asked for it: HBM is behind, back off
 #define RS_PACE_BURST          2              // tiles of credit of the token bucket
 #define RS_PACE_PERMILLE       825            // (850 is the best on a cold chip: 6.45 TB/s against 6.26; after GEMM bursts -- the chip power-limited, HBM hot -- the
@@ -73,11 +74,11 @@
 #define RS_SHIFT_TILE_BYTES  8192
 #define RS_SHIFT_LONG_RUN    4096       // rows at least this long: bulk stores (u4, 6 KiB rows: 6.12 TB/s against 5.65 from registers);
                                         // shorter: register stores, 8 warps (u1, 2 KiB rows: 5.8 against 4.1 with bulk stores)
-#define RS_SHIFT_MID_RUN     1024       // rows of 1-4 KiB (stored row by row from registers): 7 warps x 3 slots
+#define RS_SHIFT_MID_RUN     1024       // rows of 1-4 KiB (stored row by row from registers)
 #define RS_SHIFT_WARPS_MID   8          // u1 (2050-byte rows): 6 x 3: 5.38 TB/s, 7 x 3: 6.08, 8 x 2: 5.85, 8 x 3: 5.65
 #define RS_SHIFT_STAGES_MID  2          // (idle chip: 7 x 3 is best, 6.08 TB/s against 5.86-5.92; after GEMM bursts 7 x 3 falls to 4.34, 8 x 2 holds 4.92-4.97)
-#define RS_SHIFT_WARPS_LONG  8          // rows >= 1 KiB: bodies realigned in the ring and stored with bulk copies.  One warp per
-#define RS_SHIFT_STAGES_LONG 2          // scheduler hides no latency (~520 instructions per tile at ~6 cycles each), so 6 warps:
+#define RS_SHIFT_WARPS_LONG  8          // rows >= 4 KiB: bodies realigned in the ring and stored with bulk copies.  One warp per
+#define RS_SHIFT_STAGES_LONG 2          // scheduler hides no latency (~520 instructions per tile at ~6 cycles each), so many warps:
                                         // u4 4 x 4: 4.4 TB/s, 5 x 4: 5.4, 6 x 3: 6.12, 7 x 3: 6.05, 8 x 3: 5.75 (register stores, 4 x 4: 5.79) on an idle chip;
                                         // after GEMM bursts (SM clock ~1.4 GHz) 6 x 3 falls to 4.49 while 8 x 2 holds 5.69 (idle: 5.72), so 8 x 2
 
