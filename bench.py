@@ -538,6 +538,14 @@ def sweep_names(what):
     return out
 
 
+def _release(torch):
+    """give freed buffers back to the driver and let it finish with them: for some ms after a large cudaFree the device
+    is busy with the freed pages (the first ~20 launches after a 36 GiB free ran at 5.0 TB/s instead of 6.5, the same
+    launches after a 2 s wait at 6.5: profiles/r02_pacing.md part 5), which would be charged to the NEXT workload of a sweep"""
+    torch.cuda.empty_cache()
+    time.sleep(1.0)
+
+
 def _buffers(torch, dev, n, nbytes, gen):
     """n device buffers of nbytes each (256-byte aligned slices of ONE allocation), seeded bytes"""
     pitch = (nbytes + 255) // 256 * 256
@@ -628,7 +636,7 @@ def run_sweep(args):
             row["roof_1k_GB/s"] = roof
         plan.close()
         del keep, sets
-        torch.cuda.empty_cache()
+        _release(torch)
         # on-box ceiling: torch copy_ moving the same byte volume as execute (capped at 2 x 4 GiB), same protocol
         if not args.plain:
             half = min(x_bytes // 2, 4 << 30)
@@ -639,7 +647,7 @@ def run_sweep(args):
                 med, _b = time_each(lambda: pairs[0][1].copy_(pairs[0][0]), stream, K)
             row["torch_copy_same_volume_GB/s"] = 2 * half / med / 1e6
             del pairs
-            torch.cuda.empty_cache()
+            _release(torch)
         rows.append(row)
         print(json.dumps(row), flush=True)
     if args.md and args.strategies:

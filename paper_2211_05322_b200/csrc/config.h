@@ -21,15 +21,14 @@
 #define RS_BULK_STAGES       4          // ring slots per warp
 #define RS_BULK_LOOKAHEAD    2          // loads in flight per warp before the first store is issued
 #define RS_BULK_TILE_BYTES   12288      // bytes per ring slot
-#define RS_BULK_SHORT_RUN    2048       // runs up to this long: many copies per tile, use the SHORT shape (4 warps; paced when 1 : 1 and >= 128 MiB).
-                                        // 2 KiB rows on 2 warps are issue-bound once the SM clock drops under power (after GEMM bursts, ~1.4 GHz):
-                                        // P1 at 1 GiB 6.35 TB/s cold but 5.2-5.3 hot; on 4 paced warps 6.30 cold, 6.24 hot (256 MiB: 6.38 -> 6.09 cold, 4.80 -> 5.63 hot)
+#define RS_BULK_SHORT_RUN    2048       // runs up to this long: many copies per tile, use the SHORT shape (4 warps x 8 KiB) -- write-heavy operations,
+                                        // 1 : 1 ones under 128 MiB and tensor-map copies; larger 1 : 1 operations have a shape of their own (WIDE_11 below)
 #define RS_BULK_MIN_FILL     0.7        // slots less full than this on average: the SHORT shape too
 #define RS_BULK_TINY_FILL    0.3        // slots less than 30 % full (tiles under ~3.5 KiB): 8 warps x 3 slots x 4 KiB
 #define RS_BULK_WARPS_SHORT  4
 #define RS_BULK_TILE_BYTES_SHORT 8192
 #define RS_BULK_CTAS_DEN       148    // CTA counts below are out of 148 SMs
-#define RS_BULK_CTAS_LONG_NUM  132    // 1 : 1 operations whose runs are at least RS_BULK_LONG_RUN
+#define RS_BULK_CTAS_LONG_NUM  132    // large 1 : 1 operations (WIDE_11)
 // Rate matching of write-heavy (multicast) operations: every SM runs, every warp paces its tiles so that the launch
 // offers this many permille of the DRAM peak (2 x memory clock x bus width = 7 672 GB/s on B200).  Measured
 // (profiles/r02_pacing.md): achieved = 0.99 x offered up to 860 permille (6.52 TB/s on 1 + 8), collapse from 880 on
@@ -42,14 +41,12 @@
 #define RS_PACE_PERMILLE_SHORT 775            // (cold: 6.08 TB/s at 810, 5.83 at 775; hot: 4.63 at 810, 5.85 at 775)
 #define RS_PACE_PERMILLE_SHORT_DENSE 820   // short rows that are adjacent in the receivers (one bulk store per tile)
 #define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
-#define RS_PACE_PERMILLE_11    880            // 1 : 1 operations made of runs >= 1 MiB: best at 880-900, collapse from 910 (fig5_1x1 6.18 -> 6.56 TB/s,
-#define RS_PACE_PERMILLE_11_SHORT 860          // 1 : 1 operations on the 4-warp shape (rows <= 1 KiB or half-empty slots)
-#define RS_PACE_11_MIN_RUN     (1ll << 20)    //   P6 at 4 GiB 6.56 -> 6.8, unpack of P2 6.59 -> 6.76; runs of 128 KiB: no change; 2-6 KiB rows: 0 to -3 %)
+#define RS_PACE_PERMILLE_11    880            // 1 : 1 operations moving >= RS_PACE_11_MIN_BYTES through rs_copy_bulk: 4 warps x 12 KiB per SM, paced (tables.cpp
+                                              //   WIDE_11; 890 is 1 % better on an idle chip and 1 % worse on a hot one, collapse from 900 on)
+#define RS_PACE_PERMILLE_11_SHORT 860         // ... through tensor maps (rows of 64 B - 2 KiB)
 #define RS_PACE_11_MIN_BYTES   (128ll << 20)
+#define RS_WIDE_11_ALL_SMS_RUN 1024           // WIDE_11 with rows up to this long (12+ copies per tile): every SM instead of 132 of 148
 #define RS_MID_MCAST_BYTES     (768ll << 20)  // paced write-heavy operations moving up to this much: the 4-warp shape
-#define RS_BULK_LONG_RUN       4096
-#define RS_BULK_CTAS_MIN_BYTES (384ll << 20)   // operations moving less than this keep one CTA on every SM (config 2's pack, 128 + 128 MiB:
-                                               // 46.1 us on 132 CTAs, 43.3 us on 148; at 256 + 256 MiB the two are level, beyond 132 wins)
 #define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path
                                             // (no shared-memory carve-out, no mbarriers: 4 MiB + 4 MiB in 3.2 us against 6.5 us;
                                             // equal at 16 + 16 MiB; from 20 + 20 MiB on the TMA ring wins: 8.1 against 8.6 us)

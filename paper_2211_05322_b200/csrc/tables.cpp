@@ -170,7 +170,7 @@ int pick_path(const Plan &P, int64_t align, int64_t min_run, int64_t max_run, in
 // Launch shape of the two TMA kernels, from measurement on B200.
 struct BulkShape { int warps, stages, grid, pace_permille; int64_t tile_bytes; };
 
-BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_bytes, int64_t write_bytes, bool dst_dense, bool underfilled, bool tiny_tiles) {
+BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int64_t read_bytes, int64_t write_bytes, bool dst_dense, bool underfilled, bool tiny_tiles) {
     const rs_tuning &U = P.tune;
     // short runs = many bulk copies per tile: one warp issues them too slowly, so more, smaller pipelines
     // (Table 2 case 9, 512-byte runs: 3.6 TB/s with 2 warps, 5.7 with 4)
@@ -190,31 +190,29 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     // paced write-heavy operations of medium size ramp faster on 4 warps x 8 KiB (16 + 128 MiB: 26.0 -> 25.3 us, 64 + 512 MiB +1.4 %; from ~1 GiB moved
     // on the two shapes are level)
     const bool mid_mcast = !shift && !capped && write_bytes >= 2 * read_bytes && read_bytes + write_bytes >= RS_PACE_MIN_BYTES && read_bytes + write_bytes <= RS_MID_MCAST_BYTES;
-    BulkShape sh;
-    sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : shift_mid ? RS_SHIFT_WARPS_MID : RS_SHIFT_WARPS)
-                                             : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : short_runs || capped || mid_mcast ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
-    sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : shift_mid ? RS_SHIFT_STAGES_MID : RS_SHIFT_STAGES)
-                                              : pick(U.bulk_stages, small_mcast ? RS_BULK_STAGES_SMALL_MCAST : RS_BULK_STAGES)));
-    sh.tile_bytes = shift ? pick(U.shift_tile_bytes, RS_SHIFT_TILE_BYTES)
-                          : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : short_runs || mid_mcast ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
-    sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
-    while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
     // One CTA per SM.
     //  * Write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes) are an OPEN loop: stores are fire and
     //    forget, every SM can push ~65 GB/s, 148 of them offer 9.6 TB/s and HBM collapses to 5.2-5.8 TB/s.  They run on
-    //    every SM and are RATE MATCHED (kernels.cu pace_tile, config.h RS_PACE_PERMILLE): 6.4-6.5 TB/s.
-    //  * 1 : 1 operations limit themselves (loads are a closed loop: bytes in flight / latency) and stay unpaced;
-    //    with long runs (<= 3 bulk copies per tile) 132 CTAs are 1.5-3.7 % faster than 148 (a fraction of the SM count,
-    //    so the rule survives a different part); operations moving under 384 MiB are ramp-bound: every SM.
-    const bool write_heavy = write_bytes >= 2 * read_bytes, big = read_bytes + write_bytes >= RS_BULK_CTAS_MIN_BYTES;
-    //  * 1 : 1 operations made of VERY long runs (>= 1 MiB on both sides: whole-shard copies, unpack of a broadcast, P3 / P6)
-    //    do not limit themselves well enough either: on every SM and paced at 880 permille they reach 6.45-6.7 TB/s where the
-    //    unpaced 132-CTA launch gives 6.2-6.55 and `torch copy_` 6.4-6.6 (profiles/r02_pacing.md, second part); from 910 on
-    //    they collapse like the write-heavy ones.  Rows of a few KiB gain nothing (config 4) or lose 3 % (P1: 2 warps per SM
-    //    have no slack for a pause).
-    const bool long_11 = !shift && !write_heavy && min_run >= RS_PACE_11_MIN_RUN && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES;
+    //    every SM and are RATE MATCHED (kernels.cu pace_tile, config.h RS_PACE_PERMILLE): 6.2-6.3 TB/s.
+    //  * 1 : 1 operations moving >= 128 MiB through per-row bulk copies: 4 warps x 12 KiB slots on 132 of 148 SMs, paced at
+    //    880 permille (WIDE_11).  The loop of 2 unpaced warps per SM limits itself (bytes in flight / latency) and was the
+    //    round's first shape: 6.3-6.5 TB/s on an idle chip, but 4.4-4.8 for rows of 3-6 KiB once the SM clock drops under
+    //    power (latency in cycles is what it is; in ns it grows).  Twice the pipelines have the slack, and the pacing then
+    //    sets the rate: 6.39-6.56 TB/s idle AND hot on every 1 : 1 layout measured (profiles/r02_pacing.md part 5); 890 is
+    //    1 % better idle and 1 % worse hot, from 900 on it collapses.  Rows <= 1 KiB (12+ copies per tile): every SM.
+    const bool write_heavy = write_bytes >= 2 * read_bytes;
+    const bool wide_11 = !shift && !tmap && !capped && !write_heavy && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES;
+    BulkShape sh;
+    sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : shift_mid ? RS_SHIFT_WARPS_MID : RS_SHIFT_WARPS)
+                                             : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : wide_11 || short_runs || capped || mid_mcast ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
+    sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : shift_mid ? RS_SHIFT_STAGES_MID : RS_SHIFT_STAGES)
+                                              : pick(U.bulk_stages, small_mcast ? RS_BULK_STAGES_SMALL_MCAST : RS_BULK_STAGES)));
+    sh.tile_bytes = shift ? pick(U.shift_tile_bytes, RS_SHIFT_TILE_BYTES)
+                          : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : wide_11 ? RS_BULK_TILE_BYTES : short_runs || mid_mcast ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
+    sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
+    while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
     int ctas = P.sm_count;
-    if (big && !shift && !write_heavy && !long_11 && min_run >= RS_BULK_LONG_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
+    if (wide_11 && min_run > RS_WIDE_11_ALL_SMS_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
     sh.grid = std::max(1, std::min(P.sm_count, pick(write_heavy ? U.bulk_ctas_mcast : U.bulk_ctas, std::max(1, ctas))));
     if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
     // (operations under 64 MiB are over before the pacing has anything to hold back: they keep the unpaced ramp)
@@ -222,10 +220,8 @@ BulkShape bulk_shape(const Plan &P, bool shift, int64_t min_run, int64_t read_by
     // take a higher rate than rows stored one by one (Table 2 case 9: 6.12 TB/s at 810, 6.26 at 830, 6.35-6.40 at 850 on two
     // boxes but 5.98 on a third, whose edge lies lower: 830)
     sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
-                     : long_11 ? RS_PACE_PERMILLE_11
-                     // 1 : 1 on the 4-warp shape (rows <= 1 KiB, half-empty slots): twice the pipelines per SM make the loop open enough to want
-                     // pacing too (a4 6.09 -> 6.33-6.48 TB/s at 850-870, 1 KiB rows on 4x8 -> 8x4 meshes 5.81 -> 6.04, 128-byte rows through
-                     // tensor maps 5.37 -> 6.15-6.33; collapse at 890); the 2-warp shape loses 3 % when paced
+                     : wide_11 ? RS_PACE_PERMILLE_11
+                     // 1 : 1 through tensor maps (rows of 64 B - 2 KiB; always the 4-warp shape): 128-byte rows 5.37 -> 6.15-6.33 TB/s at 850-870, collapse at 890
                      : !shift && !write_heavy && short_runs && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES ? RS_PACE_PERMILLE_11_SHORT : 0;
     return sh;
 }
@@ -351,7 +347,7 @@ rs_status finish_op_impl(Plan *P, OpTables *op, int64_t read_bytes, int64_t writ
         // pacing of that shape: config 2 43.6 -> 41.8 us (torch copy_ 42.4), its unpack 43.1 -> 41.6, 64 + 64 MiB 22.2-22.4 -> 21.7-22.0;
         // unpaced the 4 warps lose (45.5 us)
         if (path == RS_PATH_TMAP && write_bytes < 2 * read_bytes && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES) underfilled = true;
-        BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, min_run, read_bytes, write_bytes, dst_dense, underfilled, tiny_tiles);
+        BulkShape sh = bulk_shape(*P, path == RS_PATH_BULK_SHIFT, path == RS_PATH_TMAP, min_run, read_bytes, write_bytes, dst_dense, underfilled, tiny_tiles);
         tile_bytes = sh.tile_bytes;
         stages = sh.stages;
         op->pace_permille = sh.pace_permille;
