@@ -1029,7 +1029,7 @@ def run_ncu_summary(args):
     out_csv.writerow(cols)
     for item in args.ncu_summary:
         key, path = item.rsplit("=", 1)
-        workload, op = key.split(":") if ":" in key else (key, "execute")
+        workload, op = key.rsplit(":", 1) if ":" in key else (key, "execute")     # (x:... workload names hold colons)
         out = subprocess.run(["ncu", "-i", path, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
         rows = list(csv.reader(io.StringIO(out)))
         hdr, units = rows[0], rows[1]

@@ -23,6 +23,8 @@
 #define RS_BULK_TILE_BYTES   12288      // bytes per ring slot
 #define RS_BULK_SHORT_RUN    2048       // runs up to this long: many copies per tile, use the SHORT shape (4 warps x 8 KiB) -- write-heavy operations,
                                         // 1 : 1 ones under 128 MiB and tensor-map copies; larger 1 : 1 operations have a shape of their own (WIDE_11 below)
+#define RS_BULK_VERY_SHORT_RUN 512      // large operations made of rows up to this long (24+ copies per 12 KiB): 8 warps x 4 slots x 6 KiB (tables.cpp many_copies)
+#define RS_BULK_TILE_BYTES_MANY 6144
 #define RS_BULK_MIN_FILL     0.7        // slots less full than this on average: the SHORT shape too
 #define RS_BULK_TINY_FILL    0.3        // slots less than 30 % full (tiles under ~3.5 KiB): 8 warps x 3 slots x 4 KiB
 #define RS_BULK_WARPS_SHORT  4
@@ -41,10 +43,12 @@
 #define RS_PACE_PERMILLE_SHORT 775            // (cold: 6.08 TB/s at 810, 5.83 at 775; hot: 4.63 at 810, 5.85 at 775)
 #define RS_PACE_PERMILLE_SHORT_DENSE 820   // short rows that are adjacent in the receivers (one bulk store per tile)
 #define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
-#define RS_PACE_PERMILLE_11    880            // 1 : 1 operations moving >= RS_PACE_11_MIN_BYTES through rs_copy_bulk: 4 warps x 12 KiB per SM, paced (tables.cpp
+#define RS_PACE_PERMILLE_11    880            // 1 : 1 operations moving >= RS_WIDE_11_MIN_BYTES through rs_copy_bulk: 4 warps x 12 KiB per SM, paced (tables.cpp
                                               //   WIDE_11; 890 is 1 % better on an idle chip and 1 % worse on a hot one, collapse from 900 on)
 #define RS_PACE_PERMILLE_11_SHORT 860         // ... through tensor maps (rows of 64 B - 2 KiB)
 #define RS_PACE_11_MIN_BYTES   (128ll << 20)
+#define RS_WIDE_11_MIN_BYTES   (256ll << 20)  // (64 + 64 MiB of long runs, CUDA graph of 50 launches: 21.9 us on 2 unpaced warps x 148 CTAs, 24.1 as WIDE_11; 128 + 128 MiB: 43.5 / 43.2;
+                                              //  256 + 256 MiB: 83.8 / 82.9)
 #define RS_WIDE_11_ALL_SMS_RUN 1024           // WIDE_11 with rows up to this long (12+ copies per tile): every SM instead of 132 of 148
 #define RS_MID_MCAST_BYTES     (768ll << 20)  // paced write-heavy operations moving up to this much: the 4-warp shape
 #define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path

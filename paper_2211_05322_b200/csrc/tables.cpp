@@ -194,21 +194,26 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     //  * Write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes) are an OPEN loop: stores are fire and
     //    forget, every SM can push ~65 GB/s, 148 of them offer 9.6 TB/s and HBM collapses to 5.2-5.8 TB/s.  They run on
     //    every SM and are RATE MATCHED (kernels.cu pace_tile, config.h RS_PACE_PERMILLE): 6.2-6.3 TB/s.
-    //  * 1 : 1 operations moving >= 128 MiB through per-row bulk copies: 4 warps x 12 KiB slots on 132 of 148 SMs, paced at
+    //  * 1 : 1 operations moving >= 256 MiB through per-row bulk copies: 4 warps x 12 KiB slots on 132 of 148 SMs, paced at
     //    880 permille (WIDE_11).  The loop of 2 unpaced warps per SM limits itself (bytes in flight / latency) and was the
     //    round's first shape: 6.3-6.5 TB/s on an idle chip, but 4.4-4.8 for rows of 3-6 KiB once the SM clock drops under
     //    power (latency in cycles is what it is; in ns it grows).  Twice the pipelines have the slack, and the pacing then
     //    sets the rate: 6.39-6.56 TB/s idle AND hot on every 1 : 1 layout measured (profiles/r02_pacing.md part 5); 890 is
     //    1 % better idle and 1 % worse hot, from 900 on it collapses.  Rows <= 1 KiB (12+ copies per tile): every SM.
     const bool write_heavy = write_bytes >= 2 * read_bytes;
-    const bool wide_11 = !shift && !tmap && !capped && !write_heavy && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES;
+    const bool wide_11 = !shift && !tmap && !capped && !write_heavy && !small_mcast && read_bytes + write_bytes >= RS_WIDE_11_MIN_BYTES;
+    //  * Rows up to 512 bytes (24+ copies per 12 KiB) in large operations, 1 : 1 or write-heavy: 8 warps x 6 KiB.  At ~2 instructions
+    //    per copy and ~6 cycles per instruction with one warp per scheduler, four warps keep up at the boost clock only (512-byte rows,
+    //    1 + 1 GiB: 6.26 TB/s idle, 5.17 hot; on 8 warps 6.33 / 6.17; Table 2 case 9: 6.19 / 5.16 -> 6.19 / 5.55).
+    const bool many_copies = !shift && !tmap && !capped && !small_mcast && min_run <= RS_BULK_VERY_SHORT_RUN &&
+                             (wide_11 || (write_heavy && read_bytes + write_bytes > RS_MID_MCAST_BYTES));
     BulkShape sh;
     sh.warps = std::max(1, std::min(8, shift ? pick(U.shift_warps, shift_long ? RS_SHIFT_WARPS_LONG : shift_mid ? RS_SHIFT_WARPS_MID : RS_SHIFT_WARPS)
-                                             : pick(U.bulk_warps, small_mcast ? RS_BULK_WARPS_SMALL_MCAST : wide_11 || short_runs || capped || mid_mcast ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
+                                             : pick(U.bulk_warps, small_mcast || many_copies ? RS_BULK_WARPS_SMALL_MCAST : wide_11 || short_runs || capped || mid_mcast ? RS_BULK_WARPS_SHORT : RS_BULK_WARPS)));
     sh.stages = std::max(2, std::min(8, shift ? pick(U.shift_stages, shift_long ? RS_SHIFT_STAGES_LONG : shift_mid ? RS_SHIFT_STAGES_MID : RS_SHIFT_STAGES)
                                               : pick(U.bulk_stages, small_mcast ? RS_BULK_STAGES_SMALL_MCAST : RS_BULK_STAGES)));
     sh.tile_bytes = shift ? pick(U.shift_tile_bytes, RS_SHIFT_TILE_BYTES)
-                          : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : wide_11 ? RS_BULK_TILE_BYTES : short_runs || mid_mcast ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
+                          : pick(U.bulk_tile_bytes, small_mcast ? RS_BULK_TILE_BYTES_SMALL_MCAST : many_copies ? RS_BULK_TILE_BYTES_MANY : wide_11 ? RS_BULK_TILE_BYTES : short_runs || mid_mcast ? RS_BULK_TILE_BYTES_SHORT : RS_BULK_TILE_BYTES);
     sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
     while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
     int ctas = P.sm_count;
