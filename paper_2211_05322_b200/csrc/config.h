@@ -47,8 +47,11 @@
                                               //   WIDE_11; 890 is 1 % better on an idle chip and 1 % worse on a hot one, collapse from 900 on)
 #define RS_PACE_PERMILLE_11_SHORT 860         // ... through tensor maps (rows of 64 B - 2 KiB)
 #define RS_PACE_11_MIN_BYTES   (128ll << 20)
-#define RS_WIDE_11_MIN_BYTES   (256ll << 20)  // (64 + 64 MiB of long runs, CUDA graph of 50 launches: 21.9 us on 2 unpaced warps x 148 CTAs, 24.1 as WIDE_11; 128 + 128 MiB: 43.5 / 43.2;
-                                              //  256 + 256 MiB: 83.8 / 82.9)
+#define RS_WIDE_11_MIN_BYTES   (384ll << 20)  // (CUDA graphs of 50+ launches.  64 + 64 MiB of long runs: 21.9 us on 2 unpaced warps x 148 CTAs, 24.1 as WIDE_11; 128 + 128 MiB: long runs
+                                              //  6.42 TB/s on 2 warps @ 880 x 148 CTAs against 6.16 as WIDE_11, config 2's pack (2 KiB rows) 6.16 on 4 x 8 KiB @ 860 against 5.86;
+                                              //  256 + 256 MiB: WIDE_11 +3-5 % on P1 / P4 / P6)
+#define RS_PACE_11_MIN_RUN     (1ll << 20)    // below RS_WIDE_11_MIN_BYTES: 1 : 1 operations made of runs this long keep 2 warps on every SM, paced at RS_PACE_PERMILLE_11
+                                              //  (64 + 64 MiB of whole-shard copies: 6.29 TB/s against 6.14 unpaced)
 #define RS_WIDE_11_ALL_SMS_RUN 1024           // WIDE_11 with rows up to this long (12+ copies per tile): every SM instead of 132 of 148
 #define RS_MID_MCAST_BYTES     (768ll << 20)  // paced write-heavy operations moving up to this much: the 4-warp shape
 #define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path

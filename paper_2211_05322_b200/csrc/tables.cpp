@@ -194,7 +194,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     //  * Write-heavy operations (a slice with k >= 2 receivers: 1 read + k writes) are an OPEN loop: stores are fire and
     //    forget, every SM can push ~65 GB/s, 148 of them offer 9.6 TB/s and HBM collapses to 5.2-5.8 TB/s.  They run on
     //    every SM and are RATE MATCHED (kernels.cu pace_tile, config.h RS_PACE_PERMILLE): 6.2-6.3 TB/s.
-    //  * 1 : 1 operations moving >= 256 MiB through per-row bulk copies: 4 warps x 12 KiB slots on 132 of 148 SMs, paced at
+    //  * 1 : 1 operations moving >= 384 MiB through per-row bulk copies: 4 warps x 12 KiB slots on 132 of 148 SMs, paced at
     //    880 permille (WIDE_11).  The loop of 2 unpaced warps per SM limits itself (bytes in flight / latency) and was the
     //    round's first shape: 6.3-6.5 TB/s on an idle chip, but 4.4-4.8 for rows of 3-6 KiB once the SM clock drops under
     //    power (latency in cycles is what it is; in ns it grows).  Twice the pipelines have the slack, and the pacing then
@@ -202,6 +202,8 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     //    1 % better idle and 1 % worse hot, from 900 on it collapses.  Rows <= 1 KiB (12+ copies per tile): every SM.
     const bool write_heavy = write_bytes >= 2 * read_bytes;
     const bool wide_11 = !shift && !tmap && !capped && !write_heavy && !small_mcast && read_bytes + write_bytes >= RS_WIDE_11_MIN_BYTES;
+    //  * Smaller 1 : 1 operations keep the ramp of the lighter shapes; those made of runs >= 1 MiB and moving >= 128 MiB are paced on their two warps.
+    const bool long_11 = !shift && !write_heavy && !wide_11 && min_run >= RS_PACE_11_MIN_RUN && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES;
     //  * Rows up to 512 bytes (24+ copies per 12 KiB) in large operations, 1 : 1 or write-heavy: 8 warps x 6 KiB.  At ~2 instructions
     //    per copy and ~6 cycles per instruction with one warp per scheduler, four warps keep up at the boost clock only (512-byte rows,
     //    1 + 1 GiB: 6.26 TB/s idle, 5.17 hot; on 8 warps 6.33 / 6.17; Table 2 case 9: 6.19 / 5.16 -> 6.19 / 5.55).
@@ -225,7 +227,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     // take a higher rate than rows stored one by one (Table 2 case 9: 6.12 TB/s at 810, 6.26 at 830, 6.35-6.40 at 850 on two
     // boxes but 5.98 on a third, whose edge lies lower: 830)
     sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
-                     : wide_11 ? RS_PACE_PERMILLE_11
+                     : wide_11 || long_11 ? RS_PACE_PERMILLE_11
                      // 1 : 1 through tensor maps (rows of 64 B - 2 KiB; always the 4-warp shape): 128-byte rows 5.37 -> 6.15-6.33 TB/s at 850-870, collapse at 890
                      : !shift && !write_heavy && short_runs && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES ? RS_PACE_PERMILLE_11_SHORT : 0;
     return sh;
