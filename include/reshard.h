@@ -135,7 +135,7 @@ typedef struct rs_tuning {
                                                           never two ring CTAs on one SM; 1 = only what the ring needs) */
     int32_t lsu_narrow;                                /* register path on layouts that are not 16-byte aligned: 1 = always at the layout's own vector
                                                           width, -1 = always the 16-byte shift kernel, 0 = library default (by row length) */
-    int32_t shift_mode;                                /* rs_copy_bulk_shift, rows >= 1 KiB: 0 = library default; 1: windows
+    int32_t shift_mode;                                /* rs_copy_bulk_shift, rows >= 1 KiB: 0 = library default (= 1); 1: windows
                                                           assembled in registers and stored with st.global; 2: row bodies
                                                           realigned in shared memory and stored with cp.async.bulk      */
 } rs_tuning;

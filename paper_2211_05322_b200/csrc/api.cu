@@ -440,8 +440,9 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     const bool as_bulk = op.info.path == RS_PATH_BULK || op.info.path == RS_PATH_TMAP;   // aligned TMA plans
     const int warps = op.info.block / 32;
     const bool pdl = !P.tune.no_pdl && !static_dev;          // (the shared table array is rewritten between launches: full stream order)
-    const int shift_mode = P.tune.shift_mode == rs::RS_SHIFT_REG || P.tune.shift_mode == rs::RS_SHIFT_BULK ? P.tune.shift_mode
-                         : op.info.min_run_bytes >= RS_SHIFT_LONG_RUN ? rs::RS_SHIFT_BULK : rs::RS_SHIFT_REG;
+    // shifted stores from registers; realigning the rows in the ring and storing them with cp.async.bulk (rs_tuning.shift_mode = 2) is 3-4 % faster for rows
+    // >= 4 KiB on an idle chip (u4 6.31 against 6.10 TB/s) and 12-18 % slower on a power-limited one (5.3 against 5.97): more instructions per tile (config.h)
+    const int shift_mode = P.tune.shift_mode == rs::RS_SHIFT_REG || P.tune.shift_mode == rs::RS_SHIFT_BULK ? P.tune.shift_mode : rs::RS_SHIFT_REG;
     if (as_bulk && align == 16) {
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         dev.early_trigger = grid >= P.sm_count;
@@ -461,14 +462,16 @@ rs_status run_op(const rs_plan *plan, int opi, const void *const *src, int n_src
     } else if (op.info.path == RS_PATH_BULK_SHIFT) {          // layout not 16-byte aligned: TMA loads, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(op.info.grid, (n_tiles + warps - 1) / warps));
         dev.early_trigger = grid >= P.sm_count;
+        const int permille = P.tune.pace_permille > 0 ? P.tune.pace_permille : P.tune.pace_permille < 0 ? 0 : op.pace_permille;
+        const float pace = permille > 0 ? (float)((double)grid * warps / (P.dram_peak_gbs * permille / 1000.0)) : 0.f;
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.info.block, op.info.smem_bytes, op.stages, op.lookahead,
-                                  op.shift_stage, shift_mode, pdl, st);
+                                  op.shift_stage, shift_mode, pace, P.tune.pace_burst > 0 ? std::min(P.tune.pace_burst, 255) : RS_PACE_BURST, pdl, st);
     } else if (as_bulk && op.alt_stage) {                     // aligned plan, under-aligned pointers: same tiles, shifted stores
         const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(P.max_ctas > 0 ? std::min(P.sm_count, P.max_ctas) : P.sm_count,
                                                                      (n_tiles + op.alt_warps - 1) / op.alt_warps));
         dev.early_trigger = grid >= P.sm_count;
         e = rs::launch_bulk_shift(dev, pt, small, grid, op.alt_warps * 32, op.alt_smem, op.alt_stages, op.alt_stages - 1,
-                                  op.alt_stage, shift_mode, pdl, st);
+                                  op.alt_stage, shift_mode, 0.f, RS_PACE_BURST, pdl, st);
     } else {                                                  // register paths
         int64_t cap = bulk_family ? (int64_t)P.sm_count * RS_LSU_CTAS_DEFAULT : op.info.grid;
         if (P.max_ctas > 0) cap = std::min<int64_t>(cap, P.max_ctas);

@@ -76,8 +76,12 @@
 #define RS_SHIFT_WARPS       8          // u4 (6145-byte runs, 2-byte aligned): 8 x 2 x 8 KiB = 5.6-5.7 TB/s; 4 x 4 x 8 KiB a little more,
 #define RS_SHIFT_STAGES      2          // but short rows (flat walk, ~100 instructions per 512 B) need the 8 warps
 #define RS_SHIFT_TILE_BYTES  8192
-#define RS_SHIFT_LONG_RUN    4096       // rows at least this long: bulk stores (u4, 6 KiB rows: 6.12 TB/s against 5.65 from registers);
-                                        // shorter: register stores, 8 warps (u1, 2 KiB rows: 5.8 against 4.1 with bulk stores)
+#define RS_PACE_PERMILLE_SHIFT       850          // rate matching of the shifted kernel, rows >= RS_PACE_SHIFT_MIN_RUN: 1 : 1 (u4: 5.96 TB/s at 800, 6.17 at 830, 6.31 at 850, 6.29 at 860; u1 5.90 / 6.11 / 6.24 / 6.30)
+#define RS_PACE_PERMILLE_SHIFT_MCAST 800          // ... write-heavy (1 + 4 of u1's rows: 5.91 TB/s at 800, 4.81 at 830 -- past the edge; unpaced 4.79)
+#define RS_PACE_SHIFT_MIN_BYTES      (256ll << 20)
+#define RS_PACE_SHIFT_MIN_RUN         2048
+#define RS_SHIFT_LONG_RUN    4096       // rows at least this long MAY leave through bulk stores (rs_tuning.shift_mode = 2; unpaced: u4 6.12 TB/s against 5.65 from registers;
+                                        // paced at 850: 6.31 against 6.10 idle, 5.3 against 5.97 after GEMM bursts, so registers are the default: api.cu)
 #define RS_SHIFT_MID_RUN     1024       // rows of 1-4 KiB (stored row by row from registers)
 #define RS_SHIFT_WARPS_MID   8          // u1 (2050-byte rows): 6 x 3: 5.38 TB/s, 7 x 3: 6.08, 8 x 2: 5.85, 8 x 3: 5.65
 #define RS_SHIFT_STAGES_MID  2          // (idle chip: 7 x 3 is best, 6.08 TB/s against 5.86-5.92; after GEMM bursts 7 x 3 falls to 4.34, 8 x 2 holds 4.92-4.97)

@@ -739,7 +739,7 @@ __device__ __forceinline__ void slot_store(const ShiftSlot &t, char *dr, uint32_
 template <int NP>
 __global__ void __launch_bounds__(256, 1)
 rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptrs, const int stages, const int lookahead,
-                   const uint32_t stage_bytes, const int mode) {
+                   const uint32_t stage_bytes, const int mode, const float pace, const int burst) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const uint32_t bars = smem_u32(smem) + warp * 64;
@@ -758,6 +758,7 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptr
     const int pending_ok = stages - lookahead - 1;            // store groups that may still read the ring (>= 0)
     int ld_slot = 0, st_slot = 0;
     uint32_t st_parity = 0;
+    uint64_t t_next = 0;                                      // rate matching (pace_tile), as in rs_copy_bulk
 
     for (int it = 0; it < n_my + lookahead; ++it) {
         if (it < n_my) {                                      // ---- load tile `it`
@@ -774,6 +775,7 @@ rs_copy_bulk_shift(const RsOpDev op, const __grid_constant__ RsPtrTableT<NP> ptr
             }
             const RsDesc *d = descs + (it & (RS_DESC_RING - 1));
             const uint32_t n_rows = d->n_rows, n = d->col_bytes, pitch = shift_pitch(n);
+            if (pace > 0.f) pace_tile(t_next, pace, burst & 0xff, n_rows * n * (1u + d->k), lane);
             const uint32_t bar = bars + 8 * ld_slot, slot = ring + (uint32_t)ld_slot * stage_bytes;
             const bool fast = d->flags & RS_TILE_FAST;
             const RsTask *__restrict__ T = op.tasks + d->task;
@@ -969,9 +971,9 @@ cudaError_t prepare_bulk(int smem_bytes) {
 }
 
 cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
-                              int stages, int lookahead, uint32_t stage_bytes, int mode, bool pdl, cudaStream_t st) {
-    if (small) return launch_k(rs_copy_bulk_shift<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes, mode);
-    return launch_k(rs_copy_bulk_shift<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes, mode);
+                              int stages, int lookahead, uint32_t stage_bytes, int mode, float pace, int burst, bool pdl, cudaStream_t st) {
+    if (small) return launch_k(rs_copy_bulk_shift<RS_PTRS_SMALL>, grid, block, (size_t)smem_bytes, st, pdl, op, small_table(ptrs), stages, lookahead, stage_bytes, mode, pace, burst);
+    return launch_k(rs_copy_bulk_shift<128>, grid, block, (size_t)smem_bytes, st, pdl, op, ptrs, stages, lookahead, stage_bytes, mode, pace, burst);
 }
 
 cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,

@@ -21,7 +21,7 @@ cudaError_t launch_bulk(const RsOpDev &op, const RsPtrTable &ptrs, bool small, i
 // mode: RS_SHIFT_REG (register stores) or RS_SHIFT_BULK (bodies of long rows realigned in the ring, bulk stores)
 enum { RS_SHIFT_REG = 1, RS_SHIFT_BULK = 2 };
 cudaError_t launch_bulk_shift(const RsOpDev &op, const RsPtrTable &ptrs, bool small, int grid, int block, int smem_bytes,
-                              int stages, int lookahead, uint32_t stage_bytes, int mode, bool pdl, cudaStream_t st);
+                              int stages, int lookahead, uint32_t stage_bytes, int mode, float pace, int burst, bool pdl, cudaStream_t st);
 // tensor-map TMA path: tmaps = RS_TMAP_TABLE_BYTES bytes, RS_TMAP_BUFS CUtensorMap per side (api.cu encodes them)
 #define RS_TMAP_TABLE_BYTES (2 * RS_TMAP_BUFS * 128)
 cudaError_t launch_tmap(const RsOpDev &op, const RsPtrTable &ptrs, const void *tmaps, int grid, int block, int smem_bytes, int stages,

@@ -226,10 +226,13 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     // short rows that are adjacent in every destination are stored with one bulk copy per tile and receiver (kernels.cu) and
     // take a higher rate than rows stored one by one (Table 2 case 9: 6.12 TB/s at 810, 6.26 at 830, 6.35-6.40 at 850 on two
     // boxes but 5.98 on a third, whose edge lies lower: 830)
-    sh.pace_permille = write_heavy && !shift && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
+    // The shifted kernel (unaligned layouts) offers too much as well -- 8 warps per SM, stores fire and forget: u4 5.65 -> 6.31 TB/s at 850 permille, u1 5.86 -> 6.24,
+    // their pack / unpack +6-15 %; write-heavy: 5.49 -> 6.08 and 4.79 -> 5.91 at 800, collapse from 830 on (profiles/r02_unaligned.md).  Rows >= 2 KiB only (1 KiB rows: issue-bound, 4.58 -> 4.47).
+    sh.pace_permille = shift ? (min_run >= RS_PACE_SHIFT_MIN_RUN && read_bytes + write_bytes >= RS_PACE_SHIFT_MIN_BYTES ? (write_heavy ? RS_PACE_PERMILLE_SHIFT_MCAST : RS_PACE_PERMILLE_SHIFT) : 0)
+                     : write_heavy && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
                      : wide_11 || long_11 ? RS_PACE_PERMILLE_11
                      // 1 : 1 through tensor maps (rows of 64 B - 2 KiB; always the 4-warp shape): 128-byte rows 5.37 -> 6.15-6.33 TB/s at 850-870, collapse at 890
-                     : !shift && !write_heavy && short_runs && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES ? RS_PACE_PERMILLE_11_SHORT : 0;
+                     : !write_heavy && short_runs && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES ? RS_PACE_PERMILLE_11_SHORT : 0;
     return sh;
 }
 

@@ -483,8 +483,10 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("t2_4") == (rs.RS_PATH_BULK, 132, 128, 880)                   # 128 KiB runs, 1 : 1
     assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 128, 825)      # write-heavy, 144 MiB moved: paced, 4 warps
     assert shape_of("t2_9") == (rs.RS_PATH_BULK, 148, 256, 820)                   # 512-byte runs, 1 + 4: 8 warps; rows adjacent in the receivers
-    assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 256, 0)                 # nothing aligned, 6 KiB rows: 8 warps, bulk stores
-    assert shape_of("u1") == (rs.RS_PATH_BULK_SHIFT, 148, 256, 0)                 # nothing aligned, 2 KiB rows: 8 warps, register stores
+    assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 256, 850)               # nothing aligned, 6 KiB rows: 8 warps, bulk stores, paced
+    assert shape_of("u1") == (rs.RS_PATH_BULK_SHIFT, 148, 256, 850)               # nothing aligned, 2 KiB rows: 8 warps, register stores, paced
+    assert shape_of("x:64x2046x4100:bf16:2x4:S0RS1:2x4:S0RR") == (rs.RS_PATH_BULK_SHIFT, 148, 256, 800)   # ... to 4 receivers: a lower target
+    assert shape_of("x:107101x257:i64:1x2:RS1:2x1:S0R")[::3] == (rs.RS_PATH_BULK_SHIFT, 0)                # ... rows of 1 KiB: issue-bound, unpaced
     assert shape_of("c2") == (rs.RS_PATH_TMAP, 148, 128, 860)                     # 256 MiB moved in 2 KiB rows: tensor-map copies, 4 warps, paced
     assert shape_of("sweep_P1_m8_1024MiB")[0] == shape_of("sweep_P2_m8_64MiB")[0] == rs.RS_PATH_BULK   # too large / rows of 4 KiB
     assert shape_of("c3") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 20 + 20 MiB: the TMA ring from 32 MiB moved on
