@@ -43,8 +43,11 @@
 #define RS_PACE_PERMILLE_SHORT 775            // (cold: 6.08 TB/s at 810, 5.83 at 775; hot: 4.63 at 810, 5.85 at 775)
 #define RS_PACE_PERMILLE_SHORT_DENSE 820   // short rows that are adjacent in the receivers (one bulk store per tile)
 #define RS_PACE_MIN_BYTES      (64ll << 20)   // 4 + 32 MiB: 8.75 us unpaced, 9.26 paced; 16 + 128 MiB: 27.3 unpaced, 26.4 paced
-#define RS_PACE_PERMILLE_11    880            // 1 : 1 operations moving >= RS_WIDE_11_MIN_BYTES through rs_copy_bulk: 4 warps x 12 KiB per SM, paced (tables.cpp
-                                              //   WIDE_11; 890 is 1 % better on an idle chip and 1 % worse on a hot one, collapse from 900 on)
+#define RS_PACE_PERMILLE_WIDE_11 860          // 1 : 1 operations moving >= RS_WIDE_11_MIN_BYTES through rs_copy_bulk: 4 warps x 12 KiB per SM, paced (tables.cpp WIDE_11).
+                                              //   Idle, 132 CTAs: +1 % per 10 permille up to 900 (c4 6.42 TB/s at 860, 6.48 at 870, 6.56 at 880, 6.62 at 890), collapse beyond; after GEMM
+                                              //   bursts three boxes held 880 (6.41-6.57) and a fourth, whose idle rates are 1-2 % lower too, fell to 5.94-6.08 at 880 and held 6.37-6.41
+                                              //   at 865, 6.26-6.39 at 850 (profiles/r02_pacing.md part 5)
+#define RS_PACE_PERMILLE_11    880            // smaller 1 : 1 operations made of runs >= RS_PACE_11_MIN_RUN (2 warps on every SM; ramp-bound, far from the edge)
 #define RS_PACE_PERMILLE_11_SHORT 860         // ... through tensor maps (rows of 64 B - 2 KiB)
 #define RS_PACE_11_MIN_BYTES   (128ll << 20)
 #define RS_WIDE_11_MIN_BYTES   (384ll << 20)  // (CUDA graphs of 50+ launches.  64 + 64 MiB of long runs: 21.9 us on 2 unpaced warps x 148 CTAs, 24.1 as WIDE_11; 128 + 128 MiB: long runs

@@ -195,11 +195,12 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     //    forget, every SM can push ~65 GB/s, 148 of them offer 9.6 TB/s and HBM collapses to 5.2-5.8 TB/s.  They run on
     //    every SM and are RATE MATCHED (kernels.cu pace_tile, config.h RS_PACE_PERMILLE): 6.2-6.3 TB/s.
     //  * 1 : 1 operations moving >= 384 MiB through per-row bulk copies: 4 warps x 12 KiB slots on 132 of 148 SMs, paced at
-    //    880 permille (WIDE_11).  The loop of 2 unpaced warps per SM limits itself (bytes in flight / latency) and was the
+    //    860 permille (WIDE_11).  The loop of 2 unpaced warps per SM limits itself (bytes in flight / latency) and was the
     //    round's first shape: 6.3-6.5 TB/s on an idle chip, but 4.4-4.8 for rows of 3-6 KiB once the SM clock drops under
     //    power (latency in cycles is what it is; in ns it grows).  Twice the pipelines have the slack, and the pacing then
-    //    sets the rate: 6.39-6.56 TB/s idle AND hot on every 1 : 1 layout measured (profiles/r02_pacing.md part 5); 890 is
-    //    1 % better idle and 1 % worse hot, from 900 on it collapses.  Rows <= 1 KiB (12+ copies per tile): every SM.
+    //    sets the rate: idle +1 % per 10 permille up to 900 (6.39-6.56 TB/s at 880 on the twelve 1 : 1 layouts measured), the edge
+    //    of the collapse at 900 idle, but at 870-880 on a hot chip of the pool's weakest box -- hence 860: 6.3-6.45 TB/s idle
+    //    and hot (profiles/r02_pacing.md part 5).  On every SM the edge lies 10-20 permille lower.  Rows <= 1 KiB: every SM.
     const bool write_heavy = write_bytes >= 2 * read_bytes;
     const bool wide_11 = !shift && !tmap && !capped && !write_heavy && !small_mcast && read_bytes + write_bytes >= RS_WIDE_11_MIN_BYTES;
     //  * Smaller 1 : 1 operations keep the ramp of the lighter shapes; those made of runs >= 1 MiB and moving >= 128 MiB are paced on their two warps.
@@ -230,7 +231,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     // their pack / unpack +6-15 %; write-heavy: 5.49 -> 6.08 and 4.79 -> 5.91 at 800, collapse from 830 on (profiles/r02_unaligned.md).  Rows >= 2 KiB only (1 KiB rows: issue-bound, 4.58 -> 4.47).
     sh.pace_permille = shift ? (min_run >= RS_PACE_SHIFT_MIN_RUN && read_bytes + write_bytes >= RS_PACE_SHIFT_MIN_BYTES ? (write_heavy ? RS_PACE_PERMILLE_SHIFT_MCAST : RS_PACE_PERMILLE_SHIFT) : 0)
                      : write_heavy && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
-                     : wide_11 || long_11 ? RS_PACE_PERMILLE_11
+                     : wide_11 ? RS_PACE_PERMILLE_WIDE_11 : long_11 ? RS_PACE_PERMILLE_11
                      // 1 : 1 through tensor maps (rows of 64 B - 2 KiB; always the 4-warp shape): 128-byte rows 5.37 -> 6.15-6.33 TB/s at 850-870, collapse at 890
                      : !write_heavy && short_runs && !small_mcast && read_bytes + write_bytes >= RS_PACE_11_MIN_BYTES ? RS_PACE_PERMILLE_11_SHORT : 0;
     return sh;

@@ -468,19 +468,19 @@ def test_launch_shapes_follow_the_measured_rules():
         p = _plan(w.shape, inputs.elem_bytes(w.dtype), w.src_mesh, w.src_spec, w.dst_mesh, w.dst_spec, 0, opts or None)
         o = p.op_info(op)
         return o.path, o.grid, o.block, o.pace_permille
-    assert shape_of("c4") == (rs.RS_PATH_BULK, 132, 128, 880)                     # large 1 : 1 operations: 4 warps x 12 KiB on 132 SMs, paced
-    assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 132, 128, 880)    # ... rows of 2 KiB (holds under power-limited clocks)
-    assert shape_of("sweep_P2_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 128, 880)   # ... 4 KiB rows (2 unpaced warps: 6.6 TB/s idle, 4.5 hot)
-    assert shape_of("x:256x2048x1024:bf16:2x4:S0RS1:2x4:S0S1R") == (rs.RS_PATH_BULK, 148, 256, 880)   # ... rows of 512 bytes: every SM, 8 warps x 6 KiB
-    assert shape_of("x:64x2048x4096:bf16:4x8:S0S1R:8x4:S1RS0") == (rs.RS_PATH_BULK, 148, 128, 880)    # ... rows of 1 KiB: every SM, 4 warps
-    assert shape_of("sweep_P3_m8_256MiB") == (rs.RS_PATH_BULK, 132, 128, 880)     # ... from 384 MiB moved on
+    assert shape_of("c4") == (rs.RS_PATH_BULK, 132, 128, 860)                     # large 1 : 1 operations: 4 warps x 12 KiB on 132 SMs, paced
+    assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 132, 128, 860)    # ... rows of 2 KiB (holds under power-limited clocks)
+    assert shape_of("sweep_P2_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 128, 860)   # ... 4 KiB rows (2 unpaced warps: 6.6 TB/s idle, 4.5 hot)
+    assert shape_of("x:256x2048x1024:bf16:2x4:S0RS1:2x4:S0S1R") == (rs.RS_PATH_BULK, 148, 256, 860)   # ... rows of 512 bytes: every SM, 8 warps x 6 KiB
+    assert shape_of("x:64x2048x4096:bf16:4x8:S0S1R:8x4:S1RS0") == (rs.RS_PATH_BULK, 148, 128, 860)    # ... rows of 1 KiB: every SM, 4 warps
+    assert shape_of("sweep_P3_m8_256MiB") == (rs.RS_PATH_BULK, 132, 128, 860)     # ... from 384 MiB moved on
     assert shape_of("sweep_P3_m8_128MiB") == (rs.RS_PATH_BULK, 148, 64, 880)      # below: 2 warps on every SM, paced when the runs are >= 1 MiB and 128 MiB move
     assert shape_of("sweep_P3_m8_32MiB") == (rs.RS_PATH_BULK, 148, 64, 0)
     assert shape_of("c2", rs.RS_OP_PACK) == (rs.RS_PATH_BULK, 148, 64, 0)         # 128 + 128 MiB, under the WIDE_11 size: 2 unpaced warps on every SM
     assert shape_of("sweep_P5_m8_1024MiB") == (rs.RS_PATH_BULK, 148, 64, 825)     # 1 read + 8 writes: every SM, rate matched
-    assert shape_of("sweep_P5_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 128, 880)   # its unpack is a 1 : 1 copy of 512 MiB runs
-    assert shape_of("fig5_1x1") == (rs.RS_PATH_BULK, 132, 128, 880)               # one sender, one receiver, one 1 GiB run
-    assert shape_of("t2_4") == (rs.RS_PATH_BULK, 132, 128, 880)                   # 128 KiB runs, 1 : 1
+    assert shape_of("sweep_P5_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 128, 860)   # its unpack is a 1 : 1 copy of 512 MiB runs
+    assert shape_of("fig5_1x1") == (rs.RS_PATH_BULK, 132, 128, 860)               # one sender, one receiver, one 1 GiB run
+    assert shape_of("t2_4") == (rs.RS_PATH_BULK, 132, 128, 860)                   # 128 KiB runs, 1 : 1
     assert shape_of("sweep_P5_m8_16MiB") == (rs.RS_PATH_BULK, 148, 128, 825)      # write-heavy, 144 MiB moved: paced, 4 warps
     assert shape_of("t2_9") == (rs.RS_PATH_BULK, 148, 256, 820)                   # 512-byte runs, 1 + 4: 8 warps; rows adjacent in the receivers
     assert shape_of("u4") == (rs.RS_PATH_BULK_SHIFT, 148, 256, 850)               # nothing aligned, 6 KiB rows: 8 warps, bulk stores, paced
