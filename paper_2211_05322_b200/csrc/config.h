@@ -55,7 +55,6 @@
                                               //  256 + 256 MiB: WIDE_11 +3-5 % on P1 / P4 / P6)
 #define RS_PACE_11_MIN_RUN     (1ll << 20)    // below RS_WIDE_11_MIN_BYTES: 1 : 1 operations made of runs this long keep 2 warps on every SM, paced at RS_PACE_PERMILLE_11
                                               //  (64 + 64 MiB of whole-shard copies: 6.29 TB/s against 6.14 unpaced)
-#define RS_WIDE_11_ALL_SMS_RUN 1024           // WIDE_11 with rows up to this long (12+ copies per tile): every SM instead of 132 of 148
 #define RS_MID_MCAST_BYTES     (768ll << 20)  // paced write-heavy operations moving up to this much: the 4-warp shape
 #define RS_SMALL_OP_BYTES    (32ll << 20)   // AUTO: aligned operations moving no more than this take the register path
                                             // (no shared-memory carve-out, no mbarriers: 4 MiB + 4 MiB in 3.2 us against 6.5 us;

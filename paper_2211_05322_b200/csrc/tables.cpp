@@ -200,7 +200,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     //    power (latency in cycles is what it is; in ns it grows).  Twice the pipelines have the slack, and the pacing then
     //    sets the rate: idle +1 % per 10 permille up to 900 (6.39-6.56 TB/s at 880 on the twelve 1 : 1 layouts measured), the edge
     //    of the collapse at 900 idle, but at 870-880 on a hot chip of the pool's weakest box -- hence 860: 6.3-6.45 TB/s idle
-    //    and hot (profiles/r02_pacing.md part 5).  On every SM the edge lies 10-20 permille lower.  Rows <= 1 KiB: every SM.
+    //    and hot (profiles/r02_pacing.md part 5).  On every SM the edge lies 10-20 permille lower, for every row length.
     const bool write_heavy = write_bytes >= 2 * read_bytes;
     const bool wide_11 = !shift && !tmap && !capped && !write_heavy && !small_mcast && read_bytes + write_bytes >= RS_WIDE_11_MIN_BYTES;
     //  * Smaller 1 : 1 operations keep the ramp of the lighter shapes; those made of runs >= 1 MiB and moving >= 128 MiB are paced on their two warps.
@@ -220,7 +220,8 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     sh.tile_bytes = std::max<int64_t>(128, sh.tile_bytes / 128 * 128);
     while ((int64_t)sh.warps * (sh.stages * sh.tile_bytes + RS_BULK_DESC_BYTES) + 1024 > RS_SMEM_MAX && sh.tile_bytes > 1024) sh.tile_bytes -= 1024;
     int ctas = P.sm_count;
-    if (wide_11 && min_run > RS_WIDE_11_ALL_SMS_RUN) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
+    // (large 1 : 1 operations through tensor maps too: 128-byte rows, 1 + 1 GiB, hot 5.75 TB/s on 148 CTAs, 6.17 on 132; idle 6.2 either way)
+    if (wide_11 || (tmap && !capped && !write_heavy && read_bytes + write_bytes >= RS_WIDE_11_MIN_BYTES)) ctas = P.sm_count * RS_BULK_CTAS_LONG_NUM / RS_BULK_CTAS_DEN;
     sh.grid = std::max(1, std::min(P.sm_count, pick(write_heavy ? U.bulk_ctas_mcast : U.bulk_ctas, std::max(1, ctas))));
     if (P.max_ctas > 0) sh.grid = std::min(sh.grid, P.max_ctas);
     // (operations under 64 MiB are over before the pacing has anything to hold back: they keep the unpaced ramp)

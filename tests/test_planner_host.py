@@ -471,8 +471,8 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("c4") == (rs.RS_PATH_BULK, 132, 128, 860)                     # large 1 : 1 operations: 4 warps x 12 KiB on 132 SMs, paced
     assert shape_of("sweep_P1_m8_1024MiB") == (rs.RS_PATH_BULK, 132, 128, 860)    # ... rows of 2 KiB (holds under power-limited clocks)
     assert shape_of("sweep_P2_m8_1024MiB", rs.RS_OP_UNPACK) == (rs.RS_PATH_BULK, 132, 128, 860)   # ... 4 KiB rows (2 unpaced warps: 6.6 TB/s idle, 4.5 hot)
-    assert shape_of("x:256x2048x1024:bf16:2x4:S0RS1:2x4:S0S1R") == (rs.RS_PATH_BULK, 148, 256, 860)   # ... rows of 512 bytes: every SM, 8 warps x 6 KiB
-    assert shape_of("x:64x2048x4096:bf16:4x8:S0S1R:8x4:S1RS0") == (rs.RS_PATH_BULK, 148, 128, 860)    # ... rows of 1 KiB: every SM, 4 warps
+    assert shape_of("x:256x2048x1024:bf16:2x4:S0RS1:2x4:S0S1R") == (rs.RS_PATH_BULK, 132, 256, 860)   # ... rows of 512 bytes: 8 warps x 6 KiB
+    assert shape_of("x:64x2048x4096:bf16:4x8:S0S1R:8x4:S1RS0") == (rs.RS_PATH_BULK, 132, 128, 860)    # ... rows of 1 KiB
     assert shape_of("sweep_P3_m8_256MiB") == (rs.RS_PATH_BULK, 132, 128, 860)     # ... from 384 MiB moved on
     assert shape_of("sweep_P3_m8_128MiB") == (rs.RS_PATH_BULK, 148, 64, 880)      # below: 2 warps on every SM, paced when the runs are >= 1 MiB and 128 MiB move
     assert shape_of("sweep_P3_m8_32MiB") == (rs.RS_PATH_BULK, 148, 64, 0)
@@ -492,7 +492,7 @@ def test_launch_shapes_follow_the_measured_rules():
     assert shape_of("c3") == (rs.RS_PATH_BULK, 148, 64, 0)                        # 20 + 20 MiB: the TMA ring from 32 MiB moved on
     assert shape_of("sweep_P1_m8_16MiB")[:2] == (rs.RS_PATH_LSU, 4 * 148)         # small operations: register path, 4 CTAs per SM
     assert shape_of("sweep_P1_m8_1MiB")[0] == rs.RS_PATH_LSU
-    assert shape_of("r128") == (rs.RS_PATH_TMAP, 148, 128, 860)                   # 128-byte rows at 1 + 1 GiB: boxes of 64 rows, paced
+    assert shape_of("r128") == (rs.RS_PATH_TMAP, 132, 128, 860)                   # 128-byte rows at 1 + 1 GiB: boxes of 64 rows, paced, 132 of 148 SMs like every large 1 : 1 operation
     assert shape_of("r128m") == (rs.RS_PATH_TMAP, 148, 128, 775)                  # ... 1 + 4 GiB
     assert shape_of("r128", rs.RS_OP_PACK)[0] == rs.RS_PATH_BULK                  # its pack copies whole 64 KiB runs
     p = _plan((262144, 4, 64), 2, (2,), "R,R,S0", (2,), "R,S0,R", 0)              # 64-byte rows, but only 2 per span: no box fits
