@@ -181,7 +181,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     // a caller-imposed CTA cap (rs_plan_opts.max_ctas) is made up for with more warps per CTA:
     // 64 CTAs x 4 warps move 6.0 TB/s of a 1 : 1 layout, 64 x 2 only 3.9
     const bool capped = P.max_ctas > 0 && P.max_ctas * 4 < P.sm_count * 3;
-    // shifted variant: rows of >= 4 KiB leave through bulk stores (config.h RS_SHIFT_LONG_RUN), shorter ones through registers
+    // shifted variant: the ring shape by row length (all three classes ended on 8 warps x 2 slots; stores leave from registers unless rs_tuning.shift_mode = 2: api.cu)
     const bool shift_long = shift && min_run >= RS_SHIFT_LONG_RUN, shift_mid = shift && !shift_long && min_run >= RS_SHIFT_MID_RUN;
     // small write-heavy operations (4 MiB to 8 receivers) are over in 5-8 us: many short pipelines ramp up faster
     // ... and so do tiles of 1-4 KiB (a span of the innermost row dim that short: feature maps resharded across H / W): at ~1 340 cycles
@@ -228,7 +228,7 @@ BulkShape bulk_shape(const Plan &P, bool shift, bool tmap, int64_t min_run, int6
     // short rows that are adjacent in every destination are stored with one bulk copy per tile and receiver (kernels.cu) and
     // take a higher rate than rows stored one by one (Table 2 case 9: 6.12 TB/s at 810, 6.26 at 830, 6.35-6.40 at 850 on two
     // boxes but 5.98 on a third, whose edge lies lower: 830)
-    // The shifted kernel (unaligned layouts) offers too much as well -- 8 warps per SM, stores fire and forget: u4 5.65 -> 6.31 TB/s at 850 permille, u1 5.86 -> 6.24,
+    // The shifted kernel (unaligned layouts) offers too much as well -- 8 warps per SM, stores fire and forget: u4 5.65 -> 6.1 TB/s at 850 permille (6.31 with bulk stores), u1 5.86 -> 6.24,
     // their pack / unpack +6-15 %; write-heavy: 5.49 -> 6.08 and 4.79 -> 5.91 at 800, collapse from 830 on (profiles/r02_unaligned.md).  Rows >= 2 KiB only (1 KiB rows: issue-bound, 4.58 -> 4.47).
     sh.pace_permille = shift ? (min_run >= RS_PACE_SHIFT_MIN_RUN && read_bytes + write_bytes >= RS_PACE_SHIFT_MIN_BYTES ? (write_heavy ? RS_PACE_PERMILLE_SHIFT_MCAST : RS_PACE_PERMILLE_SHIFT) : 0)
                      : write_heavy && read_bytes + write_bytes >= RS_PACE_MIN_BYTES ? (short_runs ? (dst_dense ? RS_PACE_PERMILLE_SHORT_DENSE : RS_PACE_PERMILLE_SHORT) : RS_PACE_PERMILLE)
